@@ -1,0 +1,135 @@
+/* ORACLE -- TEST INFRASTRUCTURE, NOT PRODUCT CODE.
+ *
+ * Plain, slow, fp64 CPU implementation of what the index-based multi-walk force path computes
+ * (arXiv 1907.02290, /root/reference/PAPER.md; "P:n" = line n of that file).  Only tests/,
+ * __graft_entry__.smoke() and bench.py's cpu_baseline / --impl reference legs may call it.  It
+ * shares no code with the CUDA library (paper_1907_02290_b200/csrc) and is never tuned.
+ *
+ * What it evaluates:
+ *   orc_monopoles  P:160, P:848  monopole (centre-of-mass) moment of every tree cell, bottom line
+ *                  of the definition: M_c = sum m_p, X_c = sum m_p x_p / M_c over the cell's
+ *                  particle range.  Kept in fp64 (never rounded to fp32).
+ *   orc_forces     P:77, P:181, P:441-477  for each i-group, each particle i of the group: the
+ *                  softened Newtonian sum over the group's shared interaction list -- EPJ entries
+ *                  are particle indices, SPJ entries are cell indices whose (X_c, M_c) act as one
+ *                  particle ("a SPJ represents a node of Barnes-Hut tree", P:387 same kernel).
+ *                  acc_i = G sum_k m_k d / (|d|^2 + eps^2)^(3/2),  d = x_k - x_i
+ *                  pot_i = -G sum_k m_k / (|d|^2 + eps^2)^(1/2)
+ *                  The paper never prints the formula; it gives eps2 = eps*eps, the
+ *                  float4 (x,y,z,m) -> (ax,ay,az,pot) layout and "monopole"
+ *                  (P:197).  Readings S1-S5 in DESIGN.md: Plummer softening, the same eps
+ *                  for EPJ and SPJ, the entry whose INDEX equals i is skipped (a different particle
+ *                  at the same position is a real pair), pot <= 0 and includes G.
+ *   orc_direct     the plain O(N^2) definition of the same sum over all other particles.
+ *
+ * Inputs are the fp32 particle array exactly as uploaded to the GPU; every value is widened to
+ * double before any arithmetic.  OpenMP only distributes groups / particles over threads; each
+ * sum runs in list order.  No blocking, no SIMD intrinsics, no reordering.
+ */
+#include <math.h>
+#include <stdint.h>
+#ifdef _OPENMP
+#include <omp.h>
+#endif
+
+int orc_num_threads(void) {
+#ifdef _OPENMP
+    return omp_get_max_threads();
+#else
+    return 1;
+#endif
+}
+
+void orc_set_num_threads(int n) {
+#ifdef _OPENMP
+    if (n > 0) omp_set_num_threads(n);
+#else
+    (void)n;
+#endif
+}
+
+/* mom[4*c + 0..2] = X_c, mom[4*c + 3] = M_c.  cells4 = (first_ptcl, n_ptcl, first_child, n_child). */
+void orc_monopoles(int64_t n_cell, const int32_t* cells4, const float* posm, double* mom) {
+    int64_t c;
+#pragma omp parallel for schedule(dynamic, 64)
+    for (c = 0; c < n_cell; ++c) {
+        int64_t first = cells4[4 * c + 0], cnt = cells4[4 * c + 1];
+        double m = 0.0, sx = 0.0, sy = 0.0, sz = 0.0;
+        for (int64_t p = first; p < first + cnt; ++p) {
+            double mp = (double)posm[4 * p + 3];
+            m += mp;
+            sx += mp * (double)posm[4 * p + 0];
+            sy += mp * (double)posm[4 * p + 1];
+            sz += mp * (double)posm[4 * p + 2];
+        }
+        mom[4 * c + 0] = sx / m;
+        mom[4 * c + 1] = sy / m;
+        mom[4 * c + 2] = sz / m;
+        mom[4 * c + 3] = m;
+    }
+}
+
+static void pair_term(double xi, double yi, double zi, double xk, double yk, double zk, double mk, double eps2,
+                      double* ax, double* ay, double* az, double* pot) {
+    double dx = xk - xi, dy = yk - yi, dz = zk - zi;
+    double r2 = dx * dx + dy * dy + dz * dz + eps2;
+    double rinv = 1.0 / sqrt(r2);
+    double mr3 = mk * rinv * rinv * rinv;
+    *ax += mr3 * dx;
+    *ay += mr3 * dy;
+    *az += mr3 * dz;
+    *pot -= mk * rinv;
+}
+
+/* Evaluates groups sel[0..n_sel) (or all groups 0..n_sel-1 when sel == NULL).
+ * acc: 3 doubles per particle, pot: 1 per particle, indexed by tree-order particle position; only the
+ * selected groups' particles are written.  mom comes from orc_monopoles on the SAME posm. */
+void orc_forces(int64_t n_sel, const int64_t* sel, const int32_t* grp_first, const int32_t* grp_n,
+                const int64_t* epj_off, const int32_t* epj_id, const int64_t* spj_off, const int32_t* spj_id,
+                const float* posm, const double* mom, double eps, double G, double* acc, double* pot) {
+    const double eps2 = eps * eps;
+    int64_t s;
+#pragma omp parallel for schedule(dynamic, 1)
+    for (s = 0; s < n_sel; ++s) {
+        int64_t g = sel ? sel[s] : s;
+        int64_t first = grp_first[g], cnt = grp_n[g];
+        for (int64_t i = first; i < first + cnt; ++i) {
+            double xi = (double)posm[4 * i + 0], yi = (double)posm[4 * i + 1], zi = (double)posm[4 * i + 2];
+            double ax = 0.0, ay = 0.0, az = 0.0, p = 0.0;
+            for (int64_t e = epj_off[g]; e < epj_off[g + 1]; ++e) {
+                int64_t k = epj_id[e];
+                if (k == i) continue;
+                pair_term(xi, yi, zi, (double)posm[4 * k + 0], (double)posm[4 * k + 1], (double)posm[4 * k + 2],
+                          (double)posm[4 * k + 3], eps2, &ax, &ay, &az, &p);
+            }
+            for (int64_t e = spj_off[g]; e < spj_off[g + 1]; ++e) {
+                int64_t c = spj_id[e];
+                pair_term(xi, yi, zi, mom[4 * c + 0], mom[4 * c + 1], mom[4 * c + 2], mom[4 * c + 3], eps2, &ax, &ay, &az, &p);
+            }
+            acc[3 * i + 0] = G * ax;
+            acc[3 * i + 1] = G * ay;
+            acc[3 * i + 2] = G * az;
+            pot[i] = G * p;
+        }
+    }
+}
+
+/* Direct summation over all other particles (the definition Barnes-Hut approximates). */
+void orc_direct(int64_t n, const float* posm, double eps, double G, double* acc, double* pot) {
+    const double eps2 = eps * eps;
+    int64_t i;
+#pragma omp parallel for schedule(static)
+    for (i = 0; i < n; ++i) {
+        double xi = (double)posm[4 * i + 0], yi = (double)posm[4 * i + 1], zi = (double)posm[4 * i + 2];
+        double ax = 0.0, ay = 0.0, az = 0.0, p = 0.0;
+        for (int64_t k = 0; k < n; ++k) {
+            if (k == i) continue;
+            pair_term(xi, yi, zi, (double)posm[4 * k + 0], (double)posm[4 * k + 1], (double)posm[4 * k + 2],
+                      (double)posm[4 * k + 3], eps2, &ax, &ay, &az, &p);
+        }
+        acc[3 * i + 0] = G * ax;
+        acc[3 * i + 1] = G * ay;
+        acc[3 * i + 2] = G * az;
+        pot[i] = G * p;
+    }
+}

@@ -1,0 +1,94 @@
+"""ctypes front end of oracle/mwf_oracle.c (fp64 CPU oracle; test infrastructure only)."""
+from __future__ import annotations
+
+import ctypes
+import os
+import subprocess
+
+import numpy as np
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+_SRC = os.path.join(_HERE, "mwf_oracle.c")
+_SO = os.path.join(_HERE, "libmwf_oracle.so")
+_lib = None
+
+
+def build(force: bool = False) -> str:
+    """Compile the oracle with gcc -O2 -fopenmp (no fast-math, no intrinsics)."""
+    if force or not os.path.exists(_SO) or os.path.getmtime(_SO) < os.path.getmtime(_SRC):
+        r = subprocess.run(["gcc", "-O2", "-fopenmp", "-ffp-contract=off", "-shared", "-fPIC", "-o", _SO, _SRC, "-lm"],
+                           capture_output=True, text=True)
+        if r.returncode != 0:
+            raise RuntimeError("oracle build failed:\n" + r.stderr)
+    return _SO
+
+
+def _load():
+    global _lib
+    if _lib is None:
+        lib = ctypes.CDLL(build())
+        vp, i64, dbl = ctypes.c_void_p, ctypes.c_int64, ctypes.c_double
+        lib.orc_num_threads.restype = ctypes.c_int
+        lib.orc_set_num_threads.argtypes = [ctypes.c_int]
+        lib.orc_monopoles.argtypes = [i64, vp, vp, vp]
+        lib.orc_forces.argtypes = [i64, vp, vp, vp, vp, vp, vp, vp, vp, vp, dbl, dbl, vp, vp]
+        lib.orc_direct.argtypes = [i64, vp, dbl, dbl, vp, vp]
+        _lib = lib
+    return _lib
+
+
+def _p(a):
+    return None if a is None else a.ctypes.data_as(ctypes.c_void_p)
+
+
+def num_threads() -> int:
+    return int(_load().orc_num_threads())
+
+
+def set_num_threads(n: int) -> None:
+    _load().orc_set_num_threads(int(n))
+
+
+def _c(a, dt):
+    a = np.ascontiguousarray(a, dtype=dt)
+    return a
+
+
+def monopoles(cells: np.ndarray, posm: np.ndarray) -> np.ndarray:
+    """[n_cell,4] float64 (X_c xyz, M_c) from the fp32 particle array."""
+    cells = _c(cells, np.int32)
+    posm = _c(posm, np.float32)
+    mom = np.empty((cells.shape[0], 4), np.float64)
+    _load().orc_monopoles(cells.shape[0], _p(cells), _p(posm), _p(mom))
+    return mom
+
+
+def forces(posm, mom, grp_first, grp_n, epj_off, epj_id, spj_off, spj_id, eps: float, G: float = 1.0, groups=None):
+    """acc [N,3], pot [N] in float64 for the selected groups (all when `groups` is None); particles of
+    other groups are left NaN."""
+    posm = _c(posm, np.float32)
+    mom = _c(mom, np.float64)
+    grp_first, grp_n = _c(grp_first, np.int32), _c(grp_n, np.int32)
+    epj_off, spj_off = _c(epj_off, np.int64), _c(spj_off, np.int64)
+    epj_id, spj_id = _c(epj_id, np.int32), _c(spj_id, np.int32)
+    n = posm.shape[0]
+    acc = np.full((n, 3), np.nan)
+    pot = np.full(n, np.nan)
+    if groups is None:
+        n_sel, sel = grp_first.shape[0], None
+    else:
+        sel = _c(groups, np.int64)
+        n_sel = sel.shape[0]
+    _load().orc_forces(n_sel, _p(sel), _p(grp_first), _p(grp_n), _p(epj_off), _p(epj_id), _p(spj_off), _p(spj_id),
+                       _p(posm), _p(mom), float(eps), float(G), _p(acc), _p(pot))
+    return acc, pot
+
+
+def direct(posm, eps: float, G: float = 1.0):
+    """Plain O(N^2) direct summation: acc [N,3], pot [N] float64."""
+    posm = _c(posm, np.float32)
+    n = posm.shape[0]
+    acc = np.empty((n, 3))
+    pot = np.empty(n)
+    _load().orc_direct(n, _p(posm), float(eps), float(G), _p(acc), _p(pot))
+    return acc, pot

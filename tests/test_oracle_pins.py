@@ -1,0 +1,242 @@
+"""Pins of the fp64 oracle (oracle/) against closed forms, invariants and brute force.
+
+Each test names the SURVEY.md section 8(c) pin (P1..P8) it implements and the mistake it is meant to
+catch.  None of these values comes from the CUDA path.
+"""
+import math
+
+import numpy as np
+import pytest
+
+import oracle
+from paper_1907_02290_b200.workload import CONFIGS, build_tree_and_lists, make_particles, make_workload
+
+
+def one_group_lists(n, i_first, n_i, epj, spj=()):
+    grp_first = np.array([i_first], np.int32)
+    grp_n = np.array([n_i], np.int32)
+    epj_off = np.array([0, len(epj)], np.int64)
+    spj_off = np.array([0, len(spj)], np.int64)
+    return grp_first, grp_n, epj_off, np.array(epj, np.int32), spj_off, np.array(spj, np.int32)
+
+
+def eval_lists(posm, mom, lists, eps, G=1.0):
+    gf, gn, eo, ei, so, si = lists
+    return oracle.forces(posm, mom, gf, gn, eo, ei, so, si, eps, G)
+
+
+# ---------------------------------------------------------------- P1: closed forms
+def test_single_source_is_a_plummer_sphere():
+    """One source of mass M with eps = a IS a Plummer sphere: phi = -GM/sqrt(r^2+a^2),
+    |a| = GM r/(r^2+a^2)^(3/2), pointing at the source.  Catches sign, exponent, eps and G errors."""
+    M, a, G = 2.0, 0.5, 3.0
+    src = np.array([1.0, -2.0, 0.5])
+    d = np.array([3.0, 4.0, 12.0])            # |d| = 13, all exactly representable in fp32
+    posm = np.array([[*src, M], [*(src + d), 0.25]], np.float32)
+    r2 = 169.0 + a * a
+    want_acc = -G * M * d / r2 ** 1.5         # test particle is pulled back toward the source
+    want_pot = -G * M / math.sqrt(r2)
+    acc, pot = oracle.direct(posm, a, G)
+    np.testing.assert_allclose(acc[1], want_acc, rtol=1e-14)
+    assert pot[1] == pytest.approx(want_pot, rel=1e-14)
+    # the same through the list path, source as an EPJ
+    mom = np.zeros((1, 4))
+    acc, pot = eval_lists(posm, mom, one_group_lists(2, 1, 1, [0, 1]), a, G)
+    np.testing.assert_allclose(acc[1], want_acc, rtol=1e-14)
+    assert pot[1] == pytest.approx(want_pot, rel=1e-14)
+    # and with the source given as an SPJ (cell 0 = a monopole at src with mass M)
+    mom = np.array([[*src, M]])
+    acc, pot = eval_lists(posm, mom, one_group_lists(2, 1, 1, [1], [0]), a, G)
+    np.testing.assert_allclose(acc[1], want_acc, rtol=1e-14)
+    assert pot[1] == pytest.approx(want_pot, rel=1e-14)
+
+
+def test_two_unequal_bodies():
+    """a_1 = G m_2 d/(..), a_2 = -G m_1 d/(..): catches using m_i where m_j belongs and a flipped d."""
+    posm = np.array([[0, 0, 0, 3.0], [1, 2, 2, 0.5]], np.float32)   # |d| = 3
+    eps = 4.0                                                      # r2 = 25
+    acc, pot = oracle.direct(posm, eps, 1.0)
+    d = np.array([1.0, 2.0, 2.0])
+    np.testing.assert_allclose(acc[0], 0.5 * d / 125.0, rtol=1e-15)
+    np.testing.assert_allclose(acc[1], -3.0 * d / 125.0, rtol=1e-15)
+    assert pot[0] == pytest.approx(-0.5 / 5.0, rel=1e-15)
+    assert pot[1] == pytest.approx(-3.0 / 5.0, rel=1e-15)
+
+
+def test_ring_on_axis():
+    """n equal masses on a ring of radius R: on the axis at height z,
+    a_z = -G n m z/(R^2+z^2+eps^2)^(3/2), a_x = a_y = 0, phi = -G n m/sqrt(R^2+z^2+eps^2).
+    Catches per-component mix-ups (a transposed coordinate breaks the cancellation)."""
+    n, R, z, m, eps = 16, 2.0, 1.5, 0.125, 0.25
+    ang = 2 * np.pi * np.arange(n) / n
+    ring = np.stack([R * np.cos(ang), R * np.sin(ang), np.zeros(n), np.full(n, m)], axis=1)
+    posm = np.concatenate([ring, [[0, 0, z, 1.0]]]).astype(np.float32)
+    acc, pot = oracle.direct(posm, eps, 1.0)
+    s = R * R + z * z + eps * eps
+    assert acc[n, 2] == pytest.approx(-n * m * z / s ** 1.5, rel=1e-6)   # fp32 rounding of the ring
+    assert abs(acc[n, 0]) < 1e-8 and abs(acc[n, 1]) < 1e-8
+    assert pot[n] == pytest.approx(-n * m / math.sqrt(s), rel=1e-6)
+
+
+def test_exact_scaling_laws():
+    """x -> 2x, eps -> 2eps gives acc/4 and pot/2; m -> 4m gives 4x both.  Powers of two are exact in
+    fp32, so this pins the -3/2 and -1/2 exponents to rounding."""
+    posm, _ = make_particles(CONFIGS[0], 256)
+    a1, p1 = oracle.direct(posm, 1 / 64, 1.0)
+    q = posm.copy()
+    q[:, :3] *= 2
+    a2, p2 = oracle.direct(q, 2 / 64, 1.0)
+    np.testing.assert_allclose(a2, a1 / 4, rtol=1e-13)
+    np.testing.assert_allclose(p2, p1 / 2, rtol=1e-13)
+    q = posm.copy()
+    q[:, 3] *= 4
+    a3, p3 = oracle.direct(q, 1 / 64, 0.5)
+    np.testing.assert_allclose(a3, a1 * 2, rtol=1e-13)
+    np.testing.assert_allclose(p3, p1 * 2, rtol=1e-13)
+
+
+def test_coincident_distinct_particles_are_a_real_pair():
+    """Reading S4: only the entry whose INDEX equals i is skipped; another particle at the same
+    position adds 0 to acc and -G m/eps to pot."""
+    posm = np.array([[1, 1, 1, 2.0], [1, 1, 1, 5.0]], np.float32)
+    acc, pot = oracle.direct(posm, 0.5, 1.0)
+    assert np.all(acc == 0)
+    assert pot[0] == -5.0 / 0.5 and pot[1] == -2.0 / 0.5
+
+
+# ---------------------------------------------------------------- P2, P3: brute force / theta -> 0
+def brute_force(posm, eps, G):
+    """Test-local O(N^2) numpy evaluation (fp64), j != i."""
+    x = posm[:, :3].astype(np.float64)
+    m = posm[:, 3].astype(np.float64)
+    d = x[None, :, :] - x[:, None, :]
+    r2 = (d ** 2).sum(-1) + eps * eps
+    np.fill_diagonal(r2, np.inf)
+    w = m[None, :] / r2 ** 1.5
+    return G * (w[:, :, None] * d).sum(1), -G * (m[None, :] / np.sqrt(r2)).sum(1)
+
+
+@pytest.mark.parametrize("n", [1, 2, 37, 700])
+def test_direct_equals_brute_force(n):
+    posm, _ = make_particles(CONFIGS[0], n)
+    a, p = oracle.direct(posm, 1 / 64, 1.5)
+    ab, pb = brute_force(posm, 1 / 64, 1.5)
+    np.testing.assert_allclose(a, ab, rtol=1e-12, atol=1e-15)
+    np.testing.assert_allclose(p, pb, rtol=1e-12, atol=1e-15)
+
+
+@pytest.mark.parametrize("theta", [0.0, 1e-3])
+def test_theta_to_zero_reproduces_direct_summation(theta):
+    """north_star pin: with theta -> 0 every list is all particles and the list path equals direct
+    summation (checks CSR offsets, group ranges and index-based self exclusion)."""
+    posm, _ = make_particles(CONFIGS[0], 1500)
+    w = build_tree_and_lists(posm, 8, 64, theta)
+    assert w.spj_off[-1] == 0
+    mom = oracle.monopoles(w.cells, w.posm)
+    acc, pot = oracle.forces(w.posm, mom, w.grp_first, w.grp_n, w.epj_off, w.epj_id, w.spj_off, w.spj_id, 1 / 64)
+    ab, pb = brute_force(w.posm, 1 / 64, 1.0)
+    np.testing.assert_allclose(acc, ab, rtol=1e-12, atol=1e-14)
+    np.testing.assert_allclose(pot, pb, rtol=1e-12)
+
+
+def test_group_subset_selection():
+    w = make_workload(CONFIGS[0], 2000)
+    mom = oracle.monopoles(w.cells, w.posm)
+    args = (w.posm, mom, w.grp_first, w.grp_n, w.epj_off, w.epj_id, w.spj_off, w.spj_id, 1 / 64)
+    acc, pot = oracle.forces(*args)
+    sel = np.arange(1, w.n_group, 3)
+    acc_s, pot_s = oracle.forces(*args, groups=sel)
+    mask = np.zeros(w.n, bool)
+    for g in sel:
+        mask[w.grp_first[g]:w.grp_first[g] + w.grp_n[g]] = True
+    assert np.array_equal(acc_s[mask], acc[mask]) and np.array_equal(pot_s[mask], pot[mask])
+    assert np.all(np.isnan(acc_s[~mask])) and np.all(np.isnan(pot_s[~mask]))
+
+
+# ---------------------------------------------------------------- P5: momentum conservation
+def test_direct_sum_conserves_momentum():
+    """Newton's third law holds term by term for direct summation: |sum m a| <= 1e-13 sum m|a|."""
+    posm, _ = make_particles(CONFIGS[2], 1024)      # unequal masses (disk + halo)
+    acc, _ = oracle.direct(posm, 0.005)
+    m = posm[:, 3].astype(np.float64)
+    resid = np.linalg.norm((m[:, None] * acc).sum(0))
+    assert resid <= 1e-13 * (m * np.linalg.norm(acc, axis=1)).sum()
+
+
+# ---------------------------------------------------------------- P6: Plummer potential energy
+def truncated_plummer_W(rc):
+    """W of a unit-mass Plummer sphere (G = a = 1) cut at r < rc and renormalised to unit mass:
+    W = -4 pi int_0^rc rho(r) M(r) r dr / M(rc)^2, by quadrature."""
+    from scipy.integrate import quad
+    rho = lambda r: 3.0 / (4 * np.pi) * (1 + r * r) ** -2.5
+    mass = lambda r: r ** 3 * (1 + r * r) ** -1.5
+    val, _ = quad(lambda r: rho(r) * mass(r) * r, 0, rc, epsabs=1e-13, epsrel=1e-12)
+    return -4 * np.pi * val / mass(rc) ** 2
+
+
+def test_plummer_potential_energy(golden):
+    """north_star pin: W = -3 pi G M^2/(32 a); with the cut at 22.8a the exact value is 1.0055x that.
+    Ties the generator, the pair sum and the sign/scale of pot (reading S3) together."""
+    w_inf = golden["plummer_W_coeff"]
+    assert w_inf == pytest.approx(-3 * math.pi / 32, rel=1e-15)
+    assert truncated_plummer_W(1e4) == pytest.approx(w_inf, rel=1e-6)
+    want = truncated_plummer_W(22.8)
+    assert want / w_inf == pytest.approx(1.0055, abs=5e-4)
+    posm, _ = make_particles(CONFIGS[0], 16384)
+    _, pot = oracle.direct(posm, 1 / 64)
+    W = 0.5 * np.sum(posm[:, 3].astype(np.float64) * pot)
+    assert W == pytest.approx(want, rel=0.02)       # sampling scatter ~0.4 % at N = 16384; eps shifts -0.05 %
+
+
+# ---------------------------------------------------------------- P7: Barnes-Hut quality of tree lists
+def test_tree_forces_converge_to_direct_sum():
+    """The list path with SPJ monopoles approximates direct summation, better as theta falls.
+    A wrong SPJ index, a missing list segment or a bad monopole gives O(1) errors here."""
+    posm, _ = make_particles(CONFIGS[0], 4096)
+    eps = 1 / 64
+    rms = []
+    for theta in (0.8, 0.5, 0.3):
+        w = build_tree_and_lists(posm, 8, 64, theta)
+        mom = oracle.monopoles(w.cells, w.posm)
+        acc, pot = oracle.forces(w.posm, mom, w.grp_first, w.grp_n, w.epj_off, w.epj_id, w.spj_off, w.spj_id, eps)
+        ad, pd = oracle.direct(w.posm, eps)
+        e = np.linalg.norm(acc - ad, axis=1) / np.linalg.norm(ad, axis=1)
+        rms.append(np.sqrt(np.mean(e ** 2)))
+        if theta == 0.5:
+            assert 5e-5 < rms[-1] < 3e-3 and e.max() < 5e-2
+            assert np.sqrt(np.mean(((pot - pd) / pd) ** 2)) < 5e-4
+            m = w.posm[:, 3].astype(np.float64)
+            assert 0.5 * np.sum(m * pot) == pytest.approx(0.5 * np.sum(m * pd), rel=3e-4)
+    assert rms[0] > rms[1] > rms[2]
+
+
+# ---------------------------------------------------------------- P8: monopoles
+def test_monopole_invariants():
+    w = make_workload(CONFIGS[2], 3000)              # unequal masses
+    mom = oracle.monopoles(w.cells, w.posm)
+    x = w.posm[:, :3].astype(np.float64)
+    m = w.posm[:, 3].astype(np.float64)
+    # root = whole system
+    assert mom[0, 3] == pytest.approx(m.sum(), rel=1e-13)
+    np.testing.assert_allclose(mom[0, :3], (m[:, None] * x).sum(0) / m.sum(), rtol=1e-12, atol=1e-15)
+    # parent = mass-weighted combination of its children (the paper's bottom-up pass)
+    for c in range(w.n_cell):
+        fc, nc = w.cells[c, 2], w.cells[c, 3]
+        if nc:
+            ch = mom[fc:fc + nc]
+            assert ch[:, 3].sum() == pytest.approx(mom[c, 3], rel=1e-13)
+            np.testing.assert_allclose((ch[:, 3:4] * ch[:, :3]).sum(0) / ch[:, 3].sum(), mom[c, :3], rtol=1e-11, atol=1e-14)
+    # centre of mass lies inside the cell cube
+    half = 0.5 * w.geom[:, 3:4] * (1 + 1e-12)
+    assert np.all(np.abs(mom[:, :3] - w.geom[:, :3]) <= half)
+    # translating all particles by t moves every X_c by t and leaves M_c alone; positions are first put
+    # on a 2^-12 grid so that the translated fp32 values are exact
+    t = np.array([64.0, -32.0, 16.0])
+    q0 = w.posm.copy()
+    q0[:, :3] = np.clip(np.round(q0[:, :3].astype(np.float64) * 4096) / 4096, -1000, 1000)
+    q1 = q0.copy()
+    q1[:, :3] = (q0[:, :3].astype(np.float64) + t).astype(np.float32)
+    assert np.all(q1[:, :3].astype(np.float64) - t == q0[:, :3])
+    mom0, mom1 = oracle.monopoles(w.cells, q0), oracle.monopoles(w.cells, q1)
+    assert np.array_equal(mom1[:, 3], mom0[:, 3])
+    np.testing.assert_allclose(mom1[:, :3] - t, mom0[:, :3], atol=1e-12)
