@@ -1,0 +1,324 @@
+#!/usr/bin/env python
+"""Benchmark of the index-based multi-walk force path on B200 (contract: see DESIGN.md "Measurement").
+
+  python bench.py [--gpus N] [--steps K] [--warmup W] [--config 1..5] [--impl ours|reference]
+
+A "step" is one pass of the whole hot path over one batch of synthetic input: a list-reuse step =
+upload particles -> refresh monopoles -> force kernel over all groups -> retrieve acc+pot (rows
+a1, a3, a4, a5 of SURVEY.md section 8(a)), with the tree and the index lists uploaded once before the
+timed region (row a2; the paper's construction step).  Default workload: BASELINE.json
+config 5 (Plummer N = 2^22, list reuse), the configuration the north_star's 50 %-of-peak target names.
+
+  value  interactions/s of the whole job with inputs resident in HBM (device source and destination)
+  e2e    the same through the C ABI with pinned HOST buffers: H2D of the particles and D2H of acc+pot
+         inside the timed region
+  roofline  force kernel alone: 23 flop x interactions / CUDA-event kernel time, against the FP32
+         non-tensor peak SMs x 128 FMA/clk x 2 x max SM clock  ("bound": "alu")
+  cpu_baseline  the fp64 oracle, as it stands, on the box's host cores, on a bounded sample of groups
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import subprocess
+import sys
+import threading
+import time
+
+import numpy as np
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+N_OP = 23  # flop per interaction, the paper's convention (Table 8, P:1208 Table A.1)
+METRIC = "particle-particle interactions/sec"
+UNIT = "interactions/s"
+
+
+def log(*a):
+    print(*a, file=sys.stderr, flush=True)
+
+
+# ----------------------------------------------------------------------------- clocks
+class ClockSampler:
+    """nvidia-smi sampled every 200 ms during the timed region (B200_PROFILING.md clocks line)."""
+    Q = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,clocks_event_reasons.hw_thermal_slowdown,"
+         "clocks_event_reasons.sw_thermal_slowdown,clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, index: int):
+        self.rows, self.proc, self.index = [], None, index
+
+    def __enter__(self):
+        try:
+            self.proc = subprocess.Popen(["nvidia-smi", "-i", str(self.index), "--query-gpu=" + self.Q, "--format=csv,noheader,nounits", "-lms", "200"],
+                                         stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
+            self.thread = threading.Thread(target=self._read, daemon=True)
+            self.thread.start()
+        except OSError:
+            self.proc = None
+        return self
+
+    def _read(self):
+        for line in self.proc.stdout:
+            parts = [x.strip() for x in line.split(",")]
+            if len(parts) >= 7:
+                self.rows.append(parts)
+
+    def __exit__(self, *exc):
+        if self.proc:
+            self.proc.terminate()
+            try:
+                self.proc.wait(timeout=5)
+            except subprocess.TimeoutExpired:
+                self.proc.kill()
+
+    def summary(self):
+        sm, mx, pw, reasons = [], [], [], set()
+        for r in self.rows:
+            try:
+                sm.append(float(r[0])); mx.append(float(r[1])); pw.append(float(r[2]))
+            except ValueError:
+                continue
+            for name, v in zip(("hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"), r[3:7]):
+                if v.lower().startswith("active"):
+                    reasons.add(name)
+        if not sm:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": [], "samples": 0}
+        busy = [s for s, p in zip(sm, pw) if p >= 0.5 * max(pw)] or sm
+        return {"sm_mhz": float(np.median(busy)), "sm_max_mhz": float(max(mx)), "reasons": sorted(reasons),
+                "samples": len(sm), "power_w_max": float(max(pw))}
+
+
+def measured_peaks():
+    try:
+        return json.load(open(os.path.join(ROOT, "MEASURED_PEAKS.json")))
+    except (OSError, ValueError):
+        return {}
+
+
+# ----------------------------------------------------------------------------- oracle legs
+def oracle_sample(w, cfg, target_s: float, seed: int = 12345):
+    """Times the fp64 oracle (monopoles excluded: forces only, like the GPU kernel figure) on a seeded
+    sample of groups sized for about `target_s` seconds.  Returns (interactions, seconds, n_groups)."""
+    import oracle
+    mom = oracle.monopoles(w.cells, w.posm)
+    rng = np.random.default_rng(seed)
+    order = rng.permutation(w.n_group)
+    per_group = w.grp_n.astype(np.int64) * w.n_list
+    args = (w.posm, mom, w.grp_first, w.grp_n, w.epj_off, w.epj_id, w.spj_off, w.spj_id, cfg.eps, 1.0)
+    # calibrate on ~2e8 interactions
+    k0 = int(np.searchsorted(np.cumsum(per_group[order]), 2e8)) + 1
+    k0 = min(k0, w.n_group)
+    t = time.perf_counter()
+    oracle.forces(*args, groups=order[:k0])
+    dt0 = time.perf_counter() - t
+    rate = per_group[order[:k0]].sum() / max(dt0, 1e-9)
+    want = rate * target_s
+    k = int(np.searchsorted(np.cumsum(per_group[order]), want)) + 1
+    k = max(k0, min(k, w.n_group))
+    sel = order[:k]
+    t = time.perf_counter()
+    oracle.forces(*args, groups=sel)
+    dt = time.perf_counter() - t
+    return int(per_group[sel].sum()), dt, k
+
+
+def run_reference(args, cfg, w, rank, world):
+    """--impl reference: the oracle as it stands on the host cores; each step a bounded sample."""
+    if rank != 0:
+        return
+    import oracle
+    per_step_s = max(2.0, min(20.0, 150.0 / max(1, args.steps + args.warmup)))
+    inter_tot, t_tot, groups = 0, 0.0, 0
+    for s in range(args.warmup + args.steps):
+        i, dt, k = oracle_sample(w, cfg, per_step_s, seed=777 + s)
+        if s >= args.warmup:
+            inter_tot += i; t_tot += dt; groups = k
+    value = inter_tot / t_tot
+    cores = oracle.num_threads()
+    sample = "%d of %d groups per step (seeded), forces only" % (groups, w.n_group)
+    out = {
+        "impl": "reference", "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": args.gpus, "steps": args.steps, "warmup": args.warmup,
+        "ms_per_step": 1e3 * t_tot / max(1, args.steps), "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+        "dtype": "f64", "data": "synthetic", "config": workload_config(cfg, w),
+        "cpu_baseline": {"value": value, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": sample},
+        "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+        "gpu_launches": 0,
+    }
+    print(json.dumps(out), flush=True)
+
+
+def workload_config(cfg, w):
+    return {"workload": "config %d: %s" % (cfg_index(cfg) + 1, cfg.name), "n": w.n, "n_group": w.n_group, "n_cell": w.n_cell,
+            "list_entries": w.n_entry, "interactions_per_step": w.interactions, "theta": cfg.theta, "eps": cfg.eps,
+            "n_leaf": cfg.n_leaf, "n_grp": cfg.n_grp, "step": "list-reuse step: upload, monopole refresh, force kernel, retrieve",
+            "l2": "inputs larger than L2 (index lists %.2f GB streamed every step)" % (4e-9 * w.n_entry), "parallelism": "replicas"}
+
+
+def cfg_index(cfg):
+    from paper_1907_02290_b200.workload import CONFIGS
+    return CONFIGS.index(cfg)
+
+
+# ----------------------------------------------------------------------------- main
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=10)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--config", type=int, default=5, help="BASELINE.json config 1..5")
+    ap.add_argument("--n", type=int, default=None, help="override the particle count (testing only)")
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--cpu-baseline-seconds", type=float, default=15.0)
+    ap.add_argument("--n-tag", type=int, default=8)
+    args = ap.parse_args()
+    args.warmup = max(args.warmup, 3) if args.impl == "ours" else args.warmup
+
+    from paper_1907_02290_b200 import replicas
+    from paper_1907_02290_b200.workload import CONFIGS, make_workload
+    cfg = CONFIGS[args.config - 1]
+
+    if args.impl == "reference":
+        rank = int(os.environ.get("RANK", "0"))
+        if rank != 0:
+            return 0
+        t = time.perf_counter()
+        w = make_workload(cfg, args.n)
+        log("[bench] workload built in %.1f s" % (time.perf_counter() - t))
+        run_reference(args, cfg, w, rank, int(os.environ.get("WORLD_SIZE", "1")))
+        return 0
+
+    import torch
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py needs a CUDA device: the product path has no CPU fallback")
+    rank, world, local = replicas.init_from_env()
+    torch.cuda.set_device(local)
+    from paper_1907_02290_b200 import binding
+
+    t = time.perf_counter()
+    w = make_workload(cfg, args.n)
+    t_build = time.perf_counter() - t
+    log("[bench r%d] %s: N=%d cells=%d groups=%d entries=%d interactions=%.4e (host tree+lists %.1f s)" % (
+        rank, cfg.name, w.n, w.n_cell, w.n_group, w.n_entry, w.interactions, t_build))
+
+    f = binding.MultiWalkForce.for_workload(w, n_tag=args.n_tag, device=local)
+    t = time.perf_counter()
+    f.upload_workload(w, binding.MAKE_LIST_FOR_REUSE)      # construction step: tree + lists, once
+    f.sync()
+    t_upload = time.perf_counter() - t
+    src_dev = torch.from_numpy(w.posm).to(f.device)
+    dst_dev = torch.zeros((w.n, 4), dtype=torch.float32, device=f.device)
+    src_host, dst_host = f.pinned(w.n), f.pinned(w.n)
+    src_host.numpy()[:] = w.posm
+    inter = w.interactions
+
+    def step_device():
+        f.begin_step(binding.REUSE_LIST)
+        f.calc_force_all(src_dev, dst_dev)
+
+    def step_host():
+        f.begin_step(binding.REUSE_LIST)
+        f.calc_force_all(src_host, dst_host)
+
+    # ---- device-resident steps (value) + kernel-only time (roofline)
+    for _ in range(args.warmup):
+        step_device()
+    torch.cuda.synchronize()
+    c0 = f.get_counters()
+    replicas.barrier(world)
+    kernel_ms = []
+    with ClockSampler(local) as clocks:
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        torch.cuda.synchronize()
+        e0.record(f.streams[0])
+        for _ in range(args.steps):
+            step_device()
+            kernel_ms.append(f.last_dispatch_ms(0))
+        e1.record(f.streams[0])
+        torch.cuda.synchronize()
+        ms_dev = e0.elapsed_time(e1)
+        c1 = f.get_counters()
+        # keep the sampler alive long enough for at least a few samples under load
+        t_end = time.perf_counter() + max(0.0, 1.0 - ms_dev * 1e-3)
+        while time.perf_counter() < t_end:
+            step_device()
+    replicas.barrier(world)
+    launches = (c1["kernel_launches"] - c0["kernel_launches"])
+    units, ms_max = replicas.reduce_timing(inter * args.steps, ms_dev, world)
+    value = units / (ms_max * 1e-3)
+
+    # ---- end to end with host buffers
+    for _ in range(2):
+        step_host()
+    torch.cuda.synchronize()
+    replicas.barrier(world)
+    t0 = time.perf_counter()
+    for _ in range(args.steps):
+        step_host()
+    torch.cuda.synchronize()
+    ms_e2e = (time.perf_counter() - t0) * 1e3
+    units_e, ms_e_max = replicas.reduce_timing(inter * args.steps, ms_e2e, world)
+    e2e_value = units_e / (ms_e_max * 1e-3)
+
+    # ---- phases, for the record (not part of the contract)
+    phases = {}
+    ev = [torch.cuda.Event(enable_timing=True) for _ in range(5)]
+    s0 = f.streams[0]
+    f.begin_step(binding.REUSE_LIST)
+    ev[0].record(s0); f.set_particles(src_dev, 0, w.n, s0)
+    ev[1].record(s0); f.refresh_monopoles(s0)
+    ev[2].record(s0); f.dispatch(0, 0, w.n_group)
+    ev[3].record(s0); f.retrieve(0, dst_dev)
+    ev[4].record(s0); torch.cuda.synchronize()
+    for k, name in enumerate(("upload_d2d", "monopole_refresh", "force_kernel", "retrieve_d2d")):
+        phases[name + "_ms"] = round(ev[k].elapsed_time(ev[k + 1]), 4)
+
+    if rank == 0:
+        peaks = measured_peaks()
+        clk = clocks.summary()
+        sm_max_mhz = peaks.get("sm_max_mhz") or clk.get("sm_max_mhz") or 1965.0
+        n_sm = torch.cuda.get_device_properties(local).multi_processor_count
+        peak_tflops = n_sm * 128 * 2 * sm_max_mhz * 1e6 / 1e12
+        k_ms = float(np.mean(kernel_ms))
+        achieved = N_OP * inter / (k_ms * 1e-3) / 1e12
+        traffic = None
+        try:
+            traffic = json.load(open(os.path.join(ROOT, "profiles", "force_kernel_traffic.json"))).get(cfg.name)
+        except (OSError, ValueError):
+            pass
+        roof = {"bound": "alu", "kernel": "mwf::k_force", "achieved": achieved, "peak": peak_tflops, "unit": "TFLOP/s",
+                "frac": achieved / peak_tflops, "traffic": traffic, "kernel_ms": k_ms,
+                "peak_source": "SMs x 128 FMA/clk x 2 x max SM clock (%d x 256 x %.0f MHz; clock from %s)" % (
+                    n_sm, sm_max_mhz, "MEASURED_PEAKS.json" if peaks.get("sm_max_mhz") else "nvidia-smi"),
+                "flop_per_interaction": N_OP, "interactions_per_launch": inter}
+        if clk.get("sm_mhz"):
+            roof["frac_at_sustained_clock"] = achieved / (n_sm * 256 * clk["sm_mhz"] * 1e6 / 1e12)
+        log("[bench] oracle cpu_baseline ...")
+        ci, cdt, ck = oracle_sample(w, cfg, args.cpu_baseline_seconds)
+        import oracle
+        cpu = {"value": ci / cdt, "unit": UNIT, "cores": oracle.num_threads(), "kind": "oracle",
+               "sample": "%d of %d groups (seeded), %.3e interactions, forces only, %.1f s" % (ck, w.n_group, ci, cdt)}
+        out = {
+            "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
+            "ms_per_step": ms_max / args.steps, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+            "dtype": "f32", "data": "synthetic", "config": workload_config(cfg, w),
+            "gflops_at_23": value * N_OP / 1e9, "frac_fp32_peak_whole_step": value * N_OP / 1e12 / (peak_tflops * world),
+            "roofline": roof, "cpu_baseline": cpu,
+            "e2e": {"value": e2e_value, "unit": UNIT, "h2d_bytes_per_step": 16 * w.n, "d2h_bytes_per_step": 16 * w.n,
+                    "ms_per_step": ms_e_max / args.steps},
+            "gpu_launches": launches, "clocks": clk, "phases": phases,
+            "construction_step": {"host_tree_and_lists_s": round(t_build, 3), "upload_tree_and_lists_s": round(t_upload, 3)},
+            "context": {"paper_fraction_of_peak": 0.27, "paper_hardware": "TITAN V (P:673), whole step"},
+        }
+        print(json.dumps(out), flush=True)
+    f.close()
+    if world > 1:
+        import torch.distributed as dist
+        dist.destroy_process_group()
+    return 0
+
+
+if __name__ == "__main__":
+    sys.exit(main())

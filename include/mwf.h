@@ -1,0 +1,167 @@
+/* mwf.h -- C ABI of the B200-native index-based multi-walk force library (libmwf.so).
+ *
+ * The hot path of "Accelerated FDPS" (arXiv 1907.02290; "P:n" = line n of the paper text the build was
+ * written from, SURVEY.md section 8 is the scope contract):
+ *
+ *   (1) upload / update particles        P:107, P:181, P:391, P:466-474  "send all EPJ and SPJ once"
+ *   (2) upload tree cells + index lists  P:181, P:391, P:441-477, P:528-546  lists are INDICES, kept on the device
+ *   (3) refresh the monopoles            P:134-136, P:160  moments recomputed every step, also on reuse steps
+ *   (4) dispatch the force kernel        P:89 multiwalk, "dispatch", P:557-569 ForceKernelIndex
+ *   (5) retrieve acc and pot             P:189 "retrieve", P:595-663 RetrieveKernel
+ *   list reuse                           P:115-143, P:242 MAKE_LIST / MAKE_LIST_FOR_REUSE / REUSE_LIST
+ *
+ * Conventions common to every call
+ *   - Return value: 0 (MWF_OK) on success, a negative MWF_E* code otherwise (the paper's callbacks return 0,
+ *     P:352).  No exceptions, no abort, no exit.  mwf_strerror() gives a text;
+ *     mwf_last_cuda_error() the CUDA text behind the last MWF_ECUDA.
+ *   - "host" pointers are ordinary CPU memory (pinned memory makes the copies truly asynchronous);
+ *     "device" pointers are CUDA global memory on the ctx's device.  Each argument says which.
+ *   - Ownership: the caller owns every array it passes.  The library copies what it needs during the
+ *     call or on the given stream; host sources of asynchronous copies must stay valid until that stream
+ *     has been synchronised (mwf_retrieve() / mwf_sync() do).  All device storage of the library lives in
+ *     one arena: either caller-allocated (e.g. a torch tensor) and handed to mwf_create(), or allocated
+ *     by the library when arena == NULL.
+ *   - Streams are `cudaStream_t` handles passed as `void*` (NULL = the legacy default stream).
+ *     Cross-stream ordering (store updates -> refresh -> force kernels -> next store update) is enforced
+ *     inside the library with CUDA events; the caller never needs to synchronise between calls.
+ *   - Not thread-safe per ctx; distinct ctxs are independent.
+ *   - All particle-indexed arrays are in TREE (Morton) ORDER: particle p of group g is
+ *     grp_first[g] <= p < grp_first[g] + grp_n[g]; the i-particles ARE the stored j-particles (the
+ *     paper's own section 7.3 proposal), so there is no separate EPI upload.
+ */
+#ifndef MWF_H
+#define MWF_H
+
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct mwf_ctx mwf_ctx; /* opaque */
+
+/* EPJ / SPJ on the device: float4 (x, y, z, m), 16 B.  SPJ = monopole of a tree cell:
+ * centre of mass and total mass, same type and same array as EPJ. */
+typedef struct { float x, y, z, m; } mwf_posm;
+/* FORCE on the device: float4 (ax, ay, az, pot), 16 B. */
+typedef struct { float ax, ay, az, pot; } mwf_accp;
+/* Tree cell: particle range [first_ptcl, first_ptcl + n_ptcl) in tree order and child range
+ * [first_child, first_child + n_child) in the cell array (n_child == 0: leaf).  Cell 0 is the root and
+ * covers [0, N).  Children of a cell are stored contiguously, after their parent (level order),
+ * and their particle ranges partition the parent's range. */
+typedef struct { int32_t first_ptcl, n_ptcl, first_child, n_child; } mwf_cell;
+
+typedef struct {
+    float eps;          /* Plummer softening length, > 0 (eps^2 must be a normal float)      */
+    float G;            /* gravitational constant, applied to acc and pot                    */
+    int64_t max_ptcl;   /* capacity: particles                                               */
+    int64_t max_cell;   /* capacity: tree cells                                              */
+    int64_t max_group;  /* capacity: i-groups                                                */
+    int64_t max_entry;  /* capacity: total list entries, EPJ + SPJ summed over groups        */
+    int32_t n_tag;      /* number of dispatch tags (= internal streams), 1 .. MWF_MAX_TAG; paper uses 8 */
+    int32_t device;     /* CUDA device ordinal                                               */
+} mwf_params;
+
+#define MWF_MAX_TAG 16
+
+/* INTERACTION_LIST_MODE of the paper. */
+enum { MWF_MAKE_LIST = 0, MWF_MAKE_LIST_FOR_REUSE = 1, MWF_REUSE_LIST = 2 };
+
+enum {
+    MWF_OK = 0,
+    MWF_EINVAL = -1,  /* null pointer, negative size, eps <= 0, bad tag or mode                          */
+    MWF_ESTATE = -2,  /* call out of order: dispatch without lists / with stale monopoles, REUSE_LIST with
+                         no saved lists (MAKE_LIST does not keep them), retrieve of an idle tag   */
+    MWF_ERANGE = -3,  /* an index, range or offset in the uploaded tree / lists is out of bounds or not
+                         monotone (found by the one-time device validation)                               */
+    MWF_ENOMEM = -4,  /* exceeds a max_* capacity or the arena is too small                              */
+    MWF_ECUDA = -5    /* a CUDA call failed; sticky text via mwf_last_cuda_error()                       */
+};
+
+/* Bytes of device memory a ctx with these capacities needs (write to *bytes). */
+int mwf_arena_bytes(const mwf_params* p, int64_t* bytes);
+
+/* Create a ctx.  arena: DEVICE pointer to at least mwf_arena_bytes() bytes, 256-B aligned, owned by the
+ * caller and kept alive until mwf_destroy(); or NULL to let the library cudaMalloc it. */
+int mwf_create(mwf_ctx** out, const mwf_params* p, void* arena, int64_t arena_bytes);
+int mwf_destroy(mwf_ctx* c);
+
+/* Bind the caller's stream (e.g. a torch.cuda.Stream) to a tag instead of the internal one. */
+int mwf_set_tag_stream(mwf_ctx* c, int32_t tag, void* cuda_stream);
+
+/* (1) Upload or update particles [first, first + n) of the store, tree order (P:466-474 H2dJptcl).
+ * src: n records, HOST if src_on_device == 0 else DEVICE.  Asynchronous on `stream`.  Marks the
+ * monopoles stale: mwf_refresh_monopoles() must follow before the next dispatch. */
+int mwf_set_particles(mwf_ctx* c, const mwf_posm* src, int64_t first, int64_t n, int src_on_device, void* stream);
+
+/* Read back particles [first, first + n) of the store (test / integration hook). dst HOST or DEVICE. Blocking. */
+int mwf_get_particles(mwf_ctx* c, mwf_posm* dst, int64_t first, int64_t n, int dst_on_device);
+
+/* (2a) Upload the tree topology (construction step only).  cells: n_cell records, HOST.
+ * Defines N = cells[0].n_ptcl.  Validated on the device (MWF_ERANGE).  Blocking. */
+int mwf_set_tree(mwf_ctx* c, const mwf_cell* cells, int64_t n_cell, void* stream);
+
+/* (2b) Upload the i-groups and their interaction lists as two CSR index lists (construction step only;
+ * EPJ indices then SPJ indices: kept on the device).  All arrays HOST.
+ *   grp_first[g], grp_n[g]   i-range of group g (any n_i >= 1); groups must be disjoint
+ *   epj_off[n_group + 1], epj_id[]   particle indices in [0, N)
+ *   spj_off[n_group + 1], spj_id[]   cell indices in [0, n_cell)
+ * A group's EPJ list must contain either all of the group's own particles (what a Barnes walk yields;
+ * their self terms are excluded) or none of them; anything else is MWF_EINVAL.
+ * mode: MWF_MAKE_LIST (lists valid for one evaluation, dropped once every dispatched tag has been
+ * retrieved) or MWF_MAKE_LIST_FOR_REUSE (kept until the next mwf_set_lists / mwf_set_tree).
+ * Requires mwf_set_tree() first.  Validates on the device, re-encodes into one padded merged list per
+ * group and builds the work schedule.  Blocking. */
+int mwf_set_lists(mwf_ctx* c, int64_t n_group, const int32_t* grp_first, const int32_t* grp_n,
+                  const int64_t* epj_off, const int32_t* epj_id, const int64_t* spj_off, const int32_t* spj_id,
+                  int mode, void* stream);
+
+/* Declare the kind of step that follows.  MWF_REUSE_LIST: MWF_ESTATE unless lists saved with
+ * MWF_MAKE_LIST_FOR_REUSE are present.  MWF_MAKE_LIST*: drops any saved lists; mwf_set_tree() and
+ * mwf_set_lists() must follow. */
+int mwf_begin_step(mwf_ctx* c, int mode);
+
+/* (3) Recompute the monopole (total mass, centre of mass) of every tree cell from the current particle
+ * store, bottom-up over the fixed tree, on the device, and write them as SPJ entries behind the
+ * particles.  Asynchronous on `stream`. */
+int mwf_refresh_monopoles(mwf_ctx* c, void* stream);
+
+/* (4) Launch the force kernel over groups [g_begin, g_end) on the stream of `tag`; non-blocking.
+ * For every particle i of those groups, over the group's list (reading S1-S5 of DESIGN.md):
+ *   acc_i =  G sum_k m_k (x_k - x_i) / (|x_k - x_i|^2 + eps^2)^(3/2)
+ *   pot_i = -G sum_k m_k / (|x_k - x_i|^2 + eps^2)^(1/2)        (k != i by index) */
+int mwf_dispatch(mwf_ctx* c, int32_t tag, int64_t g_begin, int64_t g_end);
+
+/* (5) Copy acc+pot of the particles of every group dispatched under `tag` since its last retrieve into
+ * dst and wait for it.  dst: base of an N-record array indexed by tree-order particle
+ * position, HOST or DEVICE; records of other particles are not touched. */
+int mwf_retrieve(mwf_ctx* c, int32_t tag, mwf_accp* dst, int dst_on_device);
+
+/* One whole evaluation, the analogue of calcForceAllAndWriteBackMultiWalkIndex for a step
+ * whose tree and lists are already on the device: upload all N particles (src HOST or DEVICE; NULL = keep
+ * the store), refresh, dispatch all groups split over the tags, retrieve everything into dst. */
+int mwf_calc_force_all(mwf_ctx* c, const mwf_posm* src, int src_on_device, mwf_accp* dst, int dst_on_device);
+
+/* Test hooks: monopoles as stored (float4 per cell) and device-side results without a copy. */
+int mwf_get_monopoles(mwf_ctx* c, mwf_posm* dst, int dst_on_device);
+/* DEVICE pointers into the arena: store (N particles then n_cell SPJ) and result array. */
+int mwf_device_pointers(mwf_ctx* c, mwf_posm** store, mwf_accp** accp);
+
+/* Wait for everything the ctx has enqueued. */
+int mwf_sync(mwf_ctx* c);
+
+/* Counters since creation: kernels launched by the library, interactions dispatched (sum n_i * n_list,
+ * padding excluded), entries resident in the merged list (padding included). */
+int mwf_get_counters(mwf_ctx* c, int64_t* kernel_launches, int64_t* interactions, int64_t* padded_entries);
+
+/* Timing hook: CUDA-event time in ms of the force kernels of the last mwf_dispatch on `tag`
+ * (valid after that tag's stream was synchronised). */
+int mwf_last_dispatch_ms(mwf_ctx* c, int32_t tag, float* ms);
+
+const char* mwf_strerror(int code);
+const char* mwf_last_cuda_error(mwf_ctx* c);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* MWF_H */

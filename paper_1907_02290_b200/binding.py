@@ -1,0 +1,232 @@
+"""Thin Python binding of the C-ABI CUDA library (include/mwf.h, csrc/libmwf.so).
+
+Argument marshalling only: every step of the path runs in the library's kernels.  PyTorch supplies the
+device arena, the streams and pinned host buffers; the calls carry the names of the C entry points
+without the `mwf_` prefix.  There is no CPU fallback: a missing library or a non-CUDA environment raises.
+"""
+from __future__ import annotations
+
+import ctypes
+import os
+
+import numpy as np
+
+from . import build as _build
+
+MAKE_LIST, MAKE_LIST_FOR_REUSE, REUSE_LIST = 0, 1, 2
+OK, EINVAL, ESTATE, ERANGE, ENOMEM, ECUDA = 0, -1, -2, -3, -4, -5
+MAX_TAG = 16
+
+# every symbol include/mwf.h declares (tests check that the library exports exactly these)
+SYMBOLS = (
+    "mwf_arena_bytes", "mwf_create", "mwf_destroy", "mwf_set_tag_stream", "mwf_set_particles", "mwf_get_particles",
+    "mwf_set_tree", "mwf_set_lists", "mwf_begin_step", "mwf_refresh_monopoles", "mwf_dispatch", "mwf_retrieve",
+    "mwf_calc_force_all", "mwf_get_monopoles", "mwf_device_pointers", "mwf_sync", "mwf_get_counters",
+    "mwf_last_dispatch_ms", "mwf_strerror", "mwf_last_cuda_error",
+)
+
+
+class Params(ctypes.Structure):
+    _fields_ = [("eps", ctypes.c_float), ("G", ctypes.c_float), ("max_ptcl", ctypes.c_int64), ("max_cell", ctypes.c_int64),
+                ("max_group", ctypes.c_int64), ("max_entry", ctypes.c_int64), ("n_tag", ctypes.c_int32), ("device", ctypes.c_int32)]
+
+
+class MwfError(RuntimeError):
+    def __init__(self, code: int, text: str):
+        super().__init__("mwf error %d: %s" % (code, text))
+        self.code = code
+
+
+_lib = None
+
+
+def load_library(path: str | None = None) -> ctypes.CDLL:
+    """dlopen csrc/libmwf.so (built in-tree by `build.build_mwf`) and declare the signatures."""
+    global _lib
+    if _lib is not None and path is None:
+        return _lib
+    if path is None:
+        path = os.path.join(os.path.dirname(os.path.abspath(__file__)), "csrc", "libmwf.so")
+        if not os.path.exists(path):
+            path = _build.build_mwf()
+    lib = ctypes.CDLL(path)
+    vp, i64, i32, ci = ctypes.c_void_p, ctypes.c_int64, ctypes.c_int32, ctypes.c_int
+    P = ctypes.POINTER
+    sig = {
+        "mwf_arena_bytes": [P(Params), P(i64)],
+        "mwf_create": [P(vp), P(Params), vp, i64],
+        "mwf_destroy": [vp],
+        "mwf_set_tag_stream": [vp, i32, vp],
+        "mwf_set_particles": [vp, vp, i64, i64, ci, vp],
+        "mwf_get_particles": [vp, vp, i64, i64, ci],
+        "mwf_set_tree": [vp, vp, i64, vp],
+        "mwf_set_lists": [vp, i64, vp, vp, vp, vp, vp, vp, ci, vp],
+        "mwf_begin_step": [vp, ci],
+        "mwf_refresh_monopoles": [vp, vp],
+        "mwf_dispatch": [vp, i32, i64, i64],
+        "mwf_retrieve": [vp, i32, vp, ci],
+        "mwf_calc_force_all": [vp, vp, ci, vp, ci],
+        "mwf_get_monopoles": [vp, vp, ci],
+        "mwf_device_pointers": [vp, P(vp), P(vp)],
+        "mwf_sync": [vp],
+        "mwf_get_counters": [vp, P(i64), P(i64), P(i64)],
+        "mwf_last_dispatch_ms": [vp, i32, P(ctypes.c_float)],
+    }
+    for name, args in sig.items():
+        fn = getattr(lib, name)
+        fn.argtypes = args
+        fn.restype = ci
+    lib.mwf_strerror.argtypes = [ci]
+    lib.mwf_strerror.restype = ctypes.c_char_p
+    lib.mwf_last_cuda_error.argtypes = [vp]
+    lib.mwf_last_cuda_error.restype = ctypes.c_char_p
+    _lib = lib
+    return lib
+
+
+def _host_ptr(a: np.ndarray, dtype, what: str):
+    if not isinstance(a, np.ndarray) or a.dtype != dtype or not a.flags.c_contiguous:
+        raise TypeError("%s must be a C-contiguous numpy array of %s" % (what, np.dtype(dtype)))
+    return ctypes.c_void_p(a.ctypes.data)
+
+
+def _ptr(x, dtype, what: str):
+    """(pointer, on_device) of a numpy array, a torch CPU tensor (e.g. pinned) or a torch CUDA tensor."""
+    import torch
+    if isinstance(x, np.ndarray):
+        return _host_ptr(x, dtype, what), 0
+    if isinstance(x, torch.Tensor):
+        if not x.is_contiguous() or x.dtype != torch.float32:
+            raise TypeError("%s must be a contiguous float32 tensor" % what)
+        return ctypes.c_void_p(x.data_ptr()), 1 if x.is_cuda else 0
+    raise TypeError("%s: unsupported buffer type %r" % (what, type(x)))
+
+
+def _stream_handle(stream) -> ctypes.c_void_p:
+    if stream is None:
+        import torch
+        stream = torch.cuda.current_stream()
+    return ctypes.c_void_p(int(stream.cuda_stream))
+
+
+class MultiWalkForce:
+    """One mwf_ctx.  Device memory is one torch uint8 arena; tags run on torch streams."""
+
+    def __init__(self, eps: float, G: float = 1.0, *, max_ptcl: int, max_cell: int, max_group: int, max_entry: int,
+                 n_tag: int = 8, device: int = 0):
+        import torch
+        if not torch.cuda.is_available():
+            raise RuntimeError("MultiWalkForce needs a CUDA device (sm_100a); there is no CPU path")
+        self._lib = load_library()
+        self._torch = torch
+        self.device = torch.device("cuda", device)
+        self.params = Params(float(eps), float(G), int(max_ptcl), int(max_cell), int(max_group), int(max_entry), int(n_tag), int(device))
+        nbytes = ctypes.c_int64(0)
+        self._ck(self._lib.mwf_arena_bytes(ctypes.byref(self.params), ctypes.byref(nbytes)), ctx=False)
+        self.arena_bytes = nbytes.value
+        with torch.cuda.device(self.device):
+            self._arena = torch.empty(self.arena_bytes + 256, dtype=torch.uint8, device=self.device)
+            base = (self._arena.data_ptr() + 255) // 256 * 256
+            self._h = ctypes.c_void_p(None)
+            self._ck(self._lib.mwf_create(ctypes.byref(self._h), ctypes.byref(self.params), ctypes.c_void_p(base), self.arena_bytes), ctx=False)
+            self.streams = [torch.cuda.Stream(device=self.device) for _ in range(n_tag)]
+        for t, s in enumerate(self.streams):
+            self._ck(self._lib.mwf_set_tag_stream(self._h, t, ctypes.c_void_p(int(s.cuda_stream))))
+        self.n_tag = n_tag
+
+    @classmethod
+    def for_workload(cls, w, eps: float | None = None, G: float = 1.0, n_tag: int = 8, device: int = 0):
+        return cls(w.cfg.eps if eps is None else eps, G, max_ptcl=w.n, max_cell=w.n_cell, max_group=w.n_group,
+                   max_entry=max(1, w.n_entry), n_tag=n_tag, device=device)
+
+    # -- error handling
+    def _ck(self, rc: int, ctx: bool = True):
+        if rc != 0:
+            text = self._lib.mwf_strerror(rc).decode()
+            if rc == ECUDA and ctx and self._h:
+                text += " (" + self._lib.mwf_last_cuda_error(self._h).decode() + ")"
+            raise MwfError(rc, text)
+
+    def close(self):
+        if getattr(self, "_h", None):
+            self._lib.mwf_destroy(self._h)
+            self._h = None
+            self._arena = None
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass
+
+    # -- the C entry points, same names
+    def set_particles(self, src, first: int = 0, n: int | None = None, stream=None):
+        p, on_dev = _ptr(src, np.float32, "src")
+        if n is None:
+            n = int(src.shape[0])
+        self._ck(self._lib.mwf_set_particles(self._h, p, int(first), int(n), on_dev, _stream_handle(stream)))
+
+    def get_particles(self, first: int, n: int) -> np.ndarray:
+        out = np.empty((n, 4), np.float32)
+        self._ck(self._lib.mwf_get_particles(self._h, _host_ptr(out, np.float32, "dst"), int(first), int(n), 0))
+        return out
+
+    def set_tree(self, cells: np.ndarray, stream=None):
+        self._ck(self._lib.mwf_set_tree(self._h, _host_ptr(cells, np.int32, "cells"), int(cells.shape[0]), _stream_handle(stream)))
+
+    def set_lists(self, grp_first, grp_n, epj_off, epj_id, spj_off, spj_id, mode: int = MAKE_LIST_FOR_REUSE, stream=None):
+        self._ck(self._lib.mwf_set_lists(
+            self._h, int(grp_first.shape[0]), _host_ptr(grp_first, np.int32, "grp_first"), _host_ptr(grp_n, np.int32, "grp_n"),
+            _host_ptr(epj_off, np.int64, "epj_off"), _host_ptr(epj_id, np.int32, "epj_id"),
+            _host_ptr(spj_off, np.int64, "spj_off"), _host_ptr(spj_id, np.int32, "spj_id"), int(mode), _stream_handle(stream)))
+
+    def begin_step(self, mode: int):
+        self._ck(self._lib.mwf_begin_step(self._h, int(mode)))
+
+    def refresh_monopoles(self, stream=None):
+        self._ck(self._lib.mwf_refresh_monopoles(self._h, _stream_handle(stream)))
+
+    def dispatch(self, tag: int, g_begin: int, g_end: int):
+        self._ck(self._lib.mwf_dispatch(self._h, int(tag), int(g_begin), int(g_end)))
+
+    def retrieve(self, tag: int, dst):
+        p, on_dev = _ptr(dst, np.float32, "dst")
+        self._ck(self._lib.mwf_retrieve(self._h, int(tag), p, on_dev))
+
+    def calc_force_all(self, src, dst):
+        if src is None:
+            sp, s_dev = ctypes.c_void_p(None), 0
+        else:
+            sp, s_dev = _ptr(src, np.float32, "src")
+        dp, d_dev = _ptr(dst, np.float32, "dst")
+        self._ck(self._lib.mwf_calc_force_all(self._h, sp, s_dev, dp, d_dev))
+
+    def get_monopoles(self, n_cell: int) -> np.ndarray:
+        out = np.empty((n_cell, 4), np.float32)
+        self._ck(self._lib.mwf_get_monopoles(self._h, _host_ptr(out, np.float32, "dst"), 0))
+        return out
+
+    def sync(self):
+        self._ck(self._lib.mwf_sync(self._h))
+
+    def get_counters(self):
+        a, b, c = ctypes.c_int64(0), ctypes.c_int64(0), ctypes.c_int64(0)
+        self._ck(self._lib.mwf_get_counters(self._h, ctypes.byref(a), ctypes.byref(b), ctypes.byref(c)))
+        return dict(kernel_launches=a.value, interactions=b.value, padded_entries=c.value)
+
+    def last_dispatch_ms(self, tag: int) -> float:
+        ms = ctypes.c_float(0)
+        self._ck(self._lib.mwf_last_dispatch_ms(self._h, int(tag), ctypes.byref(ms)))
+        return float(ms.value)
+
+    # -- marshalling helpers (no arithmetic)
+    def upload_workload(self, w, mode: int = MAKE_LIST_FOR_REUSE, stream=None):
+        """Construction step: particles, tree and lists of a `workload.Workload`."""
+        self.begin_step(mode)
+        self.set_particles(w.posm, 0, w.n, stream)
+        self.set_tree(w.cells, stream)
+        self.set_lists(w.grp_first, w.grp_n, w.epj_off, w.epj_id, w.spj_off, w.spj_id, mode, stream)
+
+    def pinned(self, n: int):
+        """Pinned host float32 [n,4] buffer (for truly asynchronous uploads / retrieves)."""
+        return self._torch.empty((n, 4), dtype=self._torch.float32, pin_memory=True)

@@ -1,0 +1,192 @@
+// Index-based multi-walk force kernel for sm_100a (paper: ForceKernelIndex,
+// P:557-569; multiwalk P:89; indirect addressing P:107).
+//
+// Mapping:
+//   * work item = up to 64 consecutive i-particles of one group x the group's whole merged list; one WARP
+//     owns an item from start to end, so there is no block-level barrier and no atomics on the results.
+//   * the warp streams the list in tiles of 64 entries: each lane reads two 4-byte indices (one coalesced
+//     256-B request per warp), gathers the two float4 (x,y,z,m) records through them and writes them to a
+//     warp-private shared-memory tile in PAIR layout [x0 x1 y0 y1][z0 z1 m0 m1]; the gathers of tile t+1
+//     and the indices of tile t+2 are in flight while tile t is swept.
+//   * every lane then sweeps the tile with broadcast LDS.128 and packed FP32 math (FADD2 / FMUL2 / FFMA2 of
+//     sm_100: two j per instruction), 13 packed FP32 ops + 2 MUFU.RSQ per i per j-pair.
+//   * lane utilisation: 64 i per item = 2 per lane; remainders of <= 32 / 16 / 8 particles run 1 per lane
+//     with the warp split into 1 / 2 / 4 j-slices whose partial sums are combined by warp shuffles.
+//   * accumulation is two-level (per-tile partial sums added into running totals, two independent sums
+//     per component from the j-pairing), which keeps the fp32 summation error far inside the tolerance.
+//   * the self term (an i-particle meets itself in its own EPJ list) contributes exactly 0 to acc and
+//     m_i * rsqrt(eps^2) to the potential sum; the same value is subtracted up front (reading S2).
+#include "mwf_internal.h"
+
+namespace mwf {
+
+__device__ __forceinline__ float rsqrt_approx(float x) {
+    float r;
+    asm("rsqrt.approx.ftz.f32 %0, %1;" : "=f"(r) : "f"(x));
+    return r;
+}
+
+__device__ __forceinline__ int2 ld_stream_int2(const int2* p) {
+    int2 v;
+    asm volatile("ld.global.nc.L1::no_allocate.v2.s32 {%0, %1}, [%2];" : "=r"(v.x), "=r"(v.y) : "l"(p));
+    return v;
+}
+
+// Sweep one staged tile.  NI i-particles per lane; the lane belongs to slice `sl` of S and takes pairs
+// sl, sl + S, ...  Accumulates into the per-tile sums t* (two partial sums per component).
+template <int NI, int S>
+__device__ __forceinline__ void sweep_tile(const float4* __restrict__ sA, const float4* __restrict__ sB, int sl,
+                                           const float (&nx)[NI], const float (&ny)[NI], const float (&nz)[NI], float eps2,
+                                           float2 (&tx)[NI], float2 (&ty)[NI], float2 (&tz)[NI], float2 (&tp)[NI]) {
+    const float2 e2 = make_float2(eps2, eps2);
+#pragma unroll 8
+    for (int pp = 0; pp < (TILE_J / 2) / S; ++pp) {
+        const int p = pp * S + sl;
+        const float4 A = sA[p];
+        const float4 B = sB[p];
+        const float2 jx = make_float2(A.x, A.y), jy = make_float2(A.z, A.w);
+        const float2 jz = make_float2(B.x, B.y), jm = make_float2(B.z, B.w);
+#pragma unroll
+        for (int k = 0; k < NI; ++k) {
+            const float2 dx = __fadd2_rn(jx, make_float2(nx[k], nx[k]));
+            const float2 dy = __fadd2_rn(jy, make_float2(ny[k], ny[k]));
+            const float2 dz = __fadd2_rn(jz, make_float2(nz[k], nz[k]));
+            float2 r2 = __ffma2_rn(dx, dx, e2);
+            r2 = __ffma2_rn(dy, dy, r2);
+            r2 = __ffma2_rn(dz, dz, r2);
+            float2 ri;
+            ri.x = rsqrt_approx(r2.x);
+            ri.y = rsqrt_approx(r2.y);
+            const float2 mr = __fmul2_rn(jm, ri);
+            tp[k] = __fadd2_rn(tp[k], mr);
+            const float2 ri2 = __fmul2_rn(ri, ri);
+            const float2 mr3 = __fmul2_rn(mr, ri2);
+            tx[k] = __ffma2_rn(mr3, dx, tx[k]);
+            ty[k] = __ffma2_rn(mr3, dy, ty[k]);
+            tz[k] = __ffma2_rn(mr3, dz, tz[k]);
+        }
+    }
+}
+
+template <int NI, int S>
+__device__ __forceinline__ void run_item(const ForceArgs& a, const WorkItem it, float4* __restrict__ sbuf, int lane) {
+    constexpr int W = 32 / S;
+    const int sl = lane / W;
+    const int il = lane % W;
+    const float4* __restrict__ J = a.store;
+
+    float nx[NI], ny[NI], nz[NI], mi[NI];
+    bool valid[NI];
+#pragma unroll
+    for (int k = 0; k < NI; ++k) {
+        const int off = il + 32 * k;
+        valid[k] = off < it.n_i;
+        const float4 p = __ldg(J + it.i_first + (valid[k] ? off : 0));
+        nx[k] = -p.x; ny[k] = -p.y; nz[k] = -p.z; mi[k] = p.w;
+    }
+    const float self_rinv = rsqrt_approx(a.eps2);  // what the sweep computes for d = 0
+    const bool self_in = a.grp_self[it.group] != 0;
+
+    float2 ax[NI], ay[NI], az[NI], ap[NI];
+#pragma unroll
+    for (int k = 0; k < NI; ++k) {
+        ax[k] = ay[k] = az[k] = make_float2(0.f, 0.f);
+        // start the potential sum at minus the self term (slice 0 only: the slices are added later)
+        ap[k] = make_float2((self_in && sl == 0) ? -mi[k] * self_rinv : 0.f, 0.f);
+    }
+
+    const int64_t l0 = a.list_off[it.group];
+    const int n_tiles = (int)((a.list_off[it.group + 1] - l0) / TILE_J);
+    const int2* __restrict__ lst = reinterpret_cast<const int2*>(a.list + l0);
+
+    int2 id = make_int2(0, 0), idn = make_int2(0, 0);
+    float4 j0 = make_float4(0.f, 0.f, 0.f, 0.f), j1 = j0;
+    if (n_tiles > 0) {
+        id = ld_stream_int2(lst + lane);
+        j0 = __ldg(J + id.x);
+        j1 = __ldg(J + id.y);
+        if (n_tiles > 1) idn = ld_stream_int2(lst + 32 + lane);
+    }
+    for (int t = 0; t < n_tiles; ++t) {
+        float4* sA = sbuf + (t & 1) * TILE_J;
+        float4* sB = sA + TILE_J / 2;
+        sA[lane] = make_float4(j0.x, j1.x, j0.y, j1.y);
+        sB[lane] = make_float4(j0.z, j1.z, j0.w, j1.w);
+        __syncwarp();
+        if (t + 1 < n_tiles) {
+            j0 = __ldg(J + idn.x);
+            j1 = __ldg(J + idn.y);
+            if (t + 2 < n_tiles) idn = ld_stream_int2(lst + (int64_t)(t + 2) * 32 + lane);
+        }
+        float2 tx[NI], ty[NI], tz[NI], tp[NI];
+#pragma unroll
+        for (int k = 0; k < NI; ++k) tx[k] = ty[k] = tz[k] = tp[k] = make_float2(0.f, 0.f);
+        sweep_tile<NI, S>(sA, sB, sl, nx, ny, nz, a.eps2, tx, ty, tz, tp);
+#pragma unroll
+        for (int k = 0; k < NI; ++k) {
+            ax[k] = __fadd2_rn(ax[k], tx[k]);
+            ay[k] = __fadd2_rn(ay[k], ty[k]);
+            az[k] = __fadd2_rn(az[k], tz[k]);
+            ap[k] = __fadd2_rn(ap[k], tp[k]);
+        }
+    }
+#pragma unroll
+    for (int k = 0; k < NI; ++k) {
+        float rx = ax[k].x + ax[k].y, ry = ay[k].x + ay[k].y, rz = az[k].x + az[k].y, rp = ap[k].x + ap[k].y;
+        if (S >= 4) {
+            rx += __shfl_xor_sync(0xffffffffu, rx, 8);
+            ry += __shfl_xor_sync(0xffffffffu, ry, 8);
+            rz += __shfl_xor_sync(0xffffffffu, rz, 8);
+            rp += __shfl_xor_sync(0xffffffffu, rp, 8);
+        }
+        if (S >= 2) {
+            rx += __shfl_xor_sync(0xffffffffu, rx, 16);
+            ry += __shfl_xor_sync(0xffffffffu, ry, 16);
+            rz += __shfl_xor_sync(0xffffffffu, rz, 16);
+            rp += __shfl_xor_sync(0xffffffffu, rp, 16);
+        }
+        if (valid[k] && sl == 0)
+            a.accp[it.i_first + il + 32 * k] = make_float4(a.G * rx, a.G * ry, a.G * rz, -a.G * rp);
+    }
+    __syncwarp();  // the next item reuses the warp's tile buffers
+}
+
+__global__ void __launch_bounds__(WARPS_PER_CTA * 32, 2) k_force(const ForceArgs a) {
+    __shared__ float4 s_tiles[WARPS_PER_CTA][2 * TILE_J];
+    const int lane = threadIdx.x & 31;
+    const int warp = threadIdx.x >> 5;
+    float4* sbuf = s_tiles[warp];
+    int64_t w = (int64_t)blockIdx.x * WARPS_PER_CTA + warp;  // first item: static
+    const int64_t n_warps = (int64_t)gridDim.x * WARPS_PER_CTA;
+    while (w < a.n_items) {
+        const int64_t pos = a.item_begin + w;
+        const WorkItem it = a.items[a.order ? a.order[pos] : pos];
+        switch (it.kind) {
+            case 0: run_item<2, 1>(a, it, sbuf, lane); break;
+            case 1: run_item<1, 1>(a, it, sbuf, lane); break;
+            case 2: run_item<1, 2>(a, it, sbuf, lane); break;
+            default: run_item<1, 4>(a, it, sbuf, lane); break;
+        }
+        if (a.counter) {  // dynamic: next unclaimed item
+            unsigned int nxt = 0;
+            if (lane == 0) nxt = atomicAdd(a.counter, 1u);
+            w = n_warps + (int64_t)__shfl_sync(0xffffffffu, nxt, 0);
+        } else {
+            w += n_warps;
+        }
+    }
+}
+
+cudaError_t launch_force(const ForceArgs& a, int grid, cudaStream_t s) {
+    if (a.n_items <= 0 || grid <= 0) return cudaSuccess;
+    k_force<<<grid, WARPS_PER_CTA * 32, 0, s>>>(a);
+    return cudaGetLastError();
+}
+
+int force_max_ctas_per_sm() {
+    int n = 0;
+    if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&n, k_force, WARPS_PER_CTA * 32, 0) != cudaSuccess) return 0;
+    return n;
+}
+
+}  // namespace mwf

@@ -1,0 +1,621 @@
+// Host side of libmwf.so: the C ABI of include/mwf.h -- device store, list-reuse driver (SURVEY.md
+// section 8(a) rows a1, a2, a5, a6, a7) and the launches of the kernels in this directory.
+#include <algorithm>
+#include <cstdio>
+#include <cstring>
+#include <new>
+#include <numeric>
+
+#include "mwf_internal.h"
+
+using namespace mwf;
+
+struct mwf_ctx {
+    mwf_params p{};
+    int n_sm = 0, ctas_per_sm = 0;
+    char* arena = nullptr;
+    int64_t arena_bytes = 0;
+    bool own_arena = false;
+    // carved device arrays
+    float4* store = nullptr;      // [max_ptcl + max_cell + 1]
+    float4* accp = nullptr;       // [max_ptcl]
+    mwf_cell* cells = nullptr;    // [max_cell]
+    int32_t* parent = nullptr;    // [max_cell]
+    int32_t* arrive = nullptr;    // [max_cell]
+    double4* mom64 = nullptr;     // [max_cell]
+    int32_t* grp_first = nullptr; // [max_group]
+    int32_t* grp_n = nullptr;     // [max_group]
+    uint8_t* grp_self = nullptr;  // [max_group]
+    int64_t* list_off = nullptr;  // [max_group + 1]
+    int64_t* st_epj_off = nullptr, *st_spj_off = nullptr;  // [max_group + 1] staging
+    int32_t* st_ids = nullptr;    // [max_entry] staging of the uploaded ids
+    int32_t* list = nullptr;      // [max_entry + TILE_J * max_group] merged, padded
+    WorkItem* items = nullptr;    // [max_items]
+    int32_t* order_full = nullptr, *order_split = nullptr;  // [max_items]
+    unsigned int* counters = nullptr;  // [N_COUNTER]
+    unsigned int* err = nullptr;
+    int64_t max_items = 0;
+    // state
+    int64_t n_ptcl = 0, n_cell = 0, n_group = 0, n_items = 0, ptcl_hi = 0, padded_entries = 0;
+    bool have_tree = false, have_lists = false, lists_for_reuse = false, mono_fresh = false;
+    std::vector<int64_t> h_item_off, h_inter, h_split;  // per group prefix of items / interactions; split group bounds
+    std::vector<int32_t> h_grp_first, h_grp_n;
+    int64_t groups_outstanding = 0;  // MAKE_LIST: groups dispatched and not yet retrieved
+    int64_t groups_dispatched = 0;
+    // streams and events
+    cudaStream_t tag_stream[MWF_MAX_TAG]{};
+    bool tag_own[MWF_MAX_TAG]{};
+    bool tag_inflight[MWF_MAX_TAG]{};
+    cudaEvent_t ev_tag[MWF_MAX_TAG]{}, ev_k0[MWF_MAX_TAG]{}, ev_k1[MWF_MAX_TAG]{};
+    bool tag_timed[MWF_MAX_TAG]{};
+    cudaEvent_t ev_store{};
+    bool store_event_valid = false;
+    std::vector<std::pair<int64_t, int64_t>> tag_ranges[MWF_MAX_TAG];  // particle ranges awaiting retrieve
+    std::vector<int64_t> tag_groups;                                   // groups awaiting retrieve per tag
+    uint32_t counter_seq = 0;
+    int64_t n_launch = 0, n_inter = 0;
+    std::string cuda_err;
+};
+
+namespace {
+
+constexpr int N_COUNTER = 1024;
+
+int cuda_fail(mwf_ctx* c, cudaError_t e, const char* what) {
+    if (c) {
+        char buf[256];
+        snprintf(buf, sizeof buf, "%s: %s", what, cudaGetErrorString(e));
+        c->cuda_err = buf;
+    }
+    return MWF_ECUDA;
+}
+#define CU(c, call)                                                   \
+    do {                                                              \
+        cudaError_t e__ = (call);                                     \
+        if (e__ != cudaSuccess) return cuda_fail((c), e__, #call);    \
+    } while (0)
+
+inline int64_t up(int64_t x, int64_t a) { return (x + a - 1) / a * a; }
+
+struct Layout {
+    int64_t off[32];
+    int n = 0;
+    int64_t total = 0;
+    int64_t add(int64_t bytes) {
+        off[n] = total;
+        total += up(bytes, 256);
+        return off[n++];
+    }
+};
+
+int64_t max_items_of(const mwf_params& p) { return p.max_ptcl / CHUNK_I + 2 * p.max_group + 8; }
+
+Layout make_layout(const mwf_params& p) {
+    Layout L;
+    const int64_t mi = max_items_of(p);
+    L.add((p.max_ptcl + p.max_cell + 1) * 16);          // 0 store
+    L.add(p.max_ptcl * 16);                             // 1 accp
+    L.add(p.max_cell * 16);                             // 2 cells
+    L.add(p.max_cell * 4);                              // 3 parent
+    L.add(p.max_cell * 4);                              // 4 arrive
+    L.add(p.max_cell * 32);                             // 5 mom64
+    L.add(p.max_group * 4);                             // 6 grp_first
+    L.add(p.max_group * 4);                             // 7 grp_n
+    L.add(p.max_group);                                 // 8 grp_self
+    L.add((p.max_group + 1) * 8);                       // 9 list_off
+    L.add((p.max_group + 1) * 8);                       // 10 st_epj_off
+    L.add((p.max_group + 1) * 8);                       // 11 st_spj_off
+    L.add(p.max_entry * 4);                             // 12 st_ids
+    L.add((p.max_entry + TILE_J * p.max_group) * 4);    // 13 list
+    L.add(mi * (int64_t)sizeof(WorkItem));              // 14 items
+    L.add(mi * 4);                                      // 15 order_full
+    L.add(mi * 4);                                      // 16 order_split
+    L.add(N_COUNTER * 4);                               // 17 counters
+    L.add(256);                                         // 18 err
+    return L;
+}
+
+bool params_ok(const mwf_params* p) {
+    if (!p) return false;
+    if (!(p->eps > 0.f) || !(p->eps * p->eps >= 1.17549435e-38f)) return false;
+    if (!(p->G == p->G)) return false;
+    if (p->max_ptcl < 1 || p->max_cell < 1 || p->max_group < 1 || p->max_entry < 1) return false;
+    if (p->max_ptcl + p->max_cell + 1 > 0x7fffffffLL) return false;  // 32-bit list indices
+    if (p->n_tag < 1 || p->n_tag > MWF_MAX_TAG) return false;
+    if (p->device < 0) return false;
+    return true;
+}
+
+// Every operation that writes the store / tree / lists first waits for the force kernels that read them.
+int before_store_op(mwf_ctx* c, cudaStream_t s) {
+    for (int t = 0; t < c->p.n_tag; ++t)
+        if (c->tag_inflight[t]) CU(c, cudaStreamWaitEvent(s, c->ev_tag[t], 0));
+    if (c->store_event_valid) CU(c, cudaStreamWaitEvent(s, c->ev_store, 0));
+    return MWF_OK;
+}
+int after_store_op(mwf_ctx* c, cudaStream_t s) {
+    CU(c, cudaEventRecord(c->ev_store, s));
+    c->store_event_valid = true;
+    return MWF_OK;
+}
+
+int read_err_word(mwf_ctx* c, cudaStream_t s, unsigned int* out) {
+    CU(c, cudaMemcpyAsync(out, c->err, sizeof(unsigned int), cudaMemcpyDeviceToHost, s));
+    CU(c, cudaStreamSynchronize(s));
+    return MWF_OK;
+}
+
+void drop_lists(mwf_ctx* c) {
+    c->have_lists = false;
+    c->lists_for_reuse = false;
+    c->n_group = 0;
+    c->n_items = 0;
+    c->groups_dispatched = 0;
+}
+
+// cost of an item in sweep units (j-pairs x i per lane): what the longest-first schedule sorts by
+inline int64_t item_cost(const WorkItem& it, int64_t n_tiles) {
+    static const int64_t per_tile[4] = {64, 32, 16, 8};
+    return n_tiles * per_tile[it.kind];
+}
+
+}  // namespace
+
+extern "C" {
+
+const char* mwf_strerror(int code) {
+    switch (code) {
+        case MWF_OK: return "ok";
+        case MWF_EINVAL: return "invalid argument";
+        case MWF_ESTATE: return "call out of order for the current list/monopole state";
+        case MWF_ERANGE: return "index, range or offset out of bounds in the uploaded tree or lists";
+        case MWF_ENOMEM: return "capacity exceeded";
+        case MWF_ECUDA: return "CUDA error";
+        default: return "unknown error code";
+    }
+}
+
+const char* mwf_last_cuda_error(mwf_ctx* c) { return c ? c->cuda_err.c_str() : ""; }
+
+int mwf_arena_bytes(const mwf_params* p, int64_t* bytes) {
+    if (!params_ok(p) || !bytes) return MWF_EINVAL;
+    *bytes = make_layout(*p).total;
+    return MWF_OK;
+}
+
+int mwf_create(mwf_ctx** out, const mwf_params* p, void* arena, int64_t arena_bytes) {
+    if (!out) return MWF_EINVAL;
+    *out = nullptr;
+    if (!params_ok(p)) return MWF_EINVAL;
+    mwf_ctx* c = new (std::nothrow) mwf_ctx;
+    if (!c) return MWF_ENOMEM;
+    c->p = *p;
+    cudaError_t e = cudaSetDevice(p->device);
+    if (e != cudaSuccess) { delete c; return MWF_ECUDA; }
+    cudaDeviceProp prop;
+    e = cudaGetDeviceProperties(&prop, p->device);
+    if (e != cudaSuccess) { delete c; return MWF_ECUDA; }
+    if (prop.major != 10) {  // sm_100a code only: fail loudly, there is no fallback
+        delete c;
+        return MWF_ECUDA;
+    }
+    c->n_sm = prop.multiProcessorCount;
+    c->ctas_per_sm = force_max_ctas_per_sm();
+    if (c->ctas_per_sm < 1) { delete c; return MWF_ECUDA; }
+    const Layout L = make_layout(*p);
+    if (arena) {
+        if (arena_bytes < L.total || (reinterpret_cast<uintptr_t>(arena) & 255)) { delete c; return MWF_ENOMEM; }
+        c->arena = static_cast<char*>(arena);
+    } else {
+        void* m = nullptr;
+        if (cudaMalloc(&m, (size_t)L.total) != cudaSuccess) { cudaGetLastError(); delete c; return MWF_ENOMEM; }
+        c->arena = static_cast<char*>(m);
+        c->own_arena = true;
+    }
+    c->arena_bytes = L.total;
+    char* b = c->arena;
+    c->store = (float4*)(b + L.off[0]);
+    c->accp = (float4*)(b + L.off[1]);
+    c->cells = (mwf_cell*)(b + L.off[2]);
+    c->parent = (int32_t*)(b + L.off[3]);
+    c->arrive = (int32_t*)(b + L.off[4]);
+    c->mom64 = (double4*)(b + L.off[5]);
+    c->grp_first = (int32_t*)(b + L.off[6]);
+    c->grp_n = (int32_t*)(b + L.off[7]);
+    c->grp_self = (uint8_t*)(b + L.off[8]);
+    c->list_off = (int64_t*)(b + L.off[9]);
+    c->st_epj_off = (int64_t*)(b + L.off[10]);
+    c->st_spj_off = (int64_t*)(b + L.off[11]);
+    c->st_ids = (int32_t*)(b + L.off[12]);
+    c->list = (int32_t*)(b + L.off[13]);
+    c->items = (WorkItem*)(b + L.off[14]);
+    c->order_full = (int32_t*)(b + L.off[15]);
+    c->order_split = (int32_t*)(b + L.off[16]);
+    c->counters = (unsigned int*)(b + L.off[17]);
+    c->err = (unsigned int*)(b + L.off[18]);
+    c->max_items = max_items_of(*p);
+    c->tag_groups.assign(MWF_MAX_TAG, 0);
+    bool ok = true;
+    for (int t = 0; t < p->n_tag && ok; ++t) {
+        ok = ok && cudaStreamCreateWithFlags(&c->tag_stream[t], cudaStreamNonBlocking) == cudaSuccess;
+        c->tag_own[t] = ok;
+        ok = ok && cudaEventCreateWithFlags(&c->ev_tag[t], cudaEventDisableTiming) == cudaSuccess;
+        ok = ok && cudaEventCreate(&c->ev_k0[t]) == cudaSuccess;
+        ok = ok && cudaEventCreate(&c->ev_k1[t]) == cudaSuccess;
+    }
+    ok = ok && cudaEventCreateWithFlags(&c->ev_store, cudaEventDisableTiming) == cudaSuccess;
+    ok = ok && cudaMemset(c->counters, 0, N_COUNTER * 4) == cudaSuccess;
+    ok = ok && cudaMemset(c->err, 0, 256) == cudaSuccess;
+    if (!ok) { mwf_destroy(c); return MWF_ECUDA; }
+    *out = c;
+    return MWF_OK;
+}
+
+int mwf_destroy(mwf_ctx* c) {
+    if (!c) return MWF_EINVAL;
+    cudaDeviceSynchronize();
+    for (int t = 0; t < MWF_MAX_TAG; ++t) {
+        if (c->tag_own[t] && c->tag_stream[t]) cudaStreamDestroy(c->tag_stream[t]);
+        if (c->ev_tag[t]) cudaEventDestroy(c->ev_tag[t]);
+        if (c->ev_k0[t]) cudaEventDestroy(c->ev_k0[t]);
+        if (c->ev_k1[t]) cudaEventDestroy(c->ev_k1[t]);
+    }
+    if (c->ev_store) cudaEventDestroy(c->ev_store);
+    if (c->own_arena && c->arena) cudaFree(c->arena);
+    delete c;
+    return MWF_OK;
+}
+
+int mwf_set_tag_stream(mwf_ctx* c, int32_t tag, void* cuda_stream) {
+    if (!c || tag < 0 || tag >= c->p.n_tag) return MWF_EINVAL;
+    if (c->tag_inflight[tag] || !c->tag_ranges[tag].empty()) return MWF_ESTATE;
+    if (c->tag_own[tag] && c->tag_stream[tag]) cudaStreamDestroy(c->tag_stream[tag]);
+    c->tag_own[tag] = false;
+    c->tag_stream[tag] = static_cast<cudaStream_t>(cuda_stream);
+    return MWF_OK;
+}
+
+int mwf_set_particles(mwf_ctx* c, const mwf_posm* src, int64_t first, int64_t n, int src_on_device, void* stream) {
+    if (!c || !src || first < 0 || n < 0) return MWF_EINVAL;
+    if (first + n > c->p.max_ptcl) return MWF_ENOMEM;
+    if (c->have_tree && first + n > c->n_ptcl) return MWF_ERANGE;  // [N, ..) holds the SPJ block
+    if (n == 0) return MWF_OK;
+    cudaStream_t s = static_cast<cudaStream_t>(stream);
+    int rc = before_store_op(c, s);
+    if (rc) return rc;
+    CU(c, cudaMemcpyAsync(c->store + first, src, (size_t)n * 16, src_on_device ? cudaMemcpyDeviceToDevice : cudaMemcpyHostToDevice, s));
+    c->ptcl_hi = std::max(c->ptcl_hi, first + n);
+    if (c->have_tree) c->ptcl_hi = std::min(c->ptcl_hi, c->n_ptcl);
+    c->mono_fresh = false;
+    return after_store_op(c, s);
+}
+
+int mwf_get_particles(mwf_ctx* c, mwf_posm* dst, int64_t first, int64_t n, int dst_on_device) {
+    if (!c || !dst || first < 0 || n < 0 || first + n > c->p.max_ptcl) return MWF_EINVAL;
+    CU(c, cudaDeviceSynchronize());
+    CU(c, cudaMemcpy(dst, c->store + first, (size_t)n * 16, dst_on_device ? cudaMemcpyDeviceToDevice : cudaMemcpyDeviceToHost));
+    return MWF_OK;
+}
+
+int mwf_set_tree(mwf_ctx* c, const mwf_cell* cells, int64_t n_cell, void* stream) {
+    if (!c || !cells || n_cell < 1) return MWF_EINVAL;
+    if (n_cell > c->p.max_cell) return MWF_ENOMEM;
+    const int64_t n = cells[0].n_ptcl;
+    if (n < 1) return MWF_ERANGE;
+    if (n > c->p.max_ptcl) return MWF_ENOMEM;
+    cudaStream_t s = static_cast<cudaStream_t>(stream);
+    int rc = before_store_op(c, s);
+    if (rc) return rc;
+    c->have_tree = false;
+    drop_lists(c);
+    c->mono_fresh = false;
+    CU(c, cudaMemsetAsync(c->err, 0, sizeof(unsigned int), s));
+    CU(c, cudaMemcpyAsync(c->cells, cells, (size_t)n_cell * sizeof(mwf_cell), cudaMemcpyHostToDevice, s));
+    CU(c, launch_tree_prepare(c->cells, n_cell, c->p.max_ptcl, c->parent, c->arrive, c->err, s));
+    ++c->n_launch;
+    // zero-mass dummy record behind the SPJ block: what list padding points at
+    const float4 zero = make_float4(0.f, 0.f, 0.f, 0.f);
+    CU(c, cudaMemcpyAsync(c->store + n + n_cell, &zero, 16, cudaMemcpyHostToDevice, s));
+    unsigned int e = 0;
+    rc = read_err_word(c, s, &e);
+    if (rc) return rc;
+    rc = after_store_op(c, s);
+    if (rc) return rc;
+    if (e) return MWF_ERANGE;
+    c->n_ptcl = n;
+    c->n_cell = n_cell;
+    c->ptcl_hi = std::min(c->ptcl_hi, n);
+    c->have_tree = true;
+    return MWF_OK;
+}
+
+int mwf_set_lists(mwf_ctx* c, int64_t n_group, const int32_t* grp_first, const int32_t* grp_n, const int64_t* epj_off,
+                  const int32_t* epj_id, const int64_t* spj_off, const int32_t* spj_id, int mode, void* stream) {
+    if (!c || n_group < 1 || !grp_first || !grp_n || !epj_off || !spj_off) return MWF_EINVAL;
+    if (mode != MWF_MAKE_LIST && mode != MWF_MAKE_LIST_FOR_REUSE) return MWF_EINVAL;
+    if (!c->have_tree) return MWF_ESTATE;
+    if (n_group > c->p.max_group) return MWF_ENOMEM;
+    if (epj_off[0] != 0 || spj_off[0] != 0) return MWF_ERANGE;
+    const int64_t e_epj = epj_off[n_group], e_spj = spj_off[n_group];
+    if (e_epj < 0 || e_spj < 0) return MWF_ERANGE;
+    if ((e_epj > 0 && !epj_id) || (e_spj > 0 && !spj_id)) return MWF_EINVAL;
+    if (e_epj + e_spj > c->p.max_entry) return MWF_ENOMEM;
+    // host pass: offsets, items, schedule
+    std::vector<int64_t> list_off((size_t)n_group + 1, 0);
+    c->h_item_off.assign((size_t)n_group + 1, 0);
+    c->h_inter.assign((size_t)n_group + 1, 0);
+    std::vector<WorkItem> items;
+    std::vector<int64_t> cost;
+    items.reserve((size_t)(c->n_ptcl / CHUNK_I + 2 * n_group));
+    for (int64_t g = 0; g < n_group; ++g) {
+        const int64_t ne = epj_off[g + 1] - epj_off[g], ns = spj_off[g + 1] - spj_off[g];
+        if (ne < 0 || ns < 0) return MWF_ERANGE;
+        const int64_t gf = grp_first[g], gn = grp_n[g];
+        if (gf < 0 || gn < 1 || gf + gn > c->n_ptcl) return MWF_ERANGE;
+        const int64_t n_list = ne + ns;
+        const int64_t n_tiles = (n_list + TILE_J - 1) / TILE_J;
+        list_off[(size_t)g + 1] = list_off[(size_t)g] + n_tiles * TILE_J;
+        c->h_inter[(size_t)g + 1] = c->h_inter[(size_t)g] + gn * n_list;
+        int64_t done = 0;
+        while (done < gn) {
+            const int64_t rem = gn - done;
+            WorkItem it;
+            it.i_first = (int32_t)(gf + done);
+            it.group = (int32_t)g;
+            if (rem >= CHUNK_I) { it.n_i = CHUNK_I; it.kind = 0; }
+            else if (rem > 32) { it.n_i = 32; it.kind = 1; }
+            else if (rem > 16) { it.n_i = (int32_t)rem; it.kind = 1; }
+            else if (rem > 8) { it.n_i = (int32_t)rem; it.kind = 2; }
+            else { it.n_i = (int32_t)rem; it.kind = 3; }
+            done += it.n_i;
+            items.push_back(it);
+            cost.push_back(item_cost(it, n_tiles));
+        }
+        c->h_item_off[(size_t)g + 1] = (int64_t)items.size();
+    }
+    const int64_t n_items = (int64_t)items.size();
+    if (n_items > c->max_items) return MWF_ENOMEM;
+    // longest-first schedules: over everything, and inside each of the n_tag balanced group ranges
+    std::vector<int32_t> order_full((size_t)n_items), order_split((size_t)n_items);
+    std::iota(order_full.begin(), order_full.end(), 0);
+    std::stable_sort(order_full.begin(), order_full.end(), [&](int32_t x, int32_t y) { return cost[(size_t)x] > cost[(size_t)y]; });
+    c->h_split.assign((size_t)c->p.n_tag + 1, 0);
+    {
+        const int64_t total = c->h_inter[(size_t)n_group];
+        int64_t g = 0;
+        for (int t = 1; t < c->p.n_tag; ++t) {
+            const int64_t want = total / c->p.n_tag * t;
+            while (g < n_group && c->h_inter[(size_t)g] < want) ++g;
+            c->h_split[(size_t)t] = g;
+        }
+        c->h_split[(size_t)c->p.n_tag] = n_group;
+        std::iota(order_split.begin(), order_split.end(), 0);
+        for (int t = 0; t < c->p.n_tag; ++t) {
+            const int64_t b = c->h_item_off[(size_t)c->h_split[(size_t)t]], e = c->h_item_off[(size_t)c->h_split[(size_t)t + 1]];
+            std::stable_sort(order_split.begin() + b, order_split.begin() + e,
+                             [&](int32_t x, int32_t y) { return cost[(size_t)x] > cost[(size_t)y]; });
+        }
+    }
+    cudaStream_t s = static_cast<cudaStream_t>(stream);
+    int rc = before_store_op(c, s);
+    if (rc) return rc;
+    drop_lists(c);
+    const auto H2D = cudaMemcpyHostToDevice;
+    CU(c, cudaMemsetAsync(c->err, 0, sizeof(unsigned int), s));
+    CU(c, cudaMemcpyAsync(c->grp_first, grp_first, (size_t)n_group * 4, H2D, s));
+    CU(c, cudaMemcpyAsync(c->grp_n, grp_n, (size_t)n_group * 4, H2D, s));
+    CU(c, cudaMemcpyAsync(c->st_epj_off, epj_off, (size_t)(n_group + 1) * 8, H2D, s));
+    CU(c, cudaMemcpyAsync(c->st_spj_off, spj_off, (size_t)(n_group + 1) * 8, H2D, s));
+    if (e_epj) CU(c, cudaMemcpyAsync(c->st_ids, epj_id, (size_t)e_epj * 4, H2D, s));
+    if (e_spj) CU(c, cudaMemcpyAsync(c->st_ids + e_epj, spj_id, (size_t)e_spj * 4, H2D, s));
+    CU(c, cudaMemcpyAsync(c->list_off, list_off.data(), (size_t)(n_group + 1) * 8, H2D, s));
+    CU(c, cudaMemcpyAsync(c->items, items.data(), (size_t)n_items * sizeof(WorkItem), H2D, s));
+    CU(c, cudaMemcpyAsync(c->order_full, order_full.data(), (size_t)n_items * 4, H2D, s));
+    CU(c, cudaMemcpyAsync(c->order_split, order_split.data(), (size_t)n_items * 4, H2D, s));
+    CU(c, launch_merge_lists(n_group, c->grp_first, c->grp_n, c->st_epj_off, c->st_ids, c->st_spj_off, c->st_ids + e_epj, c->list_off,
+                             c->n_ptcl, c->n_cell, c->list, c->grp_self, c->err, s));
+    ++c->n_launch;
+    unsigned int e = 0;
+    rc = read_err_word(c, s, &e);  // also makes the host vectors above safe to free
+    if (rc) return rc;
+    rc = after_store_op(c, s);
+    if (rc) return rc;
+    if (e & ~ERR_SELF_MIXED) return MWF_ERANGE;
+    if (e) return MWF_EINVAL;  // only the self-membership rule is violated
+    c->h_grp_first.assign(grp_first, grp_first + n_group);
+    c->h_grp_n.assign(grp_n, grp_n + n_group);
+    c->n_group = n_group;
+    c->n_items = n_items;
+    c->padded_entries = list_off[(size_t)n_group];
+    c->have_lists = true;
+    c->lists_for_reuse = (mode == MWF_MAKE_LIST_FOR_REUSE);
+    c->groups_dispatched = 0;
+    c->groups_outstanding = 0;
+    return MWF_OK;
+}
+
+int mwf_begin_step(mwf_ctx* c, int mode) {
+    if (!c) return MWF_EINVAL;
+    if (mode == MWF_REUSE_LIST) {
+        if (!c->have_lists || !c->lists_for_reuse) return MWF_ESTATE;  // MAKE_LIST keeps nothing
+        c->groups_dispatched = 0;
+        return MWF_OK;
+    }
+    if (mode == MWF_MAKE_LIST || mode == MWF_MAKE_LIST_FOR_REUSE) {
+        for (int t = 0; t < c->p.n_tag; ++t)
+            if (!c->tag_ranges[t].empty()) return MWF_ESTATE;  // results of the previous step not retrieved
+        drop_lists(c);
+        return MWF_OK;
+    }
+    return MWF_EINVAL;
+}
+
+int mwf_refresh_monopoles(mwf_ctx* c, void* stream) {
+    if (!c) return MWF_EINVAL;
+    if (!c->have_tree || c->ptcl_hi < c->n_ptcl) return MWF_ESTATE;
+    cudaStream_t s = static_cast<cudaStream_t>(stream);
+    int rc = before_store_op(c, s);
+    if (rc) return rc;
+    CU(c, launch_monopoles(c->cells, c->parent, c->n_cell, c->n_ptcl, c->store, c->mom64, c->arrive, s));
+    ++c->n_launch;
+    c->mono_fresh = true;
+    return after_store_op(c, s);
+}
+
+int mwf_dispatch(mwf_ctx* c, int32_t tag, int64_t g_begin, int64_t g_end) {
+    if (!c || tag < 0 || tag >= c->p.n_tag || g_begin < 0 || g_end < g_begin) return MWF_EINVAL;
+    if (!c->have_tree || !c->have_lists || !c->mono_fresh) return MWF_ESTATE;
+    if (g_end > c->n_group) return MWF_ERANGE;
+    if (g_end == g_begin) return MWF_OK;
+    cudaStream_t s = c->tag_stream[tag];
+    if (c->store_event_valid) CU(c, cudaStreamWaitEvent(s, c->ev_store, 0));
+    ForceArgs a;
+    a.store = c->store;
+    a.list = c->list;
+    a.list_off = c->list_off;
+    a.grp_self = c->grp_self;
+    a.items = c->items;
+    a.accp = c->accp;
+    a.item_begin = c->h_item_off[(size_t)g_begin];
+    a.n_items = c->h_item_off[(size_t)g_end] - a.item_begin;
+    a.eps2 = c->p.eps * c->p.eps;
+    a.G = c->p.G;
+    a.order = nullptr;
+    if (g_begin == 0 && g_end == c->n_group) {
+        a.order = c->order_full;
+    } else {
+        for (int t = 0; t < c->p.n_tag; ++t)
+            if (c->h_split[(size_t)t] == g_begin && c->h_split[(size_t)t + 1] == g_end) a.order = c->order_split;
+    }
+    const int64_t resident = (int64_t)c->n_sm * c->ctas_per_sm;
+    const int64_t want = (a.n_items + WARPS_PER_CTA - 1) / WARPS_PER_CTA;
+    const int grid = (int)std::min(want, resident);
+    a.counter = nullptr;
+    if (want > resident) {  // more items than resident warps: claim the rest dynamically
+        a.counter = c->counters + (c->counter_seq++ % N_COUNTER);
+        CU(c, cudaMemsetAsync(a.counter, 0, sizeof(unsigned int), s));
+    }
+    CU(c, cudaEventRecord(c->ev_k0[tag], s));
+    CU(c, launch_force(a, grid, s));
+    CU(c, cudaEventRecord(c->ev_k1[tag], s));
+    CU(c, cudaEventRecord(c->ev_tag[tag], s));
+    c->tag_timed[tag] = true;
+    c->tag_inflight[tag] = true;
+    ++c->n_launch;
+    c->n_inter += c->h_inter[(size_t)g_end] - c->h_inter[(size_t)g_begin];
+    // particle range covered (groups are disjoint; contiguous when they come from a tree)
+    int64_t lo = c->h_grp_first[(size_t)g_begin], hi = lo + c->h_grp_n[(size_t)g_begin];
+    auto& rs = c->tag_ranges[tag];
+    for (int64_t g = g_begin + 1; g < g_end; ++g) {
+        const int64_t f = c->h_grp_first[(size_t)g], n = c->h_grp_n[(size_t)g];
+        if (f == hi) { hi += n; continue; }
+        rs.emplace_back(lo, hi);
+        lo = f; hi = f + n;
+    }
+    rs.emplace_back(lo, hi);
+    c->tag_groups[(size_t)tag] += g_end - g_begin;
+    c->groups_dispatched += g_end - g_begin;
+    c->groups_outstanding += g_end - g_begin;
+    return MWF_OK;
+}
+
+int mwf_retrieve(mwf_ctx* c, int32_t tag, mwf_accp* dst, int dst_on_device) {
+    if (!c || tag < 0 || tag >= c->p.n_tag || !dst) return MWF_EINVAL;
+    auto& rs = c->tag_ranges[tag];
+    if (rs.empty()) return MWF_ESTATE;
+    cudaStream_t s = c->tag_stream[tag];
+    const auto kind = dst_on_device ? cudaMemcpyDeviceToDevice : cudaMemcpyDeviceToHost;
+    // merge adjacent ranges of consecutive dispatches
+    std::sort(rs.begin(), rs.end());
+    size_t k = 0;
+    while (k < rs.size()) {
+        int64_t lo = rs[k].first, hi = rs[k].second;
+        size_t j = k + 1;
+        while (j < rs.size() && rs[j].first <= hi) { hi = std::max(hi, rs[j].second); ++j; }
+        CU(c, cudaMemcpyAsync(reinterpret_cast<float4*>(dst) + lo, c->accp + lo, (size_t)(hi - lo) * 16, kind, s));
+        k = j;
+    }
+    CU(c, cudaStreamSynchronize(s));
+    rs.clear();
+    c->tag_inflight[tag] = false;
+    c->groups_outstanding -= c->tag_groups[(size_t)tag];
+    c->tag_groups[(size_t)tag] = 0;
+    // MAKE_LIST: the lists served their one evaluation
+    if (c->have_lists && !c->lists_for_reuse && c->groups_outstanding == 0 && c->groups_dispatched >= c->n_group) drop_lists(c);
+    return MWF_OK;
+}
+
+int mwf_calc_force_all(mwf_ctx* c, const mwf_posm* src, int src_on_device, mwf_accp* dst, int dst_on_device) {
+    if (!c || !dst) return MWF_EINVAL;
+    if (!c->have_tree || !c->have_lists) return MWF_ESTATE;
+    cudaStream_t s0 = c->tag_stream[0];
+    int rc;
+    if (src) {
+        rc = mwf_set_particles(c, src, 0, c->n_ptcl, src_on_device, s0);
+        if (rc) return rc;
+    }
+    if (!c->mono_fresh) {
+        rc = mwf_refresh_monopoles(c, s0);
+        if (rc) return rc;
+    }
+    // host destination: one dispatch per tag so that each D2H copy overlaps the other tags' kernels
+    const int n_part = dst_on_device ? 1 : c->p.n_tag;
+    if (n_part == 1) {
+        rc = mwf_dispatch(c, 0, 0, c->n_group);
+        if (rc) return rc;
+        return mwf_retrieve(c, 0, dst, dst_on_device);
+    }
+    bool used[MWF_MAX_TAG] = {false};
+    for (int t = 0; t < n_part; ++t) {
+        const int64_t gb = c->h_split[(size_t)t], ge = c->h_split[(size_t)t + 1];
+        if (ge == gb) continue;
+        rc = mwf_dispatch(c, t, gb, ge);
+        if (rc) return rc;
+        used[t] = true;
+    }
+    for (int t = 0; t < n_part; ++t) {
+        if (!used[t]) continue;
+        rc = mwf_retrieve(c, t, dst, dst_on_device);
+        if (rc) return rc;
+    }
+    return MWF_OK;
+}
+
+int mwf_get_monopoles(mwf_ctx* c, mwf_posm* dst, int dst_on_device) {
+    if (!c || !dst) return MWF_EINVAL;
+    if (!c->have_tree || !c->mono_fresh) return MWF_ESTATE;
+    CU(c, cudaDeviceSynchronize());
+    CU(c, cudaMemcpy(dst, c->store + c->n_ptcl, (size_t)c->n_cell * 16, dst_on_device ? cudaMemcpyDeviceToDevice : cudaMemcpyDeviceToHost));
+    return MWF_OK;
+}
+
+int mwf_device_pointers(mwf_ctx* c, mwf_posm** store, mwf_accp** accp) {
+    if (!c) return MWF_EINVAL;
+    if (store) *store = reinterpret_cast<mwf_posm*>(c->store);
+    if (accp) *accp = reinterpret_cast<mwf_accp*>(c->accp);
+    return MWF_OK;
+}
+
+int mwf_sync(mwf_ctx* c) {
+    if (!c) return MWF_EINVAL;
+    CU(c, cudaDeviceSynchronize());
+    return MWF_OK;
+}
+
+int mwf_get_counters(mwf_ctx* c, int64_t* kernel_launches, int64_t* interactions, int64_t* padded_entries) {
+    if (!c) return MWF_EINVAL;
+    if (kernel_launches) *kernel_launches = c->n_launch;
+    if (interactions) *interactions = c->n_inter;
+    if (padded_entries) *padded_entries = c->padded_entries;
+    return MWF_OK;
+}
+
+int mwf_last_dispatch_ms(mwf_ctx* c, int32_t tag, float* ms) {
+    if (!c || tag < 0 || tag >= c->p.n_tag || !ms) return MWF_EINVAL;
+    if (!c->tag_timed[tag]) return MWF_ESTATE;
+    CU(c, cudaEventSynchronize(c->ev_k1[tag]));
+    CU(c, cudaEventElapsedTime(ms, c->ev_k0[tag], c->ev_k1[tag]));
+    return MWF_OK;
+}
+
+}  // extern "C"

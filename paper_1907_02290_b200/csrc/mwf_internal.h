@@ -1,0 +1,65 @@
+// Internal declarations shared by the translation units of libmwf.so (not part of the ABI).
+#pragma once
+#include <cuda_runtime.h>
+#include <stdint.h>
+
+#include <string>
+#include <vector>
+
+#include "mwf.h"
+
+namespace mwf {
+
+constexpr int TILE_J = 64;          // j entries staged per warp tile; merged lists are padded to this
+constexpr int WARPS_PER_CTA = 8;    // force kernel block = 256 threads
+constexpr int CHUNK_I = 64;         // i-particles of a full work item (2 per lane)
+
+// One unit of work for one warp: up to 64 consecutive i-particles of one group against its whole list.
+// kind 0: 64 particles, 2 per lane.  kind 1/2/3: <= 32 / 16 / 8 particles, 1 per lane, the warp split
+// into 1 / 2 / 4 slices that share the i-particles and take every 1st / 2nd / 4th j-pair.
+struct WorkItem {
+    int32_t i_first;
+    int32_t n_i;
+    int32_t group;
+    int32_t kind;
+};
+
+struct ForceArgs {
+    const float4* store;        // particles then SPJ then one zero-mass dummy
+    const int32_t* list;        // merged, padded lists
+    const int64_t* list_off;    // per group, in entries (multiples of TILE_J)
+    const uint8_t* grp_self;    // 1: the group's own particles are in its EPJ list
+    const WorkItem* items;
+    const int32_t* order;       // cost-sorted permutation of item indices, or nullptr = identity
+    float4* accp;
+    unsigned int* counter;      // dynamic scheduling counter (zeroed before launch), or nullptr = static
+    int64_t item_begin;
+    int64_t n_items;
+    float eps2;
+    float G;
+};
+
+// kernels' host launchers (defined next to their kernels)
+cudaError_t launch_force(const ForceArgs& a, int grid, cudaStream_t s);
+int force_max_ctas_per_sm();
+
+cudaError_t launch_tree_prepare(const mwf_cell* cells, int64_t n_cell, int64_t max_ptcl, int32_t* parent, int32_t* counter,
+                                unsigned int* err, cudaStream_t s);
+cudaError_t launch_monopoles(const mwf_cell* cells, const int32_t* parent, int64_t n_cell, int64_t n_ptcl, float4* store,
+                             double4* mom64, int32_t* counter, cudaStream_t s);
+cudaError_t launch_merge_lists(int64_t n_group, const int32_t* grp_first, const int32_t* grp_n, const int64_t* epj_off,
+                               const int32_t* epj_id, const int64_t* spj_off, const int32_t* spj_id, const int64_t* list_off,
+                               int64_t n_ptcl, int64_t n_cell, int32_t* list, uint8_t* grp_self, unsigned int* err, cudaStream_t s);
+
+// bits of the device-side validation word
+enum : unsigned int {
+    ERR_CELL_RANGE = 1u,     // cell particle range outside [0, N) or empty
+    ERR_CHILD_RANGE = 2u,    // child range outside (c, n_cell)
+    ERR_CHILD_PART = 4u,     // children do not partition the parent's particle range
+    ERR_EPJ_INDEX = 8u,      // EPJ index outside [0, N)
+    ERR_SPJ_INDEX = 16u,     // SPJ index outside [0, n_cell)
+    ERR_SELF_MIXED = 32u,    // a group's EPJ list holds some but not all of its own particles
+    ERR_GROUP_RANGE = 64u    // group i-range outside [0, N)
+};
+
+}  // namespace mwf

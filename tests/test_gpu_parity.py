@@ -1,0 +1,373 @@
+"""GPU parity: the CUDA path (through the C ABI) against the fp64 oracle, element by element on the
+same seeded inputs.  Tolerances are BASELINE.json's north_star: per-particle relative acceleration
+error <= 1e-4 max and <= 2e-5 RMS, relative potential error <= 1e-5 RMS."""
+import numpy as np
+import pytest
+
+import oracle
+from paper_1907_02290_b200 import binding
+from paper_1907_02290_b200.workload import CONFIGS, make_particles, make_workload
+
+pytestmark = pytest.mark.gpu
+
+ACC_MAX, ACC_RMS, POT_RMS = 1e-4, 2e-5, 1e-5
+
+
+def gpu_eval(w, eps, G=1.0, n_tag=4, batches=None, mode=binding.MAKE_LIST_FOR_REUSE, keep=False):
+    f = binding.MultiWalkForce.for_workload(w, eps=eps, G=G, n_tag=n_tag)
+    f.upload_workload(w, mode)
+    f.refresh_monopoles()
+    out = np.full((w.n, 4), np.nan, np.float32)
+    if batches is None:
+        f.dispatch(0, 0, w.n_group)
+        f.retrieve(0, out)
+    else:
+        tag = 0
+        pending = []
+        for gb in range(0, w.n_group, batches):
+            if len(pending) == n_tag:
+                f.retrieve(pending.pop(0), out)
+            f.dispatch(tag, gb, min(w.n_group, gb + batches))
+            pending.append(tag)
+            tag = (tag + 1) % n_tag
+        for t in pending:
+            f.retrieve(t, out)
+    if keep:
+        return out, f
+    f.close()
+    return out
+
+
+def oracle_eval(w, eps, G=1.0, groups=None, posm=None):
+    posm = w.posm if posm is None else posm
+    mom = oracle.monopoles(w.cells, posm)
+    acc, pot = oracle.forces(posm, mom, w.grp_first, w.grp_n, w.epj_off, w.epj_id, w.spj_off, w.spj_id, eps, G, groups)
+    return acc, pot, mom
+
+
+def errors(out, acc, pot, mask=None):
+    a = out[:, :3].astype(np.float64)
+    p = out[:, 3].astype(np.float64)
+    if mask is not None:
+        a, p, acc, pot = a[mask], p[mask], acc[mask], pot[mask]
+    ea = np.linalg.norm(a - acc, axis=1) / np.linalg.norm(acc, axis=1)
+    ep = np.abs(p - pot) / np.abs(pot)
+    return ea, ep
+
+
+def check(out, acc, pot, mask=None, label=""):
+    ea, ep = errors(out, acc, pot, mask)
+    msg = "%s: acc max %.2e rms %.2e | pot max %.2e rms %.2e" % (
+        label, ea.max(), np.sqrt(np.mean(ea ** 2)), ep.max(), np.sqrt(np.mean(ep ** 2)))
+    print(msg)
+    assert np.all(np.isfinite(ea)) and np.all(np.isfinite(ep)), msg
+    assert ea.max() <= ACC_MAX, msg
+    assert np.sqrt(np.mean(ea ** 2)) <= ACC_RMS, msg
+    assert np.sqrt(np.mean(ep ** 2)) <= POT_RMS, msg
+
+
+def group_mask(w, groups):
+    m = np.zeros(w.n, bool)
+    for g in groups:
+        m[w.grp_first[g]:w.grp_first[g] + w.grp_n[g]] = True
+    return m
+
+
+def expect_code(fn, *a):
+    with pytest.raises(binding.MwfError) as e:
+        fn(*a)
+    return e.value.code
+
+
+# ------------------------------------------------------------------ config 1 in full, others reduced
+def test_config1_full():
+    cfg = CONFIGS[0]
+    w = make_workload(cfg)
+    out = gpu_eval(w, cfg.eps)
+    acc, pot, _ = oracle_eval(w, cfg.eps)
+    check(out, acc, pot, label=cfg.name)
+
+
+@pytest.mark.parametrize("idx,n", [(1, 60000), (2, 70001), (3, 65537), (4, 50000)])
+def test_reduced_configs_every_particle(idx, n):
+    cfg = CONFIGS[idx]
+    w = make_workload(cfg, n)
+    out = gpu_eval(w, cfg.eps)
+    acc, pot, _ = oracle_eval(w, cfg.eps)
+    check(out, acc, pot, label="%s n=%d" % (cfg.name, n))
+
+
+def test_G_and_unequal_masses():
+    cfg = CONFIGS[2]
+    w = make_workload(cfg, 20000)
+    out = gpu_eval(w, cfg.eps, G=6.5)
+    acc, pot, _ = oracle_eval(w, cfg.eps, G=6.5)
+    check(out, acc, pot, label="G=6.5")
+
+
+# ------------------------------------------------------------------ full sizes, sampled groups
+@pytest.mark.parametrize("idx,n_sample", [(1, 300), (2, 120), (3, 200), (4, 200)])
+def test_full_size_sampled_groups(idx, n_sample):
+    """BASELINE.json's full sizes in bench.py's launch configuration (one dispatch over all groups);
+    the oracle evaluates a seeded sample of groups, every particle of each."""
+    cfg = CONFIGS[idx]
+    w = make_workload(cfg)
+    out = gpu_eval(w, cfg.eps)
+    assert np.all(np.isfinite(out))
+    rng = np.random.default_rng(100 + idx)
+    groups = rng.choice(w.n_group, size=n_sample, replace=False)
+    cost = w.grp_n.astype(np.int64) * w.n_list
+    # always include the heaviest group, the smallest group and both ends
+    groups = np.unique(np.concatenate([groups, [np.argmax(cost), np.argmin(w.grp_n), 0, w.n_group - 1]]))
+    acc, pot, _ = oracle_eval(w, cfg.eps, groups=groups)
+    check(out, acc, pot, mask=group_mask(w, groups), label="%s full size" % cfg.name)
+    # properties that hold at any size: tree forces nearly conserve momentum; W matches the closed form
+    m = w.posm[:, 3].astype(np.float64)
+    a = out[:, :3].astype(np.float64)
+    assert np.linalg.norm((m[:, None] * a).sum(0)) < 1e-3 * (m * np.linalg.norm(a, axis=1)).sum()
+    if cfg.kind == "plummer":
+        W = 0.5 * np.sum(m * out[:, 3].astype(np.float64))
+        assert W == pytest.approx(-3 * np.pi / 32 * 1.0055, rel=0.005)    # pin P6 at N >= 2^20
+
+
+# ------------------------------------------------------------------ monopole refresh (row a3, reading S11)
+@pytest.mark.parametrize("idx,n", [(0, None), (2, 100000), (3, 80000)])
+def test_monopole_refresh(idx, n):
+    cfg = CONFIGS[idx]
+    w = make_workload(cfg, n)
+    f = binding.MultiWalkForce.for_workload(w)
+    f.upload_workload(w)
+    f.refresh_monopoles()
+    got = f.get_monopoles(w.n_cell).astype(np.float64)
+    f.refresh_monopoles()                      # self-cleaning counters: a second refresh gives the same bits
+    again = f.get_monopoles(w.n_cell).astype(np.float64)
+    f.close()
+    assert np.array_equal(got, again)
+    mom = oracle.monopoles(w.cells, w.posm)
+    assert np.all(np.abs(got[:, 3] - mom[:, 3]) <= 1e-6 * mom[:, 3])
+    dx = np.linalg.norm(got[:, :3] - mom[:, :3], axis=1)
+    scale = np.maximum(np.linalg.norm(mom[:, :3], axis=1), w.geom[:, 3])
+    assert np.all(dx <= 2.0 ** -22 * scale)
+
+
+# ------------------------------------------------------------------ dispatch shapes
+def test_batched_dispatch_over_tags_is_bitwise_identical():
+    """Config 2's pipeline: 64-256 groups per dispatch, tags round-robin over the streams."""
+    cfg = CONFIGS[1]
+    w = make_workload(cfg, 150000)
+    one = gpu_eval(w, cfg.eps)
+    for batch in (64, 256):
+        many = gpu_eval(w, cfg.eps, n_tag=8, batches=batch)
+        assert np.array_equal(one, many)
+
+
+def test_calc_force_all_host_and_device_destinations():
+    import torch
+    cfg = CONFIGS[1]
+    w = make_workload(cfg, 100000)
+    ref, f = gpu_eval(w, cfg.eps, n_tag=8, keep=True)
+    host = f.pinned(w.n)
+    src = f.pinned(w.n)
+    src.numpy()[:] = w.posm
+    f.begin_step(binding.REUSE_LIST)
+    f.calc_force_all(src, host)                                   # split over the 8 tags, one D2H per tag
+    assert np.array_equal(host.numpy(), ref)
+    dev = torch.zeros((w.n, 4), dtype=torch.float32, device="cuda")
+    f.calc_force_all(torch.from_numpy(w.posm).cuda(), dev)        # device source and destination, one dispatch
+    assert np.array_equal(dev.cpu().numpy(), ref)
+    f.close()
+
+
+# ------------------------------------------------------------------ edge cases of the kernel mapping
+def synthetic_groups(n, sizes):
+    """Consecutive groups of the given sizes over n particles with EVERY particle in every list
+    (theta = 0): the result must equal direct summation whatever the group sizes are."""
+    sizes = np.asarray(sizes, np.int32)
+    assert int(sizes.sum()) == n
+    first = np.concatenate([[0], np.cumsum(sizes)[:-1]]).astype(np.int32)
+    ng = len(sizes)
+    epj_off = np.arange(ng + 1, dtype=np.int64) * n
+    epj_id = np.tile(np.arange(n, dtype=np.int32), ng)
+    return first, sizes, epj_off, epj_id, np.zeros(ng + 1, np.int64), np.zeros(0, np.int32)
+
+
+@pytest.mark.parametrize("n", [1, 2, 63, 64, 65, 129, 1000])
+def test_every_remainder_width_against_direct_summation(n):
+    """Group sizes 1, 3, 7, ... 255 hit every item kind (64 = 2 per lane; <= 32, <= 16, <= 8 with 1/2/4
+    j-slices); list lengths n = 1, 63, 64, 65 hit the ragged and exact tile tails."""
+    posm, _ = make_particles(CONFIGS[0], n)
+    sizes, left, k = [], n, 1
+    while left > 0:
+        s = min(left, k)
+        sizes.append(s)
+        left -= s
+        k = k * 2 + 1 if k < 130 else 1
+    gf, gn, eo, ei, so, si = synthetic_groups(n, sizes)
+    f = binding.MultiWalkForce(1 / 64, 1.0, max_ptcl=n, max_cell=1, max_group=len(sizes), max_entry=ei.size, n_tag=2)
+    f.begin_step(binding.MAKE_LIST)
+    f.set_particles(posm)
+    f.set_tree(np.array([[0, n, 0, 0]], np.int32))
+    f.set_lists(gf, gn, eo, ei, so, si, binding.MAKE_LIST)
+    f.refresh_monopoles()
+    f.dispatch(1, 0, len(sizes))
+    out = np.full((n, 4), np.nan, np.float32)
+    f.retrieve(1, out)
+    f.close()
+    acc, pot = oracle.direct(posm, 1 / 64)
+    if n == 1:
+        assert np.all(out == 0)          # a lone particle feels nothing (self term excluded, reading S2)
+    else:
+        check(out, acc, pot, label="direct n=%d" % n)
+
+
+def test_lists_without_self_and_spj_only():
+    """A group whose EPJ list holds none of its own particles gets no self correction; a list may be
+    SPJ-only or EPJ-only."""
+    posm, _ = make_particles(CONFIGS[0], 300)
+    cells = np.array([[0, 300, 1, 2], [0, 100, 0, 0], [100, 200, 0, 0]], np.int32)
+    gf = np.array([0, 100], np.int32)
+    gn = np.array([100, 200], np.int32)
+    # group 0 sees particles 100..299 as EPJ only (no self); group 1 sees cell 1 as one SPJ and no EPJ at all
+    eo = np.array([0, 200, 200], np.int64)
+    ei = np.arange(100, 300, dtype=np.int32)
+    so = np.array([0, 0, 1], np.int64)
+    si = np.array([1], np.int32)
+    f = binding.MultiWalkForce(1 / 64, 1.0, max_ptcl=300, max_cell=3, max_group=2, max_entry=201, n_tag=1)
+    f.set_particles(posm)
+    f.set_tree(cells)
+    f.set_lists(gf, gn, eo, ei, so, si, binding.MAKE_LIST_FOR_REUSE)
+    f.refresh_monopoles()
+    f.dispatch(0, 0, 2)
+    out = np.full((300, 4), np.nan, np.float32)
+    f.retrieve(0, out)
+    f.close()
+    mom = oracle.monopoles(cells, posm)
+    acc, pot = oracle.forces(posm, mom, gf, gn, eo, ei, so, si, 1 / 64)
+    check(out, acc, pot, label="no-self / spj-only")
+
+
+def test_coincident_particles():
+    """Reading S4: distinct particles at one position are a real pair (0 to acc, -G m/eps to pot)."""
+    posm = np.array([[1, 1, 1, 2.0], [1, 1, 1, 5.0], [2, 1, 1, 1.0]], np.float32)
+    gf, gn, eo, ei, so, si = synthetic_groups(3, [3])
+    f = binding.MultiWalkForce(0.5, 1.0, max_ptcl=3, max_cell=1, max_group=1, max_entry=3, n_tag=1)
+    f.set_particles(posm)
+    f.set_tree(np.array([[0, 3, 0, 0]], np.int32))
+    f.set_lists(gf, gn, eo, ei, so, si)
+    f.refresh_monopoles()
+    f.dispatch(0, 0, 1)
+    out = np.zeros((3, 4), np.float32)
+    f.retrieve(0, out)
+    f.close()
+    acc, pot = oracle.direct(posm, 0.5)
+    np.testing.assert_allclose(out[:, :3], acc, rtol=1e-5, atol=1e-7)
+    np.testing.assert_allclose(out[:, 3], pot, rtol=1e-5)
+
+
+# ------------------------------------------------------------------ list-reuse driver (rows a6, a7)
+def test_state_machine_and_validation():
+    cfg = CONFIGS[0]
+    w = make_workload(cfg, 2000)
+    lists = (w.grp_first, w.grp_n, w.epj_off, w.epj_id, w.spj_off, w.spj_id)
+    f = binding.MultiWalkForce.for_workload(w, n_tag=2)
+    out = np.zeros((w.n, 4), np.float32)
+    assert expect_code(f.dispatch, 0, 0, 1) == binding.ESTATE                  # nothing uploaded
+    assert expect_code(f.begin_step, binding.REUSE_LIST) == binding.ESTATE     # no saved lists
+    assert expect_code(f.set_lists, *lists) == binding.ESTATE                  # no tree yet
+    assert expect_code(f.refresh_monopoles) == binding.ESTATE
+    f.set_particles(w.posm)
+    f.set_tree(w.cells)
+    f.set_lists(*lists, binding.MAKE_LIST)
+    assert expect_code(f.dispatch, 0, 0, w.n_group) == binding.ESTATE          # monopoles stale
+    f.refresh_monopoles()
+    assert expect_code(f.dispatch, 5, 0, 1) == binding.EINVAL                  # bad tag
+    assert expect_code(f.dispatch, 0, 0, w.n_group + 1) == binding.ERANGE
+    assert expect_code(f.retrieve, 0, out) == binding.ESTATE                   # idle tag
+    f.dispatch(0, 0, w.n_group)
+    f.retrieve(0, out)
+    # MAKE_LIST keeps nothing: REUSE_LIST afterwards is a user error
+    assert expect_code(f.begin_step, binding.REUSE_LIST) == binding.ESTATE
+    assert expect_code(f.dispatch, 0, 0, 1) == binding.ESTATE
+    # MAKE_LIST_FOR_REUSE keeps them; evaluation 0 is identical under either mode (pin P9)
+    f.begin_step(binding.MAKE_LIST_FOR_REUSE)
+    f.set_tree(w.cells)
+    f.set_lists(*lists, binding.MAKE_LIST_FOR_REUSE)
+    f.refresh_monopoles()
+    f.dispatch(1, 0, w.n_group)
+    out2 = np.zeros_like(out)
+    f.retrieve(1, out2)
+    assert np.array_equal(out, out2)
+    f.begin_step(binding.REUSE_LIST)
+    f.set_particles(w.posm)
+    assert expect_code(f.dispatch, 0, 0, 1) == binding.ESTATE                  # a refresh must follow an upload
+    f.refresh_monopoles()
+    f.dispatch(0, 0, w.n_group)
+    f.retrieve(0, out2)
+    assert np.array_equal(out, out2)
+    # validation of indices, offsets, self-membership, tree and capacity
+    bad = w.epj_id.copy()
+    bad[7] = w.n
+    assert expect_code(f.set_lists, w.grp_first, w.grp_n, w.epj_off, bad, w.spj_off, w.spj_id) == binding.ERANGE
+    bad = w.spj_id.copy()
+    bad[3] = -1
+    assert expect_code(f.set_lists, w.grp_first, w.grp_n, w.epj_off, w.epj_id, w.spj_off, bad) == binding.ERANGE
+    bad = w.epj_off.copy()
+    bad[2] = bad[1] - 1
+    assert expect_code(f.set_lists, w.grp_first, w.grp_n, bad, w.epj_id, w.spj_off, w.spj_id) == binding.ERANGE
+    bad = w.epj_id.copy()
+    seg = bad[: w.epj_off[1]]
+    own = np.nonzero(seg == w.grp_first[0])[0][0]
+    outsider = np.setdiff1d(np.arange(w.n), np.arange(w.grp_first[0], w.grp_first[0] + w.grp_n[0]))[0]
+    if w.grp_n[0] > 1:
+        bad[own] = outsider                                                    # one own particle missing from the list
+        assert expect_code(f.set_lists, w.grp_first, w.grp_n, w.epj_off, bad, w.spj_off, w.spj_id) == binding.EINVAL
+    cells = w.cells.copy()
+    cells[1, 0] += 1
+    assert expect_code(f.set_tree, cells) == binding.ERANGE
+    small = binding.MultiWalkForce(cfg.eps, max_ptcl=w.n, max_cell=w.n_cell, max_group=w.n_group, max_entry=10, n_tag=1)
+    small.set_particles(w.posm)
+    small.set_tree(w.cells)
+    assert expect_code(small.set_lists, *lists) == binding.ENOMEM
+    small.close()
+    f.close()
+
+
+def test_reuse_run_per_step():
+    """Config 5 at reduced N: lists built once, 8 kick-drift-kick steps reuse them while the monopoles are
+    refreshed on the device; every evaluation is compared with the oracle run on exactly the fp32
+    positions that were uploaded (reading O7).  The orbit integration is host harness code and uses the
+    GPU's forces (the system under test)."""
+    cfg = CONFIGS[4]
+    w = make_workload(cfg, 40000)
+    f = binding.MultiWalkForce.for_workload(w, n_tag=4)
+    f.upload_workload(w, binding.MAKE_LIST_FOR_REUSE)
+    x = w.posm[:, :3].astype(np.float64)
+    v = w.vel.copy()
+    posm = w.posm.copy()
+    host_in, host_out = f.pinned(w.n), f.pinned(w.n)
+    padded0, spj_prev, a = None, None, None
+    for step in range(cfg.n_reuse + 1):
+        if step > 0:
+            v += 0.5 * cfg.dt * a
+            x += cfg.dt * v
+            posm[:, :3] = x.astype(np.float32)
+            f.begin_step(binding.REUSE_LIST)
+        host_in.numpy()[:] = posm
+        f.calc_force_all(host_in, host_out)
+        out = host_out.numpy().copy()
+        acc, pot, mom = oracle_eval(w, cfg.eps, posm=posm)
+        check(out, acc, pot, label="step %d" % step)
+        spj = f.get_monopoles(w.n_cell)
+        assert np.all(np.abs(spj[:, 3] - mom[:, 3]) <= 1e-6 * mom[:, 3])
+        assert np.all(np.linalg.norm(spj[:, :3] - mom[:, :3], axis=1)
+                      <= 2.0 ** -22 * np.maximum(np.linalg.norm(mom[:, :3], axis=1), w.geom[:, 3]))
+        if spj_prev is not None:
+            assert not np.array_equal(spj, spj_prev)           # moments follow the particles
+        spj_prev = spj
+        c = f.get_counters()
+        padded0 = c["padded_entries"] if padded0 is None else padded0
+        assert c["padded_entries"] == padded0                  # lists untouched on reuse steps
+        a = out[:, :3].astype(np.float64)
+        if step > 0:
+            v += 0.5 * cfg.dt * a
+    f.close()
