@@ -1,19 +1,24 @@
 // Index-based multi-walk force kernel for sm_100a (paper: ForceKernelIndex,
 // P:557-569; multiwalk P:89; indirect addressing P:107).
 //
-// Mapping (DESIGN.md "Force kernel"):
-//   * work item = up to 64 consecutive i-particles of one group x the group's whole merged list; one WARP
-//     owns an item from start to end, so there is no block-level barrier and no atomics on the results.
+// Mapping (DESIGN.md section 6.1):
+//   * work item = 2W consecutive i-particles of one group (W = 32, 16, 8, 4 or 2) x the group's whole merged
+//     list; one WARP owns an item from start to end, so there is no block-level barrier and no atomics on
+//     the results.  Every lane holds TWO i-particles in registers (i = il and il + W, il = lane % W); the
+//     warp is split into S = 32 / W j-slices that share those i-particles and take every S-th j-pair
+//     (the north_star's "warp shuffles for splitting"); the slices' partial sums are combined by
+//     __shfl_xor at the end.  A group of n_i particles is cut on the host into 64-particle items plus
+//     power-of-two pieces, so that lanes are never padded by more than a few particles per group.
 //   * the warp streams the list in tiles of 64 entries: each lane reads two 4-byte indices (one coalesced
 //     256-B request per warp), gathers the two float4 (x,y,z,m) records through them and writes them to a
 //     warp-private shared-memory tile in PAIR layout [x0 x1 y0 y1][z0 z1 m0 m1]; the gathers of tile t+1
 //     and the indices of tile t+2 are in flight while tile t is swept.
-//   * every lane then sweeps the tile with broadcast LDS.128 and packed FP32 math (FADD2 / FMUL2 / FFMA2 of
-//     sm_100: two j per instruction), 13 packed FP32 ops + 2 MUFU.RSQ per i per j-pair.
-//   * lane utilisation: 64 i per item = 2 per lane; remainders of <= 32 / 16 / 8 particles run 1 per lane
-//     with the warp split into 1 / 2 / 4 j-slices whose partial sums are combined by warp shuffles.
-//   * accumulation is two-level (per-tile partial sums added into running totals, two independent sums
-//     per component from the j-pairing), which keeps the fp32 summation error far inside the tolerance.
+//   * every lane sweeps its slice of the tile with broadcast LDS.128 and packed FP32 math (FADD2 / FMUL2 /
+//     FFMA2 of sm_100: two j per instruction): 13 packed FP32 ops + 2 MUFU.RSQ per i per j-pair, which is
+//     exactly the paper's 23-flop interaction (3 sub, 3 fma, rsqrt, 3 mul, 3 fma, 1 add).
+//   * accumulation is two-level: partial sums over 32 j-pairs are added into running totals (two
+//     independent sums per component from the j-pairing), which keeps the fp32 summation error far inside
+//     the tolerance.
 //   * the self term (an i-particle meets itself in its own EPJ list) contributes exactly 0 to acc and
 //     m_i * rsqrt(eps^2) to the potential sum; the same value is subtracted up front (reading S2).
 #include "mwf_internal.h"
@@ -32,22 +37,40 @@ __device__ __forceinline__ int2 ld_stream_int2(const int2* p) {
     return v;
 }
 
-// Sweep one staged tile.  NI i-particles per lane; the lane belongs to slice `sl` of S and takes pairs
-// sl, sl + S, ...  Accumulates into the per-tile sums t* (two partial sums per component).
-template <int NI, int S>
+struct Acc2 {  // sums for the two i-particles of a lane; .x / .y halves are the two j of a pair
+    float2 x[2], y[2], z[2], p[2];
+};
+
+__device__ __forceinline__ void zero(Acc2& a) {
+#pragma unroll
+    for (int k = 0; k < 2; ++k) a.x[k] = a.y[k] = a.z[k] = a.p[k] = make_float2(0.f, 0.f);
+}
+
+__device__ __forceinline__ void add_into(Acc2& a, const Acc2& t) {
+#pragma unroll
+    for (int k = 0; k < 2; ++k) {
+        a.x[k] = __fadd2_rn(a.x[k], t.x[k]);
+        a.y[k] = __fadd2_rn(a.y[k], t.y[k]);
+        a.z[k] = __fadd2_rn(a.z[k], t.z[k]);
+        a.p[k] = __fadd2_rn(a.p[k], t.p[k]);
+    }
+}
+
+// Sweep one staged tile: the lane belongs to slice `sl` of S and takes pairs sl, sl + S, ... (W = 32 / S of them).
+template <int W>
 __device__ __forceinline__ void sweep_tile(const float4* __restrict__ sA, const float4* __restrict__ sB, int sl,
-                                           const float (&nx)[NI], const float (&ny)[NI], const float (&nz)[NI], float eps2,
-                                           float2 (&tx)[NI], float2 (&ty)[NI], float2 (&tz)[NI], float2 (&tp)[NI]) {
+                                           const float (&nx)[2], const float (&ny)[2], const float (&nz)[2], float eps2, Acc2& t) {
+    constexpr int S = 32 / W;
     const float2 e2 = make_float2(eps2, eps2);
-#pragma unroll 8
-    for (int pp = 0; pp < (TILE_J / 2) / S; ++pp) {
+#pragma unroll(W < 8 ? W : 8)
+    for (int pp = 0; pp < W; ++pp) {
         const int p = pp * S + sl;
         const float4 A = sA[p];
         const float4 B = sB[p];
         const float2 jx = make_float2(A.x, A.y), jy = make_float2(A.z, A.w);
         const float2 jz = make_float2(B.x, B.y), jm = make_float2(B.z, B.w);
 #pragma unroll
-        for (int k = 0; k < NI; ++k) {
+        for (int k = 0; k < 2; ++k) {
             const float2 dx = __fadd2_rn(jx, make_float2(nx[k], nx[k]));
             const float2 dy = __fadd2_rn(jy, make_float2(ny[k], ny[k]));
             const float2 dz = __fadd2_rn(jz, make_float2(nz[k], nz[k]));
@@ -58,28 +81,28 @@ __device__ __forceinline__ void sweep_tile(const float4* __restrict__ sA, const 
             ri.x = rsqrt_approx(r2.x);
             ri.y = rsqrt_approx(r2.y);
             const float2 mr = __fmul2_rn(jm, ri);
-            tp[k] = __fadd2_rn(tp[k], mr);
+            t.p[k] = __fadd2_rn(t.p[k], mr);
             const float2 ri2 = __fmul2_rn(ri, ri);
             const float2 mr3 = __fmul2_rn(mr, ri2);
-            tx[k] = __ffma2_rn(mr3, dx, tx[k]);
-            ty[k] = __ffma2_rn(mr3, dy, ty[k]);
-            tz[k] = __ffma2_rn(mr3, dz, tz[k]);
+            t.x[k] = __ffma2_rn(mr3, dx, t.x[k]);
+            t.y[k] = __ffma2_rn(mr3, dy, t.y[k]);
+            t.z[k] = __ffma2_rn(mr3, dz, t.z[k]);
         }
     }
 }
 
-template <int NI, int S>
+template <int W>
 __device__ __forceinline__ void run_item(const ForceArgs& a, const WorkItem it, float4* __restrict__ sbuf, int lane) {
-    constexpr int W = 32 / S;
+    constexpr int S = 32 / W;
     const int sl = lane / W;
     const int il = lane % W;
     const float4* __restrict__ J = a.store;
 
-    float nx[NI], ny[NI], nz[NI], mi[NI];
-    bool valid[NI];
+    float nx[2], ny[2], nz[2], mi[2];
+    bool valid[2];
 #pragma unroll
-    for (int k = 0; k < NI; ++k) {
-        const int off = il + 32 * k;
+    for (int k = 0; k < 2; ++k) {
+        const int off = il + W * k;
         valid[k] = off < it.n_i;
         const float4 p = __ldg(J + it.i_first + (valid[k] ? off : 0));
         nx[k] = -p.x; ny[k] = -p.y; nz[k] = -p.z; mi[k] = p.w;
@@ -87,22 +110,21 @@ __device__ __forceinline__ void run_item(const ForceArgs& a, const WorkItem it, 
     const float self_rinv = rsqrt_approx(a.eps2);  // what the sweep computes for d = 0
     const bool self_in = a.grp_self[it.group] != 0;
 
-    float2 ax[NI], ay[NI], az[NI], ap[NI];
+    Acc2 acc, part;
+    zero(acc);
+    zero(part);
+    // start the potential sum at minus the self term (slice 0 only: the slices are added later)
 #pragma unroll
-    for (int k = 0; k < NI; ++k) {
-        ax[k] = ay[k] = az[k] = make_float2(0.f, 0.f);
-        // start the potential sum at minus the self term (slice 0 only: the slices are added later)
-        ap[k] = make_float2((self_in && sl == 0) ? -mi[k] * self_rinv : 0.f, 0.f);
-    }
+    for (int k = 0; k < 2; ++k) acc.p[k].x = (self_in && sl == 0) ? -mi[k] * self_rinv : 0.f;
 
     const int64_t l0 = a.list_off[it.group];
     const int n_tiles = (int)((a.list_off[it.group + 1] - l0) / TILE_J);
     const int2* __restrict__ lst = reinterpret_cast<const int2*>(a.list + l0);
 
-    int2 id = make_int2(0, 0), idn = make_int2(0, 0);
+    int2 idn = make_int2(0, 0);
     float4 j0 = make_float4(0.f, 0.f, 0.f, 0.f), j1 = j0;
     if (n_tiles > 0) {
-        id = ld_stream_int2(lst + lane);
+        const int2 id = ld_stream_int2(lst + lane);
         j0 = __ldg(J + id.x);
         j1 = __ldg(J + id.y);
         if (n_tiles > 1) idn = ld_stream_int2(lst + 32 + lane);
@@ -118,35 +140,25 @@ __device__ __forceinline__ void run_item(const ForceArgs& a, const WorkItem it, 
             j1 = __ldg(J + idn.y);
             if (t + 2 < n_tiles) idn = ld_stream_int2(lst + (int64_t)(t + 2) * 32 + lane);
         }
-        float2 tx[NI], ty[NI], tz[NI], tp[NI];
-#pragma unroll
-        for (int k = 0; k < NI; ++k) tx[k] = ty[k] = tz[k] = tp[k] = make_float2(0.f, 0.f);
-        sweep_tile<NI, S>(sA, sB, sl, nx, ny, nz, a.eps2, tx, ty, tz, tp);
-#pragma unroll
-        for (int k = 0; k < NI; ++k) {
-            ax[k] = __fadd2_rn(ax[k], tx[k]);
-            ay[k] = __fadd2_rn(ay[k], ty[k]);
-            az[k] = __fadd2_rn(az[k], tz[k]);
-            ap[k] = __fadd2_rn(ap[k], tp[k]);
+        sweep_tile<W>(sA, sB, sl, nx, ny, nz, a.eps2, part);
+        if ((t & (S - 1)) == S - 1) {  // every partial sum covers 32 j-pairs whatever the slice count
+            add_into(acc, part);
+            zero(part);
         }
     }
+    add_into(acc, part);
 #pragma unroll
-    for (int k = 0; k < NI; ++k) {
-        float rx = ax[k].x + ax[k].y, ry = ay[k].x + ay[k].y, rz = az[k].x + az[k].y, rp = ap[k].x + ap[k].y;
-        if (S >= 4) {
-            rx += __shfl_xor_sync(0xffffffffu, rx, 8);
-            ry += __shfl_xor_sync(0xffffffffu, ry, 8);
-            rz += __shfl_xor_sync(0xffffffffu, rz, 8);
-            rp += __shfl_xor_sync(0xffffffffu, rp, 8);
-        }
-        if (S >= 2) {
-            rx += __shfl_xor_sync(0xffffffffu, rx, 16);
-            ry += __shfl_xor_sync(0xffffffffu, ry, 16);
-            rz += __shfl_xor_sync(0xffffffffu, rz, 16);
-            rp += __shfl_xor_sync(0xffffffffu, rp, 16);
+    for (int k = 0; k < 2; ++k) {
+        float rx = acc.x[k].x + acc.x[k].y, ry = acc.y[k].x + acc.y[k].y, rz = acc.z[k].x + acc.z[k].y, rp = acc.p[k].x + acc.p[k].y;
+#pragma unroll
+        for (int m = W; m < 32; m <<= 1) {
+            rx += __shfl_xor_sync(0xffffffffu, rx, m);
+            ry += __shfl_xor_sync(0xffffffffu, ry, m);
+            rz += __shfl_xor_sync(0xffffffffu, rz, m);
+            rp += __shfl_xor_sync(0xffffffffu, rp, m);
         }
         if (valid[k] && sl == 0)
-            a.accp[it.i_first + il + 32 * k] = make_float4(a.G * rx, a.G * ry, a.G * rz, -a.G * rp);
+            a.accp[it.i_first + il + W * k] = make_float4(a.G * rx, a.G * ry, a.G * rz, -a.G * rp);
     }
     __syncwarp();  // the next item reuses the warp's tile buffers
 }
@@ -161,11 +173,12 @@ __global__ void __launch_bounds__(WARPS_PER_CTA * 32, 2) k_force(const ForceArgs
     while (w < a.n_items) {
         const int64_t pos = a.item_begin + w;
         const WorkItem it = a.items[a.order ? a.order[pos] : pos];
-        switch (it.kind) {
-            case 0: run_item<2, 1>(a, it, sbuf, lane); break;
-            case 1: run_item<1, 1>(a, it, sbuf, lane); break;
-            case 2: run_item<1, 2>(a, it, sbuf, lane); break;
-            default: run_item<1, 4>(a, it, sbuf, lane); break;
+        switch (it.width) {
+            case 32: run_item<32>(a, it, sbuf, lane); break;
+            case 16: run_item<16>(a, it, sbuf, lane); break;
+            case 8: run_item<8>(a, it, sbuf, lane); break;
+            case 4: run_item<4>(a, it, sbuf, lane); break;
+            default: run_item<2>(a, it, sbuf, lane); break;
         }
         if (a.counter) {  // dynamic: next unclaimed item
             unsigned int nxt = 0;

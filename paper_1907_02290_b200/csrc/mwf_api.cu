@@ -1,6 +1,7 @@
 // Host side of libmwf.so: the C ABI of include/mwf.h -- device store, list-reuse driver (SURVEY.md
 // section 8(a) rows a1, a2, a5, a6, a7) and the launches of the kernels in this directory.
 #include <algorithm>
+#include <climits>
 #include <cstdio>
 #include <cstring>
 #include <new>
@@ -88,7 +89,7 @@ struct Layout {
     }
 };
 
-int64_t max_items_of(const mwf_params& p) { return p.max_ptcl / CHUNK_I + 2 * p.max_group + 8; }
+int64_t max_items_of(const mwf_params& p) { return p.max_ptcl / CHUNK_I + 5 * p.max_group + 8; }
 
 Layout make_layout(const mwf_params& p) {
     Layout L;
@@ -153,10 +154,25 @@ void drop_lists(mwf_ctx* c) {
     c->groups_dispatched = 0;
 }
 
-// cost of an item in sweep units (j-pairs x i per lane): what the longest-first schedule sorts by
-inline int64_t item_cost(const WorkItem& it, int64_t n_tiles) {
-    static const int64_t per_tile[4] = {64, 32, 16, 8};
-    return n_tiles * per_tile[it.kind];
+// Work order of items [b, e) of `order`: longest first (so the tail of the launch is made of short items),
+// except that the NARROW items (width <= 8: few j-pairs per staged tile, so they wait on the gathers rather
+// than on the FP32 pipe) are spread evenly over the first 7/8 of the schedule, where the wide items of the
+// other warps of the SM keep the pipe busy meanwhile.
+void schedule_items(std::vector<int32_t>& order, int64_t b, int64_t e, const std::vector<WorkItem>& items, const std::vector<int64_t>& cost) {
+    auto longer = [&](int32_t x, int32_t y) { return cost[(size_t)x] > cost[(size_t)y]; };
+    std::vector<int32_t> wide, narrow;
+    for (int64_t k = b; k < e; ++k) (items[(size_t)order[(size_t)k]].width > 8 ? wide : narrow).push_back(order[(size_t)k]);
+    std::stable_sort(wide.begin(), wide.end(), longer);
+    std::stable_sort(narrow.begin(), narrow.end(), longer);
+    const size_t nw = wide.size(), nn = narrow.size();
+    const size_t span = nw - nw / 8;  // narrow items go between the first `span` wide items
+    size_t iw = 0, in = 0;
+    int64_t k = b;
+    while (iw < nw || in < nn) {
+        // keep in / nn ~ iw / span
+        const bool take_narrow = in < nn && (iw >= nw || (span > 0 ? in * span <= iw * nn : true) || iw >= span);
+        order[(size_t)k++] = take_narrow ? narrow[in++] : wide[iw++];
+    }
 }
 
 }  // namespace
@@ -346,7 +362,7 @@ int mwf_set_lists(mwf_ctx* c, int64_t n_group, const int32_t* grp_first, const i
     c->h_inter.assign((size_t)n_group + 1, 0);
     std::vector<WorkItem> items;
     std::vector<int64_t> cost;
-    items.reserve((size_t)(c->n_ptcl / CHUNK_I + 2 * n_group));
+    items.reserve((size_t)(c->n_ptcl / CHUNK_I + 3 * n_group));
     for (int64_t g = 0; g < n_group; ++g) {
         const int64_t ne = epj_off[g + 1] - epj_off[g], ns = spj_off[g + 1] - spj_off[g];
         if (ne < 0 || ns < 0) return MWF_ERANGE;
@@ -356,29 +372,45 @@ int mwf_set_lists(mwf_ctx* c, int64_t n_group, const int32_t* grp_first, const i
         const int64_t n_tiles = (n_list + TILE_J - 1) / TILE_J;
         list_off[(size_t)g + 1] = list_off[(size_t)g] + n_tiles * TILE_J;
         c->h_inter[(size_t)g + 1] = c->h_inter[(size_t)g] + gn * n_list;
-        int64_t done = 0;
-        while (done < gn) {
-            const int64_t rem = gn - done;
-            WorkItem it;
-            it.i_first = (int32_t)(gf + done);
-            it.group = (int32_t)g;
-            if (rem >= CHUNK_I) { it.n_i = CHUNK_I; it.kind = 0; }
-            else if (rem > 32) { it.n_i = 32; it.kind = 1; }
-            else if (rem > 16) { it.n_i = (int32_t)rem; it.kind = 1; }
-            else if (rem > 8) { it.n_i = (int32_t)rem; it.kind = 2; }
-            else { it.n_i = (int32_t)rem; it.kind = 3; }
-            done += it.n_i;
-            items.push_back(it);
-            cost.push_back(item_cost(it, n_tiles));
+        // Cut the group into items: whole 64-particle items, then power-of-two pieces of the remainder
+        // padded to a multiple of q; q is the quantum whose modelled cost is lowest (a coarser quantum
+        // wastes lanes, a finer one re-stages the list for one more narrow item).
+        {
+            const int64_t n_full = gn / CHUNK_I, rem = gn % CHUNK_I;
+            int64_t best_q = CHUNK_I, best_cost = INT64_MAX;
+            for (int64_t q = 2 * MIN_WIDTH; q <= CHUNK_I && rem > 0; q *= 2) {
+                const int64_t padded = (rem + q - 1) / q * q;
+                int64_t cst = 0;
+                for (int64_t piece = CHUNK_I; piece >= 2 * MIN_WIDTH; piece /= 2)
+                    if (padded & piece) cst += item_cost_per_tile((int)(piece / 2));
+                if (cst < best_cost) { best_cost = cst; best_q = q; }
+            }
+            int64_t done = 0;
+            auto emit = [&](int64_t n_i, int width) {
+                WorkItem it;
+                it.i_first = (int32_t)(gf + done);
+                it.n_i = (int32_t)n_i;
+                it.group = (int32_t)g;
+                it.width = width;
+                done += n_i;
+                items.push_back(it);
+                cost.push_back(n_tiles * item_cost_per_tile(width));
+            };
+            for (int64_t k = 0; k < n_full; ++k) emit(CHUNK_I, CHUNK_I / 2);
+            if (rem > 0) {
+                const int64_t padded = (rem + best_q - 1) / best_q * best_q;
+                for (int64_t piece = CHUNK_I; piece >= 2 * MIN_WIDTH; piece /= 2)
+                    if (padded & piece) emit(std::min(piece, gn - done), (int)(piece / 2));
+            }
         }
         c->h_item_off[(size_t)g + 1] = (int64_t)items.size();
     }
     const int64_t n_items = (int64_t)items.size();
     if (n_items > c->max_items) return MWF_ENOMEM;
-    // longest-first schedules: over everything, and inside each of the n_tag balanced group ranges
+    // work schedules (see schedule_items): over everything, and inside each of the n_tag balanced group ranges
     std::vector<int32_t> order_full((size_t)n_items), order_split((size_t)n_items);
     std::iota(order_full.begin(), order_full.end(), 0);
-    std::stable_sort(order_full.begin(), order_full.end(), [&](int32_t x, int32_t y) { return cost[(size_t)x] > cost[(size_t)y]; });
+    schedule_items(order_full, 0, n_items, items, cost);
     c->h_split.assign((size_t)c->p.n_tag + 1, 0);
     {
         const int64_t total = c->h_inter[(size_t)n_group];
@@ -392,8 +424,7 @@ int mwf_set_lists(mwf_ctx* c, int64_t n_group, const int32_t* grp_first, const i
         std::iota(order_split.begin(), order_split.end(), 0);
         for (int t = 0; t < c->p.n_tag; ++t) {
             const int64_t b = c->h_item_off[(size_t)c->h_split[(size_t)t]], e = c->h_item_off[(size_t)c->h_split[(size_t)t + 1]];
-            std::stable_sort(order_split.begin() + b, order_split.begin() + e,
-                             [&](int32_t x, int32_t y) { return cost[(size_t)x] > cost[(size_t)y]; });
+            schedule_items(order_split, b, e, items, cost);
         }
     }
     cudaStream_t s = static_cast<cudaStream_t>(stream);

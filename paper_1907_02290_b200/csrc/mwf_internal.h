@@ -13,16 +13,23 @@ namespace mwf {
 constexpr int TILE_J = 64;          // j entries staged per warp tile; merged lists are padded to this
 constexpr int WARPS_PER_CTA = 8;    // force kernel block = 256 threads
 constexpr int CHUNK_I = 64;         // i-particles of a full work item (2 per lane)
+constexpr int MIN_WIDTH = 2;        // narrowest item: 2 lanes x 2 i-particles, 16 j-slices
 
-// One unit of work for one warp: up to 64 consecutive i-particles of one group against its whole list.
-// kind 0: 64 particles, 2 per lane.  kind 1/2/3: <= 32 / 16 / 8 particles, 1 per lane, the warp split
-// into 1 / 2 / 4 slices that share the i-particles and take every 1st / 2nd / 4th j-pair.
+// One unit of work for one warp: n_i <= 2 * width consecutive i-particles of one group against the
+// group's whole list.  width = 32, 16, 8, 4 or 2 lanes hold the i-particles (2 per lane); the warp is
+// split into 32 / width slices that share them and take every (32 / width)-th j-pair.
 struct WorkItem {
     int32_t i_first;
     int32_t n_i;
     int32_t group;
-    int32_t kind;
+    int32_t width;
 };
+
+// Modelled cost of an item per list tile, in issue cycles of its warp: staging + width j-pairs x 2 i.
+// Used on the host to cut groups into items and to order the items longest-first.
+constexpr int64_t COST_STAGE = 40;
+constexpr int64_t COST_PAIR = 33;
+inline int64_t item_cost_per_tile(int width) { return COST_STAGE + COST_PAIR * width; }
 
 struct ForceArgs {
     const float4* store;        // particles then SPJ then one zero-mass dummy
