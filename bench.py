@@ -275,6 +275,27 @@ def main():
     for k, name in enumerate(("upload_d2d", "monopole_refresh", "force_kernel", "retrieve_d2d")):
         phases[name + "_ms"] = round(ev[k].elapsed_time(ev[k + 1]), 4)
 
+    # ---- NEXT-1: device-resident reuse steps (kick-drift, refresh, force, kick; no host transfer)
+    dev_res = None
+    if w.vel is not None and cfg.dt > 0:
+        vel4 = np.zeros((w.n, 4), np.float32)
+        vel4[:, :3] = w.vel
+        f.set_velocities(vel4)
+        f.begin_step(binding.REUSE_LIST)
+        f.calc_force_all(src_dev, dst_dev)
+        for _ in range(2):
+            f.step_reuse(cfg.dt)
+        torch.cuda.synchronize()
+        d0, d1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        d0.record(f.streams[0])
+        for _ in range(args.steps):
+            f.step_reuse(cfg.dt)
+        d1.record(f.streams[0])
+        torch.cuda.synchronize()
+        ms_dr = d0.elapsed_time(d1) / args.steps
+        dev_res = {"ms_per_step": ms_dr, "value": inter / (ms_dr * 1e-3), "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0,
+                   "step": "mwf_step_reuse: kick-drift, monopole refresh, force kernel, kick, all on the device (dt = %g)" % cfg.dt}
+
     if rank == 0:
         peaks = measured_peaks()
         clk = clocks.summary()
@@ -285,7 +306,11 @@ def main():
         achieved = N_OP * inter / (k_ms * 1e-3) / 1e12
         traffic = None
         try:
-            traffic = json.load(open(os.path.join(ROOT, "profiles", "force_kernel_traffic.json"))).get(cfg.name)
+            # ncu dram__bytes_read.sum + dram__bytes_write.sum per k_force launch: "config_name bytes" lines
+            for line in open(os.path.join(ROOT, "profiles", "force_kernel_traffic.txt")):
+                parts = line.split("#", 1)[0].split()
+                if len(parts) == 2 and parts[0] == cfg.name:
+                    traffic = float(parts[1])
         except (OSError, ValueError):
             pass
         roof = {"bound": "alu", "kernel": "mwf::k_force", "achieved": achieved, "peak": peak_tflops, "unit": "TFLOP/s",
@@ -308,7 +333,7 @@ def main():
             "roofline": roof, "cpu_baseline": cpu,
             "e2e": {"value": e2e_value, "unit": UNIT, "h2d_bytes_per_step": 16 * w.n, "d2h_bytes_per_step": 16 * w.n,
                     "ms_per_step": ms_e_max / args.steps},
-            "gpu_launches": launches, "clocks": clk, "phases": phases,
+            "gpu_launches": launches, "clocks": clk, "phases": phases, "device_resident_step": dev_res,
             "construction_step": {"host_tree_and_lists_s": round(t_build, 3), "upload_tree_and_lists_s": round(t_upload, 3)},
             "context": {"paper_fraction_of_peak": 0.27, "paper_hardware": "TITAN V (P:673), whole step"},
         }

@@ -9,6 +9,7 @@
  *   (4) dispatch the force kernel        P:89 multiwalk, "dispatch", P:557-569 ForceKernelIndex
  *   (5) retrieve acc and pot             P:189 "retrieve", P:595-663 RetrieveKernel
  *   list reuse                           P:115-143, P:242 MAKE_LIST / MAKE_LIST_FOR_REUSE / REUSE_LIST
+ *   device-resident reuse step           P:1171-1185 section 7.3 "implement all procedures on the accelerator"
  *
  * Conventions common to every call
  *   - Return value: 0 (MWF_OK) on success, a negative MWF_E* code otherwise (the paper's callbacks return 0,
@@ -45,6 +46,8 @@ typedef struct mwf_ctx mwf_ctx; /* opaque */
 typedef struct { float x, y, z, m; } mwf_posm;
 /* FORCE on the device: float4 (ax, ay, az, pot), 16 B. */
 typedef struct { float ax, ay, az, pot; } mwf_accp;
+/* Velocity on the device: float4 (vx, vy, vz, unused), 16 B so that it moves with vector loads. */
+typedef struct { float vx, vy, vz, pad; } mwf_vel;
 /* Tree cell: particle range [first_ptcl, first_ptcl + n_ptcl) in tree order and child range
  * [first_child, first_child + n_child) in the cell array (n_child == 0: leaf).  Cell 0 is the root and
  * covers [0, N).  Children of a cell are stored contiguously, after their parent (level order),
@@ -141,6 +144,26 @@ int mwf_retrieve(mwf_ctx* c, int32_t tag, mwf_accp* dst, int dst_on_device);
  * whose tree and lists are already on the device: upload all N particles (src HOST or DEVICE; NULL = keep
  * the store), refresh, dispatch all groups split over the tags, retrieve everything into dst. */
 int mwf_calc_force_all(mwf_ctx* c, const mwf_posm* src, int src_on_device, mwf_accp* dst, int dst_on_device);
+
+/* ---- Device-resident reuse step (the paper's own conclusion, P:1171-1185:
+ * with the lists resident the per-step host<->device transfers of particles and forces are what is left,
+ * so the orbit integration (the paper's step 5) moves to the device as well).  Kick-drift-kick
+ * leapfrog in fp32 on the store (reading S14b of DESIGN.md):
+ *     mwf_kick_drift:  v += acc * dt/2 ;  x += v * dt        (marks the monopoles stale)
+ *     mwf_kick:        v += acc * dt/2
+ * acc is the result array of the last evaluation, read in place; both calls return MWF_ESTATE unless
+ * every group has been dispatched since the positions last changed and velocities for all N particles
+ * have been uploaded.  Asynchronous on `stream`; ordered after the force kernels by the library. */
+
+/* Upload / read back velocities [first, first + n), tree order.  src/dst HOST or DEVICE. */
+int mwf_set_velocities(mwf_ctx* c, const mwf_vel* src, int64_t first, int64_t n, int src_on_device, void* stream);
+int mwf_get_velocities(mwf_ctx* c, mwf_vel* dst, int64_t first, int64_t n, int dst_on_device);
+int mwf_kick_drift(mwf_ctx* c, float dt, void* stream);
+int mwf_kick(mwf_ctx* c, float dt, void* stream);
+/* One whole list-reuse step with no host transfer, all on the stream of tag 0 and non-blocking:
+ * begin_step(MWF_REUSE_LIST), kick_drift(dt), refresh_monopoles, dispatch of all groups, kick(dt).
+ * mwf_retrieve(c, 0, ...) afterwards copies out acc+pot of all particles; mwf_sync() just waits. */
+int mwf_step_reuse(mwf_ctx* c, float dt);
 
 /* Test hooks: monopoles as stored (float4 per cell) and device-side results without a copy. */
 int mwf_get_monopoles(mwf_ctx* c, mwf_posm* dst, int dst_on_device);

@@ -21,6 +21,10 @@
  *                  for EPJ and SPJ, the entry whose INDEX equals i is skipped (a different particle
  *                  at the same position is a real pair), pot <= 0 and includes G.
  *   orc_direct     the plain O(N^2) definition of the same sum over all other particles.
+ *   orc_kick_drift, orc_kick   the kick-drift-kick leapfrog BASELINE.json's config 5 names (the orbit
+ *                  integration is step 5 of the paper's procedure; section 7.3, P:1171-1185,
+ *                  proposes moving it to the accelerator): v += a dt/2, x += v dt; and v += a dt/2.
+ *                  In fp64 from fp32 inputs (reading S14b in DESIGN.md).
  *
  * Inputs are the fp32 particle array exactly as uploaded to the GPU; every value is widened to
  * double before any arithmetic.  OpenMP only distributes groups / particles over threads; each
@@ -132,4 +136,21 @@ void orc_direct(int64_t n, const float* posm, double eps, double G, double* acc,
         acc[3 * i + 2] = G * az;
         pot[i] = G * p;
     }
+}
+
+/* Kick-drift of the leapfrog: vout = v + a dt/2, xout = x + vout dt.  posm: 4 floats per particle (x,y,z,m);
+ * vel4 and accp4: 4 floats per particle (3 used).  Outputs 3 doubles per particle. */
+void orc_kick_drift(int64_t n, const float* posm, const float* vel4, const float* accp4, double dt, double* xout, double* vout) {
+    for (int64_t i = 0; i < n; ++i)
+        for (int d = 0; d < 3; ++d) {
+            double v = (double)vel4[4 * i + d] + (double)accp4[4 * i + d] * (0.5 * dt);
+            vout[3 * i + d] = v;
+            xout[3 * i + d] = (double)posm[4 * i + d] + v * dt;
+        }
+}
+
+/* Closing half kick: vout = v + a dt/2. */
+void orc_kick(int64_t n, const float* vel4, const float* accp4, double dt, double* vout) {
+    for (int64_t i = 0; i < n; ++i)
+        for (int d = 0; d < 3; ++d) vout[3 * i + d] = (double)vel4[4 * i + d] + (double)accp4[4 * i + d] * (0.5 * dt);
 }

@@ -33,6 +33,8 @@ def _load():
         lib.orc_monopoles.argtypes = [i64, vp, vp, vp]
         lib.orc_forces.argtypes = [i64, vp, vp, vp, vp, vp, vp, vp, vp, vp, dbl, dbl, vp, vp]
         lib.orc_direct.argtypes = [i64, vp, dbl, dbl, vp, vp]
+        lib.orc_kick_drift.argtypes = [i64, vp, vp, vp, dbl, vp, vp]
+        lib.orc_kick.argtypes = [i64, vp, vp, dbl, vp]
         _lib = lib
     return _lib
 
@@ -92,3 +94,21 @@ def direct(posm, eps: float, G: float = 1.0):
     pot = np.empty(n)
     _load().orc_direct(n, _p(posm), float(eps), float(G), _p(acc), _p(pot))
     return acc, pot
+
+
+def kick_drift(posm, vel4, accp4, dt: float):
+    """Leapfrog kick-drift in fp64 from fp32 state: returns (x[N,3], v[N,3]) with v = v + a dt/2, x = x + v dt."""
+    posm, vel4, accp4 = _c(posm, np.float32), _c(vel4, np.float32), _c(accp4, np.float32)
+    n = posm.shape[0]
+    x, v = np.empty((n, 3)), np.empty((n, 3))
+    _load().orc_kick_drift(n, _p(posm), _p(vel4), _p(accp4), float(dt), _p(x), _p(v))
+    return x, v
+
+
+def kick(vel4, accp4, dt: float):
+    """Closing half kick in fp64 from fp32 state: v[N,3] = v + a dt/2."""
+    vel4, accp4 = _c(vel4, np.float32), _c(accp4, np.float32)
+    n = vel4.shape[0]
+    v = np.empty((n, 3))
+    _load().orc_kick(n, _p(vel4), _p(accp4), float(dt), _p(v))
+    return v

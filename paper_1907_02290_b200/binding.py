@@ -23,6 +23,7 @@ SYMBOLS = (
     "mwf_set_tree", "mwf_set_lists", "mwf_begin_step", "mwf_refresh_monopoles", "mwf_dispatch", "mwf_retrieve",
     "mwf_calc_force_all", "mwf_get_monopoles", "mwf_device_pointers", "mwf_sync", "mwf_get_counters",
     "mwf_last_dispatch_ms", "mwf_strerror", "mwf_last_cuda_error",
+    "mwf_set_velocities", "mwf_get_velocities", "mwf_kick_drift", "mwf_kick", "mwf_step_reuse",
 )
 
 
@@ -46,7 +47,7 @@ def load_library(path: str | None = None) -> ctypes.CDLL:
     if _lib is not None and path is None:
         return _lib
     if path is None:
-        path = os.path.join(os.path.dirname(os.path.abspath(__file__)), "csrc", "libmwf.so")
+        path = os.environ.get("MWF_LIBRARY") or os.path.join(os.path.dirname(os.path.abspath(__file__)), "csrc", "libmwf.so")
         if not os.path.exists(path):
             path = _build.build_mwf()
     lib = ctypes.CDLL(path)
@@ -71,6 +72,11 @@ def load_library(path: str | None = None) -> ctypes.CDLL:
         "mwf_sync": [vp],
         "mwf_get_counters": [vp, P(i64), P(i64), P(i64)],
         "mwf_last_dispatch_ms": [vp, i32, P(ctypes.c_float)],
+        "mwf_set_velocities": [vp, vp, i64, i64, ci, vp],
+        "mwf_get_velocities": [vp, vp, i64, i64, ci],
+        "mwf_kick_drift": [vp, ctypes.c_float, vp],
+        "mwf_kick": [vp, ctypes.c_float, vp],
+        "mwf_step_reuse": [vp, ctypes.c_float],
     }
     for name, args in sig.items():
         fn = getattr(lib, name)
@@ -200,6 +206,26 @@ class MultiWalkForce:
             sp, s_dev = _ptr(src, np.float32, "src")
         dp, d_dev = _ptr(dst, np.float32, "dst")
         self._ck(self._lib.mwf_calc_force_all(self._h, sp, s_dev, dp, d_dev))
+
+    def set_velocities(self, src, first: int = 0, n: int | None = None, stream=None):
+        p, on_dev = _ptr(src, np.float32, "src")
+        if n is None:
+            n = int(src.shape[0])
+        self._ck(self._lib.mwf_set_velocities(self._h, p, int(first), int(n), on_dev, _stream_handle(stream)))
+
+    def get_velocities(self, first: int, n: int) -> np.ndarray:
+        out = np.empty((n, 4), np.float32)
+        self._ck(self._lib.mwf_get_velocities(self._h, _host_ptr(out, np.float32, "dst"), int(first), int(n), 0))
+        return out
+
+    def kick_drift(self, dt: float, stream=None):
+        self._ck(self._lib.mwf_kick_drift(self._h, float(dt), _stream_handle(stream)))
+
+    def kick(self, dt: float, stream=None):
+        self._ck(self._lib.mwf_kick(self._h, float(dt), _stream_handle(stream)))
+
+    def step_reuse(self, dt: float):
+        self._ck(self._lib.mwf_step_reuse(self._h, float(dt)))
 
     def get_monopoles(self, n_cell: int) -> np.ndarray:
         out = np.empty((n_cell, 4), np.float32)

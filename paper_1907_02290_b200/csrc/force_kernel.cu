@@ -62,7 +62,8 @@ __device__ __forceinline__ void sweep_tile(const float4* __restrict__ sA, const 
                                            const float (&nx)[2], const float (&ny)[2], const float (&nz)[2], float eps2, Acc2& t) {
     constexpr int S = 32 / W;
     const float2 e2 = make_float2(eps2, eps2);
-#pragma unroll(W < 8 ? W : 8)
+    constexpr int UNROLL = W < MWF_UNROLL_WIDE ? W : MWF_UNROLL_WIDE;
+#pragma unroll UNROLL
     for (int pp = 0; pp < W; ++pp) {
         const int p = pp * S + sl;
         const float4 A = sA[p];
@@ -141,7 +142,8 @@ __device__ __forceinline__ void run_item(const ForceArgs& a, const WorkItem it, 
             if (t + 2 < n_tiles) idn = ld_stream_int2(lst + (int64_t)(t + 2) * 32 + lane);
         }
         sweep_tile<W>(sA, sB, sl, nx, ny, nz, a.eps2, part);
-        if ((t & (S - 1)) == S - 1) {  // every partial sum covers 32 j-pairs whatever the slice count
+        constexpr int FLUSH = S > MWF_FLUSH_MIN ? S : MWF_FLUSH_MIN;
+        if ((t & (FLUSH - 1)) == FLUSH - 1) {  // every partial sum covers 32 j-pairs whatever the slice count
             add_into(acc, part);
             zero(part);
         }
@@ -163,7 +165,7 @@ __device__ __forceinline__ void run_item(const ForceArgs& a, const WorkItem it, 
     __syncwarp();  // the next item reuses the warp's tile buffers
 }
 
-__global__ void __launch_bounds__(WARPS_PER_CTA * 32, 2) k_force(const ForceArgs a) {
+__global__ void __launch_bounds__(WARPS_PER_CTA * 32, MWF_MIN_CTAS) k_force(const ForceArgs a) {
     __shared__ float4 s_tiles[WARPS_PER_CTA][2 * TILE_J];
     const int lane = threadIdx.x & 31;
     const int warp = threadIdx.x >> 5;

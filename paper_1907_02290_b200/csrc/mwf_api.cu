@@ -20,6 +20,7 @@ struct mwf_ctx {
     // carved device arrays
     float4* store = nullptr;      // [max_ptcl + max_cell + 1]
     float4* accp = nullptr;       // [max_ptcl]
+    float4* vel = nullptr;        // [max_ptcl] (vx, vy, vz, unused): device-resident integration
     mwf_cell* cells = nullptr;    // [max_cell]
     int32_t* parent = nullptr;    // [max_cell]
     int32_t* arrive = nullptr;    // [max_cell]
@@ -39,6 +40,8 @@ struct mwf_ctx {
     // state
     int64_t n_ptcl = 0, n_cell = 0, n_group = 0, n_items = 0, ptcl_hi = 0, padded_entries = 0;
     bool have_tree = false, have_lists = false, lists_for_reuse = false, mono_fresh = false;
+    bool acc_full = false;   // every group has been dispatched since the positions last changed
+    int64_t vel_hi = 0;      // velocities [0, vel_hi) have been uploaded
     std::vector<int64_t> h_item_off, h_inter, h_split;  // per group prefix of items / interactions; split group bounds
     std::vector<int32_t> h_grp_first, h_grp_n;
     int64_t groups_outstanding = 0;  // MAKE_LIST: groups dispatched and not yet retrieved
@@ -113,6 +116,7 @@ Layout make_layout(const mwf_params& p) {
     L.add(mi * 4);                                      // 16 order_split
     L.add(N_COUNTER * 4);                               // 17 counters
     L.add(256);                                         // 18 err
+    L.add(p.max_ptcl * 16);                             // 19 vel
     return L;
 }
 
@@ -152,6 +156,7 @@ void drop_lists(mwf_ctx* c) {
     c->n_group = 0;
     c->n_items = 0;
     c->groups_dispatched = 0;
+    c->acc_full = false;
 }
 
 // Work order of items [b, e) of `order`: longest first (so the tail of the launch is made of short items),
@@ -249,6 +254,7 @@ int mwf_create(mwf_ctx** out, const mwf_params* p, void* arena, int64_t arena_by
     c->order_split = (int32_t*)(b + L.off[16]);
     c->counters = (unsigned int*)(b + L.off[17]);
     c->err = (unsigned int*)(b + L.off[18]);
+    c->vel = (float4*)(b + L.off[19]);
     c->max_items = max_items_of(*p);
     c->tag_groups.assign(MWF_MAX_TAG, 0);
     bool ok = true;
@@ -303,6 +309,7 @@ int mwf_set_particles(mwf_ctx* c, const mwf_posm* src, int64_t first, int64_t n,
     c->ptcl_hi = std::max(c->ptcl_hi, first + n);
     if (c->have_tree) c->ptcl_hi = std::min(c->ptcl_hi, c->n_ptcl);
     c->mono_fresh = false;
+    c->acc_full = false;
     return after_store_op(c, s);
 }
 
@@ -547,6 +554,7 @@ int mwf_dispatch(mwf_ctx* c, int32_t tag, int64_t g_begin, int64_t g_end) {
     c->tag_groups[(size_t)tag] += g_end - g_begin;
     c->groups_dispatched += g_end - g_begin;
     c->groups_outstanding += g_end - g_begin;
+    if (c->groups_dispatched >= c->n_group) c->acc_full = true;
     return MWF_OK;
 }
 
@@ -610,6 +618,76 @@ int mwf_calc_force_all(mwf_ctx* c, const mwf_posm* src, int src_on_device, mwf_a
         if (rc) return rc;
     }
     return MWF_OK;
+}
+
+int mwf_set_velocities(mwf_ctx* c, const mwf_vel* src, int64_t first, int64_t n, int src_on_device, void* stream) {
+    if (!c || !src || first < 0 || n < 0) return MWF_EINVAL;
+    if (first + n > c->p.max_ptcl) return MWF_ENOMEM;
+    if (n == 0) return MWF_OK;
+    cudaStream_t s = static_cast<cudaStream_t>(stream);
+    int rc = before_store_op(c, s);
+    if (rc) return rc;
+    CU(c, cudaMemcpyAsync(c->vel + first, src, (size_t)n * 16, src_on_device ? cudaMemcpyDeviceToDevice : cudaMemcpyHostToDevice, s));
+    if (first <= c->vel_hi) c->vel_hi = std::max(c->vel_hi, first + n);
+    return after_store_op(c, s);
+}
+
+int mwf_get_velocities(mwf_ctx* c, mwf_vel* dst, int64_t first, int64_t n, int dst_on_device) {
+    if (!c || !dst || first < 0 || n < 0 || first + n > c->p.max_ptcl) return MWF_EINVAL;
+    CU(c, cudaDeviceSynchronize());
+    CU(c, cudaMemcpy(dst, c->vel + first, (size_t)n * 16, dst_on_device ? cudaMemcpyDeviceToDevice : cudaMemcpyDeviceToHost));
+    return MWF_OK;
+}
+
+static int integrate_ready(mwf_ctx* c, float dt) {
+    if (!c || !(dt == dt)) return MWF_EINVAL;
+    if (!c->have_tree || !c->have_lists || !c->acc_full || c->vel_hi < c->n_ptcl) return MWF_ESTATE;
+    return MWF_OK;
+}
+
+int mwf_kick_drift(mwf_ctx* c, float dt, void* stream) {
+    int rc = integrate_ready(c, dt);
+    if (rc) return rc;
+    cudaStream_t s = static_cast<cudaStream_t>(stream);
+    rc = before_store_op(c, s);  // waits for the force kernels that read the store and write accp
+    if (rc) return rc;
+    CU(c, launch_kick_drift(c->store, c->vel, c->accp, c->n_ptcl, dt, s));
+    ++c->n_launch;
+    c->mono_fresh = false;
+    c->acc_full = false;
+    return after_store_op(c, s);
+}
+
+int mwf_kick(mwf_ctx* c, float dt, void* stream) {
+    int rc = integrate_ready(c, dt);
+    if (rc) return rc;
+    cudaStream_t s = static_cast<cudaStream_t>(stream);
+    rc = before_store_op(c, s);
+    if (rc) return rc;
+    CU(c, launch_kick(c->vel, c->accp, c->n_ptcl, dt, s));
+    ++c->n_launch;
+    return after_store_op(c, s);
+}
+
+int mwf_step_reuse(mwf_ctx* c, float dt) {
+    int rc = integrate_ready(c, dt);
+    if (rc) return rc;
+    for (int t = 1; t < c->p.n_tag; ++t)
+        if (!c->tag_ranges[t].empty()) return MWF_ESTATE;  // results of another tag not retrieved
+    rc = mwf_begin_step(c, MWF_REUSE_LIST);
+    if (rc) return rc;
+    cudaStream_t s0 = c->tag_stream[0];
+    rc = mwf_kick_drift(c, dt, s0);
+    if (rc) return rc;
+    rc = mwf_refresh_monopoles(c, s0);
+    if (rc) return rc;
+    // results stay on the device: forget what earlier steps left for tag 0, a later retrieve copies all N
+    c->groups_outstanding -= c->tag_groups[0];
+    c->tag_groups[0] = 0;
+    c->tag_ranges[0].clear();
+    rc = mwf_dispatch(c, 0, 0, c->n_group);
+    if (rc) return rc;
+    return mwf_kick(c, dt, s0);
 }
 
 int mwf_get_monopoles(mwf_ctx* c, mwf_posm* dst, int dst_on_device) {

@@ -27,7 +27,19 @@ struct WorkItem {
 
 // Modelled cost of an item per list tile, in issue cycles of its warp: staging + width j-pairs x 2 i.
 // Used on the host to cut groups into items and to order the items longest-first.
-constexpr int64_t COST_STAGE = 40;
+#ifndef MWF_COST_STAGE
+#define MWF_COST_STAGE 40
+#endif
+#ifndef MWF_UNROLL_WIDE
+#define MWF_UNROLL_WIDE 16
+#endif
+#ifndef MWF_FLUSH_MIN
+#define MWF_FLUSH_MIN 2
+#endif
+#ifndef MWF_MIN_CTAS
+#define MWF_MIN_CTAS 2
+#endif
+constexpr int64_t COST_STAGE = MWF_COST_STAGE;
 constexpr int64_t COST_PAIR = 33;
 inline int64_t item_cost_per_tile(int width) { return COST_STAGE + COST_PAIR * width; }
 
@@ -57,6 +69,9 @@ cudaError_t launch_monopoles(const mwf_cell* cells, const int32_t* parent, int64
 cudaError_t launch_merge_lists(int64_t n_group, const int32_t* grp_first, const int32_t* grp_n, const int64_t* epj_off,
                                const int32_t* epj_id, const int64_t* spj_off, const int32_t* spj_id, const int64_t* list_off,
                                int64_t n_ptcl, int64_t n_cell, int32_t* list, uint8_t* grp_self, unsigned int* err, cudaStream_t s);
+
+cudaError_t launch_kick_drift(float4* store, float4* vel, const float4* accp, int64_t n, float dt, cudaStream_t s);
+cudaError_t launch_kick(float4* vel, const float4* accp, int64_t n, float dt, cudaStream_t s);
 
 // bits of the device-side validation word
 enum : unsigned int {

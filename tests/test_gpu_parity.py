@@ -371,3 +371,95 @@ def test_reuse_run_per_step():
         if step > 0:
             v += 0.5 * cfg.dt * a
     f.close()
+
+
+# ------------------------------------------------------------------ NEXT-1: device-resident reuse steps
+def _vel4(v):
+    out = np.zeros((v.shape[0], 4), np.float32)
+    out[:, :3] = v
+    return out
+
+
+def test_device_resident_reuse_run():
+    """Config 5 at reduced N with the orbit integration on the device (paper section 7.3):
+    lists built once, then 8 x mwf_step_reuse = kick-drift, monopole refresh, force over all groups, kick,
+    with no host transfer in the step.  After every step the state is read back and compared with the
+    oracle: the leapfrog update in fp64 from the previous fp32 state (within fp32 rounding of one FMA per
+    component), and the forces on exactly the fp32 positions the device now holds (north_star tolerances)."""
+    cfg = CONFIGS[4]
+    w = make_workload(cfg, 30000)
+    dt = cfg.dt
+    f = binding.MultiWalkForce.for_workload(w, n_tag=2)
+    f.upload_workload(w, binding.MAKE_LIST_FOR_REUSE)
+    assert expect_code(f.step_reuse, dt) == binding.ESTATE          # no evaluation yet, no velocities
+    f.refresh_monopoles()
+    f.dispatch(0, 0, w.n_group)
+    out = np.zeros((w.n, 4), np.float32)
+    f.retrieve(0, out)
+    assert expect_code(f.kick, dt) == binding.ESTATE                # velocities missing
+    f.set_velocities(_vel4(w.vel))
+    x_prev, v_prev, a_prev = f.get_particles(0, w.n), f.get_velocities(0, w.n), out.copy()
+    assert np.array_equal(x_prev, w.posm)
+    for step in range(1, cfg.n_reuse + 1):
+        f.step_reuse(dt)
+        f.retrieve(0, out)                                          # waits for the step, copies acc + pot
+        x_now, v_now = f.get_particles(0, w.n), f.get_velocities(0, w.n)
+        # leapfrog parity
+        x_or, vh_or = oracle.kick_drift(x_prev, v_prev, a_prev, dt)
+        tol_x = 2.0 ** -23 * (np.abs(x_or) + dt * np.abs(vh_or)) + 1e-30
+        assert np.all(np.abs(x_now[:, :3] - x_or) <= tol_x), "drift, step %d" % step
+        assert np.array_equal(x_now[:, 3], w.posm[:, 3])            # masses untouched
+        vh32 = _vel4(vh_or.astype(np.float32))
+        v_or = oracle.kick(vh32, out, dt)
+        tol_v = 2.0 ** -22 * (np.abs(v_or) + 0.5 * dt * np.abs(out[:, :3])) + 1e-30
+        assert np.all(np.abs(v_now[:, :3] - v_or) <= tol_v), "kick, step %d" % step
+        # force parity on the positions the device holds
+        acc, pot, mom = oracle_eval(w, cfg.eps, posm=x_now)
+        check(out, acc, pot, label="device-resident step %d" % step)
+        spj = f.get_monopoles(w.n_cell)
+        assert np.all(np.abs(spj[:, 3] - mom[:, 3]) <= 1e-6 * mom[:, 3])
+        x_prev, v_prev, a_prev = x_now, v_now, out.copy()
+    assert expect_code(f.kick_drift, float("nan")) == binding.EINVAL
+    f.set_particles(w.posm)                                         # positions changed: forces are stale
+    assert expect_code(f.kick_drift, dt) == binding.ESTATE
+    f.close()
+
+
+def test_device_resident_matches_host_driven_run():
+    """The same 4 steps driven from the host in fp32 (upload positions each step) and on the device give
+    bitwise identical forces when the host performs the identical fp32 FMAs: the device integrator adds
+    nothing but the update itself."""
+    cfg = CONFIGS[4]
+    w = make_workload(cfg, 20000)
+    dt = np.float32(cfg.dt)
+    f = binding.MultiWalkForce.for_workload(w, n_tag=2)
+    f.upload_workload(w, binding.MAKE_LIST_FOR_REUSE)
+    f.refresh_monopoles()
+    f.dispatch(0, 0, w.n_group)
+    out = np.zeros((w.n, 4), np.float32)
+    f.retrieve(0, out)
+    f.set_velocities(_vel4(w.vel))
+    for _ in range(4):
+        f.step_reuse(float(dt))
+    f.retrieve(0, out)
+    x_dev = f.get_particles(0, w.n)
+    g = binding.MultiWalkForce.for_workload(w, n_tag=2)
+    g.upload_workload(w, binding.MAKE_LIST_FOR_REUSE)
+    g.refresh_monopoles()
+    g.dispatch(0, 0, w.n_group)
+    ref = np.zeros((w.n, 4), np.float32)
+    g.retrieve(0, ref)
+    posm = w.posm.copy()
+    v = w.vel.astype(np.float32)
+    h = np.float32(0.5) * dt
+    fma = lambda a, b, c: (a.astype(np.float64) * np.float64(b) + c.astype(np.float64)).astype(np.float32)  # exact product, one rounding
+    for _ in range(4):
+        v = fma(ref[:, :3], h, v)
+        posm[:, :3] = fma(v, dt, posm[:, :3])
+        g.begin_step(binding.REUSE_LIST)
+        g.calc_force_all(posm, ref)
+        v = fma(ref[:, :3], h, v)
+    assert np.array_equal(x_dev, posm)
+    assert np.array_equal(out, ref)
+    f.close()
+    g.close()

@@ -240,3 +240,52 @@ def test_monopole_invariants():
     mom0, mom1 = oracle.monopoles(w.cells, q0), oracle.monopoles(w.cells, q1)
     assert np.array_equal(mom1[:, 3], mom0[:, 3])
     np.testing.assert_allclose(mom1[:, :3] - t, mom0[:, :3], atol=1e-12)
+
+
+# ---------------------------------------------------------------- leapfrog (NEXT-1): closed forms
+def _kdk(x, v, acc_of, dt, steps):
+    """Drive oracle.kick_drift / oracle.kick; the accelerations come from the test (acc_of), fp32 state."""
+    x = x.astype(np.float32); v = v.astype(np.float32)
+    a = acc_of(x.astype(np.float64)).astype(np.float32)
+    for _ in range(steps):
+        posm = np.concatenate([x, np.ones((len(x), 1), np.float32)], axis=1)
+        v4 = np.concatenate([v, np.zeros((len(x), 1), np.float32)], axis=1)
+        a4 = np.concatenate([a, np.zeros((len(x), 1), np.float32)], axis=1)
+        xn, vh = oracle.kick_drift(posm, v4, a4, dt)
+        x = xn.astype(np.float32); vh = vh.astype(np.float32)
+        a = acc_of(x.astype(np.float64)).astype(np.float32)
+        v4 = np.concatenate([vh, np.zeros((len(x), 1), np.float32)], axis=1)
+        a4 = np.concatenate([a, np.zeros((len(x), 1), np.float32)], axis=1)
+        v = oracle.kick(v4, a4, dt).astype(np.float32)
+    return x.astype(np.float64), v.astype(np.float64)
+
+
+def test_leapfrog_constant_acceleration_is_exact():
+    """Uniform acceleration g: one kick-drift-kick step gives x0 + v0 dt + g dt^2/2 and v0 + g dt exactly
+    (catches a missing 1/2, a drift that uses the old velocity, a kick applied twice).  Dyadic values:
+    every operation is exact in fp32, so equality is bitwise."""
+    x0 = np.array([[1.0, -2.0, 0.5], [0.25, 4.0, -8.0]])
+    v0 = np.array([[0.5, 0.25, -1.0], [2.0, -0.5, 0.125]])
+    g = np.array([0.5, -2.0, 4.0])
+    dt = 0.25
+    x, v = _kdk(x0, v0, lambda x: np.broadcast_to(g, x.shape), dt, 1)
+    assert np.array_equal(x, x0 + v0 * dt + 0.5 * g * dt * dt)
+    assert np.array_equal(v, v0 + g * dt)
+    x, v = _kdk(x0, v0, lambda x: np.broadcast_to(g, x.shape), dt, 4)
+    assert np.array_equal(x, x0 + v0 * (4 * dt) + 0.5 * g * (4 * dt) ** 2)
+    assert np.array_equal(v, v0 + g * (4 * dt))
+
+
+def test_leapfrog_harmonic_oscillator_second_order_and_reversible():
+    """a = -x: the exact solution is (cos t, -sin t).  The scheme must converge with order 2 (halving dt
+    quarters the error) and be time-reversible: running back with -dt returns to the start."""
+    x0 = np.array([[1.0, 0.0, 0.0]]); v0 = np.array([[0.0, 0.0, 0.0]])
+    errs = []
+    for steps in (16, 32, 64):
+        dt = 1.0 / steps
+        x, v = _kdk(x0, v0, lambda x: -x, dt, steps)
+        errs.append(math.hypot(x[0, 0] - math.cos(1.0), v[0, 0] + math.sin(1.0)))
+    assert 3.5 < errs[0] / errs[1] < 4.5 and 3.5 < errs[1] / errs[2] < 4.5
+    x, v = _kdk(x0, v0, lambda x: -x, 1.0 / 64, 64)
+    xb, vb = _kdk(x, v, lambda x: -x, -1.0 / 64, 64)
+    assert abs(xb[0, 0] - 1.0) < 1e-5 and abs(vb[0, 0]) < 1e-5
