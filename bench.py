@@ -296,6 +296,28 @@ def main():
         dev_res = {"ms_per_step": ms_dr, "value": inter / (ms_dr * 1e-3), "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0,
                    "step": "mwf_step_reuse: kick-drift, monopole refresh, force kernel, kick, all on the device (dt = %g)" % cfg.dt}
 
+    # ---- NEXT-2: the construction step on the device (sort, tree, groups, lists) from unsorted particles
+    dev_build = None
+    try:
+        from paper_1907_02290_b200.workload import make_particles
+        posm0, _ = make_particles(cfg, args.n)
+        f.begin_step(binding.MAKE_LIST_FOR_REUSE)
+        f.set_particles(posm0)
+        f.sync()
+        tb = []
+        for _ in range(3):
+            f.set_particles(posm0)
+            f.sync()
+            t = time.perf_counter()
+            f.build(w.n, cfg.n_leaf, cfg.n_grp, cfg.theta, binding.MAKE_LIST_FOR_REUSE)
+            f.sync()
+            tb.append(time.perf_counter() - t)
+        sz = f.get_build_sizes()
+        dev_build = {"device_build_s": round(min(tb), 4), "n_cell": sz["n_cell"], "n_group": sz["n_group"], "entries": sz["n_epj"] + sz["n_spj"],
+                     "same_as_host_builder": bool(sz["n_cell"] == w.n_cell and sz["n_group"] == w.n_group and sz["n_epj"] + sz["n_spj"] == w.n_entry)}
+    except binding.MwfError as ex:
+        dev_build = {"error": str(ex)}
+
     if rank == 0:
         peaks = measured_peaks()
         clk = clocks.summary()
@@ -334,7 +356,7 @@ def main():
             "e2e": {"value": e2e_value, "unit": UNIT, "h2d_bytes_per_step": 16 * w.n, "d2h_bytes_per_step": 16 * w.n,
                     "ms_per_step": ms_e_max / args.steps},
             "gpu_launches": launches, "clocks": clk, "phases": phases, "device_resident_step": dev_res,
-            "construction_step": {"host_tree_and_lists_s": round(t_build, 3), "upload_tree_and_lists_s": round(t_upload, 3)},
+            "construction_step": {"host_tree_and_lists_s": round(t_build, 3), "upload_tree_and_lists_s": round(t_upload, 3), "on_device": dev_build},
             "context": {"paper_fraction_of_peak": 0.27, "paper_hardware": "TITAN V (P:673), whole step"},
         }
         print(json.dumps(out), flush=True)

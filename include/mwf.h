@@ -145,6 +145,27 @@ int mwf_retrieve(mwf_ctx* c, int32_t tag, mwf_accp* dst, int dst_on_device);
  * the store), refresh, dispatch all groups split over the tags, retrieve everything into dst. */
 int mwf_calc_force_all(mwf_ctx* c, const mwf_posm* src, int src_on_device, mwf_accp* dst, int dst_on_device);
 
+/* ---- Device-side construction step (paper P:149-172: root cell, Morton keys,
+ * radix sort, reorder, cells linked level by level, one tree walk per i-group emitting an index list).  Works on
+ * the particles [0, n) currently in the store, in ANY order: sorts them (and the velocities, when all n have been
+ * uploaded) into tree order in place, builds cells, groups and lists on the device and leaves the ctx in the
+ * state mwf_set_tree() + mwf_set_lists(mode) leave it in.  Readings O1-O4 of DESIGN.md (the same as the host
+ * builder's): cube root cell padded by 2^-10, 21 key bits per axis, leaf = at most n_leaf particles, group =
+ * first cell on a root path with at most n_grp particles, open iff cell side > theta x distance from the cell
+ * centre to the group's particle bounding box.  theta in [0, 1].  Results of the previous step must have been
+ * retrieved (MWF_ESTATE otherwise).  MWF_ENOMEM when max_cell / max_group / max_entry are too small.  Blocking
+ * (a few stream synchronisations to size the levels and the lists). */
+int mwf_build(mwf_ctx* c, int64_t n, int32_t n_leaf, int32_t n_grp, double theta, int mode, void* stream);
+/* Sizes of what mwf_build() made. */
+int mwf_get_build_sizes(mwf_ctx* c, int64_t* n_cell, int64_t* n_group, int64_t* n_epj, int64_t* n_spj, int32_t* n_level);
+/* perm[p] = index, in the order the particles were uploaded, of the particle now at tree position p. */
+int mwf_get_permutation(mwf_ctx* c, int32_t* perm, int dst_on_device);
+/* Read-back hooks (HOST destinations): cells (n_cell records) and their geometry (centre x,y,z and side, fp64;
+ * only for a device-built tree); group ranges; the lists in the CSR form mwf_set_lists() takes. */
+int mwf_get_tree(mwf_ctx* c, mwf_cell* cells, double* geom4);
+int mwf_get_groups(mwf_ctx* c, int32_t* grp_first, int32_t* grp_n);
+int mwf_get_lists(mwf_ctx* c, int64_t* epj_off, int32_t* epj_id, int64_t* spj_off, int32_t* spj_id);
+
 /* ---- Device-resident reuse step (the paper's own conclusion, P:1171-1185:
  * with the lists resident the per-step host<->device transfers of particles and forces are what is left,
  * so the orbit integration (the paper's step 5) moves to the device as well).  Kick-drift-kick

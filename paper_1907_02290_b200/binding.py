@@ -24,6 +24,7 @@ SYMBOLS = (
     "mwf_calc_force_all", "mwf_get_monopoles", "mwf_device_pointers", "mwf_sync", "mwf_get_counters",
     "mwf_last_dispatch_ms", "mwf_strerror", "mwf_last_cuda_error",
     "mwf_set_velocities", "mwf_get_velocities", "mwf_kick_drift", "mwf_kick", "mwf_step_reuse",
+    "mwf_build", "mwf_get_build_sizes", "mwf_get_permutation", "mwf_get_tree", "mwf_get_groups", "mwf_get_lists",
 )
 
 
@@ -77,6 +78,12 @@ def load_library(path: str | None = None) -> ctypes.CDLL:
         "mwf_kick_drift": [vp, ctypes.c_float, vp],
         "mwf_kick": [vp, ctypes.c_float, vp],
         "mwf_step_reuse": [vp, ctypes.c_float],
+        "mwf_build": [vp, i64, i32, i32, ctypes.c_double, ci, vp],
+        "mwf_get_build_sizes": [vp, P(i64), P(i64), P(i64), P(i64), P(i32)],
+        "mwf_get_permutation": [vp, vp, ci],
+        "mwf_get_tree": [vp, vp, vp],
+        "mwf_get_groups": [vp, vp, vp],
+        "mwf_get_lists": [vp, vp, vp, vp, vp],
     }
     for name, args in sig.items():
         fn = getattr(lib, name)
@@ -226,6 +233,39 @@ class MultiWalkForce:
 
     def step_reuse(self, dt: float):
         self._ck(self._lib.mwf_step_reuse(self._h, float(dt)))
+
+    def build(self, n: int, n_leaf: int, n_grp: int, theta: float, mode: int = MAKE_LIST_FOR_REUSE, stream=None):
+        self._ck(self._lib.mwf_build(self._h, int(n), int(n_leaf), int(n_grp), float(theta), int(mode), _stream_handle(stream)))
+
+    def get_build_sizes(self):
+        a, b, c, d = (ctypes.c_int64(0) for _ in range(4))
+        e = ctypes.c_int32(0)
+        self._ck(self._lib.mwf_get_build_sizes(self._h, ctypes.byref(a), ctypes.byref(b), ctypes.byref(c), ctypes.byref(d), ctypes.byref(e)))
+        return dict(n_cell=a.value, n_group=b.value, n_epj=c.value, n_spj=d.value, n_level=e.value)
+
+    def get_permutation(self, n: int) -> np.ndarray:
+        out = np.empty(n, np.int32)
+        self._ck(self._lib.mwf_get_permutation(self._h, _host_ptr(out, np.int32, "perm"), 0))
+        return out
+
+    def get_tree(self, n_cell: int, with_geom: bool = True):
+        cells = np.empty((n_cell, 4), np.int32)
+        geom = np.empty((n_cell, 4), np.float64) if with_geom else None
+        self._ck(self._lib.mwf_get_tree(self._h, _host_ptr(cells, np.int32, "cells"),
+                                        _host_ptr(geom, np.float64, "geom") if with_geom else ctypes.c_void_p(None)))
+        return cells, geom
+
+    def get_groups(self, n_group: int):
+        gf, gn = np.empty(n_group, np.int32), np.empty(n_group, np.int32)
+        self._ck(self._lib.mwf_get_groups(self._h, _host_ptr(gf, np.int32, "grp_first"), _host_ptr(gn, np.int32, "grp_n")))
+        return gf, gn
+
+    def get_lists(self, n_group: int, n_epj: int, n_spj: int):
+        eo, so = np.empty(n_group + 1, np.int64), np.empty(n_group + 1, np.int64)
+        ei, si = np.empty(max(1, n_epj), np.int32), np.empty(max(1, n_spj), np.int32)
+        self._ck(self._lib.mwf_get_lists(self._h, _host_ptr(eo, np.int64, "epj_off"), _host_ptr(ei, np.int32, "epj_id"),
+                                         _host_ptr(so, np.int64, "spj_off"), _host_ptr(si, np.int32, "spj_id")))
+        return eo, ei[:n_epj], so, si[:n_spj]
 
     def get_monopoles(self, n_cell: int) -> np.ndarray:
         out = np.empty((n_cell, 4), np.float32)

@@ -1,0 +1,203 @@
+// Device-side construction step, part 2: one tree walk per i-group emitting its interaction list as indices
+// (paper: Barnes' vectorisation, one traversal per group of particles and one
+// shared list; for the index method the list holds indices).
+//
+// Reading O4 / S6-S7 of DESIGN.md, identical to the host builder: for a cell of side l and geometric centre s,
+// d = distance from s to the group's tight particle bounding box (0 inside); OPEN iff l > theta * d, evaluated
+// as l*l > theta^2 * d^2 in fp64 with explicitly rounded operations.  Opened internal cell -> its children are
+// visited; opened leaf -> its particles join the EPJ list; cell not opened -> it joins the SPJ list.
+//
+// One WARP per group, groups claimed from an atomic counter.  The warp keeps a LIFO stack of cell indices in
+// global memory (L2-resident scratch, one slab per warp), pops up to 32 cells per round, tests one per lane and
+// compacts the three outcomes with ballots / warp prefix sums.  At most 256 cells of any one level are ever on
+// the stack, so 22 levels x 256 entries bound it.  The walk runs twice: a counting pass (n_epj, n_spj per group)
+// and, after the offsets have been scanned, a fill pass that writes the merged, padded list the force kernel
+// reads: EPJ ids, then SPJ ids + N, then the dummy index up to a multiple of 64 (P:441-477 layout).
+#include "mwf_internal.h"
+#include "scan_sort.cuh"
+
+namespace mwf {
+
+namespace {
+
+template <bool FILL>
+__global__ void __launch_bounds__(256) k_walk(const mwf_cell* __restrict__ cells, const double4* __restrict__ geom, const float* __restrict__ grp_box,
+                                              int64_t n_group, double th2, int32_t* __restrict__ stacks, unsigned int* __restrict__ counter,
+                                              int32_t* __restrict__ n_epj, int32_t* __restrict__ n_spj, const int64_t* __restrict__ list_off,
+                                              int32_t* __restrict__ list, int32_t n_ptcl, int32_t dummy) {
+    const int lane = threadIdx.x & 31;
+    const unsigned lt = (1u << lane) - 1u;
+    const int64_t warp_global = ((int64_t)blockIdx.x * blockDim.x + threadIdx.x) >> 5;
+    int32_t* __restrict__ stack = stacks + warp_global * WALK_STACK;
+    for (;;) {
+        unsigned int gi = 0;
+        if (lane == 0) gi = atomicAdd(counter, 1u);
+        const int64_t g = __shfl_sync(0xffffffffu, gi, 0);
+        if (g >= n_group) break;
+        double lo[3], hi[3];
+#pragma unroll
+        for (int a = 0; a < 3; ++a) {
+            lo[a] = (double)grp_box[g * 6 + a];
+            hi[a] = (double)grp_box[g * 6 + 3 + a];
+        }
+        int64_t off_e = 0, off_s = 0;
+        if (FILL) {
+            off_e = list_off[g];
+            off_s = off_e + n_epj[g];
+        }
+        int ne = 0, ns = 0, sp = 1;
+        if (lane == 0) stack[0] = 0;
+        __syncwarp();
+        while (sp > 0) {
+            const int take = sp < 32 ? sp : 32;
+            sp -= take;
+            const int c = lane < take ? stack[sp + lane] : -1;
+            __syncwarp();
+            int kind = 0;  // 1: SPJ, 2: opened internal cell, 3: opened leaf
+            mwf_cell cc = {0, 0, 0, 0};
+            if (c >= 0) {
+                cc = cells[c];
+                const double4 gm = geom[c];
+                const double s3[3] = {gm.x, gm.y, gm.z};
+                double d2 = 0.0;
+#pragma unroll
+                for (int a = 0; a < 3; ++a) {
+                    double d = 0.0;
+                    if (s3[a] < lo[a]) d = __dsub_rn(lo[a], s3[a]);
+                    else if (s3[a] > hi[a]) d = __dsub_rn(s3[a], hi[a]);
+                    d2 = __dadd_rn(d2, __dmul_rn(d, d));
+                }
+                const bool open = __dmul_rn(gm.w, gm.w) > __dmul_rn(th2, d2);
+                kind = !open ? 1 : (cc.n_child == 0 ? 3 : 2);
+            }
+            // SPJ entries
+            const unsigned m_s = __ballot_sync(0xffffffffu, kind == 1);
+            if (FILL && kind == 1) list[off_s + ns + __popc(m_s & lt)] = n_ptcl + c;
+            ns += __popc(m_s);
+            // opened leaves: their particles
+            const unsigned m_l = __ballot_sync(0xffffffffu, kind == 3);
+            if (m_l) {
+                int cnt = kind == 3 ? cc.n_ptcl : 0, incl = cnt;
+#pragma unroll
+                for (int d = 1; d < 32; d <<= 1) {
+                    const int up = __shfl_up_sync(0xffffffffu, incl, d);
+                    if (lane >= d) incl += up;
+                }
+                const int total = __shfl_sync(0xffffffffu, incl, 31);
+                if (FILL) {
+                    const int excl = incl - cnt;
+                    unsigned m = m_l;
+                    while (m) {
+                        const int src = __ffs(m) - 1;
+                        m &= m - 1;
+                        const int first = __shfl_sync(0xffffffffu, cc.first_ptcl, src);
+                        const int n_in = __shfl_sync(0xffffffffu, cnt, src);
+                        const int base = __shfl_sync(0xffffffffu, excl, src);
+                        for (int k = lane; k < n_in; k += 32) list[off_e + ne + base + k] = first + k;
+                    }
+                }
+                ne += total;
+            }
+            // opened internal cells: push their children
+            const unsigned m_o = __ballot_sync(0xffffffffu, kind == 2);
+            if (m_o) {
+                int cnt = kind == 2 ? cc.n_child : 0, incl = cnt;
+#pragma unroll
+                for (int d = 1; d < 32; d <<= 1) {
+                    const int up = __shfl_up_sync(0xffffffffu, incl, d);
+                    if (lane >= d) incl += up;
+                }
+                const int total = __shfl_sync(0xffffffffu, incl, 31);
+                const int excl = incl - cnt;
+                for (int k = 0; k < cnt; ++k) stack[sp + excl + k] = cc.first_child + k;
+                sp += total;
+            }
+            __syncwarp();
+        }
+        if (FILL) {  // pad to whole tiles with the zero-mass dummy record
+            const int64_t end = list_off[g + 1];
+            for (int64_t k = off_e + ne + ns + lane; k < end; k += 32) list[k] = dummy;
+        } else if (lane == 0) {
+            n_epj[g] = ne;
+            n_spj[g] = ns;
+        }
+    }
+}
+
+// list_off[g] (to be scanned) = padded length of group g's merged list
+__global__ void __launch_bounds__(256) k_padded_len(const int32_t* __restrict__ n_epj, const int32_t* __restrict__ n_spj, int64_t n_group,
+                                                    int64_t* __restrict__ list_off, int64_t* __restrict__ epj_off, int64_t* __restrict__ spj_off) {
+    const int64_t g = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (g > n_group) return;
+    if (g == n_group) { list_off[g] = 0; epj_off[g] = 0; spj_off[g] = 0; return; }
+    const int64_t len = (int64_t)n_epj[g] + n_spj[g];
+    list_off[g] = (len + TILE_J - 1) / TILE_J * TILE_J;
+    epj_off[g] = n_epj[g];
+    spj_off[g] = n_spj[g];
+}
+
+// merged list -> the two CSR id arrays of the upload interface (read-back hook)
+__global__ void __launch_bounds__(256) k_unmerge(const int32_t* __restrict__ list, const int64_t* __restrict__ list_off, const int64_t* __restrict__ epj_off,
+                                                 const int64_t* __restrict__ spj_off, int64_t n_group, int32_t n_ptcl, int32_t* __restrict__ epj_id,
+                                                 int32_t* __restrict__ spj_id) {
+    for (int64_t g = blockIdx.x; g < n_group; g += gridDim.x) {
+        const int64_t l0 = list_off[g], e0 = epj_off[g], ne = epj_off[g + 1] - e0, s0 = spj_off[g], ns = spj_off[g + 1] - s0;
+        for (int64_t k = threadIdx.x; k < ne; k += blockDim.x) epj_id[e0 + k] = list[l0 + k];
+        for (int64_t k = threadIdx.x; k < ns; k += blockDim.x) spj_id[s0 + k] = list[l0 + ne + k] - n_ptcl;
+    }
+}
+
+}  // namespace
+
+#define BL(call)                                \
+    do {                                        \
+        cudaError_t e__ = (call);               \
+        if (e__ != cudaSuccess) return e__;     \
+    } while (0)
+
+int64_t walk_warps(int64_t max_group) {
+    const int64_t cap = 148 * 16;
+    return max_group < cap ? (max_group < 8 ? 8 : (max_group + 7) / 8 * 8) : cap;
+}
+
+// Counting pass + offsets.  Leaves list_off / epj_off / spj_off scanned (n_group + 1 entries each) and returns the
+// totals through *padded / *e_epj / *e_spj (one stream synchronisation).
+cudaError_t build_lists_count(const BuildBuffers& b, int64_t n_group, double theta, int64_t n_warps, int64_t* padded, int64_t* e_epj, int64_t* e_spj,
+                              cudaStream_t s) {
+    const double th2 = theta * theta;
+    BL(cudaMemsetAsync(b.walk_counter, 0, 4, s));
+    k_walk<false><<<(unsigned)(n_warps / 8), 256, 0, s>>>(b.cells, b.geom, b.grp_box, n_group, th2, b.walk_stacks, b.walk_counter, b.n_epj, b.n_spj,
+                                                          nullptr, nullptr, 0, 0);
+    BL(cudaGetLastError());
+    k_padded_len<<<(unsigned)((n_group + 1 + 255) / 256), 256, 0, s>>>(b.n_epj, b.n_spj, n_group, b.list_off, b.epj_off, b.spj_off);
+    BL(cudaGetLastError());
+    BL(scan_exclusive<int64_t>(b.list_off, n_group + 1, b.scan_scratch64, s));
+    BL(scan_exclusive<int64_t>(b.epj_off, n_group + 1, b.scan_scratch64, s));
+    BL(scan_exclusive<int64_t>(b.spj_off, n_group + 1, b.scan_scratch64, s));
+    int64_t h[3] = {0, 0, 0};
+    BL(cudaMemcpyAsync(&h[0], b.list_off + n_group, 8, cudaMemcpyDeviceToHost, s));
+    BL(cudaMemcpyAsync(&h[1], b.epj_off + n_group, 8, cudaMemcpyDeviceToHost, s));
+    BL(cudaMemcpyAsync(&h[2], b.spj_off + n_group, 8, cudaMemcpyDeviceToHost, s));
+    BL(cudaStreamSynchronize(s));
+    *padded = h[0];
+    *e_epj = h[1];
+    *e_spj = h[2];
+    return cudaSuccess;
+}
+
+cudaError_t build_lists_fill(const BuildBuffers& b, int64_t n_group, double theta, int64_t n_warps, int64_t n_ptcl, int64_t n_cell, cudaStream_t s) {
+    const double th2 = theta * theta;
+    BL(cudaMemsetAsync(b.walk_counter, 0, 4, s));
+    k_walk<true><<<(unsigned)(n_warps / 8), 256, 0, s>>>(b.cells, b.geom, b.grp_box, n_group, th2, b.walk_stacks, b.walk_counter, b.n_epj, b.n_spj,
+                                                         b.list_off, b.list, (int32_t)n_ptcl, (int32_t)(n_ptcl + n_cell));
+    return cudaGetLastError();
+}
+
+cudaError_t unmerge_lists(const BuildBuffers& b, int64_t n_group, int64_t n_ptcl, int32_t* epj_id, int32_t* spj_id, cudaStream_t s) {
+    if (n_group <= 0) return cudaSuccess;
+    const int64_t grid = n_group < 148 * 16 ? n_group : 148 * 16;
+    k_unmerge<<<(unsigned)grid, 256, 0, s>>>(b.list, b.list_off, b.epj_off, b.spj_off, n_group, (int32_t)n_ptcl, epj_id, spj_id);
+    return cudaGetLastError();
+}
+
+}  // namespace mwf

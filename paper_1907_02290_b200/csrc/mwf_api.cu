@@ -8,6 +8,7 @@
 #include <numeric>
 
 #include "mwf_internal.h"
+#include "scan_sort.cuh"
 
 using namespace mwf;
 
@@ -40,6 +41,11 @@ struct mwf_ctx {
     // state
     int64_t n_ptcl = 0, n_cell = 0, n_group = 0, n_items = 0, ptcl_hi = 0, padded_entries = 0;
     bool have_tree = false, have_lists = false, lists_for_reuse = false, mono_fresh = false;
+    BuildBuffers bb{};       // device-side construction step (NEXT-2)
+    int64_t walk_warps_n = 0;
+    bool built_on_device = false;
+    int64_t build_e_epj = 0, build_e_spj = 0;
+    int32_t build_n_level = 0;
     bool acc_full = false;   // every group has been dispatched since the positions last changed
     int64_t vel_hi = 0;      // velocities [0, vel_hi) have been uploaded
     std::vector<int64_t> h_item_off, h_inter, h_split;  // per group prefix of items / interactions; split group bounds
@@ -82,7 +88,7 @@ int cuda_fail(mwf_ctx* c, cudaError_t e, const char* what) {
 inline int64_t up(int64_t x, int64_t a) { return (x + a - 1) / a * a; }
 
 struct Layout {
-    int64_t off[32];
+    int64_t off[48];
     int n = 0;
     int64_t total = 0;
     int64_t add(int64_t bytes) {
@@ -117,6 +123,27 @@ Layout make_layout(const mwf_params& p) {
     L.add(N_COUNTER * 4);                               // 17 counters
     L.add(256);                                         // 18 err
     L.add(p.max_ptcl * 16);                             // 19 vel
+    // device-side construction step (NEXT-2)
+    const int64_t nsb = sort_blocks(p.max_ptcl);
+    const int64_t scan_n = std::max<int64_t>(std::max<int64_t>(256 * nsb + 1, p.max_ptcl + 2), p.max_cell + 2);
+    L.add(p.max_ptcl * 8);                              // 20 key_a
+    L.add(p.max_ptcl * 8);                              // 21 key_b
+    L.add(p.max_ptcl * 4);                              // 22 idx_a (the permutation after a build)
+    L.add(p.max_ptcl * 4);                              // 23 idx_b
+    L.add((256 * nsb + 1) * 4);                         // 24 hist
+    L.add(scan_scratch_elems(scan_n) * 4);              // 25 scan_scratch (int32)
+    L.add(scan_scratch_elems(p.max_group + 2) * 8);     // 26 scan_scratch64
+    L.add(148 * 4 * 6 * 4);                             // 27 bbox_part
+    L.add(8 * 8);                                       // 28 root
+    L.add(p.max_cell * 32);                             // 29 geom
+    L.add((p.max_cell + 2) * 4);                        // 30 level_cnt
+    L.add((p.max_ptcl + 2) * 4);                        // 31 mark
+    L.add(p.max_group * 4);                             // 32 grp_cell
+    L.add(p.max_group * 24);                            // 33 grp_box
+    L.add(p.max_group * 4);                             // 34 n_epj
+    L.add(p.max_group * 4);                             // 35 n_spj
+    L.add(walk_warps(p.max_group) * WALK_STACK * 4);    // 36 walk_stacks
+    L.add(256);                                         // 37 walk_counter
     return L;
 }
 
@@ -178,6 +205,100 @@ void schedule_items(std::vector<int32_t>& order, int64_t b, int64_t e, const std
         const bool take_narrow = in < nn && (iw >= nw || (span > 0 ? in * span <= iw * nn : true) || iw >= span);
         order[(size_t)k++] = take_narrow ? narrow[in++] : wide[iw++];
     }
+}
+
+// Host-side work plan of one set of lists: per-group list offsets (padded to tiles), work items, the two
+// schedules, and the per-group prefix sums the dispatcher needs.  Used by mwf_set_lists (lists from the host)
+// and by mwf_build (lists made on the device; only their lengths come back).
+struct Plan {
+    std::vector<int64_t> list_off, item_off, inter, split;
+    std::vector<WorkItem> items;
+    std::vector<int32_t> order_full, order_split;
+};
+
+int make_plan(mwf_ctx* c, int64_t n_group, const int32_t* grp_first, const int32_t* grp_n, const int64_t* n_list_of, Plan& pl) {
+    pl.list_off.assign((size_t)n_group + 1, 0);
+    pl.item_off.assign((size_t)n_group + 1, 0);
+    pl.inter.assign((size_t)n_group + 1, 0);
+    std::vector<WorkItem>& items = pl.items;
+    std::vector<int64_t> cost;
+    items.reserve((size_t)(c->n_ptcl / CHUNK_I + 3 * n_group));
+    for (int64_t g = 0; g < n_group; ++g) {
+        const int64_t gf = grp_first[g], gn = grp_n[g];
+        if (gf < 0 || gn < 1 || gf + gn > c->n_ptcl) return MWF_ERANGE;
+        const int64_t n_list = n_list_of[g];
+        const int64_t n_tiles = (n_list + TILE_J - 1) / TILE_J;
+        pl.list_off[(size_t)g + 1] = pl.list_off[(size_t)g] + n_tiles * TILE_J;
+        pl.inter[(size_t)g + 1] = pl.inter[(size_t)g] + gn * n_list;
+        // Cut the group into items: whole 64-particle items, then power-of-two pieces of the remainder
+        // padded to a multiple of q; q is the quantum whose modelled cost is lowest (a coarser quantum
+        // wastes lanes, a finer one re-stages the list for one more narrow item).
+        const int64_t n_full = gn / CHUNK_I, rem = gn % CHUNK_I;
+        int64_t best_q = CHUNK_I, best_cost = INT64_MAX;
+        for (int64_t q = 2 * MIN_WIDTH; q <= CHUNK_I && rem > 0; q *= 2) {
+            const int64_t padded = (rem + q - 1) / q * q;
+            int64_t cst = 0;
+            for (int64_t piece = CHUNK_I; piece >= 2 * MIN_WIDTH; piece /= 2)
+                if (padded & piece) cst += item_cost_per_tile((int)(piece / 2));
+            if (cst < best_cost) { best_cost = cst; best_q = q; }
+        }
+        int64_t done = 0;
+        auto emit = [&](int64_t n_i, int width) {
+            WorkItem it;
+            it.i_first = (int32_t)(gf + done);
+            it.n_i = (int32_t)n_i;
+            it.group = (int32_t)g;
+            it.width = width;
+            done += n_i;
+            items.push_back(it);
+            cost.push_back(n_tiles * item_cost_per_tile(width));
+        };
+        for (int64_t k = 0; k < n_full; ++k) emit(CHUNK_I, CHUNK_I / 2);
+        if (rem > 0) {
+            const int64_t padded = (rem + best_q - 1) / best_q * best_q;
+            for (int64_t piece = CHUNK_I; piece >= 2 * MIN_WIDTH; piece /= 2)
+                if (padded & piece) emit(std::min(piece, gn - done), (int)(piece / 2));
+        }
+        pl.item_off[(size_t)g + 1] = (int64_t)items.size();
+    }
+    const int64_t n_items = (int64_t)items.size();
+    if (n_items > c->max_items) return MWF_ENOMEM;
+    // work schedules (see schedule_items): over everything, and inside each of the n_tag balanced group ranges
+    pl.order_full.resize((size_t)n_items);
+    pl.order_split.resize((size_t)n_items);
+    std::iota(pl.order_full.begin(), pl.order_full.end(), 0);
+    schedule_items(pl.order_full, 0, n_items, items, cost);
+    pl.split.assign((size_t)c->p.n_tag + 1, 0);
+    const int64_t total = pl.inter[(size_t)n_group];
+    int64_t g = 0;
+    for (int t = 1; t < c->p.n_tag; ++t) {
+        const int64_t want = total / c->p.n_tag * t;
+        while (g < n_group && pl.inter[(size_t)g] < want) ++g;
+        pl.split[(size_t)t] = g;
+    }
+    pl.split[(size_t)c->p.n_tag] = n_group;
+    std::iota(pl.order_split.begin(), pl.order_split.end(), 0);
+    for (int t = 0; t < c->p.n_tag; ++t) {
+        const int64_t b = pl.item_off[(size_t)pl.split[(size_t)t]], e = pl.item_off[(size_t)pl.split[(size_t)t + 1]];
+        schedule_items(pl.order_split, b, e, items, cost);
+    }
+    return MWF_OK;
+}
+
+// Adopt a plan as the ctx's current lists (after the device side is in place).
+void adopt_plan(mwf_ctx* c, Plan& pl, int64_t n_group, const int32_t* grp_first, const int32_t* grp_n, int mode) {
+    c->h_item_off.swap(pl.item_off);
+    c->h_inter.swap(pl.inter);
+    c->h_split.swap(pl.split);
+    c->h_grp_first.assign(grp_first, grp_first + n_group);
+    c->h_grp_n.assign(grp_n, grp_n + n_group);
+    c->n_group = n_group;
+    c->n_items = (int64_t)pl.items.size();
+    c->padded_entries = pl.list_off[(size_t)n_group];
+    c->have_lists = true;
+    c->lists_for_reuse = (mode == MWF_MAKE_LIST_FOR_REUSE);
+    c->groups_dispatched = 0;
+    c->groups_outstanding = 0;
 }
 
 }  // namespace
@@ -255,6 +376,22 @@ int mwf_create(mwf_ctx** out, const mwf_params* p, void* arena, int64_t arena_by
     c->counters = (unsigned int*)(b + L.off[17]);
     c->err = (unsigned int*)(b + L.off[18]);
     c->vel = (float4*)(b + L.off[19]);
+    {
+        BuildBuffers& q = c->bb;
+        q.store = c->store; q.vel = c->vel; q.tmp16 = c->accp;
+        q.key_a = (uint64_t*)(b + L.off[20]); q.key_b = (uint64_t*)(b + L.off[21]);
+        q.idx_a = (int32_t*)(b + L.off[22]); q.idx_b = (int32_t*)(b + L.off[23]);
+        q.hist = (int32_t*)(b + L.off[24]); q.scan_scratch = (int32_t*)(b + L.off[25]); q.scan_scratch64 = (int64_t*)(b + L.off[26]);
+        q.bbox_part = (float*)(b + L.off[27]); q.root = (double*)(b + L.off[28]);
+        q.cells = c->cells; q.geom = (double4*)(b + L.off[29]); q.parent = c->parent;
+        q.level_cnt = (int32_t*)(b + L.off[30]); q.level_cap = p->max_cell + 2;
+        q.mark = (int32_t*)(b + L.off[31]); q.grp_cell = (int32_t*)(b + L.off[32]);
+        q.grp_first = c->grp_first; q.grp_n = c->grp_n; q.grp_box = (float*)(b + L.off[33]);
+        q.n_epj = (int32_t*)(b + L.off[34]); q.n_spj = (int32_t*)(b + L.off[35]);
+        q.list_off = c->list_off; q.epj_off = c->st_epj_off; q.spj_off = c->st_spj_off; q.list = c->list;
+        q.walk_stacks = (int32_t*)(b + L.off[36]); q.walk_counter = (unsigned int*)(b + L.off[37]); q.err = c->err;
+        c->walk_warps_n = walk_warps(p->max_group);
+    }
     c->max_items = max_items_of(*p);
     c->tag_groups.assign(MWF_MAX_TAG, 0);
     bool ok = true;
@@ -330,6 +467,7 @@ int mwf_set_tree(mwf_ctx* c, const mwf_cell* cells, int64_t n_cell, void* stream
     int rc = before_store_op(c, s);
     if (rc) return rc;
     c->have_tree = false;
+    c->built_on_device = false;
     drop_lists(c);
     c->mono_fresh = false;
     CU(c, cudaMemsetAsync(c->err, 0, sizeof(unsigned int), s));
@@ -364,76 +502,21 @@ int mwf_set_lists(mwf_ctx* c, int64_t n_group, const int32_t* grp_first, const i
     if ((e_epj > 0 && !epj_id) || (e_spj > 0 && !spj_id)) return MWF_EINVAL;
     if (e_epj + e_spj > c->p.max_entry) return MWF_ENOMEM;
     // host pass: offsets, items, schedule
-    std::vector<int64_t> list_off((size_t)n_group + 1, 0);
-    c->h_item_off.assign((size_t)n_group + 1, 0);
-    c->h_inter.assign((size_t)n_group + 1, 0);
-    std::vector<WorkItem> items;
-    std::vector<int64_t> cost;
-    items.reserve((size_t)(c->n_ptcl / CHUNK_I + 3 * n_group));
+    std::vector<int64_t> n_list((size_t)n_group);
     for (int64_t g = 0; g < n_group; ++g) {
         const int64_t ne = epj_off[g + 1] - epj_off[g], ns = spj_off[g + 1] - spj_off[g];
         if (ne < 0 || ns < 0) return MWF_ERANGE;
-        const int64_t gf = grp_first[g], gn = grp_n[g];
-        if (gf < 0 || gn < 1 || gf + gn > c->n_ptcl) return MWF_ERANGE;
-        const int64_t n_list = ne + ns;
-        const int64_t n_tiles = (n_list + TILE_J - 1) / TILE_J;
-        list_off[(size_t)g + 1] = list_off[(size_t)g] + n_tiles * TILE_J;
-        c->h_inter[(size_t)g + 1] = c->h_inter[(size_t)g] + gn * n_list;
-        // Cut the group into items: whole 64-particle items, then power-of-two pieces of the remainder
-        // padded to a multiple of q; q is the quantum whose modelled cost is lowest (a coarser quantum
-        // wastes lanes, a finer one re-stages the list for one more narrow item).
-        {
-            const int64_t n_full = gn / CHUNK_I, rem = gn % CHUNK_I;
-            int64_t best_q = CHUNK_I, best_cost = INT64_MAX;
-            for (int64_t q = 2 * MIN_WIDTH; q <= CHUNK_I && rem > 0; q *= 2) {
-                const int64_t padded = (rem + q - 1) / q * q;
-                int64_t cst = 0;
-                for (int64_t piece = CHUNK_I; piece >= 2 * MIN_WIDTH; piece /= 2)
-                    if (padded & piece) cst += item_cost_per_tile((int)(piece / 2));
-                if (cst < best_cost) { best_cost = cst; best_q = q; }
-            }
-            int64_t done = 0;
-            auto emit = [&](int64_t n_i, int width) {
-                WorkItem it;
-                it.i_first = (int32_t)(gf + done);
-                it.n_i = (int32_t)n_i;
-                it.group = (int32_t)g;
-                it.width = width;
-                done += n_i;
-                items.push_back(it);
-                cost.push_back(n_tiles * item_cost_per_tile(width));
-            };
-            for (int64_t k = 0; k < n_full; ++k) emit(CHUNK_I, CHUNK_I / 2);
-            if (rem > 0) {
-                const int64_t padded = (rem + best_q - 1) / best_q * best_q;
-                for (int64_t piece = CHUNK_I; piece >= 2 * MIN_WIDTH; piece /= 2)
-                    if (padded & piece) emit(std::min(piece, gn - done), (int)(piece / 2));
-            }
-        }
-        c->h_item_off[(size_t)g + 1] = (int64_t)items.size();
+        n_list[(size_t)g] = ne + ns;
     }
-    const int64_t n_items = (int64_t)items.size();
-    if (n_items > c->max_items) return MWF_ENOMEM;
-    // work schedules (see schedule_items): over everything, and inside each of the n_tag balanced group ranges
-    std::vector<int32_t> order_full((size_t)n_items), order_split((size_t)n_items);
-    std::iota(order_full.begin(), order_full.end(), 0);
-    schedule_items(order_full, 0, n_items, items, cost);
-    c->h_split.assign((size_t)c->p.n_tag + 1, 0);
+    Plan plan;
     {
-        const int64_t total = c->h_inter[(size_t)n_group];
-        int64_t g = 0;
-        for (int t = 1; t < c->p.n_tag; ++t) {
-            const int64_t want = total / c->p.n_tag * t;
-            while (g < n_group && c->h_inter[(size_t)g] < want) ++g;
-            c->h_split[(size_t)t] = g;
-        }
-        c->h_split[(size_t)c->p.n_tag] = n_group;
-        std::iota(order_split.begin(), order_split.end(), 0);
-        for (int t = 0; t < c->p.n_tag; ++t) {
-            const int64_t b = c->h_item_off[(size_t)c->h_split[(size_t)t]], e = c->h_item_off[(size_t)c->h_split[(size_t)t + 1]];
-            schedule_items(order_split, b, e, items, cost);
-        }
+        const int prc = make_plan(c, n_group, grp_first, grp_n, n_list.data(), plan);
+        if (prc) return prc;
     }
+    const std::vector<int64_t>& list_off = plan.list_off;
+    const std::vector<WorkItem>& items = plan.items;
+    const std::vector<int32_t>&order_full = plan.order_full, &order_split = plan.order_split;
+    const int64_t n_items = (int64_t)items.size();
     cudaStream_t s = static_cast<cudaStream_t>(stream);
     int rc = before_store_op(c, s);
     if (rc) return rc;
@@ -460,15 +543,7 @@ int mwf_set_lists(mwf_ctx* c, int64_t n_group, const int32_t* grp_first, const i
     if (rc) return rc;
     if (e & ~ERR_SELF_MIXED) return MWF_ERANGE;
     if (e) return MWF_EINVAL;  // only the self-membership rule is violated
-    c->h_grp_first.assign(grp_first, grp_first + n_group);
-    c->h_grp_n.assign(grp_n, grp_n + n_group);
-    c->n_group = n_group;
-    c->n_items = n_items;
-    c->padded_entries = list_off[(size_t)n_group];
-    c->have_lists = true;
-    c->lists_for_reuse = (mode == MWF_MAKE_LIST_FOR_REUSE);
-    c->groups_dispatched = 0;
-    c->groups_outstanding = 0;
+    adopt_plan(c, plan, n_group, grp_first, grp_n, mode);
     return MWF_OK;
 }
 
@@ -617,6 +692,130 @@ int mwf_calc_force_all(mwf_ctx* c, const mwf_posm* src, int src_on_device, mwf_a
         rc = mwf_retrieve(c, t, dst, dst_on_device);
         if (rc) return rc;
     }
+    return MWF_OK;
+}
+
+int mwf_build(mwf_ctx* c, int64_t n, int32_t n_leaf, int32_t n_grp, double theta, int mode, void* stream) {
+    if (!c || n < 1 || n_leaf < 1 || n_grp < 1 || !(theta >= 0.0) || theta > 1.0) return MWF_EINVAL;
+    if (mode != MWF_MAKE_LIST && mode != MWF_MAKE_LIST_FOR_REUSE) return MWF_EINVAL;
+    if (n > c->p.max_ptcl) return MWF_ENOMEM;
+    if (c->ptcl_hi < n && !(c->have_tree && c->n_ptcl >= n)) return MWF_ESTATE;  // particles [0, n) must have been uploaded
+    for (int t = 0; t < c->p.n_tag; ++t)
+        if (!c->tag_ranges[t].empty()) return MWF_ESTATE;  // tmp16 aliases the result array: retrieve first
+    cudaStream_t s = static_cast<cudaStream_t>(stream);
+    int rc = before_store_op(c, s);
+    if (rc) return rc;
+    c->have_tree = false;
+    c->built_on_device = false;
+    drop_lists(c);
+    c->mono_fresh = false;
+    CU(c, cudaMemsetAsync(c->err, 0, sizeof(unsigned int), s));
+    const bool with_vel = c->vel_hi >= n;
+    int64_t n_cell = 0, n_group = 0;
+    int n_level = 0;
+    CU(c, build_tree_device(c->bb, n, n_leaf, n_grp, c->p.max_cell, c->p.max_group, with_vel, &n_cell, &n_group, &n_level, s));
+    c->n_launch += 8 + 3 * 8 + 3 * n_level;
+    if (n_cell > c->p.max_cell || n_group > c->p.max_group) { after_store_op(c, s); return MWF_ENOMEM; }
+    unsigned int e = 0;
+    rc = read_err_word(c, s, &e);
+    if (rc) return rc;
+    if (e) { after_store_op(c, s); return MWF_ENOMEM; }
+    // tree state as mwf_set_tree leaves it: arrival counters zero, dummy record behind the SPJ block
+    CU(c, cudaMemsetAsync(c->arrive, 0, (size_t)n_cell * 4, s));
+    const float4 zero = make_float4(0.f, 0.f, 0.f, 0.f);
+    CU(c, cudaMemcpyAsync(c->store + n + n_cell, &zero, 16, cudaMemcpyHostToDevice, s));
+    c->n_ptcl = n;
+    c->n_cell = n_cell;
+    c->ptcl_hi = n;
+    // lists: counting walk, offsets, capacity check, fill walk
+    int64_t padded = 0, e_epj = 0, e_spj = 0;
+    CU(c, build_lists_count(c->bb, n_group, theta, c->walk_warps_n, &padded, &e_epj, &e_spj, s));
+    if (e_epj + e_spj > c->p.max_entry) { after_store_op(c, s); return MWF_ENOMEM; }
+    CU(c, build_lists_fill(c->bb, n_group, theta, c->walk_warps_n, n, n_cell, s));
+    CU(c, cudaMemsetAsync(c->grp_self, 1, (size_t)n_group, s));  // theta <= 1: a group's own cells are always opened
+    c->n_launch += 6;
+    // work plan on the host from the group sizes and list lengths
+    std::vector<int32_t> h_first((size_t)n_group), h_n((size_t)n_group), h_ne((size_t)n_group), h_ns((size_t)n_group);
+    const auto D2H = cudaMemcpyDeviceToHost;
+    CU(c, cudaMemcpyAsync(h_first.data(), c->grp_first, (size_t)n_group * 4, D2H, s));
+    CU(c, cudaMemcpyAsync(h_n.data(), c->grp_n, (size_t)n_group * 4, D2H, s));
+    CU(c, cudaMemcpyAsync(h_ne.data(), c->bb.n_epj, (size_t)n_group * 4, D2H, s));
+    CU(c, cudaMemcpyAsync(h_ns.data(), c->bb.n_spj, (size_t)n_group * 4, D2H, s));
+    CU(c, cudaStreamSynchronize(s));
+    std::vector<int64_t> n_list((size_t)n_group);
+    for (int64_t g = 0; g < n_group; ++g) n_list[(size_t)g] = (int64_t)h_ne[(size_t)g] + h_ns[(size_t)g];
+    Plan plan;
+    rc = make_plan(c, n_group, h_first.data(), h_n.data(), n_list.data(), plan);
+    if (rc) { after_store_op(c, s); return rc; }
+    if (plan.list_off[(size_t)n_group] != padded) { after_store_op(c, s); return MWF_ERANGE; }  // host and device offsets must agree
+    const int64_t n_items = (int64_t)plan.items.size();
+    const auto H2D = cudaMemcpyHostToDevice;
+    CU(c, cudaMemcpyAsync(c->items, plan.items.data(), (size_t)n_items * sizeof(WorkItem), H2D, s));
+    CU(c, cudaMemcpyAsync(c->order_full, plan.order_full.data(), (size_t)n_items * 4, H2D, s));
+    CU(c, cudaMemcpyAsync(c->order_split, plan.order_split.data(), (size_t)n_items * 4, H2D, s));
+    CU(c, cudaStreamSynchronize(s));  // the plan's host vectors die with this call
+    rc = after_store_op(c, s);
+    if (rc) return rc;
+    c->have_tree = true;
+    c->built_on_device = true;
+    c->build_e_epj = e_epj;
+    c->build_e_spj = e_spj;
+    c->build_n_level = n_level;
+    adopt_plan(c, plan, n_group, h_first.data(), h_n.data(), mode);
+    return MWF_OK;
+}
+
+int mwf_get_build_sizes(mwf_ctx* c, int64_t* n_cell, int64_t* n_group, int64_t* n_epj, int64_t* n_spj, int32_t* n_level) {
+    if (!c) return MWF_EINVAL;
+    if (!c->built_on_device || !c->have_lists) return MWF_ESTATE;
+    if (n_cell) *n_cell = c->n_cell;
+    if (n_group) *n_group = c->n_group;
+    if (n_epj) *n_epj = c->build_e_epj;
+    if (n_spj) *n_spj = c->build_e_spj;
+    if (n_level) *n_level = c->build_n_level;
+    return MWF_OK;
+}
+
+int mwf_get_permutation(mwf_ctx* c, int32_t* perm, int dst_on_device) {
+    if (!c || !perm) return MWF_EINVAL;
+    if (!c->built_on_device) return MWF_ESTATE;
+    CU(c, cudaDeviceSynchronize());
+    CU(c, cudaMemcpy(perm, c->bb.idx_a, (size_t)c->n_ptcl * 4, dst_on_device ? cudaMemcpyDeviceToDevice : cudaMemcpyDeviceToHost));
+    return MWF_OK;
+}
+
+int mwf_get_tree(mwf_ctx* c, mwf_cell* cells, double* geom4) {
+    if (!c || (!cells && !geom4)) return MWF_EINVAL;
+    if (!c->have_tree) return MWF_ESTATE;
+    if (geom4 && !c->built_on_device) return MWF_ESTATE;  // an uploaded tree carries no geometry
+    CU(c, cudaDeviceSynchronize());
+    if (cells) CU(c, cudaMemcpy(cells, c->cells, (size_t)c->n_cell * sizeof(mwf_cell), cudaMemcpyDeviceToHost));
+    if (geom4) CU(c, cudaMemcpy(geom4, c->bb.geom, (size_t)c->n_cell * 32, cudaMemcpyDeviceToHost));
+    return MWF_OK;
+}
+
+int mwf_get_groups(mwf_ctx* c, int32_t* grp_first, int32_t* grp_n) {
+    if (!c || !grp_first || !grp_n) return MWF_EINVAL;
+    if (!c->have_lists) return MWF_ESTATE;
+    std::memcpy(grp_first, c->h_grp_first.data(), (size_t)c->n_group * 4);
+    std::memcpy(grp_n, c->h_grp_n.data(), (size_t)c->n_group * 4);
+    return MWF_OK;
+}
+
+int mwf_get_lists(mwf_ctx* c, int64_t* epj_off, int32_t* epj_id, int64_t* spj_off, int32_t* spj_id) {
+    if (!c || !epj_off || !spj_off || !epj_id || !spj_id) return MWF_EINVAL;
+    if (!c->built_on_device || !c->have_lists) return MWF_ESTATE;
+    CU(c, cudaDeviceSynchronize());
+    // un-merge into the staging area of the upload path, then two bulk copies
+    if (c->build_e_epj + c->build_e_spj > c->p.max_entry) return MWF_ENOMEM;
+    int32_t* d_epj = c->st_ids;
+    int32_t* d_spj = c->st_ids + c->build_e_epj;
+    CU(c, unmerge_lists(c->bb, c->n_group, c->n_ptcl, d_epj, d_spj, nullptr));
+    CU(c, cudaDeviceSynchronize());
+    CU(c, cudaMemcpy(epj_off, c->bb.epj_off, (size_t)(c->n_group + 1) * 8, cudaMemcpyDeviceToHost));
+    CU(c, cudaMemcpy(spj_off, c->bb.spj_off, (size_t)(c->n_group + 1) * 8, cudaMemcpyDeviceToHost));
+    if (c->build_e_epj) CU(c, cudaMemcpy(epj_id, d_epj, (size_t)c->build_e_epj * 4, cudaMemcpyDeviceToHost));
+    if (c->build_e_spj) CU(c, cudaMemcpy(spj_id, d_spj, (size_t)c->build_e_spj * 4, cudaMemcpyDeviceToHost));
     return MWF_OK;
 }
 

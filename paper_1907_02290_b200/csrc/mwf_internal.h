@@ -70,6 +70,28 @@ cudaError_t launch_merge_lists(int64_t n_group, const int32_t* grp_first, const 
                                const int32_t* epj_id, const int64_t* spj_off, const int32_t* spj_id, const int64_t* list_off,
                                int64_t n_ptcl, int64_t n_cell, int32_t* list, uint8_t* grp_self, unsigned int* err, cudaStream_t s);
 
+// ---- device-side construction step (NEXT-2): buffers carved from the arena, see build_tree.cu / build_lists.cu
+constexpr int WALK_STACK = 6144;  // >= 22 levels x 256 cells (bound derived in build_lists.cu)
+
+struct BuildBuffers {
+    float4* store; float4* vel; float4* tmp16;          // tmp16 aliases the result array (free during construction)
+    uint64_t* key_a; uint64_t* key_b; int32_t* idx_a; int32_t* idx_b;
+    int32_t* hist; int32_t* scan_scratch; int64_t* scan_scratch64;
+    float* bbox_part; double* root;
+    mwf_cell* cells; double4* geom; int32_t* parent; int32_t* level_cnt; int64_t level_cap;
+    int32_t* mark; int32_t* grp_cell; int32_t* grp_first; int32_t* grp_n; float* grp_box;
+    int32_t* n_epj; int32_t* n_spj; int64_t* list_off; int64_t* epj_off; int64_t* spj_off; int32_t* list;
+    int32_t* walk_stacks; unsigned int* walk_counter; unsigned int* err;
+};
+
+cudaError_t build_tree_device(const BuildBuffers& b, int64_t n, int n_leaf, int n_grp, int64_t max_cell, int64_t max_group, bool with_vel,
+                              int64_t* n_cell_out, int64_t* n_group_out, int* n_level_out, cudaStream_t s);
+int64_t walk_warps(int64_t max_group);
+cudaError_t build_lists_count(const BuildBuffers& b, int64_t n_group, double theta, int64_t n_warps, int64_t* padded, int64_t* e_epj, int64_t* e_spj,
+                              cudaStream_t s);
+cudaError_t build_lists_fill(const BuildBuffers& b, int64_t n_group, double theta, int64_t n_warps, int64_t n_ptcl, int64_t n_cell, cudaStream_t s);
+cudaError_t unmerge_lists(const BuildBuffers& b, int64_t n_group, int64_t n_ptcl, int32_t* epj_id, int32_t* spj_id, cudaStream_t s);
+
 cudaError_t launch_kick_drift(float4* store, float4* vel, const float4* accp, int64_t n, float dt, cudaStream_t s);
 cudaError_t launch_kick(float4* vel, const float4* accp, int64_t n, float dt, cudaStream_t s);
 
@@ -81,7 +103,8 @@ enum : unsigned int {
     ERR_EPJ_INDEX = 8u,      // EPJ index outside [0, N)
     ERR_SPJ_INDEX = 16u,     // SPJ index outside [0, n_cell)
     ERR_SELF_MIXED = 32u,    // a group's EPJ list holds some but not all of its own particles
-    ERR_GROUP_RANGE = 64u    // group i-range outside [0, N)
+    ERR_GROUP_RANGE = 64u,   // group i-range outside [0, N)
+    ERR_BUILD_CAPACITY = 128u  // device-side construction: more cells than max_cell
 };
 
 }  // namespace mwf

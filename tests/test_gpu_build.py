@@ -1,0 +1,150 @@
+"""GPU parity of the device-side construction step (mwf_build; paper P:149-172):
+sort order, cells, cell geometry, groups and index lists must be exactly those of the plain Python restatement of
+readings O1-O4 (oracle/bhtree_ref.py, small N) and of the independent host builder (full sizes); lists are
+compared per group as sorted sets (the walk order is free, reading S10).  Then the forces evaluated on the
+device-built lists must match the fp64 oracle run on those same lists (north_star tolerances)."""
+import numpy as np
+import pytest
+
+import oracle
+from oracle import bhtree_ref
+from paper_1907_02290_b200 import binding
+from paper_1907_02290_b200.workload import CONFIGS, build_tree_and_lists, make_particles, make_workload
+
+pytestmark = pytest.mark.gpu
+
+ACC_MAX, ACC_RMS, POT_RMS = 1e-4, 2e-5, 1e-5
+
+
+def device_build(posm, n_leaf, n_grp, theta, eps=1 / 64, max_cell=None, max_group=None, max_entry=None, vel=None, keep=False):
+    n = posm.shape[0]
+    f = binding.MultiWalkForce(eps, 1.0, max_ptcl=n, max_cell=max_cell or 2 * n + 64, max_group=max_group or n + 8,
+                               max_entry=max_entry or max(64, min(n * n + 64 * n, 400 * n + 4096)), n_tag=2)
+    f.begin_step(binding.MAKE_LIST_FOR_REUSE)
+    f.set_particles(posm)                      # caller order, NOT tree order
+    if vel is not None:
+        v4 = np.zeros((n, 4), np.float32)
+        v4[:, :3] = vel
+        f.set_velocities(v4)
+    f.build(n, n_leaf, n_grp, theta, binding.MAKE_LIST_FOR_REUSE)
+    sz = f.get_build_sizes()
+    out = dict(sizes=sz, perm=f.get_permutation(n))
+    out["cells"], out["geom"] = f.get_tree(sz["n_cell"])
+    out["grp_first"], out["grp_n"] = f.get_groups(sz["n_group"])
+    out["epj_off"], out["epj_id"], out["spj_off"], out["spj_id"] = f.get_lists(sz["n_group"], sz["n_epj"], sz["n_spj"])
+    out["posm"] = f.get_particles(0, n)
+    if keep:
+        return out, f
+    f.close()
+    return out
+
+
+@pytest.mark.parametrize("cfg_idx,n,theta,n_leaf,n_grp", [(0, 700, 0.5, 8, 64), (2, 1500, 0.4, 8, 64), (3, 1200, 0.5, 8, 64),
+                                                             (0, 300, 0.0, 8, 64), (0, 900, 1.0, 4, 16), (1, 2049, 0.5, 16, 256), (0, 5000, 0.7, 1, 1)])
+def test_device_build_matches_plain_restatement(cfg_idx, n, theta, n_leaf, n_grp):
+    posm, _ = make_particles(CONFIGS[cfg_idx], n)
+    ref = bhtree_ref.build(posm, n_leaf, n_grp, theta)
+    got = device_build(posm, n_leaf, n_grp, theta)
+    assert np.array_equal(got["perm"], ref["perm"])
+    assert np.array_equal(got["posm"], posm[ref["perm"]])
+    assert np.array_equal(got["cells"], ref["cells"])
+    assert np.array_equal(got["geom"], ref["geom"])            # bitwise: same fp64 operations in the same order
+    assert np.array_equal(got["grp_first"], ref["cells"][ref["groups"], 0])
+    assert np.array_equal(got["grp_n"], ref["cells"][ref["groups"], 1])
+    for g in range(len(ref["groups"])):
+        e = got["epj_id"][got["epj_off"][g]:got["epj_off"][g + 1]]
+        s = got["spj_id"][got["spj_off"][g]:got["spj_off"][g + 1]]
+        assert np.array_equal(np.sort(e), np.sort(np.array(ref["epj"][g], np.int32))), "EPJ set of group %d" % g
+        assert np.array_equal(np.sort(s), np.sort(np.array(ref["spj"][g], np.int32))), "SPJ set of group %d" % g
+
+
+def test_device_build_degenerate_inputs():
+    # one particle; two particles; many coincident particles (a depth-21 leaf with more than n_leaf particles)
+    for posm in (np.array([[0.5, 0.25, -1.0, 1.0]], np.float32),
+                 np.array([[0, 0, 0, 1.0], [1, 1, 1, 2.0]], np.float32),
+                 np.concatenate([np.tile(np.array([[0.3, 0.3, 0.3, 1.0]], np.float32), (40, 1)), np.array([[1, 2, 3, 1.0]], np.float32)])):
+        ref = bhtree_ref.build(posm, 8, 16, 0.5)
+        got = device_build(posm, 8, 16, 0.5)
+        assert np.array_equal(got["perm"], ref["perm"])
+        assert np.array_equal(got["cells"], ref["cells"])
+        assert np.array_equal(got["geom"], ref["geom"])
+        for g in range(len(ref["groups"])):
+            assert sorted(got["epj_id"][got["epj_off"][g]:got["epj_off"][g + 1]]) == sorted(ref["epj"][g])
+            assert sorted(got["spj_id"][got["spj_off"][g]:got["spj_off"][g + 1]]) == sorted(ref["spj"][g])
+
+
+def test_device_build_errors():
+    posm, _ = make_particles(CONFIGS[0], 3000)
+    f = binding.MultiWalkForce(1 / 64, 1.0, max_ptcl=3000, max_cell=100, max_group=3000, max_entry=10 ** 6, n_tag=1)
+    with pytest.raises(binding.MwfError) as e:
+        f.build(3000, 8, 64, 0.5)
+    assert e.value.code == binding.ESTATE                       # no particles uploaded
+    f.set_particles(posm)
+    for bad in ((0, 8, 64, 0.5), (3000, 0, 64, 0.5), (3000, 8, 0, 0.5), (3000, 8, 64, -0.1), (3000, 8, 64, 1.5), (3000, 8, 64, float("nan"))):
+        with pytest.raises(binding.MwfError) as e:
+            f.build(*bad)
+        assert e.value.code == binding.EINVAL
+    with pytest.raises(binding.MwfError) as e:
+        f.build(3000, 8, 64, 0.5)
+    assert e.value.code == binding.ENOMEM                       # max_cell = 100
+    f.close()
+    f = binding.MultiWalkForce(1 / 64, 1.0, max_ptcl=3000, max_cell=6000, max_group=3000, max_entry=1000, n_tag=1)
+    f.set_particles(posm)
+    with pytest.raises(binding.MwfError) as e:
+        f.build(3000, 8, 64, 0.5)
+    assert e.value.code == binding.ENOMEM                       # max_entry = 1000
+    with pytest.raises(binding.MwfError) as e:
+        f.dispatch(0, 0, 1)
+    assert e.value.code == binding.ESTATE                       # a failed build leaves no lists
+    f.close()
+
+
+def check_forces(out, acc, pot, label):
+    a = out[:, :3].astype(np.float64)
+    p = out[:, 3].astype(np.float64)
+    ea = np.linalg.norm(a - acc, axis=1) / np.linalg.norm(acc, axis=1)
+    ep = np.abs(p - pot) / np.abs(pot)
+    msg = "%s: acc max %.2e rms %.2e | pot rms %.2e" % (label, ea.max(), np.sqrt(np.mean(ea ** 2)), np.sqrt(np.mean(ep ** 2)))
+    print(msg)
+    assert ea.max() <= ACC_MAX and np.sqrt(np.mean(ea ** 2)) <= ACC_RMS and np.sqrt(np.mean(ep ** 2)) <= POT_RMS, msg
+
+
+@pytest.mark.parametrize("cfg_idx,n", [(0, None), (2, 50000), (3, 60000)])
+def test_forces_on_device_built_lists(cfg_idx, n):
+    """Whole construction step on the device, then the usual evaluation; the oracle evaluates the lists the
+    device built (read back), on the particles in the device's tree order."""
+    cfg = CONFIGS[cfg_idx]
+    posm, vel = make_particles(cfg, n)
+    got, f = device_build(posm, cfg.n_leaf, cfg.n_grp, cfg.theta, eps=cfg.eps, vel=vel, keep=True)
+    f.refresh_monopoles()
+    ng = got["sizes"]["n_group"]
+    f.dispatch(0, 0, ng)
+    out = np.zeros((posm.shape[0], 4), np.float32)
+    f.retrieve(0, out)
+    if vel is not None:                                         # velocities travel with their particles
+        v = f.get_velocities(0, posm.shape[0])
+        assert np.array_equal(v[:, :3], vel.astype(np.float32)[got["perm"]])
+    f.close()
+    mom = oracle.monopoles(got["cells"], got["posm"])
+    acc, pot = oracle.forces(got["posm"], mom, got["grp_first"], got["grp_n"], got["epj_off"], got["epj_id"], got["spj_off"], got["spj_id"], cfg.eps)
+    check_forces(out, acc, pot, "device-built %s" % cfg.name)
+
+
+@pytest.mark.parametrize("cfg_idx", [1, 4])
+def test_device_build_full_size_against_host_builder(cfg_idx):
+    """Full-size configs: the device-built tree equals the host builder's (itself pinned by the plain
+    restatement) cell for cell; list lengths equal for every group; list contents equal on sampled groups."""
+    cfg = CONFIGS[cfg_idx]
+    posm, _ = make_particles(cfg)
+    w = build_tree_and_lists(posm, cfg.n_leaf, cfg.n_grp, cfg.theta)
+    got = device_build(posm, cfg.n_leaf, cfg.n_grp, cfg.theta, eps=cfg.eps, max_cell=w.n_cell + 10, max_group=w.n_group + 10,
+                       max_entry=w.n_entry + 10)
+    assert np.array_equal(got["perm"], w.perm)
+    assert np.array_equal(got["cells"], w.cells)
+    assert np.array_equal(got["geom"], w.geom)
+    assert np.array_equal(got["grp_first"], w.grp_first) and np.array_equal(got["grp_n"], w.grp_n)
+    assert np.array_equal(got["epj_off"], w.epj_off) and np.array_equal(got["spj_off"], w.spj_off)
+    rng = np.random.default_rng(7)
+    for g in rng.choice(w.n_group, 300, replace=False):
+        assert np.array_equal(np.sort(got["epj_id"][w.epj_off[g]:w.epj_off[g + 1]]), np.sort(w.epj_id[w.epj_off[g]:w.epj_off[g + 1]]))
+        assert np.array_equal(np.sort(got["spj_id"][w.spj_off[g]:w.spj_off[g + 1]]), np.sort(w.spj_id[w.spj_off[g]:w.spj_off[g + 1]]))
