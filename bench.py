@@ -301,6 +301,8 @@ def main():
     try:
         from paper_1907_02290_b200.workload import make_particles
         posm0, _ = make_particles(cfg, args.n)
+        if dev_res is not None:
+            f.retrieve(0, dst_dev)                 # the device-resident leg leaves its results on tag 0
         f.begin_step(binding.MAKE_LIST_FOR_REUSE)
         f.set_particles(posm0)
         f.sync()

@@ -1,6 +1,8 @@
 // Host side of libmwf.so: the C ABI of include/mwf.h -- device store, list-reuse driver (SURVEY.md
 // section 8(a) rows a1, a2, a5, a6, a7) and the launches of the kernels in this directory.
 #include <algorithm>
+#include <chrono>
+#include <cstdlib>
 #include <climits>
 #include <cstdio>
 #include <cstring>
@@ -70,6 +72,21 @@ struct mwf_ctx {
 namespace {
 
 constexpr int N_COUNTER = 1024;
+
+// MWF_TRACE=1 in the environment: wall-clock phase times of the construction step on stderr
+bool trace_on() {
+    static const bool on = [] { const char* e = std::getenv("MWF_TRACE"); return e && e[0] && e[0] != '0'; }();
+    return on;
+}
+struct PhaseTimer {
+    std::chrono::steady_clock::time_point t0 = std::chrono::steady_clock::now();
+    void lap(const char* what) {
+        if (!trace_on()) return;
+        const auto t1 = std::chrono::steady_clock::now();
+        fprintf(stderr, "[mwf trace] %-28s %8.3f ms\n", what, std::chrono::duration<double, std::milli>(t1 - t0).count());
+        t0 = t1;
+    }
+};
 
 int cuda_fail(mwf_ctx* c, cudaError_t e, const char* what) {
     if (c) {
@@ -190,12 +207,31 @@ void drop_lists(mwf_ctx* c) {
 // except that the NARROW items (width <= 8: few j-pairs per staged tile, so they wait on the gathers rather
 // than on the FP32 pipe) are spread evenly over the first 7/8 of the schedule, where the wide items of the
 // other warps of the SM keep the pipe busy meanwhile.
+// Stable LSD radix sort (11-bit digits) of item indices by DESCENDING cost: O(n), ties keep item order.
+void sort_longest_first(std::vector<int32_t>& v, const std::vector<int64_t>& cost, std::vector<int32_t>& tmp) {
+    const size_t n = v.size();
+    if (n < 2) return;
+    int64_t cmax = 0;
+    for (int32_t it : v) cmax = std::max(cmax, cost[(size_t)it]);
+    tmp.resize(n);
+    for (int shift = 0; shift < 63 && (cmax >> shift) > 0; shift += 11) {
+        size_t count[2049] = {0};
+        for (int32_t it : v) ++count[(size_t)(((cmax - cost[(size_t)it]) >> shift) & 2047) + 1];
+        for (int d = 0; d < 2048; ++d) count[d + 1] += count[d];
+        for (int32_t it : v) tmp[count[(size_t)(((cmax - cost[(size_t)it]) >> shift) & 2047)]++] = it;
+        v.swap(tmp);
+    }
+}
+
 void schedule_items(std::vector<int32_t>& order, int64_t b, int64_t e, const std::vector<WorkItem>& items, const std::vector<int64_t>& cost) {
-    auto longer = [&](int32_t x, int32_t y) { return cost[(size_t)x] > cost[(size_t)y]; };
-    std::vector<int32_t> wide, narrow;
-    for (int64_t k = b; k < e; ++k) (items[(size_t)order[(size_t)k]].width > 8 ? wide : narrow).push_back(order[(size_t)k]);
-    std::stable_sort(wide.begin(), wide.end(), longer);
-    std::stable_sort(narrow.begin(), narrow.end(), longer);
+    std::vector<int32_t> wide, narrow, tmp;
+    wide.reserve((size_t)(e - b));
+    for (int64_t k = b; k < e; ++k) {
+        const int32_t it = order[(size_t)k];
+        (items[(size_t)it].width > 8 ? wide : narrow).push_back(it);
+    }
+    sort_longest_first(wide, cost, tmp);
+    sort_longest_first(narrow, cost, tmp);
     const size_t nw = wide.size(), nn = narrow.size();
     const size_t span = nw - nw / 8;  // narrow items go between the first `span` wide items
     size_t iw = 0, in = 0;
@@ -713,8 +749,10 @@ int mwf_build(mwf_ctx* c, int64_t n, int32_t n_leaf, int32_t n_grp, double theta
     const bool with_vel = c->vel_hi >= n;
     int64_t n_cell = 0, n_group = 0;
     int n_level = 0;
+    PhaseTimer tm;
     CU(c, build_tree_device(c->bb, n, n_leaf, n_grp, c->p.max_cell, c->p.max_group, with_vel, &n_cell, &n_group, &n_level, s));
     c->n_launch += 8 + 3 * 8 + 3 * n_level;
+    tm.lap("sort + tree + groups");
     if (n_cell > c->p.max_cell || n_group > c->p.max_group) { after_store_op(c, s); return MWF_ENOMEM; }
     unsigned int e = 0;
     rc = read_err_word(c, s, &e);
@@ -730,11 +768,9 @@ int mwf_build(mwf_ctx* c, int64_t n, int32_t n_leaf, int32_t n_grp, double theta
     // lists: counting walk, offsets, capacity check, fill walk
     int64_t padded = 0, e_epj = 0, e_spj = 0;
     CU(c, build_lists_count(c->bb, n_group, theta, c->walk_warps_n, &padded, &e_epj, &e_spj, s));
+    tm.lap("list walk: count + offsets");
     if (e_epj + e_spj > c->p.max_entry) { after_store_op(c, s); return MWF_ENOMEM; }
-    CU(c, build_lists_fill(c->bb, n_group, theta, c->walk_warps_n, n, n_cell, s));
-    CU(c, cudaMemsetAsync(c->grp_self, 1, (size_t)n_group, s));  // theta <= 1: a group's own cells are always opened
-    c->n_launch += 6;
-    // work plan on the host from the group sizes and list lengths
+    // group sizes and list lengths come back for the host work plan; the fill walk runs meanwhile
     std::vector<int32_t> h_first((size_t)n_group), h_n((size_t)n_group), h_ne((size_t)n_group), h_ns((size_t)n_group);
     const auto D2H = cudaMemcpyDeviceToHost;
     CU(c, cudaMemcpyAsync(h_first.data(), c->grp_first, (size_t)n_group * 4, D2H, s));
@@ -742,10 +778,14 @@ int mwf_build(mwf_ctx* c, int64_t n, int32_t n_leaf, int32_t n_grp, double theta
     CU(c, cudaMemcpyAsync(h_ne.data(), c->bb.n_epj, (size_t)n_group * 4, D2H, s));
     CU(c, cudaMemcpyAsync(h_ns.data(), c->bb.n_spj, (size_t)n_group * 4, D2H, s));
     CU(c, cudaStreamSynchronize(s));
+    CU(c, build_lists_fill(c->bb, n_group, theta, c->walk_warps_n, n, n_cell, s));
+    CU(c, cudaMemsetAsync(c->grp_self, 1, (size_t)n_group, s));  // theta <= 1: a group's own cells are always opened
+    c->n_launch += 6;
     std::vector<int64_t> n_list((size_t)n_group);
     for (int64_t g = 0; g < n_group; ++g) n_list[(size_t)g] = (int64_t)h_ne[(size_t)g] + h_ns[(size_t)g];
     Plan plan;
     rc = make_plan(c, n_group, h_first.data(), h_n.data(), n_list.data(), plan);
+    tm.lap("host work plan | fill walk");
     if (rc) { after_store_op(c, s); return rc; }
     if (plan.list_off[(size_t)n_group] != padded) { after_store_op(c, s); return MWF_ERANGE; }  // host and device offsets must agree
     const int64_t n_items = (int64_t)plan.items.size();
@@ -754,6 +794,7 @@ int mwf_build(mwf_ctx* c, int64_t n, int32_t n_leaf, int32_t n_grp, double theta
     CU(c, cudaMemcpyAsync(c->order_full, plan.order_full.data(), (size_t)n_items * 4, H2D, s));
     CU(c, cudaMemcpyAsync(c->order_split, plan.order_split.data(), (size_t)n_items * 4, H2D, s));
     CU(c, cudaStreamSynchronize(s));  // the plan's host vectors die with this call
+    tm.lap("plan upload");
     rc = after_store_op(c, s);
     if (rc) return rc;
     c->have_tree = true;
