@@ -137,7 +137,8 @@ int mwf_dispatch(mwf_ctx* c, int32_t tag, int64_t g_begin, int64_t g_end);
 
 /* (5) Copy acc+pot of the particles of every group dispatched under `tag` since its last retrieve into
  * dst and wait for it.  dst: base of an N-record array indexed by tree-order particle
- * position, HOST or DEVICE; records of other particles are not touched. */
+ * position, HOST or DEVICE; records of other particles are not touched.  dst == NULL: wait for the tag and
+ * discard its results (they stay in the library's result array; a device-resident loop needs no copy). */
 int mwf_retrieve(mwf_ctx* c, int32_t tag, mwf_accp* dst, int dst_on_device);
 
 /* One whole evaluation, the analogue of calcForceAllAndWriteBackMultiWalkIndex for a step

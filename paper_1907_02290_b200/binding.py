@@ -203,7 +203,10 @@ class MultiWalkForce:
         self._ck(self._lib.mwf_dispatch(self._h, int(tag), int(g_begin), int(g_end)))
 
     def retrieve(self, tag: int, dst):
-        p, on_dev = _ptr(dst, np.float32, "dst")
+        if dst is None:
+            p, on_dev = ctypes.c_void_p(None), 0
+        else:
+            p, on_dev = _ptr(dst, np.float32, "dst")
         self._ck(self._lib.mwf_retrieve(self._h, int(tag), p, on_dev))
 
     def calc_force_all(self, src, dst):

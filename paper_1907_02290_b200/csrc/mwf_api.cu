@@ -670,14 +670,14 @@ int mwf_dispatch(mwf_ctx* c, int32_t tag, int64_t g_begin, int64_t g_end) {
 }
 
 int mwf_retrieve(mwf_ctx* c, int32_t tag, mwf_accp* dst, int dst_on_device) {
-    if (!c || tag < 0 || tag >= c->p.n_tag || !dst) return MWF_EINVAL;
+    if (!c || tag < 0 || tag >= c->p.n_tag) return MWF_EINVAL;
     auto& rs = c->tag_ranges[tag];
     if (rs.empty()) return MWF_ESTATE;
     cudaStream_t s = c->tag_stream[tag];
     const auto kind = dst_on_device ? cudaMemcpyDeviceToDevice : cudaMemcpyDeviceToHost;
     // merge adjacent ranges of consecutive dispatches
     std::sort(rs.begin(), rs.end());
-    size_t k = 0;
+    size_t k = dst ? 0 : rs.size();  // dst == NULL: wait for the tag and discard its results
     while (k < rs.size()) {
         int64_t lo = rs[k].first, hi = rs[k].second;
         size_t j = k + 1;

@@ -148,3 +148,52 @@ def test_device_build_full_size_against_host_builder(cfg_idx):
     for g in rng.choice(w.n_group, 300, replace=False):
         assert np.array_equal(np.sort(got["epj_id"][w.epj_off[g]:w.epj_off[g + 1]]), np.sort(w.epj_id[w.epj_off[g]:w.epj_off[g + 1]]))
         assert np.array_equal(np.sort(got["spj_id"][w.spj_off[g]:w.spj_off[g + 1]]), np.sort(w.spj_id[w.spj_off[g]:w.spj_off[g + 1]]))
+
+
+def test_whole_loop_on_the_device():
+    """Construction on the device, 3 device-resident reuse steps, construction again from the moved particles
+    (now in the previous tree order), evaluation: nothing but the initial upload and the final read-back crosses
+    the host link.  The second tree must be the one the plain restatement builds from the moved particles, and
+    its forces must match the oracle."""
+    cfg = CONFIGS[4]
+    posm, vel = make_particles(cfg, 6000)
+    got, f = device_build(posm, cfg.n_leaf, cfg.n_grp, cfg.theta, eps=cfg.eps, vel=vel, keep=True)
+    n = posm.shape[0]
+    ng = got["sizes"]["n_group"]
+    f.refresh_monopoles()
+    f.dispatch(0, 0, ng)
+    f.retrieve(0, None)                                        # wait, keep the forces on the device
+    for _ in range(3):
+        f.step_reuse(cfg.dt)
+    with pytest.raises(binding.MwfError) as e:
+        f.build(n, cfg.n_leaf, cfg.n_grp, cfg.theta)
+    assert e.value.code == binding.ESTATE                      # results of the last step neither retrieved nor discarded
+    f.retrieve(0, None)
+    moved = f.get_particles(0, n)                              # tree order of the FIRST build
+    v_before = f.get_velocities(0, n)
+    f.begin_step(binding.MAKE_LIST_FOR_REUSE)
+    f.build(n, cfg.n_leaf, cfg.n_grp, cfg.theta)
+    sz = f.get_build_sizes()
+    perm2 = f.get_permutation(n)
+    ref = bhtree_ref.build(moved, cfg.n_leaf, cfg.n_grp, cfg.theta)
+    assert np.array_equal(perm2, ref["perm"])
+    cells, geom = f.get_tree(sz["n_cell"])
+    assert np.array_equal(cells, ref["cells"]) and np.array_equal(geom, ref["geom"])
+    assert np.array_equal(f.get_particles(0, n), moved[perm2])
+    assert np.array_equal(f.get_velocities(0, n), v_before[perm2])
+    with pytest.raises(binding.MwfError) as e:
+        f.kick_drift(cfg.dt)
+    assert e.value.code == binding.ESTATE                      # new lists: forces must be evaluated first
+    f.refresh_monopoles()
+    f.dispatch(0, 0, sz["n_group"])
+    out = np.zeros((n, 4), np.float32)
+    f.retrieve(0, out)
+    gf, gn = f.get_groups(sz["n_group"])
+    eo, ei, so, si = f.get_lists(sz["n_group"], sz["n_epj"], sz["n_spj"])
+    f.step_reuse(cfg.dt)                                       # and the loop goes on
+    f.retrieve(0, None)
+    f.close()
+    p2 = moved[perm2]
+    mom = oracle.monopoles(cells, p2)
+    acc, pot = oracle.forces(p2, mom, gf, gn, eo, ei, so, si, cfg.eps)
+    check_forces(out, acc, pot, "second construction")
