@@ -162,6 +162,33 @@ def cfg_index(cfg):
     return CONFIGS.index(cfg)
 
 
+def construction_leg(args, cfg, binding, device):
+    """Only the device-side construction step (mwf_build): unsorted particles resident in the store ->
+    Morton order, tree, groups, index lists, work plan.  One JSON line; wall-clock per build (the call
+    synchronises), W warm-up builds, K timed ones."""
+    from paper_1907_02290_b200.workload import make_particles
+    posm, _ = make_particles(cfg, args.n)
+    n = posm.shape[0]
+    f = binding.MultiWalkForce(cfg.eps, 1.0, max_ptcl=n, max_cell=n, max_group=max(64, n // 8), max_entry=80 * n, n_tag=args.n_tag, device=device)
+    times = []
+    for it in range(args.warmup + args.steps):
+        f.begin_step(binding.MAKE_LIST_FOR_REUSE)
+        f.set_particles(posm)
+        f.sync()
+        t = time.perf_counter()
+        f.build(n, cfg.n_leaf, cfg.n_grp, cfg.theta, binding.MAKE_LIST_FOR_REUSE)
+        f.sync()
+        if it >= args.warmup:
+            times.append(time.perf_counter() - t)
+    sz = f.get_build_sizes()
+    f.close()
+    print(json.dumps({"leg": "construction", "metric": "device-side construction step", "value": 1e3 * float(np.median(times)), "unit": "ms",
+                      "min_ms": 1e3 * min(times), "steps": args.steps, "warmup": args.warmup, "higher_is_better": False,
+                      "config": {"workload": "config %d: %s" % (cfg_index(cfg) + 1, cfg.name), "n": n, "n_leaf": cfg.n_leaf, "n_grp": cfg.n_grp, "theta": cfg.theta},
+                      "built": sz, "data": "synthetic"}), flush=True)
+    return 0
+
+
 # ----------------------------------------------------------------------------- main
 def main():
     ap = argparse.ArgumentParser()
@@ -173,6 +200,8 @@ def main():
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--cpu-baseline-seconds", type=float, default=15.0)
     ap.add_argument("--n-tag", type=int, default=8)
+    ap.add_argument("--leg", default="step", choices=["step", "construction"],
+                    help="step: the list-reuse step (the contract's JSON line); construction: only the device-side construction step")
     args = ap.parse_args()
     args.warmup = max(args.warmup, 3) if args.impl == "ours" else args.warmup
 
@@ -196,6 +225,9 @@ def main():
     rank, world, local = replicas.init_from_env()
     torch.cuda.set_device(local)
     from paper_1907_02290_b200 import binding
+
+    if args.leg == "construction":
+        return construction_leg(args, cfg, binding, local)
 
     t = time.perf_counter()
     w = make_workload(cfg, args.n)
