@@ -307,6 +307,33 @@ def main():
     for k, name in enumerate(("upload_d2d", "monopole_refresh", "force_kernel", "retrieve_d2d")):
         phases[name + "_ms"] = round(ev[k].elapsed_time(ev[k + 1]), 4)
 
+    # ---- config 2's pipeline: 64-256 groups per dispatch, tags round-robin over the streams
+    batched = None
+    if cfg.groups_per_dispatch > 0:
+        def step_batched():
+            f.begin_step(binding.REUSE_LIST)
+            f.set_particles(src_dev, 0, w.n, f.streams[0])
+            f.refresh_monopoles(f.streams[0])
+            tag, pending = 0, []
+            for gb in range(0, w.n_group, cfg.groups_per_dispatch):
+                if len(pending) == f.n_tag:
+                    f.retrieve(pending.pop(0), dst_dev)
+                f.dispatch(tag, gb, min(w.n_group, gb + cfg.groups_per_dispatch))
+                pending.append(tag)
+                tag = (tag + 1) % f.n_tag
+            for t in pending:
+                f.retrieve(t, dst_dev)
+        for _ in range(3):
+            step_batched()
+        torch.cuda.synchronize()
+        t0 = time.perf_counter()
+        for _ in range(args.steps):
+            step_batched()
+        torch.cuda.synchronize()
+        ms_b = (time.perf_counter() - t0) * 1e3 / args.steps
+        batched = {"groups_per_dispatch": cfg.groups_per_dispatch, "dispatches_per_step": -(-w.n_group // cfg.groups_per_dispatch),
+                   "ms_per_step": ms_b, "value": inter / (ms_b * 1e-3), "unit": UNIT, "timing": "host wall clock, device-resident source and destination"}
+
     # ---- NEXT-1: device-resident reuse steps (kick-drift, refresh, force, kick; no host transfer)
     dev_res = None
     if w.vel is not None and cfg.dt > 0:
@@ -389,7 +416,7 @@ def main():
             "roofline": roof, "cpu_baseline": cpu,
             "e2e": {"value": e2e_value, "unit": UNIT, "h2d_bytes_per_step": 16 * w.n, "d2h_bytes_per_step": 16 * w.n,
                     "ms_per_step": ms_e_max / args.steps},
-            "gpu_launches": launches, "clocks": clk, "phases": phases, "device_resident_step": dev_res,
+            "gpu_launches": launches, "clocks": clk, "phases": phases, "device_resident_step": dev_res, "batched_dispatch": batched,
             "construction_step": {"host_tree_and_lists_s": round(t_build, 3), "upload_tree_and_lists_s": round(t_upload, 3), "on_device": dev_build},
             "context": {"paper_fraction_of_peak": 0.27, "paper_hardware": "TITAN V (P:673), whole step"},
         }

@@ -52,6 +52,9 @@ struct mwf_ctx {
     int64_t vel_hi = 0;      // velocities [0, vel_hi) have been uploaded
     std::vector<int64_t> h_item_off, h_inter, h_split;  // per group prefix of items / interactions; split group bounds
     std::vector<int32_t> h_grp_first, h_grp_n;
+    std::vector<WorkItem> h_items;   // kept for the per-tag schedule, which is made on first use
+    std::vector<int64_t> h_cost;
+    bool split_ready = false;
     int64_t groups_outstanding = 0;  // MAKE_LIST: groups dispatched and not yet retrieved
     int64_t groups_dispatched = 0;
     // streams and events
@@ -249,7 +252,8 @@ void schedule_items(std::vector<int32_t>& order, int64_t b, int64_t e, const std
 struct Plan {
     std::vector<int64_t> list_off, item_off, inter, split;
     std::vector<WorkItem> items;
-    std::vector<int32_t> order_full, order_split;
+    std::vector<int64_t> cost;
+    std::vector<int32_t> order_full;
 };
 
 int make_plan(mwf_ctx* c, int64_t n_group, const int32_t* grp_first, const int32_t* grp_n, const int64_t* n_list_of, Plan& pl) {
@@ -257,7 +261,7 @@ int make_plan(mwf_ctx* c, int64_t n_group, const int32_t* grp_first, const int32
     pl.item_off.assign((size_t)n_group + 1, 0);
     pl.inter.assign((size_t)n_group + 1, 0);
     std::vector<WorkItem>& items = pl.items;
-    std::vector<int64_t> cost;
+    std::vector<int64_t>& cost = pl.cost;
     items.reserve((size_t)(c->n_ptcl / CHUNK_I + 3 * n_group));
     for (int64_t g = 0; g < n_group; ++g) {
         const int64_t gf = grp_first[g], gn = grp_n[g];
@@ -299,9 +303,9 @@ int make_plan(mwf_ctx* c, int64_t n_group, const int32_t* grp_first, const int32
     }
     const int64_t n_items = (int64_t)items.size();
     if (n_items > c->max_items) return MWF_ENOMEM;
-    // work schedules (see schedule_items): over everything, and inside each of the n_tag balanced group ranges
+    // work schedule over everything (see schedule_items); the schedules inside the n_tag interaction-balanced group
+    // ranges that mwf_calc_force_all uses for a host destination are made on first use (ensure_split_order)
     pl.order_full.resize((size_t)n_items);
-    pl.order_split.resize((size_t)n_items);
     std::iota(pl.order_full.begin(), pl.order_full.end(), 0);
     schedule_items(pl.order_full, 0, n_items, items, cost);
     pl.split.assign((size_t)c->p.n_tag + 1, 0);
@@ -313,11 +317,6 @@ int make_plan(mwf_ctx* c, int64_t n_group, const int32_t* grp_first, const int32
         pl.split[(size_t)t] = g;
     }
     pl.split[(size_t)c->p.n_tag] = n_group;
-    std::iota(pl.order_split.begin(), pl.order_split.end(), 0);
-    for (int t = 0; t < c->p.n_tag; ++t) {
-        const int64_t b = pl.item_off[(size_t)pl.split[(size_t)t]], e = pl.item_off[(size_t)pl.split[(size_t)t + 1]];
-        schedule_items(pl.order_split, b, e, items, cost);
-    }
     return MWF_OK;
 }
 
@@ -326,15 +325,33 @@ void adopt_plan(mwf_ctx* c, Plan& pl, int64_t n_group, const int32_t* grp_first,
     c->h_item_off.swap(pl.item_off);
     c->h_inter.swap(pl.inter);
     c->h_split.swap(pl.split);
+    c->h_items.swap(pl.items);
+    c->h_cost.swap(pl.cost);
+    c->split_ready = false;
     c->h_grp_first.assign(grp_first, grp_first + n_group);
     c->h_grp_n.assign(grp_n, grp_n + n_group);
     c->n_group = n_group;
-    c->n_items = (int64_t)pl.items.size();
+    c->n_items = (int64_t)c->h_items.size();
     c->padded_entries = pl.list_off[(size_t)n_group];
     c->have_lists = true;
     c->lists_for_reuse = (mode == MWF_MAKE_LIST_FOR_REUSE);
     c->groups_dispatched = 0;
     c->groups_outstanding = 0;
+}
+
+// Per-tag schedules: made and uploaded the first time a dispatch covers exactly one of the balanced ranges.
+int ensure_split_order(mwf_ctx* c, cudaStream_t s) {
+    if (c->split_ready) return MWF_OK;
+    std::vector<int32_t> order((size_t)c->n_items);
+    std::iota(order.begin(), order.end(), 0);
+    for (int t = 0; t < c->p.n_tag; ++t) {
+        const int64_t b = c->h_item_off[(size_t)c->h_split[(size_t)t]], e = c->h_item_off[(size_t)c->h_split[(size_t)t + 1]];
+        schedule_items(order, b, e, c->h_items, c->h_cost);
+    }
+    CU(c, cudaMemcpyAsync(c->order_split, order.data(), (size_t)c->n_items * 4, cudaMemcpyHostToDevice, s));
+    CU(c, cudaStreamSynchronize(s));
+    c->split_ready = true;
+    return MWF_OK;
 }
 
 }  // namespace
@@ -551,7 +568,7 @@ int mwf_set_lists(mwf_ctx* c, int64_t n_group, const int32_t* grp_first, const i
     }
     const std::vector<int64_t>& list_off = plan.list_off;
     const std::vector<WorkItem>& items = plan.items;
-    const std::vector<int32_t>&order_full = plan.order_full, &order_split = plan.order_split;
+    const std::vector<int32_t>& order_full = plan.order_full;
     const int64_t n_items = (int64_t)items.size();
     cudaStream_t s = static_cast<cudaStream_t>(stream);
     int rc = before_store_op(c, s);
@@ -568,7 +585,6 @@ int mwf_set_lists(mwf_ctx* c, int64_t n_group, const int32_t* grp_first, const i
     CU(c, cudaMemcpyAsync(c->list_off, list_off.data(), (size_t)(n_group + 1) * 8, H2D, s));
     CU(c, cudaMemcpyAsync(c->items, items.data(), (size_t)n_items * sizeof(WorkItem), H2D, s));
     CU(c, cudaMemcpyAsync(c->order_full, order_full.data(), (size_t)n_items * 4, H2D, s));
-    CU(c, cudaMemcpyAsync(c->order_split, order_split.data(), (size_t)n_items * 4, H2D, s));
     CU(c, launch_merge_lists(n_group, c->grp_first, c->grp_n, c->st_epj_off, c->st_ids, c->st_spj_off, c->st_ids + e_epj, c->list_off,
                              c->n_ptcl, c->n_cell, c->list, c->grp_self, c->err, s));
     ++c->n_launch;
@@ -634,7 +650,11 @@ int mwf_dispatch(mwf_ctx* c, int32_t tag, int64_t g_begin, int64_t g_end) {
         a.order = c->order_full;
     } else {
         for (int t = 0; t < c->p.n_tag; ++t)
-            if (c->h_split[(size_t)t] == g_begin && c->h_split[(size_t)t + 1] == g_end) a.order = c->order_split;
+            if (c->h_split[(size_t)t] == g_begin && c->h_split[(size_t)t + 1] == g_end) {
+                const int rc = ensure_split_order(c, s);
+                if (rc) return rc;
+                a.order = c->order_split;
+            }
     }
     const int64_t resident = (int64_t)c->n_sm * c->ctas_per_sm;
     const int64_t want = (a.n_items + WARPS_PER_CTA - 1) / WARPS_PER_CTA;
@@ -792,7 +812,6 @@ int mwf_build(mwf_ctx* c, int64_t n, int32_t n_leaf, int32_t n_grp, double theta
     const auto H2D = cudaMemcpyHostToDevice;
     CU(c, cudaMemcpyAsync(c->items, plan.items.data(), (size_t)n_items * sizeof(WorkItem), H2D, s));
     CU(c, cudaMemcpyAsync(c->order_full, plan.order_full.data(), (size_t)n_items * 4, H2D, s));
-    CU(c, cudaMemcpyAsync(c->order_split, plan.order_split.data(), (size_t)n_items * 4, H2D, s));
     CU(c, cudaStreamSynchronize(s));  // the plan's host vectors die with this call
     tm.lap("plan upload");
     rc = after_store_op(c, s);
