@@ -156,7 +156,7 @@ __global__ void __launch_bounds__(256) k_unmerge(const int32_t* __restrict__ lis
     } while (0)
 
 int64_t walk_warps(int64_t max_group) {
-    const int64_t cap = 148 * 16;
+    const int64_t cap = 148 * 32;
     return max_group < cap ? (max_group < 8 ? 8 : (max_group + 7) / 8 * 8) : cap;
 }
 

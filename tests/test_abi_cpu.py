@@ -49,9 +49,9 @@ def test_strerror_and_arena_bytes(lib):
     n = ctypes.c_int64(0)
     assert lib.mwf_arena_bytes(ctypes.byref(p), ctypes.byref(n)) == 0
     # store + results + merged list + staging dominate; velocities, the sort / tree-build buffers of the
-    # device-side construction step and its walk stacks (<= 148 x 16 warps x 24 KB) come on top
+    # device-side construction step and its walk stacks (<= 148 x 32 warps x 24 KB) come on top
     lower = (p.max_ptcl + p.max_cell) * 16 + p.max_ptcl * 16 + 2 * p.max_entry * 4
-    assert lower < n.value < lower * 1.1 + 80 * p.max_ptcl + 48 * p.max_cell + 148 * 16 * 24576 + (1 << 20)
+    assert lower < n.value < lower * 1.1 + 80 * p.max_ptcl + 48 * p.max_cell + 148 * 32 * 24576 + (1 << 20)
     bad = binding.Params(0.0, 1.0, 10, 10, 10, 10, 8, 0)          # eps must be > 0 (reading S2)
     assert lib.mwf_arena_bytes(ctypes.byref(bad), ctypes.byref(n)) == binding.EINVAL
     bad = binding.Params(0.1, 1.0, 10, 10, 10, 10, 99, 0)
