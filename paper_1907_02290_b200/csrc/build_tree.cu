@@ -101,33 +101,40 @@ __global__ void __launch_bounds__(256) k_gather16(const float4* __restrict__ src
 }
 
 // ---- cells, one level at a time ----------------------------------------------------------------------
-// For every cell of the level: octant boundaries by binary search in its sorted key range; n_child.
+// Eight lanes per cell: lane o finds, by binary search in the cell's sorted key range, the first position whose
+// digit at this level exceeds o (the end of octant o); the eight boundaries are kept for k_level_emit.
 __global__ void __launch_bounds__(128) k_level_count(const mwf_cell* __restrict__ cells, int64_t lev_begin, int64_t lev_end,
-                                                     const uint64_t* __restrict__ key, int shift, int n_leaf, int32_t* __restrict__ n_child) {
-    const int64_t c = lev_begin + (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
-    if (c >= lev_end) return;
-    const mwf_cell cc = cells[c];
-    int nc = 0;
-    if (cc.n_ptcl > n_leaf && shift >= 0) {
+                                                     const uint64_t* __restrict__ key, int shift, int n_leaf, int32_t* __restrict__ n_child,
+                                                     int32_t* __restrict__ bounds) {
+    const int64_t t = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    const int64_t c = lev_begin + (t >> 3);
+    const int oct = (int)(t & 7);
+    const bool live = c < lev_end;
+    mwf_cell cc = {0, 0, 0, 0};
+    if (live) cc = cells[c];
+    int end = 0;
+    const bool split = live && cc.n_ptcl > n_leaf;
+    if (split) {
         const uint64_t* kb = key + cc.first_ptcl;
-        int p = 0;
-        for (int oct = 0; oct < 8; ++oct) {
-            // first position in [p, n) whose digit exceeds oct
-            int lo = p, hi = cc.n_ptcl;
-            while (lo < hi) {
-                const int mid = (lo + hi) >> 1;
-                if ((int)((kb[mid] >> shift) & 7) <= oct) lo = mid + 1; else hi = mid;
-            }
-            if (lo > p) ++nc;
-            p = lo;
+        int lo = 0, hi = cc.n_ptcl;
+        while (lo < hi) {
+            const int mid = (lo + hi) >> 1;
+            if ((int)((kb[mid] >> shift) & 7) <= oct) lo = mid + 1; else hi = mid;
         }
+        end = lo;
     }
-    n_child[c - lev_begin] = nc;
+    const int prev = __shfl_up_sync(0xffffffffu, end, 1);
+    const int begin = oct == 0 ? 0 : prev;
+    const unsigned nonempty = __ballot_sync(0xffffffffu, split && end > begin);
+    if (live) {
+        bounds[(c - lev_begin) * 8 + oct] = end;
+        if (oct == 0) n_child[c - lev_begin] = __popc((nonempty >> (threadIdx.x & 24)) & 0xffu);
+    }
 }
 
 // Writes the children of every cell of the level behind the level (child offsets = exclusive scan of n_child).
 __global__ void __launch_bounds__(128) k_level_emit(mwf_cell* __restrict__ cells, double4* __restrict__ geom, int32_t* __restrict__ parent,
-                                                    int64_t lev_begin, int64_t lev_end, const uint64_t* __restrict__ key, int shift, int n_leaf,
+                                                    int64_t lev_begin, int64_t lev_end, const int32_t* __restrict__ bounds,
                                                     const int32_t* __restrict__ child_off, int64_t max_cell, unsigned int* __restrict__ err) {
     const int64_t c = lev_begin + (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
     if (c >= lev_end) return;
@@ -144,14 +151,13 @@ __global__ void __launch_bounds__(128) k_level_emit(mwf_cell* __restrict__ cells
             cc.n_child = nc;
             const double4 g = geom[c];
             const double hs = __dmul_rn(0.5, g.w), qs = __dmul_rn(0.25, g.w);
-            const uint64_t* kb = key + cc.first_ptcl;
+            const int4 b0 = *reinterpret_cast<const int4*>(bounds + (c - lev_begin) * 8);
+            const int4 b1 = *reinterpret_cast<const int4*>(bounds + (c - lev_begin) * 8 + 4);
+            const int be[8] = {b0.x, b0.y, b0.z, b0.w, b1.x, b1.y, b1.z, b1.w};
             int p = 0, k = 0;
+#pragma unroll
             for (int oct = 0; oct < 8; ++oct) {
-                int lo = p, hi = cc.n_ptcl;
-                while (lo < hi) {
-                    const int mid = (lo + hi) >> 1;
-                    if ((int)((kb[mid] >> shift) & 7) <= oct) lo = mid + 1; else hi = mid;
-                }
+                const int lo = be[oct];
                 if (lo > p) {
                     mwf_cell ch;
                     ch.first_ptcl = cc.first_ptcl + p;
@@ -289,12 +295,11 @@ cudaError_t build_tree_device(const BuildBuffers& b, int64_t n, int n_leaf, int 
         const int64_t m = lev_end - lev_begin;
         if (m + 1 > b.level_cap) return cudaErrorInvalidValue;
         const int shift = 3 * (KEY_BITS - 1 - lev);
-        k_level_count<<<(unsigned)((m + 127) / 128), 128, 0, s>>>(b.cells, lev_begin, lev_end, b.key_a, shift, n_leaf, b.level_cnt);
+        k_level_count<<<(unsigned)((m * 8 + 127) / 128), 128, 0, s>>>(b.cells, lev_begin, lev_end, b.key_a, shift, n_leaf, b.level_cnt, b.level_bounds);
         BT(cudaGetLastError());
         BT(cudaMemsetAsync(b.level_cnt + m, 0, 4, s));
         BT(scan_exclusive<int32_t>(b.level_cnt, m + 1, b.scan_scratch, s));
-        k_level_emit<<<(unsigned)((m + 127) / 128), 128, 0, s>>>(b.cells, b.geom, b.parent, lev_begin, lev_end, b.key_a, shift, n_leaf, b.level_cnt,
-                                                                 max_cell, b.err);
+        k_level_emit<<<(unsigned)((m + 127) / 128), 128, 0, s>>>(b.cells, b.geom, b.parent, lev_begin, lev_end, b.level_bounds, b.level_cnt, max_cell, b.err);
         BT(cudaGetLastError());
         int32_t n_new = 0;
         BT(cudaMemcpyAsync(&n_new, b.level_cnt + m, 4, cudaMemcpyDeviceToHost, s));

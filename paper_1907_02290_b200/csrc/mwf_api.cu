@@ -164,6 +164,7 @@ Layout make_layout(const mwf_params& p) {
     L.add(p.max_group * 4);                             // 35 n_spj
     L.add(walk_warps(p.max_group) * WALK_STACK * 4);    // 36 walk_stacks
     L.add(256);                                         // 37 walk_counter
+    L.add((p.max_cell + 2) * 32);                       // 38 level_bounds (8 octant ends per cell of the level being split)
     return L;
 }
 
@@ -443,6 +444,7 @@ int mwf_create(mwf_ctx** out, const mwf_params* p, void* arena, int64_t arena_by
         q.n_epj = (int32_t*)(b + L.off[34]); q.n_spj = (int32_t*)(b + L.off[35]);
         q.list_off = c->list_off; q.epj_off = c->st_epj_off; q.spj_off = c->st_spj_off; q.list = c->list;
         q.walk_stacks = (int32_t*)(b + L.off[36]); q.walk_counter = (unsigned int*)(b + L.off[37]); q.err = c->err;
+        q.level_bounds = (int32_t*)(b + L.off[38]);
         c->walk_warps_n = walk_warps(p->max_group);
     }
     c->max_items = max_items_of(*p);

@@ -78,7 +78,7 @@ struct BuildBuffers {
     uint64_t* key_a; uint64_t* key_b; int32_t* idx_a; int32_t* idx_b;
     int32_t* hist; int32_t* scan_scratch; int64_t* scan_scratch64;
     float* bbox_part; double* root;
-    mwf_cell* cells; double4* geom; int32_t* parent; int32_t* level_cnt; int64_t level_cap;
+    mwf_cell* cells; double4* geom; int32_t* parent; int32_t* level_cnt; int32_t* level_bounds; int64_t level_cap;
     int32_t* mark; int32_t* grp_cell; int32_t* grp_first; int32_t* grp_n; float* grp_box;
     int32_t* n_epj; int32_t* n_spj; int64_t* list_off; int64_t* epj_off; int64_t* spj_off; int32_t* list;
     int32_t* walk_stacks; unsigned int* walk_counter; unsigned int* err;
