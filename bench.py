@@ -189,6 +189,45 @@ def construction_leg(args, cfg, binding, device):
     return 0
 
 
+def sweep_leg(args, cfg, binding, device):
+    """The paper's appendix-A experiment (Fig. A.1, eq. A.1) on this kernel: force-kernel time per
+    interaction as a function of the mean group size <n_i> (n_grp swept) for theta = 1, 0.5, 0.3.  The paper's
+    finding: independent of theta, falling with <n_i> and then flat.  Lists are built on the device."""
+    import torch
+    from paper_1907_02290_b200.workload import make_particles
+    n = args.n or (1 << 20)
+    posm, _ = make_particles(cfg, n)
+    n_sm = torch.cuda.get_device_properties(device).multi_processor_count
+    peak = n_sm * 256 * (measured_peaks().get("sm_max_mhz") or 1965.0) * 1e6
+    f = binding.MultiWalkForce(cfg.eps, 1.0, max_ptcl=n, max_cell=n, max_group=n, max_entry=700 * n, n_tag=2, device=device)
+    rows = []
+    for theta in (1.0, 0.5, 0.3):
+        for n_grp in (8, 16, 32, 64, 128, 256, 512, 1024, 2048):
+            f.begin_step(binding.MAKE_LIST_FOR_REUSE)
+            f.set_particles(posm)
+            try:
+                f.build(n, cfg.n_leaf, n_grp, theta, binding.MAKE_LIST_FOR_REUSE)
+            except binding.MwfError as ex:
+                rows.append({"theta": theta, "n_grp": n_grp, "error": str(ex)})
+                continue
+            sz = f.get_build_sizes()
+            f.refresh_monopoles()
+            ms = []
+            c0 = f.get_counters()["interactions"]
+            for it in range(args.warmup + args.steps):
+                f.dispatch(0, 0, sz["n_group"])
+                f.retrieve(0, None)
+                if it >= args.warmup:
+                    ms.append(f.last_dispatch_ms(0))
+            inter = (f.get_counters()["interactions"] - c0) // (args.warmup + args.steps)
+            t = float(np.median(ms)) * 1e-3
+            rows.append({"theta": theta, "n_grp": n_grp, "mean_n_i": n / sz["n_group"], "mean_n_list": inter / n, "interactions": inter,
+                         "kernel_ms": t * 1e3, "ps_per_interaction": 1e12 * t / inter, "frac_fp32_peak": N_OP * inter / t / peak})
+    f.close()
+    print(json.dumps({"leg": "sweep", "workload": "%s generator, N = %d, eps = %g, n_leaf = %d" % (cfg.kind, n, cfg.eps, cfg.n_leaf), "rows": rows}), flush=True)
+    return 0
+
+
 # ----------------------------------------------------------------------------- main
 def main():
     ap = argparse.ArgumentParser()
@@ -200,8 +239,9 @@ def main():
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--cpu-baseline-seconds", type=float, default=15.0)
     ap.add_argument("--n-tag", type=int, default=8)
-    ap.add_argument("--leg", default="step", choices=["step", "construction"],
-                    help="step: the list-reuse step (the contract's JSON line); construction: only the device-side construction step")
+    ap.add_argument("--leg", default="step", choices=["step", "construction", "sweep"],
+                    help="step: the list-reuse step (the contract's JSON line); construction: only the device-side construction step; "
+                         "sweep: kernel time per interaction against <n_i> and theta (the paper's Fig. A.1, P:1197-1212)")
     args = ap.parse_args()
     args.warmup = max(args.warmup, 3) if args.impl == "ours" else args.warmup
 
@@ -228,6 +268,8 @@ def main():
 
     if args.leg == "construction":
         return construction_leg(args, cfg, binding, local)
+    if args.leg == "sweep":
+        return sweep_leg(args, cfg, binding, local)
 
     t = time.perf_counter()
     w = make_workload(cfg, args.n)
