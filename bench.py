@@ -228,6 +228,104 @@ def sweep_leg(args, cfg, binding, device):
     return 0
 
 
+def g1_leg(args, cfg, binding, device):
+    """A/B of the paper's two GPU methods on this machine (Table 1, Fig. 5, Table 2): G2 = index lists resident
+    on the device and reused (the product path) against G1 = multiwalk whose lists carry the j records (16 B per entry,
+    P:969) and are packed on the host and sent with every dispatch, every step.  Same groups, same lists, same
+    kernel sweep; one reuse-type step each, host source and destination.  One JSON line."""
+    import torch
+    from paper_1907_02290_b200.workload import make_workload, pack_data_lists
+    w = make_workload(cfg, args.n)
+    f = binding.MultiWalkForce.for_workload(w, n_tag=args.n_tag, device=device)
+    f.upload_workload(w, binding.MAKE_LIST_FOR_REUSE)
+    src_host, dst_host = f.pinned(w.n), f.pinned(w.n)
+    src_host.numpy()[:] = w.posm
+    inter = w.interactions
+    # batches of whole groups of about E / (4 n_tag) entries each
+    per_batch = max(int(w.n_list.max()), w.n_entry // (4 * args.n_tag) + 1)
+    bounds, acc = [0], 0
+    for g in range(w.n_group):
+        if acc + int(w.n_list[g]) > per_batch and acc > 0:
+            bounds.append(g); acc = 0
+        acc += int(w.n_list[g])
+    bounds.append(w.n_group)
+    f.reserve_data_lists(per_batch)
+    stage = [torch.empty((per_batch, 4), dtype=torch.float32, pin_memory=True) for _ in range(args.n_tag)]
+    spj_host = np.empty((w.n_cell, 4), np.float32)
+
+    def step_g2():
+        f.begin_step(binding.REUSE_LIST)
+        f.calc_force_all(src_host, dst_host)
+
+    t_pack = [0.0]
+    k_ms = [0.0]
+
+    def step_g1(timed=False):
+        f.begin_step(binding.REUSE_LIST)
+        f.set_particles(src_host, 0, w.n, f.streams[0])
+        f.refresh_monopoles(f.streams[0])           # the paper computes the moments on the host; here they come back from the device
+        spj_host[:] = f.get_monopoles(w.n_cell)
+        posm_h = src_host.numpy()
+        tag, pending = 0, []
+        for b in range(len(bounds) - 1):
+            if len(pending) == f.n_tag:
+                t = pending.pop(0)
+                f.retrieve(t, dst_host)
+                if timed:
+                    k_ms[0] += f.last_dispatch_ms(t)
+            t0 = time.perf_counter()
+            rec, joff = pack_data_lists(w, bounds[b], bounds[b + 1], posm_h, spj_host, out=stage[tag].numpy())
+            t_pack[0] += time.perf_counter() - t0
+            f.dispatch_data(tag, bounds[b], bounds[b + 1], stage[tag][: rec.shape[0]], joff)
+            pending.append(tag)
+            tag = (tag + 1) % f.n_tag
+        for t in pending:
+            f.retrieve(t, dst_host)
+            if timed:
+                k_ms[0] += f.last_dispatch_ms(t)
+
+    res = {}
+    for name, fn in (("g2_index_reuse", step_g2), ("g1_data_lists", step_g1)):
+        for _ in range(2):
+            fn()
+        torch.cuda.synchronize()
+        t_pack[0] = 0.0
+        t0 = time.perf_counter()
+        for _ in range(args.steps):
+            fn()
+        torch.cuda.synchronize()
+        ms = (time.perf_counter() - t0) * 1e3 / args.steps
+        res[name] = {"ms_per_step": ms, "value": inter / (ms * 1e-3), "unit": UNIT}
+    res["g1_data_lists"].update({"host_pack_ms_per_step": 1e3 * t_pack[0] / args.steps, "dispatches_per_step": len(bounds) - 1,
+                                 "h2d_bytes_per_step": 16 * w.n + 16 * w.n_entry + 8 * (w.n_group + len(bounds) - 1), "d2h_bytes_per_step": 16 * w.n + 16 * w.n_cell})
+    res["g2_index_reuse"].update({"h2d_bytes_per_step": 16 * w.n, "d2h_bytes_per_step": 16 * w.n})
+    step_g1(timed=True)
+    res["g1_data_lists"]["kernel_ms_sum"] = k_ms[0]
+    # kernel-only A/B with everything resident: what the index gather costs inside the kernel
+    kern = {}
+    try:
+        rec, joff = pack_data_lists(w, 0, w.n_group, src_host.numpy(), spj_host)
+        f.reserve_data_lists(rec.shape[0])
+        rec_dev = torch.from_numpy(rec).to(f.device)
+        a, bms = [], []
+        for it in range(args.warmup + args.steps):
+            f.begin_step(binding.REUSE_LIST)
+            f.dispatch(0, 0, w.n_group); f.retrieve(0, None)
+            a.append(f.last_dispatch_ms(0))
+            f.begin_step(binding.REUSE_LIST)
+            f.dispatch_data(1, 0, w.n_group, rec_dev, joff); f.retrieve(1, None)
+            bms.append(f.last_dispatch_ms(1))
+        kern = {"k_force_index_ms": float(np.median(a[args.warmup:])), "k_force_data_ms": float(np.median(bms[args.warmup:])),
+                "data_list_bytes": 16 * int(rec.shape[0]), "index_list_bytes": 4 * int(rec.shape[0])}
+    except binding.MwfError as ex:
+        kern = {"error": str(ex)}
+    f.close()
+    print(json.dumps({"leg": "g1", "metric": METRIC, "config": workload_config(cfg, w), "steps": args.steps, "timing": "host wall clock, pinned host source and destination",
+                      "methods": res, "kernel_only": kern, "speedup_g2_over_g1": res["g1_data_lists"]["ms_per_step"] / res["g2_index_reuse"]["ms_per_step"],
+                      "context": {"paper_g1_s": 0.36, "paper_g2_reuse_s": 0.095, "paper_hardware": "TITAN V + Xeon E5-2670 v3, PCIe 3 (P:716 Table 2)"}}), flush=True)
+    return 0
+
+
 # ----------------------------------------------------------------------------- main
 def main():
     ap = argparse.ArgumentParser()
@@ -239,9 +337,10 @@ def main():
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--cpu-baseline-seconds", type=float, default=15.0)
     ap.add_argument("--n-tag", type=int, default=8)
-    ap.add_argument("--leg", default="step", choices=["step", "construction", "sweep"],
+    ap.add_argument("--leg", default="step", choices=["step", "construction", "sweep", "g1"],
                     help="step: the list-reuse step (the contract's JSON line); construction: only the device-side construction step; "
-                         "sweep: kernel time per interaction against <n_i> and theta (the paper's Fig. A.1, P:1197-1212)")
+                         "sweep: kernel time per interaction against <n_i> and theta (the paper's Fig. A.1, P:1197-1212); "
+                         "g1: the paper's method G1 (lists carry j records, sent every step) against the index method")
     args = ap.parse_args()
     args.warmup = max(args.warmup, 3) if args.impl == "ours" else args.warmup
 
@@ -270,6 +369,8 @@ def main():
         return construction_leg(args, cfg, binding, local)
     if args.leg == "sweep":
         return sweep_leg(args, cfg, binding, local)
+    if args.leg == "g1":
+        return g1_leg(args, cfg, binding, local)
 
     t = time.perf_counter()
     w = make_workload(cfg, args.n)

@@ -135,6 +135,25 @@ int mwf_refresh_monopoles(mwf_ctx* c, void* stream);
  *   pot_i = -G sum_k m_k / (|x_k - x_i|^2 + eps^2)^(1/2)        (k != i by index) */
 int mwf_dispatch(mwf_ctx* c, int32_t tag, int64_t g_begin, int64_t g_end);
 
+/* ---- Method G1 of the paper, for A/B comparison with the index method (paper
+ * P:170-177 "multiwalk", Fig. 2 DispatchKernelStream, Table 1, Fig. 5): the interaction list of every
+ * group carries the j-particle DATA (16 B per entry) instead of 4-byte indices, and is sent with every
+ * dispatch -- on reuse steps too, because particle data changes every step.
+ *
+ * mwf_reserve_data_lists: allocate (cudaMalloc, outside the arena) one staging buffer of max_entry_per_tag j
+ * records per tag; frees any earlier reservation.  MWF_ESTATE while a tag is in flight.
+ * mwf_dispatch_data: like mwf_dispatch over groups [g_begin, g_end), but group g_begin + k interacts with the
+ * records jdata[joff[k] .. joff[k+1]) (EPJ records, then the SPJ records = monopoles of its list's cells) instead
+ * of gathering through its index list.  jdata: HOST (pinned for overlap) or DEVICE, joff: HOST, ng + 1 offsets in
+ * records, joff[0] == 0; both are copied on the tag's stream, so they must stay valid until the tag is retrieved.
+ * The groups, their i-ranges, the self-exclusion rule and the work schedule are those of the lists given to
+ * mwf_set_lists()/mwf_build(); each run must have exactly the length of the group's index list (MWF_ERANGE).
+ * The i-particles are read from the store; the monopoles need not be fresh (SPJ data travels in jdata).
+ * MWF_ENOMEM when joff[ng] exceeds the reservation, MWF_ESTATE when the tag has not been retrieved yet. */
+int mwf_reserve_data_lists(mwf_ctx* c, int64_t max_entry_per_tag);
+int mwf_dispatch_data(mwf_ctx* c, int32_t tag, int64_t g_begin, int64_t g_end, const mwf_posm* jdata, const int64_t* joff,
+                      int jdata_on_device);
+
 /* (5) Copy acc+pot of the particles of every group dispatched under `tag` since its last retrieve into
  * dst and wait for it.  dst: base of an N-record array indexed by tree-order particle
  * position, HOST or DEVICE; records of other particles are not touched.  dst == NULL: wait for the tag and

@@ -24,6 +24,7 @@ SYMBOLS = (
     "mwf_calc_force_all", "mwf_get_monopoles", "mwf_device_pointers", "mwf_sync", "mwf_get_counters",
     "mwf_last_dispatch_ms", "mwf_strerror", "mwf_last_cuda_error",
     "mwf_set_velocities", "mwf_get_velocities", "mwf_kick_drift", "mwf_kick", "mwf_step_reuse",
+    "mwf_reserve_data_lists", "mwf_dispatch_data",
     "mwf_build", "mwf_get_build_sizes", "mwf_get_permutation", "mwf_get_tree", "mwf_get_groups", "mwf_get_lists",
 )
 
@@ -78,6 +79,8 @@ def load_library(path: str | None = None) -> ctypes.CDLL:
         "mwf_kick_drift": [vp, ctypes.c_float, vp],
         "mwf_kick": [vp, ctypes.c_float, vp],
         "mwf_step_reuse": [vp, ctypes.c_float],
+        "mwf_reserve_data_lists": [vp, i64],
+        "mwf_dispatch_data": [vp, i32, i64, i64, vp, vp, ci],
         "mwf_build": [vp, i64, i32, i32, ctypes.c_double, ci, vp],
         "mwf_get_build_sizes": [vp, P(i64), P(i64), P(i64), P(i64), P(i32)],
         "mwf_get_permutation": [vp, vp, ci],
@@ -201,6 +204,14 @@ class MultiWalkForce:
 
     def dispatch(self, tag: int, g_begin: int, g_end: int):
         self._ck(self._lib.mwf_dispatch(self._h, int(tag), int(g_begin), int(g_end)))
+
+    def reserve_data_lists(self, max_entry_per_tag: int):
+        self._ck(self._lib.mwf_reserve_data_lists(self._h, int(max_entry_per_tag)))
+
+    def dispatch_data(self, tag: int, g_begin: int, g_end: int, jdata, joff: np.ndarray):
+        """Method G1: jdata = [n,4] float32 j records (numpy, pinned torch CPU tensor or CUDA tensor), joff = int64 offsets."""
+        p, on_dev = _ptr(jdata, np.float32, "jdata")
+        self._ck(self._lib.mwf_dispatch_data(self._h, int(tag), int(g_begin), int(g_end), p, _host_ptr(joff, np.int64, "joff"), on_dev))
 
     def retrieve(self, tag: int, dst):
         if dst is None:

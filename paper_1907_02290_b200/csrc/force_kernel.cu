@@ -92,7 +92,16 @@ __device__ __forceinline__ void sweep_tile(const float4* __restrict__ sA, const 
     }
 }
 
-template <int W>
+// Entries (2 * lane, 2 * lane + 1) of tile t of a DATA list (method G1: the list carries the records themselves);
+// entries past the end of the list read as a zero-mass record at the origin.
+__device__ __forceinline__ void ld_data_pair(const float4* __restrict__ jd, int64_t n_list, int t, int lane, float4& j0, float4& j1) {
+    const int64_t e = (int64_t)t * TILE_J + 2 * lane;
+    const float4 zero = make_float4(0.f, 0.f, 0.f, 0.f);
+    j0 = e < n_list ? __ldg(jd + e) : zero;
+    j1 = e + 1 < n_list ? __ldg(jd + e + 1) : zero;
+}
+
+template <int W, bool INDEXED>
 __device__ __forceinline__ void run_item(const ForceArgs& a, const WorkItem it, float4* __restrict__ sbuf, int lane) {
     constexpr int S = 32 / W;
     const int sl = lane / W;
@@ -118,17 +127,30 @@ __device__ __forceinline__ void run_item(const ForceArgs& a, const WorkItem it, 
 #pragma unroll
     for (int k = 0; k < 2; ++k) acc.p[k].x = (self_in && sl == 0) ? -mi[k] * self_rinv : 0.f;
 
-    const int64_t l0 = a.list_off[it.group];
-    const int n_tiles = (int)((a.list_off[it.group + 1] - l0) / TILE_J);
-    const int2* __restrict__ lst = reinterpret_cast<const int2*>(a.list + l0);
+    int64_t l0, n_list = 0;
+    int n_tiles;
+    if constexpr (INDEXED) {
+        l0 = a.list_off[it.group];
+        n_tiles = (int)((a.list_off[it.group + 1] - l0) / TILE_J);
+    } else {
+        l0 = a.joff[it.group - a.g_base];
+        n_list = a.joff[it.group - a.g_base + 1] - l0;
+        n_tiles = (int)((n_list + TILE_J - 1) / TILE_J);
+    }
+    const int2* __restrict__ lst = reinterpret_cast<const int2*>(a.list + (INDEXED ? l0 : 0));
+    const float4* __restrict__ jd = a.jdata + (INDEXED ? 0 : l0);
 
     int2 idn = make_int2(0, 0);
     float4 j0 = make_float4(0.f, 0.f, 0.f, 0.f), j1 = j0;
     if (n_tiles > 0) {
-        const int2 id = ld_stream_int2(lst + lane);
-        j0 = __ldg(J + id.x);
-        j1 = __ldg(J + id.y);
-        if (n_tiles > 1) idn = ld_stream_int2(lst + 32 + lane);
+        if constexpr (INDEXED) {
+            const int2 id = ld_stream_int2(lst + lane);
+            j0 = __ldg(J + id.x);
+            j1 = __ldg(J + id.y);
+            if (n_tiles > 1) idn = ld_stream_int2(lst + 32 + lane);
+        } else {
+            ld_data_pair(jd, n_list, 0, lane, j0, j1);
+        }
     }
     for (int t = 0; t < n_tiles; ++t) {
         float4* sA = sbuf + (t & 1) * TILE_J;
@@ -137,9 +159,13 @@ __device__ __forceinline__ void run_item(const ForceArgs& a, const WorkItem it, 
         sB[lane] = make_float4(j0.z, j1.z, j0.w, j1.w);
         __syncwarp();
         if (t + 1 < n_tiles) {
-            j0 = __ldg(J + idn.x);
-            j1 = __ldg(J + idn.y);
-            if (t + 2 < n_tiles) idn = ld_stream_int2(lst + (int64_t)(t + 2) * 32 + lane);
+            if constexpr (INDEXED) {
+                j0 = __ldg(J + idn.x);
+                j1 = __ldg(J + idn.y);
+                if (t + 2 < n_tiles) idn = ld_stream_int2(lst + (int64_t)(t + 2) * 32 + lane);
+            } else {
+                ld_data_pair(jd, n_list, t + 1, lane, j0, j1);
+            }
         }
         sweep_tile<W>(sA, sB, sl, nx, ny, nz, a.eps2, part);
         constexpr int FLUSH = S > MWF_FLUSH_MIN ? S : MWF_FLUSH_MIN;
@@ -165,8 +191,8 @@ __device__ __forceinline__ void run_item(const ForceArgs& a, const WorkItem it, 
     __syncwarp();  // the next item reuses the warp's tile buffers
 }
 
-__global__ void __launch_bounds__(WARPS_PER_CTA * 32, MWF_MIN_CTAS) k_force(const ForceArgs a) {
-    __shared__ float4 s_tiles[WARPS_PER_CTA][2 * TILE_J];
+template <bool INDEXED>
+__device__ __forceinline__ void force_body(const ForceArgs& a, float4 (*s_tiles)[2 * TILE_J]) {
     const int lane = threadIdx.x & 31;
     const int warp = threadIdx.x >> 5;
     float4* sbuf = s_tiles[warp];
@@ -176,11 +202,11 @@ __global__ void __launch_bounds__(WARPS_PER_CTA * 32, MWF_MIN_CTAS) k_force(cons
         const int64_t pos = a.item_begin + w;
         const WorkItem it = a.items[a.order ? a.order[pos] : pos];
         switch (it.width) {
-            case 32: run_item<32>(a, it, sbuf, lane); break;
-            case 16: run_item<16>(a, it, sbuf, lane); break;
-            case 8: run_item<8>(a, it, sbuf, lane); break;
-            case 4: run_item<4>(a, it, sbuf, lane); break;
-            default: run_item<2>(a, it, sbuf, lane); break;
+            case 32: run_item<32, INDEXED>(a, it, sbuf, lane); break;
+            case 16: run_item<16, INDEXED>(a, it, sbuf, lane); break;
+            case 8: run_item<8, INDEXED>(a, it, sbuf, lane); break;
+            case 4: run_item<4, INDEXED>(a, it, sbuf, lane); break;
+            default: run_item<2, INDEXED>(a, it, sbuf, lane); break;
         }
         if (a.counter) {  // dynamic: next unclaimed item
             unsigned int nxt = 0;
@@ -192,9 +218,24 @@ __global__ void __launch_bounds__(WARPS_PER_CTA * 32, MWF_MIN_CTAS) k_force(cons
     }
 }
 
+__global__ void __launch_bounds__(WARPS_PER_CTA * 32, MWF_MIN_CTAS) k_force(const ForceArgs a) {
+    __shared__ float4 s_tiles[WARPS_PER_CTA][2 * TILE_J];
+    force_body<true>(a, s_tiles);
+}
+
+// Method G1 of the paper (multiwalk without indirect addressing, Fig. 2): same items, same sweep, but
+// every group's list is a contiguous run of j RECORDS sent with the dispatch.  A/B variant.
+__global__ void __launch_bounds__(WARPS_PER_CTA * 32, MWF_MIN_CTAS) k_force_data(const ForceArgs a) {
+    __shared__ float4 s_tiles[WARPS_PER_CTA][2 * TILE_J];
+    force_body<false>(a, s_tiles);
+}
+
 cudaError_t launch_force(const ForceArgs& a, int grid, cudaStream_t s) {
     if (a.n_items <= 0 || grid <= 0) return cudaSuccess;
-    k_force<<<grid, WARPS_PER_CTA * 32, 0, s>>>(a);
+    if (a.jdata)
+        k_force_data<<<grid, WARPS_PER_CTA * 32, 0, s>>>(a);
+    else
+        k_force<<<grid, WARPS_PER_CTA * 32, 0, s>>>(a);
     return cudaGetLastError();
 }
 

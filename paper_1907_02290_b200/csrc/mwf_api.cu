@@ -67,6 +67,10 @@ struct mwf_ctx {
     bool store_event_valid = false;
     std::vector<std::pair<int64_t, int64_t>> tag_ranges[MWF_MAX_TAG];  // particle ranges awaiting retrieve
     std::vector<int64_t> tag_groups;                                   // groups awaiting retrieve per tag
+    // method G1 (data lists, NEXT-3): per-tag staging of j records and their offsets, cudaMalloc'ed on demand
+    float4* data_buf[MWF_MAX_TAG]{};
+    int64_t* data_off[MWF_MAX_TAG]{};
+    int64_t data_cap = 0;
     uint32_t counter_seq = 0;
     int64_t n_launch = 0, n_inter = 0;
     std::string cuda_err;
@@ -475,6 +479,10 @@ int mwf_destroy(mwf_ctx* c) {
         if (c->ev_k1[t]) cudaEventDestroy(c->ev_k1[t]);
     }
     if (c->ev_store) cudaEventDestroy(c->ev_store);
+    for (int t = 0; t < MWF_MAX_TAG; ++t) {
+        if (c->data_buf[t]) cudaFree(c->data_buf[t]);
+        if (c->data_off[t]) cudaFree(c->data_off[t]);
+    }
     if (c->own_arena && c->arena) cudaFree(c->arena);
     delete c;
     return MWF_OK;
@@ -629,19 +637,19 @@ int mwf_refresh_monopoles(mwf_ctx* c, void* stream) {
     return after_store_op(c, s);
 }
 
-int mwf_dispatch(mwf_ctx* c, int32_t tag, int64_t g_begin, int64_t g_end) {
-    if (!c || tag < 0 || tag >= c->p.n_tag || g_begin < 0 || g_end < g_begin) return MWF_EINVAL;
-    if (!c->have_tree || !c->have_lists || !c->mono_fresh) return MWF_ESTATE;
-    if (g_end > c->n_group) return MWF_ERANGE;
-    if (g_end == g_begin) return MWF_OK;
+// Launch of the force kernel over groups [g_begin, g_end) on the tag's stream and the bookkeeping that goes with it.
+// jdata / joff (device) non-null: method G1, the lists are runs of j records instead of indices into the store.
+static int dispatch_launch(mwf_ctx* c, int32_t tag, int64_t g_begin, int64_t g_end, const float4* jdata, const int64_t* joff) {
     cudaStream_t s = c->tag_stream[tag];
-    if (c->store_event_valid) CU(c, cudaStreamWaitEvent(s, c->ev_store, 0));
     ForceArgs a;
     a.store = c->store;
     a.list = c->list;
     a.list_off = c->list_off;
     a.grp_self = c->grp_self;
     a.items = c->items;
+    a.jdata = jdata;
+    a.joff = joff;
+    a.g_base = g_begin;
     a.accp = c->accp;
     a.item_begin = c->h_item_off[(size_t)g_begin];
     a.n_items = c->h_item_off[(size_t)g_end] - a.item_begin;
@@ -689,6 +697,60 @@ int mwf_dispatch(mwf_ctx* c, int32_t tag, int64_t g_begin, int64_t g_end) {
     c->groups_outstanding += g_end - g_begin;
     if (c->groups_dispatched >= c->n_group) c->acc_full = true;
     return MWF_OK;
+}
+
+int mwf_dispatch(mwf_ctx* c, int32_t tag, int64_t g_begin, int64_t g_end) {
+    if (!c || tag < 0 || tag >= c->p.n_tag || g_begin < 0 || g_end < g_begin) return MWF_EINVAL;
+    if (!c->have_tree || !c->have_lists || !c->mono_fresh) return MWF_ESTATE;
+    if (g_end > c->n_group) return MWF_ERANGE;
+    if (g_end == g_begin) return MWF_OK;
+    if (c->store_event_valid) CU(c, cudaStreamWaitEvent(c->tag_stream[tag], c->ev_store, 0));
+    return dispatch_launch(c, tag, g_begin, g_end, nullptr, nullptr);
+}
+
+int mwf_reserve_data_lists(mwf_ctx* c, int64_t max_entry_per_tag) {
+    if (!c || max_entry_per_tag < 1) return MWF_EINVAL;
+    for (int t = 0; t < c->p.n_tag; ++t)
+        if (c->tag_inflight[t] || !c->tag_ranges[t].empty()) return MWF_ESTATE;
+    CU(c, cudaDeviceSynchronize());
+    for (int t = 0; t < c->p.n_tag; ++t) {
+        if (c->data_buf[t]) { cudaFree(c->data_buf[t]); c->data_buf[t] = nullptr; }
+        if (c->data_off[t]) { cudaFree(c->data_off[t]); c->data_off[t] = nullptr; }
+    }
+    c->data_cap = 0;
+    for (int t = 0; t < c->p.n_tag; ++t) {
+        void *a = nullptr, *b = nullptr;
+        if (cudaMalloc(&a, (size_t)max_entry_per_tag * 16) != cudaSuccess || cudaMalloc(&b, (size_t)(c->p.max_group + 1) * 8) != cudaSuccess) {
+            cudaGetLastError();
+            if (a) cudaFree(a);
+            return MWF_ENOMEM;
+        }
+        c->data_buf[t] = static_cast<float4*>(a);
+        c->data_off[t] = static_cast<int64_t*>(b);
+    }
+    c->data_cap = max_entry_per_tag;
+    return MWF_OK;
+}
+
+int mwf_dispatch_data(mwf_ctx* c, int32_t tag, int64_t g_begin, int64_t g_end, const mwf_posm* jdata, const int64_t* joff, int jdata_on_device) {
+    if (!c || tag < 0 || tag >= c->p.n_tag || g_begin < 0 || g_end < g_begin || !jdata || !joff) return MWF_EINVAL;
+    if (!c->have_tree || !c->have_lists || c->data_cap < 1) return MWF_ESTATE;
+    if (c->ptcl_hi < c->n_ptcl) return MWF_ESTATE;  // the i-particles are read from the store
+    if (g_end > c->n_group) return MWF_ERANGE;
+    if (g_end == g_begin) return MWF_OK;
+    if (c->tag_inflight[tag]) return MWF_ESTATE;  // the tag's staging buffer is still being read: retrieve first
+    const int64_t ng = g_end - g_begin;
+    if (joff[0] != 0) return MWF_ERANGE;
+    for (int64_t g = 0; g < ng; ++g)  // the run of group g_begin + g must be as long as the group's index list
+        if (joff[g + 1] - joff[g] != (c->h_inter[(size_t)(g_begin + g) + 1] - c->h_inter[(size_t)(g_begin + g)]) / c->h_grp_n[(size_t)(g_begin + g)])
+            return MWF_ERANGE;
+    if (joff[ng] > c->data_cap) return MWF_ENOMEM;
+    cudaStream_t s = c->tag_stream[tag];
+    if (c->store_event_valid) CU(c, cudaStreamWaitEvent(s, c->ev_store, 0));
+    CU(c, cudaMemcpyAsync(c->data_off[tag], joff, (size_t)(ng + 1) * 8, cudaMemcpyHostToDevice, s));
+    if (joff[ng] > 0)
+        CU(c, cudaMemcpyAsync(c->data_buf[tag], jdata, (size_t)joff[ng] * 16, jdata_on_device ? cudaMemcpyDeviceToDevice : cudaMemcpyHostToDevice, s));
+    return dispatch_launch(c, tag, g_begin, g_end, c->data_buf[tag], c->data_off[tag]);
 }
 
 int mwf_retrieve(mwf_ctx* c, int32_t tag, mwf_accp* dst, int dst_on_device) {

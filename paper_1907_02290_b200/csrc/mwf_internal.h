@@ -50,6 +50,9 @@ struct ForceArgs {
     const uint8_t* grp_self;    // 1: the group's own particles are in its EPJ list
     const WorkItem* items;
     const int32_t* order;       // cost-sorted permutation of item indices, or nullptr = identity
+    const float4* jdata;        // method G1 (data lists): j records of groups [g_base, ...), else nullptr
+    const int64_t* joff;        // G1: offsets of those groups' runs in jdata, in records
+    int64_t g_base;
     float4* accp;
     unsigned int* counter;      // dynamic scheduling counter (zeroed before launch), or nullptr = static
     int64_t item_begin;

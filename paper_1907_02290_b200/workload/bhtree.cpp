@@ -285,4 +285,20 @@ void bh_get_lists(void* h, int32_t* epj_id, int32_t* spj_id) {
     t->blk_epj.clear(); t->blk_spj.clear();
 }
 
+// Method G1's host-side packing (Fig. 2 "DispatchKernelStream" copies EPJ and SPJ data per walk):
+// for groups [g0, g1) write the records of their EPJ ids (from posm) and then of their SPJ ids (from spj, one
+// float4 per cell) contiguously into out, and the run offsets (in records, relative to out) into joff[g1 - g0 + 1].
+// A pure gather: no arithmetic.  OpenMP over groups.
+void bh_pack_data_lists(int64_t g0, int64_t g1, const float* posm, const float* spj, const int64_t* epj_off, const int32_t* epj_id,
+                        const int64_t* spj_off, const int32_t* spj_id, float* out, int64_t* joff) {
+    joff[0] = 0;
+    for (int64_t g = g0; g < g1; ++g) joff[g - g0 + 1] = joff[g - g0] + (epj_off[g + 1] - epj_off[g]) + (spj_off[g + 1] - spj_off[g]);
+#pragma omp parallel for schedule(dynamic, 16)
+    for (int64_t g = g0; g < g1; ++g) {
+        float* o = out + 4 * joff[g - g0];
+        for (int64_t k = epj_off[g]; k < epj_off[g + 1]; ++k, o += 4) std::memcpy(o, posm + 4 * (int64_t)epj_id[k], 16);
+        for (int64_t k = spj_off[g]; k < spj_off[g + 1]; ++k, o += 4) std::memcpy(o, spj + 4 * (int64_t)spj_id[k], 16);
+    }
+}
+
 }  // extern "C"

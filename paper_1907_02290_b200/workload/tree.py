@@ -38,6 +38,7 @@ def _load():
         lib.bh_build_lists.restype = ctypes.c_int
         lib.bh_build_lists.argtypes = [vp, dbl, vp, vp, ctypes.POINTER(i64), ctypes.POINTER(i64)]
         lib.bh_get_lists.argtypes = [vp, vp, vp]
+        lib.bh_pack_data_lists.argtypes = [i64, i64] + [vp] * 8
         _lib = lib
     return _lib
 
@@ -129,6 +130,23 @@ def build_tree_and_lists(posm: np.ndarray, n_leaf: int, n_grp: int, theta: float
                     perm=perm, cells=cells, geom=geom, level=level, level_first=level_first, root=root,
                     grp_cell=grp_cell, grp_first=grp_first, grp_n=grp_n,
                     epj_off=epj_off, epj_id=epj_id, spj_off=spj_off, spj_id=spj_id, theta=float(theta))
+
+
+def pack_data_lists(w: Workload, g0: int, g1: int, posm: np.ndarray, spj: np.ndarray, out: np.ndarray | None = None):
+    """Method G1's host-side packing (Fig. 2): the j RECORDS of groups [g0, g1) -- EPJ from posm [N,4], then SPJ
+    from spj [n_cell,4] (the monopoles as the device refresh made them) -- gathered into one contiguous float32 [E,4] array
+    (out, e.g. a pinned buffer viewed as numpy) plus the int64 run offsets.  Returns (records, joff)."""
+    lib = _load()
+    n_e = int(w.epj_off[g1] - w.epj_off[g0] + w.spj_off[g1] - w.spj_off[g0])
+    if out is None:
+        out = np.empty((max(1, n_e), 4), np.float32)
+    if out.shape[0] < n_e or out.dtype != np.float32 or not out.flags.c_contiguous:
+        raise ValueError("out must be a C-contiguous float32 [>= %d, 4] array" % n_e)
+    posm = np.ascontiguousarray(posm, dtype=np.float32)
+    spj = np.ascontiguousarray(spj, dtype=np.float32)
+    joff = np.empty(g1 - g0 + 1, np.int64)
+    lib.bh_pack_data_lists(int(g0), int(g1), _p(posm), _p(spj), _p(w.epj_off), _p(w.epj_id), _p(w.spj_off), _p(w.spj_id), _p(out), _p(joff))
+    return out[:n_e], joff
 
 
 def make_workload(cfg: Config, n: int | None = None, theta: float | None = None) -> Workload:

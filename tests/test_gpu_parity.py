@@ -6,7 +6,7 @@ import pytest
 
 import oracle
 from paper_1907_02290_b200 import binding
-from paper_1907_02290_b200.workload import CONFIGS, make_particles, make_workload
+from paper_1907_02290_b200.workload import CONFIGS, build_tree_and_lists, make_particles, make_workload, pack_data_lists
 
 pytestmark = pytest.mark.gpu
 
@@ -150,6 +150,43 @@ def test_monopole_refresh(idx, n):
     assert np.all(dx <= 2.0 ** -22 * scale)
 
 
+def _check_monopoles(cells, posm, side):
+    n_cell = cells.shape[0]
+    f = binding.MultiWalkForce(0.01, max_ptcl=posm.shape[0], max_cell=n_cell, max_group=4, max_entry=64, n_tag=1)
+    f.set_particles(posm)
+    f.set_tree(cells)
+    f.refresh_monopoles()
+    got = f.get_monopoles(n_cell).astype(np.float64)
+    f.refresh_monopoles()
+    assert np.array_equal(got, f.get_monopoles(n_cell).astype(np.float64))
+    f.close()
+    mom = oracle.monopoles(cells, posm)
+    assert np.all(np.abs(got[:, 3] - mom[:, 3]) <= 1e-6 * mom[:, 3])
+    dx = np.linalg.norm(got[:, :3] - mom[:, :3], axis=1)
+    assert np.all(dx <= 2.0 ** -22 * np.maximum(np.linalg.norm(mom[:, :3], axis=1), side))
+
+
+def test_monopole_refresh_tree_shapes():
+    """Tree shapes beyond the configs': very large leaves (n_leaf = 5000), one particle per leaf, a small tree, and a
+    hand-made chain 90 levels deep (far deeper than 21-bit keys can make)."""
+    posm, _ = make_particles(CONFIGS[0], 30011)
+    for n_leaf, n in ((5000, 30011), (16, 2048), (1, 1500), (3, 9000)):
+        w = build_tree_and_lists(posm[:n], n_leaf, 64, 0.9)
+        _check_monopoles(w.cells, w.posm, w.geom[:, 3])
+    # chain: cell 2k (k >= 1) is internal with a one-particle leaf 2k+1 and the next internal cell 2k+2 as children
+    depth, rng = 90, np.random.default_rng(11)
+    n = depth + 1
+    pts = np.concatenate([rng.normal(size=(n, 3)), rng.uniform(0.5, 2.0, size=(n, 1))], axis=1).astype(np.float32)
+    cells = [(0, n, 1, 2)]
+    for k in range(depth):
+        first = k                                   # particles [k, n) are below the k-th chain cell
+        cells.append((first, 1, 0, 0))              # leaf with particle k
+        last = k == depth - 1
+        cells.append((first + 1, n - first - 1, 0 if last else len(cells) + 1, 0 if last else 2))
+    cells = np.array(cells, np.int32)
+    _check_monopoles(cells, pts, np.full(cells.shape[0], 8.0))
+
+
 # ------------------------------------------------------------------ dispatch shapes
 def test_batched_dispatch_over_tags_is_bitwise_identical():
     """Config 2's pipeline: 64-256 groups per dispatch, tags round-robin over the streams."""
@@ -262,6 +299,51 @@ def test_coincident_particles():
     acc, pot = oracle.direct(posm, 0.5)
     np.testing.assert_allclose(out[:, :3], acc, rtol=1e-5, atol=1e-7)
     np.testing.assert_allclose(out[:, 3], pot, rtol=1e-5)
+
+
+# ------------------------------------------------------------------ method G1: data lists (NEXT-3; Fig. 2)
+def test_data_lists_equal_index_lists():
+    """The paper's method G1 (the lists carry j records, sent with every dispatch) against its method G2 (indices into
+    the device store) on the same lists: same sweep and summation order, so the results are bitwise equal; and both
+    match the oracle."""
+    cfg = CONFIGS[1]
+    w = make_workload(cfg, 60001)
+    out_idx, f = gpu_eval(w, cfg.eps, keep=True)
+    spj = f.get_monopoles(w.n_cell)
+    assert expect_code(f.dispatch_data, 0, 0, 1, np.zeros((4, 4), np.float32), np.zeros(2, np.int64)) == binding.ESTATE   # nothing reserved
+    cap = int(w.n_list.max()) * 40
+    f.reserve_data_lists(cap)
+    out = np.full((w.n, 4), np.nan, np.float32)
+    tag, pending, keep_alive = 0, [], {}
+    for gb in range(0, w.n_group, 37):
+        ge = min(w.n_group, gb + 37)
+        if len(pending) == f.n_tag:
+            f.retrieve(pending.pop(0), out)
+        rec, joff = pack_data_lists(w, gb, ge, w.posm, spj)
+        keep_alive[tag] = (rec, joff)                      # host sources stay valid until the tag is retrieved
+        f.dispatch_data(tag, gb, ge, rec, joff)
+        pending.append(tag)
+        tag = (tag + 1) % f.n_tag
+    for t in pending:
+        f.retrieve(t, out)
+    assert np.array_equal(out, out_idx)
+    acc, pot, _ = oracle_eval(w, cfg.eps)
+    check(out, acc, pot, label="G1 data lists")
+    # device-resident records, one dispatch over everything
+    import torch
+    rec, joff = pack_data_lists(w, 0, w.n_group, w.posm, spj)
+    f.reserve_data_lists(rec.shape[0])
+    out2 = np.full((w.n, 4), np.nan, np.float32)
+    f.dispatch_data(1, 0, w.n_group, torch.from_numpy(rec).cuda(), joff)
+    assert expect_code(f.dispatch_data, 1, 0, 1, rec, joff[:2].copy()) == binding.ESTATE              # tag still in flight
+    f.retrieve(1, out2)
+    assert np.array_equal(out2, out_idx)
+    bad = joff.copy()
+    bad[1] += 1
+    assert expect_code(f.dispatch_data, 0, 0, w.n_group, rec, bad) == binding.ERANGE                  # run length != list length
+    f.reserve_data_lists(10)
+    assert expect_code(f.dispatch_data, 0, 0, w.n_group, rec, joff) == binding.ENOMEM
+    f.close()
 
 
 # ------------------------------------------------------------------ list-reuse driver (rows a6, a7; P:242)

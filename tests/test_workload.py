@@ -160,3 +160,20 @@ def test_config_table_matches_baseline_json():
     assert [c.n_leaf for c in CONFIGS] == [8, 16, 16, 16, 16]
     assert [c.eps for c in CONFIGS] == [1 / 64, 1 / 256, 0.005, 1e-4, 1 / 512]
     assert CONFIGS[4].n_reuse == 8 and CONFIGS[4].dt == 1 / 1024
+
+
+def test_pack_data_lists_is_a_plain_gather():
+    """Method G1's host packing: EPJ records then SPJ records per group, contiguous, with run offsets."""
+    from paper_1907_02290_b200.workload import pack_data_lists
+    cfg = CONFIGS[0]
+    w = make_workload(cfg, 3000)
+    rng = np.random.default_rng(3)
+    spj = rng.normal(size=(w.n_cell, 4)).astype(np.float32)
+    g0, g1 = 5, min(w.n_group, 41)
+    rec, joff = pack_data_lists(w, g0, g1, w.posm, spj)
+    assert joff[0] == 0 and rec.shape[0] == joff[-1]
+    for g in range(g0, g1):
+        e = w.epj_id[w.epj_off[g]:w.epj_off[g + 1]]
+        c = w.spj_id[w.spj_off[g]:w.spj_off[g + 1]]
+        want = np.concatenate([w.posm[e], spj[c]])
+        assert np.array_equal(rec[joff[g - g0]:joff[g - g0 + 1]], want)
