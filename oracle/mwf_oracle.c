@@ -21,6 +21,14 @@
  *                  for EPJ and SPJ, the entry whose INDEX equals i is skipped (a different particle
  *                  at the same position is a real pair), pot <= 0 and includes G.
  *   orc_direct     the plain O(N^2) definition of the same sum over all other particles.
+ *   orc_quadrupoles, orc_forces_quad   (the paper says "multipole moments", and
+ *                  measures the monopole case only)  second moment of every cell about its centre of mass,
+ *                  Q_c = sum m_p (x_p - X_c)(x_p - X_c)^T, and the list evaluation in which an SPJ entry acts
+ *                  through M_c and Q_c: the Taylor expansion to second order in (x_p - X_c) of the SAME softened
+ *                  kernel (reading S22 in DESIGN.md), with R = X_c - x_i, s^2 = |R|^2 + eps^2:
+ *                    pot_i -= G [ M/s - tr(Q)/(2 s^3) + 3 (R.Q.R)/(2 s^5) ]
+ *                    acc_i += G [ M R/s^3 - 3 tr(Q) R/(2 s^5) - 3 (Q R)/s^5 + 15 (R.Q.R) R/(2 s^7) ]
+ *                  EPJ entries are evaluated exactly as in orc_forces.
  *   orc_kick_drift, orc_kick   the kick-drift-kick leapfrog BASELINE.json's config 5 names (the orbit
  *                  integration is step 5 of the paper's procedure; section 7.3, P:1171-1185,
  *                  proposes moving it to the accelerator): v += a dt/2, x += v dt; and v += a dt/2.
@@ -109,6 +117,80 @@ void orc_forces(int64_t n_sel, const int64_t* sel, const int32_t* grp_first, con
             for (int64_t e = spj_off[g]; e < spj_off[g + 1]; ++e) {
                 int64_t c = spj_id[e];
                 pair_term(xi, yi, zi, mom[4 * c + 0], mom[4 * c + 1], mom[4 * c + 2], mom[4 * c + 3], eps2, &ax, &ay, &az, &p);
+            }
+            acc[3 * i + 0] = G * ax;
+            acc[3 * i + 1] = G * ay;
+            acc[3 * i + 2] = G * az;
+            pot[i] = G * p;
+        }
+    }
+}
+
+/* quad[6*c + 0..5] = (Qxx, Qyy, Qzz, Qxy, Qxz, Qyz) of cell c about its centre of mass mom[4*c + 0..2], straight
+ * from the definition over the cell's particle range. */
+void orc_quadrupoles(int64_t n_cell, const int32_t* cells4, const float* posm, const double* mom, double* quad) {
+    int64_t c;
+#pragma omp parallel for schedule(dynamic, 64)
+    for (c = 0; c < n_cell; ++c) {
+        int64_t first = cells4[4 * c + 0], cnt = cells4[4 * c + 1];
+        double q[6] = {0.0, 0.0, 0.0, 0.0, 0.0, 0.0};
+        for (int64_t p = first; p < first + cnt; ++p) {
+            double mp = (double)posm[4 * p + 3];
+            double yx = (double)posm[4 * p + 0] - mom[4 * c + 0];
+            double yy = (double)posm[4 * p + 1] - mom[4 * c + 1];
+            double yz = (double)posm[4 * p + 2] - mom[4 * c + 2];
+            q[0] += mp * yx * yx;
+            q[1] += mp * yy * yy;
+            q[2] += mp * yz * yz;
+            q[3] += mp * yx * yy;
+            q[4] += mp * yx * yz;
+            q[5] += mp * yy * yz;
+        }
+        for (int k = 0; k < 6; ++k) quad[6 * c + k] = q[k];
+    }
+}
+
+/* Monopole + quadrupole term of one cell on particle i (see the header). */
+static void cell_term_quad(double xi, double yi, double zi, const double* X, double M, const double* Q, double eps2,
+                           double* ax, double* ay, double* az, double* pot) {
+    double Rx = X[0] - xi, Ry = X[1] - yi, Rz = X[2] - zi;
+    double s2 = Rx * Rx + Ry * Ry + Rz * Rz + eps2;
+    double s1 = sqrt(s2);
+    double s3 = s2 * s1, s5 = s3 * s2, s7 = s5 * s2;
+    double tr = Q[0] + Q[1] + Q[2];
+    double QRx = Q[0] * Rx + Q[3] * Ry + Q[4] * Rz;
+    double QRy = Q[3] * Rx + Q[1] * Ry + Q[5] * Rz;
+    double QRz = Q[4] * Rx + Q[5] * Ry + Q[2] * Rz;
+    double RQR = Rx * QRx + Ry * QRy + Rz * QRz;
+    *pot -= M / s1 - tr / (2.0 * s3) + 3.0 * RQR / (2.0 * s5);
+    double cR = M / s3 - 3.0 * tr / (2.0 * s5) + 15.0 * RQR / (2.0 * s7);
+    *ax += cR * Rx - 3.0 * QRx / s5;
+    *ay += cR * Ry - 3.0 * QRy / s5;
+    *az += cR * Rz - 3.0 * QRz / s5;
+}
+
+/* As orc_forces, with SPJ entries acting through monopole and quadrupole (quad from orc_quadrupoles). */
+void orc_forces_quad(int64_t n_sel, const int64_t* sel, const int32_t* grp_first, const int32_t* grp_n,
+                     const int64_t* epj_off, const int32_t* epj_id, const int64_t* spj_off, const int32_t* spj_id,
+                     const float* posm, const double* mom, const double* quad, double eps, double G, double* acc, double* pot) {
+    const double eps2 = eps * eps;
+    int64_t s;
+#pragma omp parallel for schedule(dynamic, 1)
+    for (s = 0; s < n_sel; ++s) {
+        int64_t g = sel ? sel[s] : s;
+        int64_t first = grp_first[g], cnt = grp_n[g];
+        for (int64_t i = first; i < first + cnt; ++i) {
+            double xi = (double)posm[4 * i + 0], yi = (double)posm[4 * i + 1], zi = (double)posm[4 * i + 2];
+            double ax = 0.0, ay = 0.0, az = 0.0, p = 0.0;
+            for (int64_t e = epj_off[g]; e < epj_off[g + 1]; ++e) {
+                int64_t k = epj_id[e];
+                if (k == i) continue;
+                pair_term(xi, yi, zi, (double)posm[4 * k + 0], (double)posm[4 * k + 1], (double)posm[4 * k + 2],
+                          (double)posm[4 * k + 3], eps2, &ax, &ay, &az, &p);
+            }
+            for (int64_t e = spj_off[g]; e < spj_off[g + 1]; ++e) {
+                int64_t c = spj_id[e];
+                cell_term_quad(xi, yi, zi, mom + 4 * c, mom[4 * c + 3], quad + 6 * c, eps2, &ax, &ay, &az, &p);
             }
             acc[3 * i + 0] = G * ax;
             acc[3 * i + 1] = G * ay;

@@ -33,6 +33,8 @@ def _load():
         lib.orc_monopoles.argtypes = [i64, vp, vp, vp]
         lib.orc_forces.argtypes = [i64, vp, vp, vp, vp, vp, vp, vp, vp, vp, dbl, dbl, vp, vp]
         lib.orc_direct.argtypes = [i64, vp, dbl, dbl, vp, vp]
+        lib.orc_quadrupoles.argtypes = [i64, vp, vp, vp, vp]
+        lib.orc_forces_quad.argtypes = [i64, vp, vp, vp, vp, vp, vp, vp, vp, vp, vp, dbl, dbl, vp, vp]
         lib.orc_kick_drift.argtypes = [i64, vp, vp, vp, dbl, vp, vp]
         lib.orc_kick.argtypes = [i64, vp, vp, dbl, vp]
         _lib = lib
@@ -65,9 +67,19 @@ def monopoles(cells: np.ndarray, posm: np.ndarray) -> np.ndarray:
     return mom
 
 
-def forces(posm, mom, grp_first, grp_n, epj_off, epj_id, spj_off, spj_id, eps: float, G: float = 1.0, groups=None):
+def quadrupoles(cells: np.ndarray, posm: np.ndarray, mom: np.ndarray) -> np.ndarray:
+    """[n_cell,6] float64 (Qxx, Qyy, Qzz, Qxy, Qxz, Qyz): second moments about the centres of mass in `mom`."""
+    cells = _c(cells, np.int32)
+    posm = _c(posm, np.float32)
+    mom = _c(mom, np.float64)
+    quad = np.empty((cells.shape[0], 6), np.float64)
+    _load().orc_quadrupoles(cells.shape[0], _p(cells), _p(posm), _p(mom), _p(quad))
+    return quad
+
+
+def forces(posm, mom, grp_first, grp_n, epj_off, epj_id, spj_off, spj_id, eps: float, G: float = 1.0, groups=None, quad=None):
     """acc [N,3], pot [N] in float64 for the selected groups (all when `groups` is None); particles of
-    other groups are left NaN."""
+    other groups are left NaN.  quad (from `quadrupoles`): SPJ entries act through monopole and quadrupole."""
     posm = _c(posm, np.float32)
     mom = _c(mom, np.float64)
     grp_first, grp_n = _c(grp_first, np.int32), _c(grp_n, np.int32)
@@ -81,6 +93,11 @@ def forces(posm, mom, grp_first, grp_n, epj_off, epj_id, spj_off, spj_id, eps: f
     else:
         sel = _c(groups, np.int64)
         n_sel = sel.shape[0]
+    if quad is not None:
+        quad = _c(quad, np.float64)
+        _load().orc_forces_quad(n_sel, _p(sel), _p(grp_first), _p(grp_n), _p(epj_off), _p(epj_id), _p(spj_off), _p(spj_id),
+                                _p(posm), _p(mom), _p(quad), float(eps), float(G), _p(acc), _p(pot))
+        return acc, pot
     _load().orc_forces(n_sel, _p(sel), _p(grp_first), _p(grp_n), _p(epj_off), _p(epj_id), _p(spj_off), _p(spj_id),
                        _p(posm), _p(mom), float(eps), float(G), _p(acc), _p(pot))
     return acc, pot

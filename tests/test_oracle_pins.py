@@ -289,3 +289,151 @@ def test_leapfrog_harmonic_oscillator_second_order_and_reversible():
     x, v = _kdk(x0, v0, lambda x: -x, 1.0 / 64, 64)
     xb, vb = _kdk(x, v, lambda x: -x, -1.0 / 64, 64)
     assert abs(xb[0, 0] - 1.0) < 1e-5 and abs(vb[0, 0]) < 1e-5
+
+
+# ---------------------------------------------------------------- NEXT-3: quadrupole SPJ (reading S22)
+def _cell_on_points(src_posm, test_points, eps, G=1.0, quad=True):
+    """Sources = one cell (cell 0, particles [0, n)); every test point is its own one-particle group whose
+    list is that single SPJ entry.  Returns (acc, pot) at the test points."""
+    n, k = src_posm.shape[0], test_points.shape[0]
+    posm = np.concatenate([src_posm, np.concatenate([test_points, np.zeros((k, 1))], axis=1)]).astype(np.float32)
+    cells = np.array([[0, n, 0, 0]], np.int32)
+    mom = oracle.monopoles(cells, posm)
+    q = oracle.quadrupoles(cells, posm, mom) if quad else None
+    gf = np.arange(n, n + k, dtype=np.int32)
+    gn = np.ones(k, np.int32)
+    eo = np.zeros(k + 1, np.int64)
+    so = np.arange(k + 1, dtype=np.int64)
+    acc, pot = oracle.forces(posm, mom, gf, gn, eo, np.zeros(0, np.int32), so, np.zeros(k, np.int32), eps, G, quad=q)
+    return acc[n:], pot[n:], posm
+
+
+def test_quadrupole_two_masses_closed_form():
+    """Two masses m at (0,0,+-a), eps = 0.  Taylor series of the exact potential to order a^2 (textbook):
+    on the x axis  phi = -G (2m/d - m a^2/d^3), on the z axis  phi = -G (2m/d + 2 m a^2/d^3).  Values typed from the
+    series, not from the oracle's formula; catches a wrong coefficient or sign of either quadrupole term."""
+    m, a, d, G = 0.75, 0.5, 8.0, 2.0
+    src = np.array([[0, 0, a, m], [0, 0, -a, m]], np.float64)
+    pts = np.array([[d, 0, 0], [0, 0, d], [0, -d, 0]], np.float64)
+    acc, pot, _ = _cell_on_points(src, pts, 0.0, G)
+    assert pot[0] == pytest.approx(-G * (2 * m / d - m * a * a / d ** 3), rel=1e-14)
+    assert pot[1] == pytest.approx(-G * (2 * m / d + 2 * m * a * a / d ** 3), rel=1e-14)
+    assert pot[2] == pytest.approx(pot[0], rel=1e-14)
+    # radial derivative of the same series: a_x = -d phi/dx on the x axis, a_z = -d phi/dz on the z axis
+    np.testing.assert_allclose(acc[0], [-G * (2 * m / d ** 2 - 3 * m * a * a / d ** 4), 0, 0], rtol=1e-13, atol=1e-16)
+    np.testing.assert_allclose(acc[1], [0, 0, -G * (2 * m / d ** 2 + 6 * m * a * a / d ** 4)], rtol=1e-13, atol=1e-16)
+
+
+def test_quadrupole_of_an_octahedron_vanishes():
+    """Six equal masses at +-a on the axes have Q = 2 m a^2 * identity: no quadrupole field for eps = 0, so the
+    quadrupole evaluation equals the monopole one.  Catches a wrong trace term."""
+    a, m = 0.3, 1.5
+    src = np.array([[a, 0, 0, m], [-a, 0, 0, m], [0, a, 0, m], [0, -a, 0, m], [0, 0, a, m], [0, 0, -a, m]], np.float64)
+    pts = np.array([[3.0, 1.0, -2.0], [0.5, 4.0, 0.25]])
+    acc_q, pot_q, _ = _cell_on_points(src, pts, 0.0)
+    acc_m, pot_m, _ = _cell_on_points(src, pts, 0.0, quad=False)
+    np.testing.assert_allclose(acc_q, acc_m, rtol=1e-13)
+    np.testing.assert_allclose(pot_q, pot_m, rtol=1e-13)
+
+
+@pytest.mark.parametrize("eps", [0.0, 0.7])
+def test_quadrupole_convergence_order(eps):
+    """Against direct summation over the cluster, the error of the monopole evaluation falls as d^-3 (potential) and
+    d^-4 (acceleration) with distance d, that of the quadrupole evaluation one power faster -- also with softening,
+    because the expansion is of the softened kernel itself.  A dropped term or a wrong coefficient anywhere leaves a
+    residual of the lower order and fails the ratio."""
+    rng = np.random.default_rng(5)
+    n = 60
+    src = np.concatenate([rng.uniform(-0.5, 0.5, size=(n, 3)), rng.uniform(0.5, 1.5, size=(n, 1))], axis=1)
+    u = np.array([0.36, -0.48, 0.8])
+    dist = np.array([8.0, 16.0, 32.0, 64.0])
+    err = {}
+    for quad in (False, True):
+        acc, pot, posm = _cell_on_points(src, dist[:, None] * u[None, :], eps, quad=quad)
+        # direct sum over the (fp32-rounded) sources at the (fp32-rounded) test points
+        ea, ep = [], []
+        for k in range(len(dist)):
+            d = posm[:n, :3].astype(np.float64) - posm[n + k, :3].astype(np.float64)
+            r2 = (d * d).sum(1) + eps * eps
+            mk = posm[:n, 3].astype(np.float64)
+            ep.append(abs(pot[k] - (-(mk / np.sqrt(r2)).sum())))
+            ea.append(np.linalg.norm(acc[k] - (mk[:, None] * d / r2[:, None] ** 1.5).sum(0)))
+        err[quad] = (np.array(ea), np.array(ep))
+    for quad, p_pot in ((False, 3), (True, 4)):
+        ea, ep = err[quad]
+        # the source centre of mass is the expansion centre, so the dipole vanishes; ratios per doubling of d
+        assert np.all(np.abs(np.log2(ep[:-1] / ep[1:]) - p_pot) < 0.35), (quad, ep)
+        assert np.all(np.abs(np.log2(ea[:-1] / ea[1:]) - (p_pot + 1)) < 0.35), (quad, ea)
+    assert np.all(err[True][1] < 0.2 * err[False][1])
+
+
+def test_quadrupole_acc_is_minus_grad_pot():
+    """acc = -grad(pot) by central differences of the oracle's own potential at displaced test points (positions
+    chosen exactly representable in fp32): ties the acceleration formula to the potential that the pins above fix."""
+    rng = np.random.default_rng(9)
+    src = np.concatenate([rng.uniform(-0.5, 0.5, size=(20, 3)), rng.uniform(0.5, 1.5, size=(20, 1))], axis=1)
+    x0 = np.array([3.0, -2.5, 4.25])
+    h = 2.0 ** -10
+    pts = [x0]
+    for ax in range(3):
+        for sgn in (+1, -1):
+            p = x0.copy()
+            p[ax] += sgn * h
+            pts.append(p)
+    acc, pot, _ = _cell_on_points(src, np.array(pts), 0.3)
+    grad = np.array([(pot[1 + 2 * ax] - pot[2 + 2 * ax]) / (2 * h) for ax in range(3)])
+    np.testing.assert_allclose(acc[0], -grad, rtol=3e-6)
+
+
+def test_quadrupole_moment_invariants():
+    """Q_c on a real tree: parallel-axis theorem (parent = sum over children of Q_child + M_child dd^T, d = X_child - X),
+    trace = sum m |x - X|^2 >= 0, translation invariance, and the root equals the numpy definition."""
+    cfg = CONFIGS[0]
+    w = make_workload(cfg, 3000)
+    mom = oracle.monopoles(w.cells, w.posm)
+    q = oracle.quadrupoles(w.cells, w.posm, mom)
+
+    def full(v):
+        return np.array([[v[0], v[3], v[4]], [v[3], v[1], v[5]], [v[4], v[5], v[2]]])
+
+    x = w.posm[:, :3].astype(np.float64)
+    m = w.posm[:, 3].astype(np.float64)
+    y = x - mom[0, :3]
+    np.testing.assert_allclose(full(q[0]), np.einsum("p,pa,pb->ab", m, y, y), rtol=1e-12, atol=1e-15)
+    assert np.all(q[:, :3].sum(1) >= 0)
+    for c in range(w.n_cell):
+        fc, nc = w.cells[c, 2], w.cells[c, 3]
+        if nc == 0:
+            continue
+        tot = np.zeros((3, 3))
+        for ch in range(fc, fc + nc):
+            d = mom[ch, :3] - mom[c, :3]
+            tot += full(q[ch]) + mom[ch, 3] * np.outer(d, d)
+        np.testing.assert_allclose(full(q[c]), tot, rtol=1e-9, atol=1e-14)
+    shifted = w.posm.copy()
+    shifted[:, :3] += np.array([0.5, -0.25, 2.0], np.float32)        # exact in fp32 for these magnitudes? compare loosely
+    mom2 = oracle.monopoles(w.cells, shifted)
+    q2 = oracle.quadrupoles(w.cells, shifted, mom2)
+    np.testing.assert_allclose(q2, q, rtol=2e-4, atol=1e-9)
+
+
+def test_quadrupole_tree_forces_beat_monopole():
+    """On Barnes-Hut lists the quadrupole evaluation is closer to direct summation than the monopole one (by more
+    than 2x in RMS at theta = 0.7 and 0.4), and both converge as theta falls."""
+    cfg = CONFIGS[0]
+    posm, _ = make_particles(cfg, 4096)
+    rms = {}
+    for theta in (0.7, 0.4):
+        w = build_tree_and_lists(posm, cfg.n_leaf, cfg.n_grp, theta)
+        acc_d, _ = oracle.direct(w.posm, cfg.eps)
+        mom = oracle.monopoles(w.cells, w.posm)
+        q = oracle.quadrupoles(w.cells, w.posm, mom)
+        lists = (w.grp_first, w.grp_n, w.epj_off, w.epj_id, w.spj_off, w.spj_id)
+        for name, quad in (("mono", None), ("quad", q)):
+            acc, _ = oracle.forces(w.posm, mom, *lists, cfg.eps, quad=quad)
+            e = np.linalg.norm(acc - acc_d, axis=1) / np.linalg.norm(acc_d, axis=1)
+            rms[(name, theta)] = np.sqrt(np.mean(e ** 2))
+    assert rms[("quad", 0.7)] < rms[("mono", 0.7)] / 2
+    assert rms[("quad", 0.4)] < rms[("mono", 0.4)] / 2
+    assert rms[("quad", 0.4)] < rms[("quad", 0.7)]
+    print(rms)
