@@ -326,6 +326,51 @@ def g1_leg(args, cfg, binding, device):
     return 0
 
 
+def quad_leg(args, cfg, binding, device):
+    """Quadrupole SPJ (NEXT-3): the list-reuse step with order 2 -- refresh of monopoles AND quadrupoles, force kernel,
+    quadrupole correction kernel -- device-resident source and destination.  k_quad is ALU-bound like k_force: 36 packed
+    FP32 operations + 2 MUFU per i per j-pair = 60 flop per SPJ correction (FMA = 2, rsqrt = 4, the paper's counting)."""
+    import torch
+    from paper_1907_02290_b200.workload import make_workload
+    N_OP_QUAD = 60
+    w = make_workload(cfg, args.n)
+    f = binding.MultiWalkForce.for_workload(w, n_tag=args.n_tag, device=device)
+    f.upload_workload(w, binding.MAKE_LIST_FOR_REUSE)
+    src_dev = torch.from_numpy(w.posm).to(f.device)
+    dst_dev = torch.zeros((w.n, 4), dtype=torch.float32, device=f.device)
+    n_sm = torch.cuda.get_device_properties(device).multi_processor_count
+    peak = n_sm * 256 * (measured_peaks().get("sm_max_mhz") or 1965.0) * 1e6
+    inter = w.interactions
+    inter_spj = int(np.sum(w.grp_n.astype(np.int64) * np.diff(w.spj_off)))
+    res = {}
+    for order in (1, 2):
+        f.set_spj_order(order)
+        ms_step, ms_force, ms_quad, ms_ref = [], [], [], []
+        s0 = f.streams[0]
+        for it in range(args.warmup + args.steps):
+            ev = [torch.cuda.Event(enable_timing=True) for _ in range(4)]
+            f.begin_step(binding.REUSE_LIST)
+            ev[0].record(s0); f.set_particles(src_dev, 0, w.n, s0)
+            ev[1].record(s0); f.refresh_monopoles(s0)
+            ev[2].record(s0); f.dispatch(0, 0, w.n_group); f.retrieve(0, dst_dev)
+            ev[3].record(s0); torch.cuda.synchronize()
+            if it >= args.warmup:
+                ms_step.append(ev[0].elapsed_time(ev[3])); ms_ref.append(ev[1].elapsed_time(ev[2]))
+                q = f.last_quad_ms(0) if order == 2 else 0.0
+                ms_quad.append(q); ms_force.append(f.last_dispatch_ms(0) - q)
+        r = {"ms_per_step": float(np.median(ms_step)), "refresh_ms": float(np.median(ms_ref)), "k_force_ms": float(np.median(ms_force))}
+        if order == 2:
+            tq = float(np.median(ms_quad)) * 1e-3
+            r.update({"k_quad_ms": tq * 1e3, "spj_interactions": inter_spj, "flop_per_correction": N_OP_QUAD,
+                      "k_quad_tflops": N_OP_QUAD * inter_spj / tq / 1e12, "k_quad_frac_fp32_peak": N_OP_QUAD * inter_spj / tq / peak})
+        res["order_%d" % order] = r
+    f.close()
+    print(json.dumps({"leg": "quad", "config": workload_config(cfg, w), "steps": args.steps, "warmup": args.warmup,
+                      "interactions": inter, "spj_fraction_of_interactions": inter_spj / inter, "results": res,
+                      "peak_tflops": peak / 1e12, "timing": "CUDA events, device-resident source and destination"}), flush=True)
+    return 0
+
+
 # ----------------------------------------------------------------------------- main
 def main():
     ap = argparse.ArgumentParser()
@@ -337,10 +382,11 @@ def main():
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--cpu-baseline-seconds", type=float, default=15.0)
     ap.add_argument("--n-tag", type=int, default=8)
-    ap.add_argument("--leg", default="step", choices=["step", "construction", "sweep", "g1"],
+    ap.add_argument("--leg", default="step", choices=["step", "construction", "sweep", "g1", "quad"],
                     help="step: the list-reuse step (the contract's JSON line); construction: only the device-side construction step; "
                          "sweep: kernel time per interaction against <n_i> and theta (the paper's Fig. A.1, P:1197-1212); "
-                         "g1: the paper's method G1 (lists carry j records, sent every step) against the index method")
+                         "g1: the paper's method G1 (lists carry j records, sent every step) against the index method; "
+                         "quad: the reuse step with quadrupole SPJ (refresh + force + quadrupole kernels)")
     args = ap.parse_args()
     args.warmup = max(args.warmup, 3) if args.impl == "ours" else args.warmup
 
@@ -371,6 +417,8 @@ def main():
         return sweep_leg(args, cfg, binding, local)
     if args.leg == "g1":
         return g1_leg(args, cfg, binding, local)
+    if args.leg == "quad":
+        return quad_leg(args, cfg, binding, local)
 
     t = time.perf_counter()
     w = make_workload(cfg, args.n)

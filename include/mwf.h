@@ -154,6 +154,22 @@ int mwf_reserve_data_lists(mwf_ctx* c, int64_t max_entry_per_tag);
 int mwf_dispatch_data(mwf_ctx* c, int32_t tag, int64_t g_begin, int64_t g_end, const mwf_posm* jdata, const int64_t* joff,
                       int jdata_on_device);
 
+/* ---- Quadrupole SPJ (the paper computes "multipole moments" of the cells, and
+ * measures the monopole case).  order = 1 (default): an SPJ entry is a point mass at the cell's centre of mass.
+ * order = 2: it also carries Q = sum m (x - X)(x - X)^T about the centre of mass X and acts through the second-order
+ * Taylor expansion of the same softened kernel (reading S22 of DESIGN.md; R = X - x_i, s^2 = |R|^2 + eps^2):
+ *     pot_i -= G [ M/s - tr(Q)/(2 s^3) + 3 (R.Q.R)/(2 s^5) ]
+ *     acc_i += G [ M R/s^3 - 3 tr(Q) R/(2 s^5) - 3 (Q R)/s^5 + 15 (R.Q.R) R/(2 s^7) ]
+ * mwf_refresh_monopoles() then also computes Q bottom-up (parallel-axis theorem, fp64), and every mwf_dispatch()
+ * runs a second kernel behind the force kernel that adds the Q terms of the SPJ part of each group's list.
+ * Allocates 80 B per max_cell with cudaMalloc on first use (MWF_ENOMEM); marks the moments stale when the order
+ * changes; MWF_ESTATE while a tag is in flight or unretrieved.  mwf_dispatch_data() supports order 1 only. */
+int mwf_set_spj_order(mwf_ctx* c, int order);
+/* Test hook: 8 floats per cell (Qxx Qyy Qzz Qxy Qxz Qyz tr(Q)/2 0) as the refresh stored them.  dst HOST or DEVICE. */
+int mwf_get_quadrupoles(mwf_ctx* c, float* dst, int dst_on_device);
+/* Timing hook: ms of the quadrupole kernel of the last mwf_dispatch on `tag` (mwf_last_dispatch_ms covers both kernels). */
+int mwf_last_quad_ms(mwf_ctx* c, int32_t tag, float* ms);
+
 /* (5) Copy acc+pot of the particles of every group dispatched under `tag` since its last retrieve into
  * dst and wait for it.  dst: base of an N-record array indexed by tree-order particle
  * position, HOST or DEVICE; records of other particles are not touched.  dst == NULL: wait for the tag and

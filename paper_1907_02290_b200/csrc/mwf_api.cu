@@ -71,6 +71,13 @@ struct mwf_ctx {
     float4* data_buf[MWF_MAX_TAG]{};
     int64_t* data_off[MWF_MAX_TAG]{};
     int64_t data_cap = 0;
+    // quadrupole SPJ (NEXT-3): cudaMalloc'ed when mwf_set_spj_order(2) is first called
+    int spj_order = 1;
+    double* quad64 = nullptr;   // [6 * max_cell]
+    float4* quad = nullptr;     // [2 * max_cell]
+    int quad_ctas_per_sm = 0;
+    cudaEvent_t ev_kq[MWF_MAX_TAG]{};
+    bool tag_quad[MWF_MAX_TAG]{};
     uint32_t counter_seq = 0;
     int64_t n_launch = 0, n_inter = 0;
     std::string cuda_err;
@@ -460,6 +467,7 @@ int mwf_create(mwf_ctx** out, const mwf_params* p, void* arena, int64_t arena_by
         ok = ok && cudaEventCreateWithFlags(&c->ev_tag[t], cudaEventDisableTiming) == cudaSuccess;
         ok = ok && cudaEventCreate(&c->ev_k0[t]) == cudaSuccess;
         ok = ok && cudaEventCreate(&c->ev_k1[t]) == cudaSuccess;
+        ok = ok && cudaEventCreate(&c->ev_kq[t]) == cudaSuccess;
     }
     ok = ok && cudaEventCreateWithFlags(&c->ev_store, cudaEventDisableTiming) == cudaSuccess;
     ok = ok && cudaMemset(c->counters, 0, N_COUNTER * 4) == cudaSuccess;
@@ -477,7 +485,10 @@ int mwf_destroy(mwf_ctx* c) {
         if (c->ev_tag[t]) cudaEventDestroy(c->ev_tag[t]);
         if (c->ev_k0[t]) cudaEventDestroy(c->ev_k0[t]);
         if (c->ev_k1[t]) cudaEventDestroy(c->ev_k1[t]);
+        if (c->ev_kq[t]) cudaEventDestroy(c->ev_kq[t]);
     }
+    if (c->quad64) cudaFree(c->quad64);
+    if (c->quad) cudaFree(c->quad);
     if (c->ev_store) cudaEventDestroy(c->ev_store);
     for (int t = 0; t < MWF_MAX_TAG; ++t) {
         if (c->data_buf[t]) cudaFree(c->data_buf[t]);
@@ -631,7 +642,8 @@ int mwf_refresh_monopoles(mwf_ctx* c, void* stream) {
     cudaStream_t s = static_cast<cudaStream_t>(stream);
     int rc = before_store_op(c, s);
     if (rc) return rc;
-    CU(c, launch_monopoles(c->cells, c->parent, c->n_cell, c->n_ptcl, c->store, c->mom64, c->arrive, s));
+    CU(c, launch_monopoles(c->cells, c->parent, c->n_cell, c->n_ptcl, c->store, c->mom64, c->arrive,
+                           c->spj_order == 2 ? c->quad64 : nullptr, c->spj_order == 2 ? c->quad : nullptr, s));
     ++c->n_launch;
     c->mono_fresh = true;
     return after_store_op(c, s);
@@ -676,6 +688,25 @@ static int dispatch_launch(mwf_ctx* c, int32_t tag, int64_t g_begin, int64_t g_e
     }
     CU(c, cudaEventRecord(c->ev_k0[tag], s));
     CU(c, launch_force(a, grid, s));
+    c->tag_quad[tag] = false;
+    if (c->spj_order == 2) {  // quadrupole terms of the SPJ entries, added behind the monopole kernel
+        QuadArgs q;
+        q.store = c->store; q.quad = c->quad; q.list = c->list; q.list_off = c->list_off;
+        q.epj_off = c->st_epj_off; q.spj_off = c->st_spj_off;
+        q.items = c->items; q.order = a.order; q.accp = c->accp;
+        q.item_begin = a.item_begin; q.n_items = a.n_items; q.n_ptcl = c->n_ptcl; q.eps2 = a.eps2; q.G = a.G;
+        const int64_t qres = (int64_t)c->n_sm * c->quad_ctas_per_sm;
+        const int qgrid = (int)std::min(want, qres);
+        q.counter = nullptr;
+        if (want > qres) {
+            q.counter = c->counters + (c->counter_seq++ % N_COUNTER);
+            CU(c, cudaMemsetAsync(q.counter, 0, sizeof(unsigned int), s));
+        }
+        CU(c, cudaEventRecord(c->ev_kq[tag], s));
+        CU(c, launch_quad(q, qgrid, s));
+        c->tag_quad[tag] = true;
+        ++c->n_launch;
+    }
     CU(c, cudaEventRecord(c->ev_k1[tag], s));
     CU(c, cudaEventRecord(c->ev_tag[tag], s));
     c->tag_timed[tag] = true;
@@ -734,7 +765,7 @@ int mwf_reserve_data_lists(mwf_ctx* c, int64_t max_entry_per_tag) {
 
 int mwf_dispatch_data(mwf_ctx* c, int32_t tag, int64_t g_begin, int64_t g_end, const mwf_posm* jdata, const int64_t* joff, int jdata_on_device) {
     if (!c || tag < 0 || tag >= c->p.n_tag || g_begin < 0 || g_end < g_begin || !jdata || !joff) return MWF_EINVAL;
-    if (!c->have_tree || !c->have_lists || c->data_cap < 1) return MWF_ESTATE;
+    if (!c->have_tree || !c->have_lists || c->data_cap < 1 || c->spj_order != 1) return MWF_ESTATE;
     if (c->ptcl_hi < c->n_ptcl) return MWF_ESTATE;  // the i-particles are read from the store
     if (g_end > c->n_group) return MWF_ERANGE;
     if (g_end == g_begin) return MWF_OK;
@@ -1011,6 +1042,46 @@ int mwf_step_reuse(mwf_ctx* c, float dt) {
     rc = mwf_dispatch(c, 0, 0, c->n_group);
     if (rc) return rc;
     return mwf_kick(c, dt, s0);
+}
+
+int mwf_set_spj_order(mwf_ctx* c, int order) {
+    if (!c || (order != 1 && order != 2)) return MWF_EINVAL;
+    for (int t = 0; t < c->p.n_tag; ++t)
+        if (c->tag_inflight[t] || !c->tag_ranges[t].empty()) return MWF_ESTATE;
+    if (order == 2 && !c->quad) {
+        void *a = nullptr, *b = nullptr;
+        if (cudaMalloc(&a, (size_t)c->p.max_cell * 48) != cudaSuccess || cudaMalloc(&b, (size_t)c->p.max_cell * 32) != cudaSuccess) {
+            cudaGetLastError();
+            if (a) cudaFree(a);
+            return MWF_ENOMEM;
+        }
+        c->quad64 = static_cast<double*>(a);
+        c->quad = static_cast<float4*>(b);
+        c->quad_ctas_per_sm = quad_max_ctas_per_sm();
+        if (c->quad_ctas_per_sm < 1) return MWF_ECUDA;
+    }
+    if (order != c->spj_order) {
+        c->mono_fresh = false;  // the moments on the device are those of the other order
+        c->acc_full = false;
+    }
+    c->spj_order = order;
+    return MWF_OK;
+}
+
+int mwf_get_quadrupoles(mwf_ctx* c, float* dst, int dst_on_device) {
+    if (!c || !dst) return MWF_EINVAL;
+    if (!c->have_tree || !c->mono_fresh || c->spj_order != 2) return MWF_ESTATE;
+    CU(c, cudaDeviceSynchronize());
+    CU(c, cudaMemcpy(dst, c->quad, (size_t)c->n_cell * 32, dst_on_device ? cudaMemcpyDeviceToDevice : cudaMemcpyDeviceToHost));
+    return MWF_OK;
+}
+
+int mwf_last_quad_ms(mwf_ctx* c, int32_t tag, float* ms) {
+    if (!c || tag < 0 || tag >= c->p.n_tag || !ms) return MWF_EINVAL;
+    if (!c->tag_timed[tag] || !c->tag_quad[tag]) return MWF_ESTATE;
+    CU(c, cudaEventSynchronize(c->ev_k1[tag]));
+    CU(c, cudaEventElapsedTime(ms, c->ev_kq[tag], c->ev_k1[tag]));
+    return MWF_OK;
 }
 
 int mwf_get_monopoles(mwf_ctx* c, mwf_posm* dst, int dst_on_device) {

@@ -61,14 +61,36 @@ struct ForceArgs {
     float G;
 };
 
+// Quadrupole correction of the SPJ entries (NEXT-3, quad_kernel.cu): same items and schedule as the force kernel.
+struct QuadArgs {
+    const float4* store;
+    const float4* quad;         // two float4 per cell: (Qxx Qyy Qzz Qxy) (Qxz Qyz tr(Q)/2 0)
+    const int32_t* list;
+    const int64_t* list_off;
+    const int64_t* epj_off;     // scanned EPJ / SPJ counts per group: the SPJ part of group g starts at
+    const int64_t* spj_off;     //   list_off[g] + epj_off[g+1] - epj_off[g] and has spj_off[g+1] - spj_off[g] entries
+    const WorkItem* items;
+    const int32_t* order;
+    float4* accp;
+    unsigned int* counter;
+    int64_t item_begin;
+    int64_t n_items;
+    int64_t n_ptcl;
+    float eps2;
+    float G;
+};
+cudaError_t launch_quad(const QuadArgs& a, int grid, cudaStream_t s);
+int quad_max_ctas_per_sm();
+
 // kernels' host launchers (defined next to their kernels)
 cudaError_t launch_force(const ForceArgs& a, int grid, cudaStream_t s);
 int force_max_ctas_per_sm();
 
 cudaError_t launch_tree_prepare(const mwf_cell* cells, int64_t n_cell, int64_t max_ptcl, int32_t* parent, int32_t* counter,
                                 unsigned int* err, cudaStream_t s);
+// quad64 / quad non-null: also the second moments about the centres of mass (6 doubles per cell) and their float record
 cudaError_t launch_monopoles(const mwf_cell* cells, const int32_t* parent, int64_t n_cell, int64_t n_ptcl, float4* store,
-                             double4* mom64, int32_t* counter, cudaStream_t s);
+                             double4* mom64, int32_t* counter, double* quad64, float4* quad, cudaStream_t s);
 cudaError_t launch_merge_lists(int64_t n_group, const int32_t* grp_first, const int32_t* grp_n, const int64_t* epj_off,
                                const int32_t* epj_id, const int64_t* spj_off, const int32_t* spj_id, const int64_t* list_off,
                                int64_t n_ptcl, int64_t n_cell, int32_t* list, uint8_t* grp_self, unsigned int* err, cudaStream_t s);

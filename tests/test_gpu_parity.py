@@ -346,6 +346,89 @@ def test_data_lists_equal_index_lists():
     f.close()
 
 
+# ------------------------------------------------------------------ quadrupole SPJ (NEXT-3, reading S22)
+@pytest.mark.parametrize("idx,n", [(0, None), (2, 65537), (3, 50000)])
+def test_quadrupole_spj(idx, n):
+    """order 2: the refresh also makes Q bottom-up, the dispatch adds the Q terms of the SPJ entries behind the force
+    kernel.  Moments and forces against the oracle's quadrupole evaluation on the same lists; switching back to order 1
+    reproduces the monopole result bit for bit."""
+    cfg = CONFIGS[idx]
+    w = make_workload(cfg, n)
+    out1, f = gpu_eval(w, cfg.eps, keep=True)
+    assert expect_code(f.get_quadrupoles, w.n_cell) == binding.ESTATE             # order 1 keeps no quadrupoles
+    f.set_spj_order(2)
+    assert expect_code(f.dispatch, 0, 0, w.n_group) == binding.ESTATE             # moments of the other order are stale
+    f.refresh_monopoles()
+    got = f.get_quadrupoles(w.n_cell).astype(np.float64)
+    mom = oracle.monopoles(w.cells, w.posm)
+    quad = oracle.quadrupoles(w.cells, w.posm, mom)
+    tr = quad[:, :3].sum(1)
+    assert np.all(np.abs(got[:, :6] - quad) <= 1e-6 * tr[:, None] + 1e-30)
+    assert np.all(np.abs(got[:, 6] - 0.5 * tr) <= 1e-6 * tr + 1e-30)
+    out2 = np.full((w.n, 4), np.nan, np.float32)
+    f.dispatch(0, 0, w.n_group)
+    f.retrieve(0, out2)
+    assert f.last_quad_ms(0) > 0
+    lists = (w.grp_first, w.grp_n, w.epj_off, w.epj_id, w.spj_off, w.spj_id)
+    acc, pot = oracle.forces(w.posm, mom, *lists, cfg.eps, quad=quad)
+    check(out2, acc, pot, label="%s quadrupole" % cfg.name)
+    acc1, pot1 = oracle.forces(w.posm, mom, *lists, cfg.eps)
+    ea, _ = errors(out2, acc1, pot1)
+    assert ea.max() > 10 * ACC_MAX or idx == 0                                     # it is not the monopole answer
+    # batched over tags: same bits
+    out3 = np.full((w.n, 4), np.nan, np.float32)
+    step = max(1, w.n_group // 7)
+    tags = []
+    for k, gb in enumerate(range(0, w.n_group, step)):
+        t = k % f.n_tag
+        if t in tags:
+            f.retrieve(t, out3)
+            tags.remove(t)
+        f.dispatch(t, gb, min(w.n_group, gb + step))
+        tags.append(t)
+    for t in tags:
+        f.retrieve(t, out3)
+    assert np.array_equal(out2, out3)
+    if idx == 0:
+        f.reserve_data_lists(64)
+        assert expect_code(f.dispatch_data, 0, 0, 1, np.zeros((4, 4), np.float32), np.zeros(2, np.int64)) == binding.ESTATE
+    f.set_spj_order(1)
+    f.refresh_monopoles()
+    out4 = np.full((w.n, 4), np.nan, np.float32)
+    f.dispatch(0, 0, w.n_group)
+    f.retrieve(0, out4)
+    assert np.array_equal(out1, out4)
+    assert expect_code(f.last_quad_ms, 0) == binding.ESTATE
+    f.close()
+
+
+def test_quadrupole_device_resident_steps():
+    """mwf_step_reuse with order 2: kick-drift, refresh (monopoles + quadrupoles), both kernels, kick -- per step the
+    forces match the oracle's quadrupole evaluation at the positions the device holds."""
+    cfg = CONFIGS[4]
+    w = make_workload(cfg, 30000)
+    f = binding.MultiWalkForce.for_workload(w, n_tag=2)
+    f.upload_workload(w)
+    f.set_spj_order(2)
+    vel4 = np.zeros((w.n, 4), np.float32)
+    vel4[:, :3] = w.vel
+    f.set_velocities(vel4)
+    f.refresh_monopoles()
+    out = np.zeros((w.n, 4), np.float32)
+    f.dispatch(0, 0, w.n_group)
+    f.retrieve(0, out)
+    lists = (w.grp_first, w.grp_n, w.epj_off, w.epj_id, w.spj_off, w.spj_id)
+    for step in range(3):
+        f.step_reuse(cfg.dt)
+        f.retrieve(0, out)
+        posm = f.get_particles(0, w.n)
+        mom = oracle.monopoles(w.cells, posm)
+        quad = oracle.quadrupoles(w.cells, posm, mom)
+        acc, pot = oracle.forces(posm, mom, *lists, cfg.eps, quad=quad)
+        check(out, acc, pot, label="quadrupole reuse step %d" % (step + 1))
+    f.close()
+
+
 # ------------------------------------------------------------------ list-reuse driver (rows a6, a7; P:242)
 def test_state_machine_and_validation():
     cfg = CONFIGS[0]
