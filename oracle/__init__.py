@@ -6,4 +6,5 @@ paper_1907_02290_b200/ imports this package; only tests/, __graft_entry__.smoke(
 cpu_baseline / --impl reference legs do.  Parity status: every function here is pinned by
 tests/test_oracle_pins.py (closed forms, brute force, invariants); nothing is "parity unpinned".
 """
-from .oracle import build, direct, forces, kick, kick_drift, monopoles, num_threads, quadrupoles, set_num_threads  # noqa: F401
+from .oracle import (build, direct, forces, kick, kick_drift, monopoles, num_threads, quadrupoles, set_num_threads,  # noqa: F401
+                     sph_density, sph_density_direct, sph_dwdr, sph_hydro, sph_hydro_direct, sph_w)

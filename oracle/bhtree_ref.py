@@ -22,7 +22,11 @@ def _key(ix: int, iy: int, iz: int) -> int:
     return k
 
 
-def build(posm: np.ndarray, n_leaf: int, n_grp: int, theta: float):
+def build(posm: np.ndarray, n_leaf: int, n_grp: int, theta: float, h=None, skin: float = 0.0):
+    """theta-lists (long range, O4).  With `h` (smoothing length per particle, caller's order): the short-range
+    neighbour-search criterion instead (reading S24 of DESIGN.md): a cell is opened iff the gap between its
+    cube and the group's particle box is <= max(R_g, R_c), R = 2 (1 + skin) x the largest h among the group's / the
+    cell's particles; an opened leaf gives its particles as EPJ, anything else is dropped (no SPJ)."""
     pos = np.asarray(posm, dtype=np.float32)[:, :3].astype(np.float64)
     n = pos.shape[0]
     # O1 root cell
@@ -85,6 +89,42 @@ def build(posm: np.ndarray, n_leaf: int, n_grp: int, theta: float):
                 descend(fc + k)
 
     descend(0)
+    if h is not None:
+        hs = np.asarray(h, dtype=np.float32).astype(np.float64)[perm]
+        reach = 2.0 * (1.0 + skin)
+        epj, spj = [], []
+        for gc in groups:
+            first, cnt = cells[gc][0], cells[gc][1]
+            blo = spos[first:first + cnt].min(axis=0)
+            bhi = spos[first:first + cnt].max(axis=0)
+            rg = reach * hs[first:first + cnt].max()
+            e = []
+
+            def search(c):
+                cx, cy, cz, l = geom[c]
+                rc = reach * hs[cells[c][0]:cells[c][0] + cells[c][1]].max()
+                r = rg if rg > rc else rc
+                d2 = 0.0
+                for a, sc in enumerate((cx, cy, cz)):
+                    d = 0.0
+                    if sc + 0.5 * l < blo[a]:
+                        d = blo[a] - (sc + 0.5 * l)
+                    elif sc - 0.5 * l > bhi[a]:
+                        d = (sc - 0.5 * l) - bhi[a]
+                    d2 += d * d
+                if d2 <= r * r:
+                    if cells[c][3] == 0:
+                        e.extend(range(cells[c][0], cells[c][0] + cells[c][1]))
+                    else:
+                        for k in range(cells[c][3]):
+                            search(cells[c][2] + k)
+
+            search(0)
+            epj.append(e)
+            spj.append([])
+        return dict(perm=np.array(perm, np.int32), cells=np.array(cells, np.int32), geom=np.array(geom),
+                    level=np.array(level, np.int32), groups=np.array(groups, np.int32), epj=epj, spj=spj,
+                    root=np.array(centre + [side]))
     # O4 lists
     th2 = theta * theta
     epj, spj = [], []

@@ -9,14 +9,15 @@ import numpy as np
 
 _HERE = os.path.dirname(os.path.abspath(__file__))
 _SRC = os.path.join(_HERE, "mwf_oracle.c")
+_SRC_SPH = os.path.join(_HERE, "sph_oracle.c")
 _SO = os.path.join(_HERE, "libmwf_oracle.so")
 _lib = None
 
 
 def build(force: bool = False) -> str:
     """Compile the oracle with gcc -O2 -fopenmp (no fast-math, no intrinsics)."""
-    if force or not os.path.exists(_SO) or os.path.getmtime(_SO) < os.path.getmtime(_SRC):
-        r = subprocess.run(["gcc", "-O2", "-fopenmp", "-ffp-contract=off", "-shared", "-fPIC", "-o", _SO, _SRC, "-lm"],
+    if force or not os.path.exists(_SO) or os.path.getmtime(_SO) < max(os.path.getmtime(_SRC), os.path.getmtime(_SRC_SPH)):
+        r = subprocess.run(["gcc", "-O2", "-fopenmp", "-ffp-contract=off", "-shared", "-fPIC", "-o", _SO, _SRC, _SRC_SPH, "-lm"],
                            capture_output=True, text=True)
         if r.returncode != 0:
             raise RuntimeError("oracle build failed:\n" + r.stderr)
@@ -37,6 +38,14 @@ def _load():
         lib.orc_forces_quad.argtypes = [i64, vp, vp, vp, vp, vp, vp, vp, vp, vp, vp, dbl, dbl, vp, vp]
         lib.orc_kick_drift.argtypes = [i64, vp, vp, vp, dbl, vp, vp]
         lib.orc_kick.argtypes = [i64, vp, vp, dbl, vp]
+        lib.orc_sph_w.restype = dbl
+        lib.orc_sph_w.argtypes = [dbl, dbl]
+        lib.orc_sph_dwdr.restype = dbl
+        lib.orc_sph_dwdr.argtypes = [dbl, dbl]
+        lib.orc_sph_density.argtypes = [i64, vp, vp, vp, vp, vp, vp, vp, dbl, vp, vp]
+        lib.orc_sph_density_direct.argtypes = [i64, vp, vp, vp]
+        lib.orc_sph_hydro.argtypes = [i64, vp, vp, vp, vp, vp, vp, vp, vp, vp]
+        lib.orc_sph_hydro_direct.argtypes = [i64, vp, vp, vp, vp]
         _lib = lib
     return _lib
 
@@ -129,3 +138,59 @@ def kick(vel4, accp4, dt: float):
     v = np.empty((n, 3))
     _load().orc_kick(n, _p(vel4), _p(accp4), float(dt), _p(v))
     return v
+
+
+# ---- short-range workload (NEXT-4): SPH density and pressure-gradient acceleration, oracle/sph_oracle.c
+
+def sph_w(r: float, h: float) -> float:
+    """Cubic-spline kernel W(r, h) in 3-D, support 2h."""
+    return float(_load().orc_sph_w(float(r), float(h)))
+
+
+def sph_dwdr(r: float, h: float) -> float:
+    return float(_load().orc_sph_dwdr(float(r), float(h)))
+
+
+def _sel(groups, grp_first):
+    if groups is None:
+        return grp_first.shape[0], None
+    sel = _c(groups, np.int64)
+    return sel.shape[0], sel
+
+
+def sph_density(posm, sph4, grp_first, grp_n, epj_off, epj_id, gamma: float, groups=None):
+    """rho [N], P/rho^2 [N] (float64) over the groups' neighbour lists; sph4 = [N,4] float32 (h, u, rho, P/rho^2),
+    of which h and u are read.  Particles of unselected groups are NaN."""
+    posm, sph4 = _c(posm, np.float32), _c(sph4, np.float32)
+    grp_first, grp_n, epj_off, epj_id = _c(grp_first, np.int32), _c(grp_n, np.int32), _c(epj_off, np.int64), _c(epj_id, np.int32)
+    n = posm.shape[0]
+    rho, pr2 = np.full(n, np.nan), np.full(n, np.nan)
+    n_sel, sel = _sel(groups, grp_first)
+    _load().orc_sph_density(n_sel, _p(sel), _p(grp_first), _p(grp_n), _p(epj_off), _p(epj_id), _p(posm), _p(sph4), float(gamma), _p(rho), _p(pr2))
+    return rho, pr2
+
+
+def sph_density_direct(posm, sph4):
+    posm, sph4 = _c(posm, np.float32), _c(sph4, np.float32)
+    rho = np.empty(posm.shape[0])
+    _load().orc_sph_density_direct(posm.shape[0], _p(posm), _p(sph4), _p(rho))
+    return rho
+
+
+def sph_hydro(posm, sph4, grp_first, grp_n, epj_off, epj_id, groups=None):
+    """acc [N,3] and scale [N] (sum of the magnitudes of the pair terms) in float64; reads h and P/rho^2 of sph4."""
+    posm, sph4 = _c(posm, np.float32), _c(sph4, np.float32)
+    grp_first, grp_n, epj_off, epj_id = _c(grp_first, np.int32), _c(grp_n, np.int32), _c(epj_off, np.int64), _c(epj_id, np.int32)
+    n = posm.shape[0]
+    acc, scale = np.full((n, 3), np.nan), np.full(n, np.nan)
+    n_sel, sel = _sel(groups, grp_first)
+    _load().orc_sph_hydro(n_sel, _p(sel), _p(grp_first), _p(grp_n), _p(epj_off), _p(epj_id), _p(posm), _p(sph4), _p(acc), _p(scale))
+    return acc, scale
+
+
+def sph_hydro_direct(posm, sph4):
+    posm, sph4 = _c(posm, np.float32), _c(sph4, np.float32)
+    n = posm.shape[0]
+    acc, scale = np.empty((n, 3)), np.empty(n)
+    _load().orc_sph_hydro_direct(n, _p(posm), _p(sph4), _p(acc), _p(scale))
+    return acc, scale

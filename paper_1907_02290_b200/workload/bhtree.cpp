@@ -265,6 +265,92 @@ int bh_build_lists(void* h, double theta, int64_t* epj_off, int64_t* spj_off, in
     return 0;
 }
 
+// Short-range neighbour search ("we still use treewalk but with cell-opening criterion different from the
+// standard opening angle", reading S24 of DESIGN.md).  hsml: smoothing length per
+// particle in the CALLER's order (as posm was given to bh_build).  With R = 2 (1 + skin) x the largest h among a
+// set of particles, cell c is opened for group g iff the gap between c's cube and g's particle box is <= max(R_g, R_c)
+// (gather and scatter neighbours: a pair interacts when r < 2 max(h_i, h_k)); an opened leaf contributes its particles
+// as EPJ, everything else is dropped -- there are no SPJ.  Purely geometric: no kernel arithmetic here.
+int bh_build_neighbour_lists(void* h, const float* hsml, double skin, int64_t* epj_off, int64_t* spj_off, int64_t* e_epj) {
+    Tree* t = (Tree*)h;
+    if (!hsml || !(skin >= 0)) return -1;
+    const int64_t ng = (int64_t)t->grp_first.size();
+    const int64_t nc = (int64_t)t->cell.size();
+    const double reach = 2.0 * (1.0 + skin);
+    std::vector<double> hs((size_t)t->n), cell_h((size_t)nc, 0.0);
+#pragma omp parallel for schedule(static)
+    for (int64_t i = 0; i < t->n; ++i) hs[(size_t)i] = (double)hsml[t->perm[(size_t)i]];
+    for (int64_t c = nc - 1; c >= 0; --c) {  // children sit behind their parent: bottom-up in one reverse sweep
+        const Cell& cc = t->cell[(size_t)c];
+        double m = 0;
+        if (cc.n_child == 0) {
+            for (int32_t i = cc.first_ptcl; i < cc.first_ptcl + cc.n_ptcl; ++i) m = std::max(m, hs[(size_t)i]);
+        } else {
+            for (int k = 0; k < cc.n_child; ++k) m = std::max(m, cell_h[(size_t)(cc.first_child + k)]);
+        }
+        cell_h[(size_t)c] = m;
+    }
+    const int64_t BLK = 64;
+    const int64_t nblk = (ng + BLK - 1) / BLK;
+    t->blk_groups = BLK;
+    t->blk_epj.assign((size_t)nblk, {});
+    t->blk_spj.assign((size_t)nblk, {});
+    t->epj_off.assign((size_t)ng + 1, 0);
+    t->spj_off.assign((size_t)ng + 1, 0);
+#pragma omp parallel
+    {
+        std::vector<int32_t> stack;
+#pragma omp for schedule(dynamic, 1)
+        for (int64_t b = 0; b < nblk; ++b) {
+            std::vector<int32_t>& ve = t->blk_epj[(size_t)b];
+            for (int64_t g = b * BLK; g < std::min(ng, (b + 1) * BLK); ++g) {
+                const int32_t f = t->grp_first[(size_t)g], cnt = t->grp_n[(size_t)g];
+                double lo[3], hi[3], hg = 0;
+                for (int a = 0; a < 3; ++a) lo[a] = hi[a] = t->pos[(size_t)f * 3 + a];
+                for (int32_t i = f; i < f + cnt; ++i) {
+                    hg = std::max(hg, hs[(size_t)i]);
+                    for (int a = 0; a < 3; ++a) {
+                        double v = t->pos[(size_t)i * 3 + a];
+                        if (v < lo[a]) lo[a] = v;
+                        if (v > hi[a]) hi[a] = v;
+                    }
+                }
+                const double rg = reach * hg;
+                const size_t e0 = ve.size();
+                stack.clear();
+                stack.push_back(0);
+                while (!stack.empty()) {
+                    const int32_t c = stack.back(); stack.pop_back();
+                    const double* gm = &t->geom[(size_t)c * 4];
+                    const double half = 0.5 * gm[3];
+                    double d2 = 0;
+                    for (int a = 0; a < 3; ++a) {
+                        double d = 0;
+                        if (gm[a] + half < lo[a]) d = lo[a] - (gm[a] + half);
+                        else if (gm[a] - half > hi[a]) d = (gm[a] - half) - hi[a];
+                        d2 += d * d;
+                    }
+                    const double rc = reach * cell_h[(size_t)c];
+                    const double r = rg > rc ? rg : rc;
+                    if (!(d2 <= r * r)) continue;
+                    const Cell& cc = t->cell[(size_t)c];
+                    if (cc.n_child == 0) {
+                        for (int32_t i = cc.first_ptcl; i < cc.first_ptcl + cc.n_ptcl; ++i) ve.push_back(i);
+                    } else {
+                        for (int k = cc.n_child - 1; k >= 0; --k) stack.push_back(cc.first_child + k);
+                    }
+                }
+                t->epj_off[(size_t)g + 1] = (int64_t)(ve.size() - e0);
+            }
+        }
+    }
+    for (int64_t g = 0; g < ng; ++g) t->epj_off[(size_t)g + 1] += t->epj_off[(size_t)g];
+    std::memcpy(epj_off, t->epj_off.data(), ((size_t)ng + 1) * sizeof(int64_t));
+    std::memcpy(spj_off, t->spj_off.data(), ((size_t)ng + 1) * sizeof(int64_t));
+    *e_epj = t->epj_off[(size_t)ng];
+    return 0;
+}
+
 // Copies the lists built by bh_build_lists into caller arrays and releases the internal blocks.
 void bh_get_lists(void* h, int32_t* epj_id, int32_t* spj_id) {
     Tree* t = (Tree*)h;

@@ -27,6 +27,9 @@ class Config:
     n_reuse: int = 0       # extra evaluations that reuse the lists (config 5)
     dt: float = 0.0
     groups_per_dispatch: int = 0  # 0 = all groups in one dispatch
+    eta: float = 1.2       # short-range configs: h = eta (m / rho)^(1/3)
+    gamma: float = 5.0 / 3.0
+    skin: float = 0.0      # neighbour lists reach 2 (1 + skin) h, so that they stay complete over the reuse steps
 
 
 # BASELINE.json "configs", in order (config k is CONFIGS[k-1]).
@@ -36,6 +39,15 @@ CONFIGS = (
     Config("disk_halo_4m", 1 << 22, 3, 0.005, 0.4, 16, 512, "disk_halo"),
     Config("clumpy_box_8m", 1 << 23, 4, 1e-4, 0.5, 16, 256, "clumpy_box"),
     Config("plummer_4m_reuse", 1 << 22, 5, 1.0 / 512, 0.5, 16, 256, "plummer", n_reuse=8, dt=1.0 / 1024),
+)
+
+
+# Short-range (SPH) stand-ins for SURVEY.md section 8(f) NEXT-4: the paper names SPH runs and
+# measures none, so these are this build's own workloads: a gas Plummer sphere with adaptive smoothing lengths.
+SPH_CONFIGS = (
+    Config("sph_plummer_32k", 1 << 15, 6, 0.0, 0.0, 16, 64, "sph_plummer"),
+    Config("sph_plummer_1m", 1 << 20, 7, 0.0, 0.0, 16, 64, "sph_plummer", n_reuse=4, dt=1.0 / 4096, skin=0.1),
+    Config("sph_plummer_4m", 1 << 22, 8, 0.0, 0.0, 16, 128, "sph_plummer", n_reuse=4, dt=1.0 / 4096, skin=0.1),
 )
 
 
@@ -129,11 +141,23 @@ def clumpy_box(n: int, seed: int, n_clump: int = 512):
     return pos, None, mass
 
 
+def make_sph_fields(cfg: Config, posm: np.ndarray) -> np.ndarray:
+    """[N,4] float32 (h, u, 0, 0) in the order of posm for a short-range config.  Smoothing length from the ANALYTIC
+    Plummer density rho(r) = 3/(4 pi) (1 + r^2)^(-5/2) (M = a = 1): h = min(eta (m / rho)^(1/3), 1), which gives
+    about (32/3) pi eta^3 = 58 neighbours inside 2h; specific internal energy u = 0.1 (1 + r^2)^(-1/2) (a hot core)."""
+    r2 = np.sum(posm[:, :3].astype(np.float64) ** 2, axis=1)
+    rho = 3.0 / (4.0 * np.pi) * (1.0 + r2) ** -2.5
+    out = np.zeros((posm.shape[0], 4), np.float32)
+    out[:, 0] = np.minimum(cfg.eta * np.cbrt(posm[:, 3].astype(np.float64) / rho), 1.0)
+    out[:, 1] = 0.1 / np.sqrt(1.0 + r2)
+    return out
+
+
 def make_particles(cfg: Config, n: int | None = None):
     """Returns (posm float32 [n,4], vel float64 [n,3] or None) for a config; `n` overrides the
     particle count (same recipe, smaller problem) for tests."""
     n = cfg.n if n is None else int(n)
-    if cfg.kind == "plummer":
+    if cfg.kind in ("plummer", "sph_plummer"):
         pos, vel, mass = plummer(n, cfg.seed)
     elif cfg.kind == "disk_halo":
         pos, vel, mass = disk_halo(n, cfg.seed)

@@ -13,7 +13,7 @@ import os
 import numpy as np
 
 from .. import build as _build
-from .generators import Config, make_particles
+from .generators import Config, make_particles, make_sph_fields
 
 _lib = None
 
@@ -38,6 +38,8 @@ def _load():
         lib.bh_build_lists.restype = ctypes.c_int
         lib.bh_build_lists.argtypes = [vp, dbl, vp, vp, ctypes.POINTER(i64), ctypes.POINTER(i64)]
         lib.bh_get_lists.argtypes = [vp, vp, vp]
+        lib.bh_build_neighbour_lists.restype = ctypes.c_int
+        lib.bh_build_neighbour_lists.argtypes = [vp, vp, dbl, vp, vp, ctypes.POINTER(i64)]
         lib.bh_pack_data_lists.argtypes = [i64, i64] + [vp] * 8
         _lib = lib
     return _lib
@@ -67,6 +69,8 @@ class Workload:
     spj_off: np.ndarray     # [n_group+1] int64
     spj_id: np.ndarray      # [E_spj] int32 cell indices
     theta: float
+    sph: np.ndarray | None = None  # [N,4] float32 (h, u, 0, 0), Morton order: short-range workload (NEXT-4) only
+    skin: float = 0.0              # neighbour lists were built with search radii 2 (1 + skin) h
 
     @property
     def n(self) -> int:
@@ -95,10 +99,16 @@ class Workload:
 
 
 def build_tree_and_lists(posm: np.ndarray, n_leaf: int, n_grp: int, theta: float, cfg: Config | None = None,
-                         vel: np.ndarray | None = None) -> Workload:
+                         vel: np.ndarray | None = None, sph: np.ndarray | None = None, skin: float = 0.0) -> Workload:
+    """sph ([N,4] float32 (h, u, ., .) in the caller's order) switches the list walk to the short-range neighbour
+    search (reading S24): EPJ lists only, search radii 2 (1 + skin) h; theta is then ignored."""
     lib = _load()
     posm = np.ascontiguousarray(posm, dtype=np.float32)
     n = posm.shape[0]
+    if sph is not None:
+        sph = np.ascontiguousarray(sph, dtype=np.float32)
+        if sph.shape != (n, 4):
+            raise ValueError("sph must be [N,4]")
     h = lib.bh_build(n, _p(posm), int(n_leaf), int(n_grp))
     if not h:
         raise ValueError("bh_build rejected its arguments")
@@ -118,7 +128,11 @@ def build_tree_and_lists(posm: np.ndarray, n_leaf: int, n_grp: int, theta: float
         epj_off = np.empty(n_group + 1, np.int64)
         spj_off = np.empty(n_group + 1, np.int64)
         e_epj, e_spj = ctypes.c_int64(0), ctypes.c_int64(0)
-        rc = lib.bh_build_lists(h, float(theta), _p(epj_off), _p(spj_off), ctypes.byref(e_epj), ctypes.byref(e_spj))
+        if sph is None:
+            rc = lib.bh_build_lists(h, float(theta), _p(epj_off), _p(spj_off), ctypes.byref(e_epj), ctypes.byref(e_spj))
+        else:
+            hsml = np.ascontiguousarray(sph[:, 0])
+            rc = lib.bh_build_neighbour_lists(h, _p(hsml), float(skin), _p(epj_off), _p(spj_off), ctypes.byref(e_epj))
         if rc != 0:
             raise ValueError("bh_build_lists failed")
         epj_id = np.empty(e_epj.value, np.int32)
@@ -129,7 +143,8 @@ def build_tree_and_lists(posm: np.ndarray, n_leaf: int, n_grp: int, theta: float
     return Workload(cfg=cfg, posm=np.ascontiguousarray(posm[perm]), vel=None if vel is None else np.ascontiguousarray(vel[perm]),
                     perm=perm, cells=cells, geom=geom, level=level, level_first=level_first, root=root,
                     grp_cell=grp_cell, grp_first=grp_first, grp_n=grp_n,
-                    epj_off=epj_off, epj_id=epj_id, spj_off=spj_off, spj_id=spj_id, theta=float(theta))
+                    epj_off=epj_off, epj_id=epj_id, spj_off=spj_off, spj_id=spj_id, theta=float(theta),
+                    sph=None if sph is None else np.ascontiguousarray(sph[perm]), skin=float(skin))
 
 
 def pack_data_lists(w: Workload, g0: int, g1: int, posm: np.ndarray, spj: np.ndarray, out: np.ndarray | None = None):
@@ -152,4 +167,6 @@ def pack_data_lists(w: Workload, g0: int, g1: int, posm: np.ndarray, spj: np.nda
 def make_workload(cfg: Config, n: int | None = None, theta: float | None = None) -> Workload:
     """Generate a config's particles and build its tree, groups and lists (construction step)."""
     posm, vel = make_particles(cfg, n)
-    return build_tree_and_lists(posm, cfg.n_leaf, cfg.n_grp, cfg.theta if theta is None else theta, cfg=cfg, vel=vel)
+    sph = make_sph_fields(cfg, posm) if cfg.kind.startswith("sph_") else None
+    return build_tree_and_lists(posm, cfg.n_leaf, cfg.n_grp, cfg.theta if theta is None else theta, cfg=cfg, vel=vel,
+                                sph=sph, skin=cfg.skin)
