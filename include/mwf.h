@@ -170,6 +170,40 @@ int mwf_get_quadrupoles(mwf_ctx* c, float* dst, int dst_on_device);
 /* Timing hook: ms of the quadrupole kernel of the last mwf_dispatch on `tag` (mwf_last_dispatch_ms covers both kernels). */
 int mwf_last_quad_ms(mwf_ctx* c, int32_t tag, float* ms);
 
+/* ---- Short-range workload through the same index lists (paper P:79: "In the case of
+ * short-range interaction such as SPH interaction between particles, we still use treewalk but with cell-opening
+ * criterion different from the standard opening angle"; particle records "much larger in the case of SPH";
+ * such lists can be reused because the time step is stability-limited).  The lists are EPJ-only neighbour
+ * lists given to mwf_set_lists() (all spj offsets 0): every particle k with |x_i - x_k| < 2 max(h_i, h_k) for some i
+ * of the group must be in the group's list; extra entries cost time, never accuracy (compact support).  The paper
+ * prints no SPH formula; reading S23 of DESIGN.md takes the cubic-spline (M4) kernel with support 2h,
+ *     W(r,h) = 1/(pi h^3) { 1 - 3/2 q^2 + 3/4 q^3 (q < 1); 1/4 (2 - q)^3 (1 <= q < 2); 0 (q >= 2) },  q = r/h.
+ * Per-particle record, tree order, 16 B: smoothing length h > 0, specific internal energy u, density rho,
+ * P/rho^2.  mwf_set_sph() uploads records [first, first + n) (all four fields; HOST or DEVICE source, asynchronous on
+ * `stream`; the array is cudaMalloc'ed on first use, 16 B x max_ptcl, MWF_ENOMEM); mwf_get_sph() reads them back
+ * (blocking).
+ *
+ * mwf_dispatch_density: for every particle i of groups [g_begin, g_end), on the stream of `tag`, non-blocking:
+ *     rho_i = sum_{k in list} m_k W(|x_i - x_k|, h_i)      (gather form, self term included)
+ *     (P/rho^2)_i = (gamma - 1) u_i / rho_i                (ideal gas; gamma > 1 else MWF_EINVAL)
+ *   written into the rho and P/rho^2 fields of the records.  mwf_retrieve(tag, dst, ..) then copies the RECORDS of those
+ *   particles (dst is an array of mwf_sph indexed by tree position); dst == NULL just waits.
+ * mwf_dispatch_hydro: pressure-gradient acceleration with the symmetrised kernel gradient,
+ *     a_i = - sum_{k != i} m_k [(P/rho^2)_i + (P/rho^2)_k] 1/2 [gradW(r_ik, h_i) + gradW(r_ik, h_k)],
+ *   gradW(r, h) = dW/dr (x_i - x_k)/r (a pair at zero distance contributes nothing), written as (ax, ay, az, 0) into
+ *   the result array that mwf_retrieve() copies out.  Reads h and P/rho^2 of every listed particle: these must be
+ *   current (from density dispatches over all groups, or uploaded); the library orders a hydro dispatch behind the
+ *   density kernels in flight on every tag.
+ * Both need the tree, the lists, particles and records for all N (MWF_ESTATE otherwise); no monopoles are involved.
+ * A tag holds one kind of result at a time: MWF_ESTATE when its previous results of the other kind (records vs
+ * accelerations) have not been retrieved.  Lists set with MWF_MAKE_LIST stay until the next mwf_begin_step /
+ * mwf_set_lists (a step needs them twice).  Artificial viscosity and the energy equation are not evaluated. */
+typedef struct { float h, u, rho, pr2; } mwf_sph;
+int mwf_set_sph(mwf_ctx* c, const mwf_sph* src, int64_t first, int64_t n, int src_on_device, void* stream);
+int mwf_get_sph(mwf_ctx* c, mwf_sph* dst, int64_t first, int64_t n, int dst_on_device);
+int mwf_dispatch_density(mwf_ctx* c, int32_t tag, int64_t g_begin, int64_t g_end, float gamma);
+int mwf_dispatch_hydro(mwf_ctx* c, int32_t tag, int64_t g_begin, int64_t g_end);
+
 /* (5) Copy acc+pot of the particles of every group dispatched under `tag` since its last retrieve into
  * dst and wait for it.  dst: base of an N-record array indexed by tree-order particle
  * position, HOST or DEVICE; records of other particles are not touched.  dst == NULL: wait for the tag and

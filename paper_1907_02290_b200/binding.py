@@ -25,6 +25,7 @@ SYMBOLS = (
     "mwf_last_dispatch_ms", "mwf_strerror", "mwf_last_cuda_error",
     "mwf_set_velocities", "mwf_get_velocities", "mwf_kick_drift", "mwf_kick", "mwf_step_reuse",
     "mwf_reserve_data_lists", "mwf_dispatch_data", "mwf_set_spj_order", "mwf_get_quadrupoles", "mwf_last_quad_ms",
+    "mwf_set_sph", "mwf_get_sph", "mwf_dispatch_density", "mwf_dispatch_hydro",
     "mwf_build", "mwf_get_build_sizes", "mwf_get_permutation", "mwf_get_tree", "mwf_get_groups", "mwf_get_lists",
 )
 
@@ -84,6 +85,10 @@ def load_library(path: str | None = None) -> ctypes.CDLL:
         "mwf_last_quad_ms": [vp, i32, P(ctypes.c_float)],
         "mwf_reserve_data_lists": [vp, i64],
         "mwf_dispatch_data": [vp, i32, i64, i64, vp, vp, ci],
+        "mwf_set_sph": [vp, vp, i64, i64, ci, vp],
+        "mwf_get_sph": [vp, vp, i64, i64, ci],
+        "mwf_dispatch_density": [vp, i32, i64, i64, ctypes.c_float],
+        "mwf_dispatch_hydro": [vp, i32, i64, i64],
         "mwf_build": [vp, i64, i32, i32, ctypes.c_double, ci, vp],
         "mwf_get_build_sizes": [vp, P(i64), P(i64), P(i64), P(i64), P(i32)],
         "mwf_get_permutation": [vp, vp, ci],
@@ -155,7 +160,9 @@ class MultiWalkForce:
 
     @classmethod
     def for_workload(cls, w, eps: float | None = None, G: float = 1.0, n_tag: int = 8, device: int = 0):
-        return cls(w.cfg.eps if eps is None else eps, G, max_ptcl=w.n, max_cell=w.n_cell, max_group=w.n_group,
+        if eps is None:
+            eps = w.cfg.eps if w.cfg.eps > 0 else 1.0   # short-range workloads have no softening; the ctx still wants one
+        return cls(eps, G, max_ptcl=w.n, max_cell=w.n_cell, max_group=w.n_group,
                    max_entry=max(1, w.n_entry), n_tag=n_tag, device=device)
 
     # -- error handling
@@ -264,6 +271,24 @@ class MultiWalkForce:
     def step_reuse(self, dt: float):
         self._ck(self._lib.mwf_step_reuse(self._h, float(dt)))
 
+    def set_sph(self, src, first: int = 0, n: int | None = None, stream=None):
+        """Short-range workload: [n,4] float32 records (h, u, rho, P/rho^2)."""
+        p, on_dev = _ptr(src, np.float32, "src")
+        if n is None:
+            n = int(src.shape[0])
+        self._ck(self._lib.mwf_set_sph(self._h, p, int(first), int(n), on_dev, _stream_handle(stream)))
+
+    def get_sph(self, first: int, n: int) -> np.ndarray:
+        out = np.empty((n, 4), np.float32)
+        self._ck(self._lib.mwf_get_sph(self._h, _host_ptr(out, np.float32, "dst"), int(first), int(n), 0))
+        return out
+
+    def dispatch_density(self, tag: int, g_begin: int, g_end: int, gamma: float):
+        self._ck(self._lib.mwf_dispatch_density(self._h, int(tag), int(g_begin), int(g_end), float(gamma)))
+
+    def dispatch_hydro(self, tag: int, g_begin: int, g_end: int):
+        self._ck(self._lib.mwf_dispatch_hydro(self._h, int(tag), int(g_begin), int(g_end)))
+
     def build(self, n: int, n_leaf: int, n_grp: int, theta: float, mode: int = MAKE_LIST_FOR_REUSE, stream=None):
         self._ck(self._lib.mwf_build(self._h, int(n), int(n_leaf), int(n_grp), float(theta), int(mode), _stream_handle(stream)))
 
@@ -322,6 +347,8 @@ class MultiWalkForce:
         self.set_particles(w.posm, 0, w.n, stream)
         self.set_tree(w.cells, stream)
         self.set_lists(w.grp_first, w.grp_n, w.epj_off, w.epj_id, w.spj_off, w.spj_id, mode, stream)
+        if getattr(w, "sph", None) is not None:
+            self.set_sph(w.sph, 0, w.n, stream)
 
     def pinned(self, n: int):
         """Pinned host float32 [n,4] buffer (for truly asynchronous uploads / retrieves)."""

@@ -78,6 +78,11 @@ struct mwf_ctx {
     int quad_ctas_per_sm = 0;
     cudaEvent_t ev_kq[MWF_MAX_TAG]{};
     bool tag_quad[MWF_MAX_TAG]{};
+    // short-range workload (NEXT-4): per-particle SPH record, cudaMalloc'ed when mwf_set_sph() is first called
+    float4* sph = nullptr;      // [max_ptcl] (h, u, rho, P/rho^2)
+    int64_t sph_hi = 0;         // records [0, sph_hi) have been uploaded
+    int sph_ctas_per_sm[2] = {0, 0};
+    int tag_kind[MWF_MAX_TAG]{};  // what the tag's pending results are: 0 = acc/pot (or hydro acc), 1 = SPH records
     uint32_t counter_seq = 0;
     int64_t n_launch = 0, n_inter = 0;
     std::string cuda_err;
@@ -478,6 +483,7 @@ int mwf_create(mwf_ctx** out, const mwf_params* p, void* arena, int64_t arena_by
 }
 
 int mwf_destroy(mwf_ctx* c) {
+    if (c && c->sph) { cudaFree(c->sph); c->sph = nullptr; }
     if (!c) return MWF_EINVAL;
     cudaDeviceSynchronize();
     for (int t = 0; t < MWF_MAX_TAG; ++t) {
@@ -649,6 +655,41 @@ int mwf_refresh_monopoles(mwf_ctx* c, void* stream) {
     return after_store_op(c, s);
 }
 
+// The schedule of a dispatch over groups [g_begin, g_end): the full one, a per-tag one, or none (item order).
+static int pick_order(mwf_ctx* c, int64_t g_begin, int64_t g_end, cudaStream_t s, const int32_t** order) {
+    *order = nullptr;
+    if (g_begin == 0 && g_end == c->n_group) {
+        *order = c->order_full;
+        return MWF_OK;
+    }
+    for (int t = 0; t < c->p.n_tag; ++t)
+        if (c->h_split[(size_t)t] == g_begin && c->h_split[(size_t)t + 1] == g_end) {
+            const int rc = ensure_split_order(c, s);
+            if (rc) return rc;
+            *order = c->order_split;
+        }
+    return MWF_OK;
+}
+
+// Bookkeeping common to every kind of dispatch: the tag is in flight, its particle ranges await a retrieve.
+static void book_dispatch(mwf_ctx* c, int32_t tag, int64_t g_begin, int64_t g_end) {
+    c->tag_inflight[tag] = true;
+    ++c->n_launch;
+    c->n_inter += c->h_inter[(size_t)g_end] - c->h_inter[(size_t)g_begin];
+    // particle range covered (groups are disjoint; contiguous when they come from a tree)
+    int64_t lo = c->h_grp_first[(size_t)g_begin], hi = lo + c->h_grp_n[(size_t)g_begin];
+    auto& rs = c->tag_ranges[tag];
+    for (int64_t g = g_begin + 1; g < g_end; ++g) {
+        const int64_t f = c->h_grp_first[(size_t)g], n = c->h_grp_n[(size_t)g];
+        if (f == hi) { hi += n; continue; }
+        rs.emplace_back(lo, hi);
+        lo = f; hi = f + n;
+    }
+    rs.emplace_back(lo, hi);
+    c->tag_groups[(size_t)tag] += g_end - g_begin;
+    c->groups_outstanding += g_end - g_begin;
+}
+
 // Launch of the force kernel over groups [g_begin, g_end) on the tag's stream and the bookkeeping that goes with it.
 // jdata / joff (device) non-null: method G1, the lists are runs of j records instead of indices into the store.
 static int dispatch_launch(mwf_ctx* c, int32_t tag, int64_t g_begin, int64_t g_end, const float4* jdata, const int64_t* joff) {
@@ -667,16 +708,9 @@ static int dispatch_launch(mwf_ctx* c, int32_t tag, int64_t g_begin, int64_t g_e
     a.n_items = c->h_item_off[(size_t)g_end] - a.item_begin;
     a.eps2 = c->p.eps * c->p.eps;
     a.G = c->p.G;
-    a.order = nullptr;
-    if (g_begin == 0 && g_end == c->n_group) {
-        a.order = c->order_full;
-    } else {
-        for (int t = 0; t < c->p.n_tag; ++t)
-            if (c->h_split[(size_t)t] == g_begin && c->h_split[(size_t)t + 1] == g_end) {
-                const int rc = ensure_split_order(c, s);
-                if (rc) return rc;
-                a.order = c->order_split;
-            }
+    {
+        const int rc = pick_order(c, g_begin, g_end, s, &a.order);
+        if (rc) return rc;
     }
     const int64_t resident = (int64_t)c->n_sm * c->ctas_per_sm;
     const int64_t want = (a.n_items + WARPS_PER_CTA - 1) / WARPS_PER_CTA;
@@ -710,22 +744,8 @@ static int dispatch_launch(mwf_ctx* c, int32_t tag, int64_t g_begin, int64_t g_e
     CU(c, cudaEventRecord(c->ev_k1[tag], s));
     CU(c, cudaEventRecord(c->ev_tag[tag], s));
     c->tag_timed[tag] = true;
-    c->tag_inflight[tag] = true;
-    ++c->n_launch;
-    c->n_inter += c->h_inter[(size_t)g_end] - c->h_inter[(size_t)g_begin];
-    // particle range covered (groups are disjoint; contiguous when they come from a tree)
-    int64_t lo = c->h_grp_first[(size_t)g_begin], hi = lo + c->h_grp_n[(size_t)g_begin];
-    auto& rs = c->tag_ranges[tag];
-    for (int64_t g = g_begin + 1; g < g_end; ++g) {
-        const int64_t f = c->h_grp_first[(size_t)g], n = c->h_grp_n[(size_t)g];
-        if (f == hi) { hi += n; continue; }
-        rs.emplace_back(lo, hi);
-        lo = f; hi = f + n;
-    }
-    rs.emplace_back(lo, hi);
-    c->tag_groups[(size_t)tag] += g_end - g_begin;
+    book_dispatch(c, tag, g_begin, g_end);
     c->groups_dispatched += g_end - g_begin;
-    c->groups_outstanding += g_end - g_begin;
     if (c->groups_dispatched >= c->n_group) c->acc_full = true;
     return MWF_OK;
 }
@@ -735,6 +755,8 @@ int mwf_dispatch(mwf_ctx* c, int32_t tag, int64_t g_begin, int64_t g_end) {
     if (!c->have_tree || !c->have_lists || !c->mono_fresh) return MWF_ESTATE;
     if (g_end > c->n_group) return MWF_ERANGE;
     if (g_end == g_begin) return MWF_OK;
+    if (!c->tag_ranges[tag].empty() && c->tag_kind[tag] != 0) return MWF_ESTATE;  // SPH records await their retrieve
+    c->tag_kind[tag] = 0;
     if (c->store_event_valid) CU(c, cudaStreamWaitEvent(c->tag_stream[tag], c->ev_store, 0));
     return dispatch_launch(c, tag, g_begin, g_end, nullptr, nullptr);
 }
@@ -770,6 +792,7 @@ int mwf_dispatch_data(mwf_ctx* c, int32_t tag, int64_t g_begin, int64_t g_end, c
     if (g_end > c->n_group) return MWF_ERANGE;
     if (g_end == g_begin) return MWF_OK;
     if (c->tag_inflight[tag]) return MWF_ESTATE;  // the tag's staging buffer is still being read: retrieve first
+    c->tag_kind[tag] = 0;
     const int64_t ng = g_end - g_begin;
     if (joff[0] != 0) return MWF_ERANGE;
     for (int64_t g = 0; g < ng; ++g)  // the run of group g_begin + g must be as long as the group's index list
@@ -797,7 +820,8 @@ int mwf_retrieve(mwf_ctx* c, int32_t tag, mwf_accp* dst, int dst_on_device) {
         int64_t lo = rs[k].first, hi = rs[k].second;
         size_t j = k + 1;
         while (j < rs.size() && rs[j].first <= hi) { hi = std::max(hi, rs[j].second); ++j; }
-        CU(c, cudaMemcpyAsync(reinterpret_cast<float4*>(dst) + lo, c->accp + lo, (size_t)(hi - lo) * 16, kind, s));
+        const float4* from = c->tag_kind[tag] == 1 ? c->sph : c->accp;
+        CU(c, cudaMemcpyAsync(reinterpret_cast<float4*>(dst) + lo, from + lo, (size_t)(hi - lo) * 16, kind, s));
         k = j;
     }
     CU(c, cudaStreamSynchronize(s));
@@ -1042,6 +1066,84 @@ int mwf_step_reuse(mwf_ctx* c, float dt) {
     rc = mwf_dispatch(c, 0, 0, c->n_group);
     if (rc) return rc;
     return mwf_kick(c, dt, s0);
+}
+
+// ---- short-range workload (NEXT-4)
+
+int mwf_set_sph(mwf_ctx* c, const mwf_sph* src, int64_t first, int64_t n, int src_on_device, void* stream) {
+    if (!c || !src || first < 0 || n < 0) return MWF_EINVAL;
+    if (first + n > c->p.max_ptcl) return MWF_ENOMEM;
+    if (!c->sph) {
+        void* q = nullptr;
+        if (cudaMalloc(&q, (size_t)c->p.max_ptcl * 16) != cudaSuccess) { cudaGetLastError(); return MWF_ENOMEM; }
+        c->sph = static_cast<float4*>(q);
+        c->sph_ctas_per_sm[0] = sph_max_ctas_per_sm(false);
+        c->sph_ctas_per_sm[1] = sph_max_ctas_per_sm(true);
+        if (c->sph_ctas_per_sm[0] < 1 || c->sph_ctas_per_sm[1] < 1) return cuda_fail(c, cudaErrorLaunchFailure, "occupancy of the SPH kernels");
+    }
+    if (n == 0) return MWF_OK;
+    cudaStream_t s = static_cast<cudaStream_t>(stream);
+    int rc = before_store_op(c, s);
+    if (rc) return rc;
+    CU(c, cudaMemcpyAsync(c->sph + first, src, (size_t)n * 16, src_on_device ? cudaMemcpyDeviceToDevice : cudaMemcpyHostToDevice, s));
+    if (first <= c->sph_hi) c->sph_hi = std::max(c->sph_hi, first + n);
+    return after_store_op(c, s);
+}
+
+int mwf_get_sph(mwf_ctx* c, mwf_sph* dst, int64_t first, int64_t n, int dst_on_device) {
+    if (!c || !dst || first < 0 || n < 0) return MWF_EINVAL;
+    if (!c->sph || first + n > c->sph_hi) return MWF_ESTATE;
+    CU(c, cudaDeviceSynchronize());
+    CU(c, cudaMemcpy(dst, c->sph + first, (size_t)n * 16, dst_on_device ? cudaMemcpyDeviceToDevice : cudaMemcpyDeviceToHost));
+    return MWF_OK;
+}
+
+static int sph_dispatch(mwf_ctx* c, int32_t tag, int64_t g_begin, int64_t g_end, bool hydro, float gamma) {
+    if (!c || tag < 0 || tag >= c->p.n_tag || g_begin < 0 || g_end < g_begin) return MWF_EINVAL;
+    if (!hydro && !(gamma > 1.f)) return MWF_EINVAL;
+    if (!c->have_tree || !c->have_lists || !c->sph || c->sph_hi < c->n_ptcl || c->ptcl_hi < c->n_ptcl) return MWF_ESTATE;
+    if (g_end > c->n_group) return MWF_ERANGE;
+    if (g_end == g_begin) return MWF_OK;
+    const int kind = hydro ? 0 : 1;
+    if (!c->tag_ranges[tag].empty() && c->tag_kind[tag] != kind) return MWF_ESTATE;
+    c->tag_kind[tag] = kind;
+    cudaStream_t s = c->tag_stream[tag];
+    if (c->store_event_valid) CU(c, cudaStreamWaitEvent(s, c->ev_store, 0));
+    // the hydro kernel reads the densities of every particle in its lists: wait for the density kernels of all tags;
+    // the density kernel overwrites records the hydro kernels of other tags may still be reading
+    for (int t = 0; t < c->p.n_tag; ++t)
+        if (t != tag && c->tag_inflight[t]) CU(c, cudaStreamWaitEvent(s, c->ev_tag[t], 0));
+    SphArgs a;
+    a.store = c->store; a.sph = c->sph; a.list = c->list; a.list_off = c->list_off; a.items = c->items;
+    a.accp = c->accp; a.n_ptcl = c->n_ptcl; a.gamma_m1 = gamma - 1.f;
+    a.item_begin = c->h_item_off[(size_t)g_begin];
+    a.n_items = c->h_item_off[(size_t)g_end] - a.item_begin;
+    int rc = pick_order(c, g_begin, g_end, s, &a.order);
+    if (rc) return rc;
+    const int64_t resident = (int64_t)c->n_sm * c->sph_ctas_per_sm[hydro ? 1 : 0];
+    const int64_t want = (a.n_items + WARPS_PER_CTA - 1) / WARPS_PER_CTA;
+    const int grid = (int)std::min(want, resident);
+    a.counter = nullptr;
+    if (want > resident) {
+        a.counter = c->counters + (c->counter_seq++ % N_COUNTER);
+        CU(c, cudaMemsetAsync(a.counter, 0, sizeof(unsigned int), s));
+    }
+    CU(c, cudaEventRecord(c->ev_k0[tag], s));
+    CU(c, launch_sph(a, hydro, grid, s));
+    CU(c, cudaEventRecord(c->ev_k1[tag], s));
+    CU(c, cudaEventRecord(c->ev_tag[tag], s));
+    c->tag_timed[tag] = true;
+    c->tag_quad[tag] = false;
+    book_dispatch(c, tag, g_begin, g_end);
+    return MWF_OK;
+}
+
+int mwf_dispatch_density(mwf_ctx* c, int32_t tag, int64_t g_begin, int64_t g_end, float gamma) {
+    return sph_dispatch(c, tag, g_begin, g_end, false, gamma);
+}
+
+int mwf_dispatch_hydro(mwf_ctx* c, int32_t tag, int64_t g_begin, int64_t g_end) {
+    return sph_dispatch(c, tag, g_begin, g_end, true, 0.f);
 }
 
 int mwf_set_spj_order(mwf_ctx* c, int order) {

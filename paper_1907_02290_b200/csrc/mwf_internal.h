@@ -82,6 +82,24 @@ struct QuadArgs {
 cudaError_t launch_quad(const QuadArgs& a, int grid, cudaStream_t s);
 int quad_max_ctas_per_sm();
 
+// Short-range workload (NEXT-4, sph_kernel.cu): same lists, items and schedule as the force kernel.
+struct SphArgs {
+    const float4* store;
+    float4* sph;                // per particle (h, u, rho, P/rho^2): density writes the last two, hydro reads h and P/rho^2
+    const int32_t* list;
+    const int64_t* list_off;
+    const WorkItem* items;
+    const int32_t* order;
+    float4* accp;               // hydro: (ax, ay, az, 0)
+    unsigned int* counter;
+    int64_t item_begin;
+    int64_t n_items;
+    int64_t n_ptcl;
+    float gamma_m1;             // density: adiabatic index - 1
+};
+cudaError_t launch_sph(const SphArgs& a, bool hydro, int grid, cudaStream_t s);
+int sph_max_ctas_per_sm(bool hydro);
+
 // kernels' host launchers (defined next to their kernels)
 cudaError_t launch_force(const ForceArgs& a, int grid, cudaStream_t s);
 int force_max_ctas_per_sm();
