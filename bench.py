@@ -371,6 +371,78 @@ def quad_leg(args, cfg, binding, device):
     return 0
 
 
+def sph_leg(args, binding, device):
+    """Short-range workload (NEXT-4): one list-reuse step of the SPH pair of passes -- upload particles, density over all
+    groups, pressure-gradient acceleration over all groups, retrieve -- on the gas Plummer sphere `sph_plummer_4m`
+    (N = 2^22, neighbour lists with 10 % skin).  Both kernels are ALU-bound like k_force.  Flop convention (FMA = 2,
+    sqrt / rsqrt = 4 as in the paper's 23, max = 1): density 25 flop per list interaction (3 sub, mul + 2 fma, sqrt, 1 mul,
+    two clamped differences, two cubes, 1 fma, 1 fma), hydro 45 (3 sub, 3 fma, rsqrt, 3 mul, two clamped-difference
+    polynomials of 8, 2 mul + fma, 1 add, 2 mul, 3 fma).  Interactions counted as for gravity: sum n_i x n_list."""
+    import torch
+    import oracle
+    from paper_1907_02290_b200.workload import SPH_CONFIGS, make_workload
+    N_OP = {"density": 25, "hydro": 45}
+    cfg = SPH_CONFIGS[2] if args.n is None else SPH_CONFIGS[1]
+    t = time.perf_counter()
+    w = make_workload(cfg, args.n)
+    log("[bench sph] %s: N=%d groups=%d entries=%d interactions=%.4e (host tree+lists %.1f s)" % (
+        cfg.name, w.n, w.n_group, w.n_entry, w.interactions, time.perf_counter() - t))
+    f = binding.MultiWalkForce.for_workload(w, n_tag=args.n_tag, device=device)
+    f.upload_workload(w, binding.MAKE_LIST_FOR_REUSE)
+    src_dev = torch.from_numpy(w.posm).to(f.device)
+    rec_dev = torch.from_numpy(w.sph).to(f.device)
+    dst_dev = torch.zeros((w.n, 4), dtype=torch.float32, device=f.device)
+    n_sm = torch.cuda.get_device_properties(device).multi_processor_count
+    peak = n_sm * 256 * (measured_peaks().get("sm_max_mhz") or 1965.0) * 1e6
+    inter = w.interactions
+    s0 = f.streams[0]
+    ms = {"step": [], "density": [], "hydro": []}
+    with ClockSampler(device) as clk:
+        for it in range(args.warmup + args.steps):
+            e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            f.begin_step(binding.REUSE_LIST)
+            e0.record(s0)
+            f.set_particles(src_dev, 0, w.n, s0)
+            f.set_sph(rec_dev, 0, w.n, s0)
+            f.dispatch_density(0, 0, w.n_group, cfg.gamma)
+            f.retrieve(0, None)
+            t_d = f.last_dispatch_ms(0)
+            f.dispatch_hydro(0, 0, w.n_group)
+            f.retrieve(0, dst_dev)
+            e1.record(s0)
+            torch.cuda.synchronize()
+            if it >= args.warmup:
+                ms["step"].append(e0.elapsed_time(e1)); ms["density"].append(t_d); ms["hydro"].append(f.last_dispatch_ms(0))
+    launches = f.get_counters()["kernel_launches"]
+    f.close()
+    med = {k: float(np.median(v)) for k, v in ms.items()}
+    kern = {k: {"ms": med[k], "interactions_per_s": inter / (med[k] * 1e-3), "flop_per_interaction": N_OP[k],
+                "tflops": N_OP[k] * inter / (med[k] * 1e-3) / 1e12, "frac_fp32_peak": N_OP[k] * inter / (med[k] * 1e-3) / peak}
+            for k in ("density", "hydro")}
+    # the oracle on the host cores, on a seeded sample of groups (density pass)
+    rng = np.random.default_rng(12345)
+    order = rng.permutation(w.n_group)
+    per_group = w.grp_n.astype(np.int64) * w.n_list
+    budget = 3e8 * max(1, oracle.num_threads()) * args.cpu_baseline_seconds / 16.0
+    k = int(np.searchsorted(np.cumsum(per_group[order]), budget)) + 1
+    sel = np.sort(order[:min(k, w.n_group)]).astype(np.int64)
+    t = time.perf_counter()
+    oracle.sph_density(w.posm, w.sph, w.grp_first, w.grp_n, w.epj_off, w.epj_id, cfg.gamma, sel)
+    t_cpu = time.perf_counter() - t
+    n_cpu = int(per_group[sel].sum())
+    print(json.dumps({"leg": "sph", "metric": "particle-particle interactions/sec", "unit": "interactions/s",
+                      "value": 2 * inter / (med["step"] * 1e-3), "ms_per_step": med["step"], "steps": args.steps, "warmup": args.warmup,
+                      "dtype": "f32", "data": "synthetic",
+                      "config": {"workload": "short-range: " + cfg.name, "n": w.n, "n_group": w.n_group, "list_entries": w.n_entry,
+                                 "interactions_per_pass": inter, "n_leaf": cfg.n_leaf, "n_grp": cfg.n_grp, "eta": cfg.eta, "skin": cfg.skin,
+                                 "step": "list-reuse step: upload particles and records, density pass, hydro pass, retrieve (device-resident)"},
+                      "kernels": kern, "peak_tflops": peak / 1e12, "gpu_launches": launches, "clocks": clk.summary(),
+                      "cpu_baseline": {"value": n_cpu / t_cpu, "unit": "interactions/s", "cores": oracle.num_threads(), "kind": "oracle",
+                                       "sample": "density pass, %d of %d groups (seeded), %.3e interactions, %.1f s" % (len(sel), w.n_group, n_cpu, t_cpu)}}),
+          flush=True)
+    return 0
+
+
 # ----------------------------------------------------------------------------- main
 def main():
     ap = argparse.ArgumentParser()
@@ -382,11 +454,12 @@ def main():
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--cpu-baseline-seconds", type=float, default=15.0)
     ap.add_argument("--n-tag", type=int, default=8)
-    ap.add_argument("--leg", default="step", choices=["step", "construction", "sweep", "g1", "quad"],
+    ap.add_argument("--leg", default="step", choices=["step", "construction", "sweep", "g1", "quad", "sph"],
                     help="step: the list-reuse step (the contract's JSON line); construction: only the device-side construction step; "
                          "sweep: kernel time per interaction against <n_i> and theta (the paper's Fig. A.1, P:1197-1212); "
                          "g1: the paper's method G1 (lists carry j records, sent every step) against the index method; "
-                         "quad: the reuse step with quadrupole SPJ (refresh + force + quadrupole kernels)")
+                         "quad: the reuse step with quadrupole SPJ (refresh + force + quadrupole kernels); "
+                         "sph: the short-range workload (SPH density and pressure-gradient passes over neighbour lists)")
     args = ap.parse_args()
     args.warmup = max(args.warmup, 3) if args.impl == "ours" else args.warmup
 
@@ -419,6 +492,8 @@ def main():
         return g1_leg(args, cfg, binding, local)
     if args.leg == "quad":
         return quad_leg(args, cfg, binding, local)
+    if args.leg == "sph":
+        return sph_leg(args, binding, local)
 
     t = time.perf_counter()
     w = make_workload(cfg, args.n)
