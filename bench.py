@@ -415,6 +415,29 @@ def sph_leg(args, binding, device):
                 ms["step"].append(e0.elapsed_time(e1)); ms["density"].append(t_d); ms["hydro"].append(f.last_dispatch_ms(0))
     launches = f.get_counters()["kernel_launches"]
     f.close()
+    # construction step on the device (mwf_build_neighbours) from particles in generator order, against the host builder
+    from paper_1907_02290_b200.workload import build_tree_and_lists, make_particles, make_sph_fields
+    posm0, _ = make_particles(cfg, args.n)
+    rec0 = make_sph_fields(cfg, posm0)
+    t = time.perf_counter()
+    build_tree_and_lists(posm0, cfg.n_leaf, cfg.n_grp, 0.0, cfg=cfg, sph=rec0, skin=cfg.skin)
+    t_host_build = time.perf_counter() - t
+    fb = binding.MultiWalkForce(1.0, 1.0, max_ptcl=w.n, max_cell=w.n_cell + 1024, max_group=w.n_group + 1024, max_entry=w.n_entry + 4096,
+                                n_tag=1, device=device)
+    p_dev, r_dev = torch.from_numpy(posm0).to(fb.device), torch.from_numpy(rec0).to(fb.device)
+    ms_build = []
+    for it in range(4):
+        fb.begin_step(binding.MAKE_LIST_FOR_REUSE)
+        fb.set_particles(p_dev)
+        fb.set_sph(r_dev)
+        torch.cuda.synchronize()
+        t = time.perf_counter()
+        fb.build_neighbours(w.n, cfg.n_leaf, cfg.n_grp, cfg.skin)
+        fb.sync()
+        ms_build.append((time.perf_counter() - t) * 1e3)
+    sizes = fb.get_build_sizes()
+    fb.close()
+    assert sizes["n_group"] == w.n_group and sizes["n_epj"] == w.n_entry
     med = {k: float(np.median(v)) for k, v in ms.items()}
     kern = {k: {"ms": med[k], "interactions_per_s": inter / (med[k] * 1e-3), "flop_per_interaction": N_OP[k],
                 "tflops": N_OP[k] * inter / (med[k] * 1e-3) / 1e12, "frac_fp32_peak": N_OP[k] * inter / (med[k] * 1e-3) / peak}
@@ -436,7 +459,9 @@ def sph_leg(args, binding, device):
                       "config": {"workload": "short-range: " + cfg.name, "n": w.n, "n_group": w.n_group, "list_entries": w.n_entry,
                                  "interactions_per_pass": inter, "n_leaf": cfg.n_leaf, "n_grp": cfg.n_grp, "eta": cfg.eta, "skin": cfg.skin,
                                  "step": "list-reuse step: upload particles and records, density pass, hydro pass, retrieve (device-resident)"},
-                      "kernels": kern, "peak_tflops": peak / 1e12, "gpu_launches": launches, "clocks": clk.summary(),
+                      "kernels": kern, "peak_tflops": peak / 1e12, "gpu_launches": launches,
+                      "construction_step": {"device_ms": float(np.median(ms_build[1:])), "host_builder_s": t_host_build,
+                                            "what": "mwf_build_neighbours: sort, tree, groups, neighbour-search walk (host wall clock around the blocking call)"}, "clocks": clk.summary(),
                       "cpu_baseline": {"value": n_cpu / t_cpu, "unit": "interactions/s", "cores": oracle.num_threads(), "kind": "oracle",
                                        "sample": "density pass, %d of %d groups (seeded), %.3e interactions, %.1f s" % (len(sel), w.n_group, n_cpu, t_cpu)}}),
           flush=True)

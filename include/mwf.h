@@ -226,7 +226,14 @@ int mwf_calc_force_all(mwf_ctx* c, const mwf_posm* src, int src_on_device, mwf_a
  * retrieved (MWF_ESTATE otherwise).  MWF_ENOMEM when max_cell / max_group / max_entry are too small.  Blocking
  * (a few stream synchronisations to size the levels and the lists). */
 int mwf_build(mwf_ctx* c, int64_t n, int32_t n_leaf, int32_t n_grp, double theta, int mode, void* stream);
-/* Sizes of what mwf_build() made. */
+/* The same construction step for the short-range workload (NEXT-4): the list walk uses the neighbour-search criterion
+ * of reading S24 instead of the opening angle -- a cell is opened iff the gap between its cube and the group's particle
+ * box is <= max(R_g, R_c), R = 2 (1 + skin) x the largest smoothing length among the group's / the cell's particles;
+ * opened leaves give EPJ entries, nothing else is listed (no SPJ).  Needs the SPH records of particles [0, n)
+ * (mwf_set_sph, in the same order as the particles; MWF_ESTATE otherwise); they are sorted into tree order with the
+ * particles (mwf_build does the same when all n records have been uploaded).  skin >= 0. */
+int mwf_build_neighbours(mwf_ctx* c, int64_t n, int32_t n_leaf, int32_t n_grp, double skin, int mode, void* stream);
+/* Sizes of what mwf_build() / mwf_build_neighbours() made. */
 int mwf_get_build_sizes(mwf_ctx* c, int64_t* n_cell, int64_t* n_group, int64_t* n_epj, int64_t* n_spj, int32_t* n_level);
 /* perm[p] = index, in the order the particles were uploaded, of the particle now at tree position p. */
 int mwf_get_permutation(mwf_ctx* c, int32_t* perm, int dst_on_device);

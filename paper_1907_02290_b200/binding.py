@@ -26,7 +26,7 @@ SYMBOLS = (
     "mwf_set_velocities", "mwf_get_velocities", "mwf_kick_drift", "mwf_kick", "mwf_step_reuse",
     "mwf_reserve_data_lists", "mwf_dispatch_data", "mwf_set_spj_order", "mwf_get_quadrupoles", "mwf_last_quad_ms",
     "mwf_set_sph", "mwf_get_sph", "mwf_dispatch_density", "mwf_dispatch_hydro",
-    "mwf_build", "mwf_get_build_sizes", "mwf_get_permutation", "mwf_get_tree", "mwf_get_groups", "mwf_get_lists",
+    "mwf_build", "mwf_build_neighbours", "mwf_get_build_sizes", "mwf_get_permutation", "mwf_get_tree", "mwf_get_groups", "mwf_get_lists",
 )
 
 
@@ -90,6 +90,7 @@ def load_library(path: str | None = None) -> ctypes.CDLL:
         "mwf_dispatch_density": [vp, i32, i64, i64, ctypes.c_float],
         "mwf_dispatch_hydro": [vp, i32, i64, i64],
         "mwf_build": [vp, i64, i32, i32, ctypes.c_double, ci, vp],
+        "mwf_build_neighbours": [vp, i64, i32, i32, ctypes.c_double, ci, vp],
         "mwf_get_build_sizes": [vp, P(i64), P(i64), P(i64), P(i64), P(i32)],
         "mwf_get_permutation": [vp, vp, ci],
         "mwf_get_tree": [vp, vp, vp],
@@ -291,6 +292,9 @@ class MultiWalkForce:
 
     def build(self, n: int, n_leaf: int, n_grp: int, theta: float, mode: int = MAKE_LIST_FOR_REUSE, stream=None):
         self._ck(self._lib.mwf_build(self._h, int(n), int(n_leaf), int(n_grp), float(theta), int(mode), _stream_handle(stream)))
+
+    def build_neighbours(self, n: int, n_leaf: int, n_grp: int, skin: float, mode: int = MAKE_LIST_FOR_REUSE, stream=None):
+        self._ck(self._lib.mwf_build_neighbours(self._h, int(n), int(n_leaf), int(n_grp), float(skin), int(mode), _stream_handle(stream)))
 
     def get_build_sizes(self):
         a, b, c, d = (ctypes.c_int64(0) for _ in range(4))

@@ -20,9 +20,10 @@ namespace mwf {
 
 namespace {
 
-template <bool FILL>
+template <bool FILL, bool NEIGH>
 __global__ void __launch_bounds__(256) k_walk(const mwf_cell* __restrict__ cells, const double4* __restrict__ geom, const float* __restrict__ grp_box,
-                                              int64_t n_group, double th2, int32_t* __restrict__ stacks, unsigned int* __restrict__ counter,
+                                              int64_t n_group, double th2, double reach, const float* __restrict__ cell_h, const float* __restrict__ grp_h,
+                                              int32_t* __restrict__ stacks, unsigned int* __restrict__ counter,
                                               int32_t* __restrict__ n_epj, int32_t* __restrict__ n_spj, const int64_t* __restrict__ list_off,
                                               int32_t* __restrict__ list, int32_t n_ptcl, int32_t dummy) {
     const int lane = threadIdx.x & 31;
@@ -40,6 +41,8 @@ __global__ void __launch_bounds__(256) k_walk(const mwf_cell* __restrict__ cells
             lo[a] = (double)grp_box[g * 6 + a];
             hi[a] = (double)grp_box[g * 6 + 3 + a];
         }
+        double rg = 0.0;
+        if constexpr (NEIGH) rg = __dmul_rn(reach, (double)grp_h[g]);
         int64_t off_e = 0, off_s = 0;
         if (FILL) {
             off_e = list_off[g];
@@ -60,15 +63,30 @@ __global__ void __launch_bounds__(256) k_walk(const mwf_cell* __restrict__ cells
                 const double4 gm = geom[c];
                 const double s3[3] = {gm.x, gm.y, gm.z};
                 double d2 = 0.0;
+                if constexpr (NEIGH) {  // gap between the cell's cube and the group's box against the search radius
+                    const double half = __dmul_rn(0.5, gm.w);
 #pragma unroll
-                for (int a = 0; a < 3; ++a) {
-                    double d = 0.0;
-                    if (s3[a] < lo[a]) d = __dsub_rn(lo[a], s3[a]);
-                    else if (s3[a] > hi[a]) d = __dsub_rn(s3[a], hi[a]);
-                    d2 = __dadd_rn(d2, __dmul_rn(d, d));
+                    for (int a = 0; a < 3; ++a) {
+                        const double top = __dadd_rn(s3[a], half), bot = __dsub_rn(s3[a], half);
+                        double d = 0.0;
+                        if (top < lo[a]) d = __dsub_rn(lo[a], top);
+                        else if (bot > hi[a]) d = __dsub_rn(bot, hi[a]);
+                        d2 = __dadd_rn(d2, __dmul_rn(d, d));
+                    }
+                    const double rc = __dmul_rn(reach, (double)cell_h[c]);
+                    const double r = rg > rc ? rg : rc;
+                    kind = !(d2 <= __dmul_rn(r, r)) ? 0 : (cc.n_child == 0 ? 3 : 2);  // out of reach: dropped, there are no SPJ
+                } else {
+#pragma unroll
+                    for (int a = 0; a < 3; ++a) {
+                        double d = 0.0;
+                        if (s3[a] < lo[a]) d = __dsub_rn(lo[a], s3[a]);
+                        else if (s3[a] > hi[a]) d = __dsub_rn(s3[a], hi[a]);
+                        d2 = __dadd_rn(d2, __dmul_rn(d, d));
+                    }
+                    const bool open = __dmul_rn(gm.w, gm.w) > __dmul_rn(th2, d2);
+                    kind = !open ? 1 : (cc.n_child == 0 ? 3 : 2);
                 }
-                const bool open = __dmul_rn(gm.w, gm.w) > __dmul_rn(th2, d2);
-                kind = !open ? 1 : (cc.n_child == 0 ? 3 : 2);
             }
             // SPJ entries
             const unsigned m_s = __ballot_sync(0xffffffffu, kind == 1);
@@ -124,6 +142,37 @@ __global__ void __launch_bounds__(256) k_walk(const mwf_cell* __restrict__ cells
     }
 }
 
+// Largest smoothing length among the particles of every cell (bits of a positive float order like ints): each leaf
+// takes the maximum over its particles and raises its ancestors with atomicMax until one is already as large.
+__global__ void __launch_bounds__(256) k_cell_hmax(const mwf_cell* __restrict__ cells, const int32_t* __restrict__ parent, const float4* __restrict__ sph,
+                                                   int64_t n_cell, int* __restrict__ cell_h) {
+    const int64_t c0 = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (c0 >= n_cell) return;
+    const mwf_cell cc = cells[c0];
+    if (cc.n_child != 0) return;
+    float m = 0.f;
+    for (int k = 0; k < cc.n_ptcl; ++k) m = fmaxf(m, sph[cc.first_ptcl + k].x);
+    const int bits = __float_as_int(m);
+    int32_t c = (int32_t)c0;
+    while (c >= 0) {
+        if (atomicMax(&cell_h[c], bits) >= bits && c != (int32_t)c0) break;
+        c = parent[c];
+    }
+}
+
+__global__ void __launch_bounds__(256) k_group_hmax(const float4* __restrict__ sph, const int32_t* __restrict__ grp_first, const int32_t* __restrict__ grp_n,
+                                                    int64_t n_group, float* __restrict__ grp_h) {
+    const int lane = threadIdx.x & 31;
+    const int64_t g = ((int64_t)blockIdx.x * blockDim.x + threadIdx.x) >> 5;
+    if (g >= n_group) return;
+    const int f = grp_first[g], cnt = grp_n[g];
+    float m = 0.f;
+    for (int i = lane; i < cnt; i += 32) m = fmaxf(m, sph[f + i].x);
+#pragma unroll
+    for (int d = 16; d > 0; d >>= 1) m = fmaxf(m, __shfl_xor_sync(0xffffffffu, m, d));
+    if (lane == 0) grp_h[g] = m;
+}
+
 // list_off[g] (to be scanned) = padded length of group g's merged list
 __global__ void __launch_bounds__(256) k_padded_len(const int32_t* __restrict__ n_epj, const int32_t* __restrict__ n_spj, int64_t n_group,
                                                     int64_t* __restrict__ list_off, int64_t* __restrict__ epj_off, int64_t* __restrict__ spj_off) {
@@ -162,12 +211,24 @@ int64_t walk_warps(int64_t max_group) {
 
 // Counting pass + offsets.  Leaves list_off / epj_off / spj_off scanned (n_group + 1 entries each) and returns the
 // totals through *padded / *e_epj / *e_spj (one stream synchronisation).
-cudaError_t build_lists_count(const BuildBuffers& b, int64_t n_group, double theta, int64_t n_warps, int64_t* padded, int64_t* e_epj, int64_t* e_spj,
+cudaError_t build_smoothing_reach(const BuildBuffers& b, const float4* sph, int64_t n_cell, int64_t n_group, float* cell_h, float* grp_h, cudaStream_t s) {
+    BL(cudaMemsetAsync(cell_h, 0, (size_t)n_cell * 4, s));
+    k_cell_hmax<<<(unsigned)((n_cell + 255) / 256), 256, 0, s>>>(b.cells, b.parent, sph, n_cell, reinterpret_cast<int*>(cell_h));
+    BL(cudaGetLastError());
+    k_group_hmax<<<(unsigned)((n_group * 32 + 255) / 256), 256, 0, s>>>(sph, b.grp_first, b.grp_n, n_group, grp_h);
+    return cudaGetLastError();
+}
+
+cudaError_t build_lists_count(const BuildBuffers& b, int64_t n_group, const WalkRule& rule, int64_t n_warps, int64_t* padded, int64_t* e_epj, int64_t* e_spj,
                               cudaStream_t s) {
-    const double th2 = theta * theta;
+    const double th2 = rule.theta * rule.theta;
     BL(cudaMemsetAsync(b.walk_counter, 0, 4, s));
-    k_walk<false><<<(unsigned)(n_warps / 8), 256, 0, s>>>(b.cells, b.geom, b.grp_box, n_group, th2, b.walk_stacks, b.walk_counter, b.n_epj, b.n_spj,
-                                                          nullptr, nullptr, 0, 0);
+    if (rule.neighbours)
+        k_walk<false, true><<<(unsigned)(n_warps / 8), 256, 0, s>>>(b.cells, b.geom, b.grp_box, n_group, th2, rule.reach, rule.cell_h, rule.grp_h, b.walk_stacks,
+                                                                    b.walk_counter, b.n_epj, b.n_spj, nullptr, nullptr, 0, 0);
+    else
+        k_walk<false, false><<<(unsigned)(n_warps / 8), 256, 0, s>>>(b.cells, b.geom, b.grp_box, n_group, th2, 0.0, nullptr, nullptr, b.walk_stacks,
+                                                                     b.walk_counter, b.n_epj, b.n_spj, nullptr, nullptr, 0, 0);
     BL(cudaGetLastError());
     k_padded_len<<<(unsigned)((n_group + 1 + 255) / 256), 256, 0, s>>>(b.n_epj, b.n_spj, n_group, b.list_off, b.epj_off, b.spj_off);
     BL(cudaGetLastError());
@@ -185,11 +246,15 @@ cudaError_t build_lists_count(const BuildBuffers& b, int64_t n_group, double the
     return cudaSuccess;
 }
 
-cudaError_t build_lists_fill(const BuildBuffers& b, int64_t n_group, double theta, int64_t n_warps, int64_t n_ptcl, int64_t n_cell, cudaStream_t s) {
-    const double th2 = theta * theta;
+cudaError_t build_lists_fill(const BuildBuffers& b, int64_t n_group, const WalkRule& rule, int64_t n_warps, int64_t n_ptcl, int64_t n_cell, cudaStream_t s) {
+    const double th2 = rule.theta * rule.theta;
     BL(cudaMemsetAsync(b.walk_counter, 0, 4, s));
-    k_walk<true><<<(unsigned)(n_warps / 8), 256, 0, s>>>(b.cells, b.geom, b.grp_box, n_group, th2, b.walk_stacks, b.walk_counter, b.n_epj, b.n_spj,
-                                                         b.list_off, b.list, (int32_t)n_ptcl, (int32_t)(n_ptcl + n_cell));
+    if (rule.neighbours)
+        k_walk<true, true><<<(unsigned)(n_warps / 8), 256, 0, s>>>(b.cells, b.geom, b.grp_box, n_group, th2, rule.reach, rule.cell_h, rule.grp_h, b.walk_stacks,
+                                                                   b.walk_counter, b.n_epj, b.n_spj, b.list_off, b.list, (int32_t)n_ptcl, (int32_t)(n_ptcl + n_cell));
+    else
+        k_walk<true, false><<<(unsigned)(n_warps / 8), 256, 0, s>>>(b.cells, b.geom, b.grp_box, n_group, th2, 0.0, nullptr, nullptr, b.walk_stacks,
+                                                                    b.walk_counter, b.n_epj, b.n_spj, b.list_off, b.list, (int32_t)n_ptcl, (int32_t)(n_ptcl + n_cell));
     return cudaGetLastError();
 }
 

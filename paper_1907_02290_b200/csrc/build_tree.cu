@@ -267,7 +267,7 @@ inline unsigned grid_for(int64_t n, int block, int cap) {
 // cells, their geometry, parents and the groups.  Synchronises the stream once per tree level to learn the
 // level's size.  Outputs the counts through *n_cell / *n_group; ERR_BUILD_CAPACITY in *err when max_cell /
 // max_group are too small.
-cudaError_t build_tree_device(const BuildBuffers& b, int64_t n, int n_leaf, int n_grp, int64_t max_cell, int64_t max_group, bool with_vel,
+cudaError_t build_tree_device(const BuildBuffers& b, int64_t n, int n_leaf, int n_grp, int64_t max_cell, int64_t max_group, bool with_vel, float4* sph,
                               int64_t* n_cell_out, int64_t* n_group_out, int* n_level_out, cudaStream_t s) {
     const int n_part = 148 * 4;
     k_bbox_partial<<<n_part, 256, 0, s>>>(b.store, n, b.bbox_part);
@@ -285,6 +285,11 @@ cudaError_t build_tree_device(const BuildBuffers& b, int64_t n, int n_leaf, int 
         k_gather16<<<grid_for(n, 256, 148 * 8), 256, 0, s>>>(b.vel, b.idx_a, n, b.tmp16);
         BT(cudaGetLastError());
         BT(cudaMemcpyAsync(b.vel, b.tmp16, (size_t)n * 16, cudaMemcpyDeviceToDevice, s));
+    }
+    if (sph) {  // short-range workload: the per-particle SPH records travel with their particles
+        k_gather16<<<grid_for(n, 256, 148 * 8), 256, 0, s>>>(sph, b.idx_a, n, b.tmp16);
+        BT(cudaGetLastError());
+        BT(cudaMemcpyAsync(sph, b.tmp16, (size_t)n * 16, cudaMemcpyDeviceToDevice, s));
     }
     // cells level by level
     k_root_cell<<<1, 32, 0, s>>>(b.cells, b.geom, b.parent, b.root, (int32_t)n);

@@ -870,10 +870,13 @@ int mwf_calc_force_all(mwf_ctx* c, const mwf_posm* src, int src_on_device, mwf_a
     return MWF_OK;
 }
 
-int mwf_build(mwf_ctx* c, int64_t n, int32_t n_leaf, int32_t n_grp, double theta, int mode, void* stream) {
-    if (!c || n < 1 || n_leaf < 1 || n_grp < 1 || !(theta >= 0.0) || theta > 1.0) return MWF_EINVAL;
+// The device-side construction step behind mwf_build (opening angle theta) and mwf_build_neighbours (search radii 2 (1 + skin) h).
+static int build_impl(mwf_ctx* c, int64_t n, int32_t n_leaf, int32_t n_grp, double theta, bool neighbours, double skin, int mode, void* stream) {
+    if (!c || n < 1 || n_leaf < 1 || n_grp < 1) return MWF_EINVAL;
+    if (neighbours ? !(skin >= 0.0) : (!(theta >= 0.0) || theta > 1.0)) return MWF_EINVAL;
     if (mode != MWF_MAKE_LIST && mode != MWF_MAKE_LIST_FOR_REUSE) return MWF_EINVAL;
     if (n > c->p.max_ptcl) return MWF_ENOMEM;
+    if (neighbours && (!c->sph || c->sph_hi < n)) return MWF_ESTATE;  // the smoothing lengths of particles [0, n) must have been uploaded
     if (c->ptcl_hi < n && !(c->have_tree && c->n_ptcl >= n)) return MWF_ESTATE;  // particles [0, n) must have been uploaded
     for (int t = 0; t < c->p.n_tag; ++t)
         if (!c->tag_ranges[t].empty()) return MWF_ESTATE;  // tmp16 aliases the result array: retrieve first
@@ -889,7 +892,8 @@ int mwf_build(mwf_ctx* c, int64_t n, int32_t n_leaf, int32_t n_grp, double theta
     int64_t n_cell = 0, n_group = 0;
     int n_level = 0;
     PhaseTimer tm;
-    CU(c, build_tree_device(c->bb, n, n_leaf, n_grp, c->p.max_cell, c->p.max_group, with_vel, &n_cell, &n_group, &n_level, s));
+    float4* sph = (c->sph && c->sph_hi >= n) ? c->sph : nullptr;
+    CU(c, build_tree_device(c->bb, n, n_leaf, n_grp, c->p.max_cell, c->p.max_group, with_vel, sph, &n_cell, &n_group, &n_level, s));
     c->n_launch += 8 + 3 * 8 + 3 * n_level;
     tm.lap("sort + tree + groups");
     if (n_cell > c->p.max_cell || n_group > c->p.max_group) { after_store_op(c, s); return MWF_ENOMEM; }
@@ -906,7 +910,17 @@ int mwf_build(mwf_ctx* c, int64_t n, int32_t n_leaf, int32_t n_grp, double theta
     c->ptcl_hi = n;
     // lists: counting walk, offsets, capacity check, fill walk
     int64_t padded = 0, e_epj = 0, e_spj = 0;
-    CU(c, build_lists_count(c->bb, n_group, theta, c->walk_warps_n, &padded, &e_epj, &e_spj, s));
+    WalkRule rule;
+    rule.theta = theta;
+    if (neighbours) {  // per-cell and per-group search radii; level_cnt and mark are free once the tree and the groups exist
+        rule.neighbours = true;
+        rule.reach = 2.0 * (1.0 + skin);
+        rule.cell_h = reinterpret_cast<float*>(c->bb.level_cnt);
+        rule.grp_h = reinterpret_cast<float*>(c->bb.mark);
+        CU(c, build_smoothing_reach(c->bb, c->sph, n_cell, n_group, reinterpret_cast<float*>(c->bb.level_cnt), reinterpret_cast<float*>(c->bb.mark), s));
+        c->n_launch += 2;
+    }
+    CU(c, build_lists_count(c->bb, n_group, rule, c->walk_warps_n, &padded, &e_epj, &e_spj, s));
     tm.lap("list walk: count + offsets");
     if (e_epj + e_spj > c->p.max_entry) { after_store_op(c, s); return MWF_ENOMEM; }
     // group sizes and list lengths come back for the host work plan; the fill walk runs meanwhile
@@ -917,7 +931,7 @@ int mwf_build(mwf_ctx* c, int64_t n, int32_t n_leaf, int32_t n_grp, double theta
     CU(c, cudaMemcpyAsync(h_ne.data(), c->bb.n_epj, (size_t)n_group * 4, D2H, s));
     CU(c, cudaMemcpyAsync(h_ns.data(), c->bb.n_spj, (size_t)n_group * 4, D2H, s));
     CU(c, cudaStreamSynchronize(s));
-    CU(c, build_lists_fill(c->bb, n_group, theta, c->walk_warps_n, n, n_cell, s));
+    CU(c, build_lists_fill(c->bb, n_group, rule, c->walk_warps_n, n, n_cell, s));
     CU(c, cudaMemsetAsync(c->grp_self, 1, (size_t)n_group, s));  // theta <= 1: a group's own cells are always opened
     c->n_launch += 6;
     std::vector<int64_t> n_list((size_t)n_group);
@@ -942,6 +956,14 @@ int mwf_build(mwf_ctx* c, int64_t n, int32_t n_leaf, int32_t n_grp, double theta
     c->build_n_level = n_level;
     adopt_plan(c, plan, n_group, h_first.data(), h_n.data(), mode);
     return MWF_OK;
+}
+
+int mwf_build(mwf_ctx* c, int64_t n, int32_t n_leaf, int32_t n_grp, double theta, int mode, void* stream) {
+    return build_impl(c, n, n_leaf, n_grp, theta, false, 0.0, mode, stream);
+}
+
+int mwf_build_neighbours(mwf_ctx* c, int64_t n, int32_t n_leaf, int32_t n_grp, double skin, int mode, void* stream) {
+    return build_impl(c, n, n_leaf, n_grp, 0.0, true, skin, mode, stream);
 }
 
 int mwf_get_build_sizes(mwf_ctx* c, int64_t* n_cell, int64_t* n_group, int64_t* n_epj, int64_t* n_spj, int32_t* n_level) {

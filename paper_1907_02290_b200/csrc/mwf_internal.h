@@ -127,12 +127,23 @@ struct BuildBuffers {
     int32_t* walk_stacks; unsigned int* walk_counter; unsigned int* err;
 };
 
-cudaError_t build_tree_device(const BuildBuffers& b, int64_t n, int n_leaf, int n_grp, int64_t max_cell, int64_t max_group, bool with_vel,
+cudaError_t build_tree_device(const BuildBuffers& b, int64_t n, int n_leaf, int n_grp, int64_t max_cell, int64_t max_group, bool with_vel, float4* sph,
                               int64_t* n_cell_out, int64_t* n_group_out, int* n_level_out, cudaStream_t s);
 int64_t walk_warps(int64_t max_group);
-cudaError_t build_lists_count(const BuildBuffers& b, int64_t n_group, double theta, int64_t n_warps, int64_t* padded, int64_t* e_epj, int64_t* e_spj,
+// Which cells a group's walk opens: the opening angle (gravity) or the short-range neighbour search (reading S24:
+// gap between cell cube and group box <= max over (group, cell) of reach x the largest smoothing length).
+struct WalkRule {
+    double theta = 0.0;
+    bool neighbours = false;
+    double reach = 0.0;          // 2 (1 + skin)
+    const float* cell_h = nullptr;  // [n_cell] largest h among the cell's particles
+    const float* grp_h = nullptr;   // [n_group]
+};
+cudaError_t build_lists_count(const BuildBuffers& b, int64_t n_group, const WalkRule& rule, int64_t n_warps, int64_t* padded, int64_t* e_epj, int64_t* e_spj,
                               cudaStream_t s);
-cudaError_t build_lists_fill(const BuildBuffers& b, int64_t n_group, double theta, int64_t n_warps, int64_t n_ptcl, int64_t n_cell, cudaStream_t s);
+cudaError_t build_lists_fill(const BuildBuffers& b, int64_t n_group, const WalkRule& rule, int64_t n_warps, int64_t n_ptcl, int64_t n_cell, cudaStream_t s);
+// cell_h / grp_h of a WalkRule from the h field of the SPH records (tree order)
+cudaError_t build_smoothing_reach(const BuildBuffers& b, const float4* sph, int64_t n_cell, int64_t n_group, float* cell_h, float* grp_h, cudaStream_t s);
 cudaError_t unmerge_lists(const BuildBuffers& b, int64_t n_group, int64_t n_ptcl, int32_t* epj_id, int32_t* spj_id, cudaStream_t s);
 
 cudaError_t launch_kick_drift(float4* store, float4* vel, const float4* accp, int64_t n, float dt, cudaStream_t s);

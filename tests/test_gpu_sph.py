@@ -237,3 +237,75 @@ def test_sph_full_size_sampled_groups_with_reuse():
         m = posm[:, 3].astype(np.float64)
         assert np.linalg.norm(np.sum(m[:, None] * out[:, :3].astype(np.float64), 0)) < 1e-5 * np.sum(m[mask] * scale[mask]) * w.n / mask.sum()
     f.close()
+
+
+# ------------------------------------------------------------------ device-side construction of the neighbour lists
+def device_neighbour_build(posm, rec, n_leaf, n_grp, skin, max_entry=None):
+    n = posm.shape[0]
+    f = binding.MultiWalkForce(1.0, 1.0, max_ptcl=n, max_cell=2 * n + 64, max_group=n + 8,
+                               max_entry=max_entry or max(64, min(n * n + 64 * n, 3000 * n + 4096)), n_tag=2)
+    f.begin_step(binding.MAKE_LIST_FOR_REUSE)
+    f.set_particles(posm)                      # caller order, NOT tree order
+    with pytest.raises(binding.MwfError) as e:
+        f.build_neighbours(n, n_leaf, n_grp, skin)
+    assert e.value.code == binding.ESTATE      # no smoothing lengths yet
+    f.set_sph(rec)
+    f.build_neighbours(n, n_leaf, n_grp, skin)
+    sz = f.get_build_sizes()
+    out = dict(sizes=sz, perm=f.get_permutation(n), posm=f.get_particles(0, n), sph=f.get_sph(0, n))
+    out["grp_first"], out["grp_n"] = f.get_groups(sz["n_group"])
+    out["epj_off"], out["epj_id"], out["spj_off"], out["spj_id"] = f.get_lists(sz["n_group"], sz["n_epj"], sz["n_spj"])
+    return out, f
+
+
+@pytest.mark.parametrize("n,n_leaf,n_grp,skin", [(700, 8, 32, 0.0), (1500, 16, 64, 0.2), (64, 4, 8, 0.0), (3000, 8, 48, 10.0), (1, 8, 8, 0.0)])
+def test_device_neighbour_build_matches_plain_restatement(n, n_leaf, n_grp, skin):
+    """mwf_build_neighbours against oracle/bhtree_ref.py (reading S24 step by step): permutation, records carried along,
+    groups, and per-group EPJ sets; there are no SPJ."""
+    from oracle import bhtree_ref
+    from paper_1907_02290_b200.workload import make_particles, make_sph_fields
+    cfg = SPH_CONFIGS[0]
+    posm, _ = make_particles(cfg, n)
+    rec = make_sph_fields(cfg, posm)
+    ref = bhtree_ref.build(posm, n_leaf, n_grp, 0.0, h=rec[:, 0], skin=skin)
+    got, f = device_neighbour_build(posm, rec, n_leaf, n_grp, skin)
+    f.close()
+    assert np.array_equal(got["perm"], ref["perm"])
+    assert np.array_equal(got["posm"], posm[ref["perm"]])
+    assert np.array_equal(got["sph"], rec[ref["perm"]])
+    assert np.array_equal(got["grp_first"], ref["cells"][ref["groups"], 0])
+    assert got["sizes"]["n_spj"] == 0
+    for g in range(len(ref["groups"])):
+        e = got["epj_id"][got["epj_off"][g]:got["epj_off"][g + 1]]
+        assert np.array_equal(np.sort(e), np.sort(np.array(ref["epj"][g], np.int32))), "EPJ set of group %d" % g
+
+
+def test_device_neighbour_build_full_size_then_both_passes():
+    """sph_plummer_1m built on the device from particles in generator order: every list offset and 300 sampled lists equal
+    the independent host builder's; then density and hydro on the device-built lists against the oracle on sampled groups."""
+    from paper_1907_02290_b200.workload import make_particles, make_sph_fields
+    cfg = SPH_CONFIGS[1]
+    posm, _ = make_particles(cfg)
+    rec = make_sph_fields(cfg, posm)
+    w = build_tree_and_lists(posm, cfg.n_leaf, cfg.n_grp, 0.0, cfg=cfg, sph=rec, skin=cfg.skin)
+    got, f = device_neighbour_build(posm, rec, cfg.n_leaf, cfg.n_grp, cfg.skin, max_entry=w.n_entry + 1024)
+    assert np.array_equal(got["perm"], w.perm)
+    assert np.array_equal(got["grp_first"], w.grp_first) and np.array_equal(got["grp_n"], w.grp_n)
+    assert np.array_equal(got["epj_off"], w.epj_off) and got["sizes"]["n_spj"] == 0
+    rng = np.random.default_rng(5)
+    sample = np.sort(rng.choice(w.n_group, 300, replace=False)).astype(np.int64)
+    for g in sample:
+        a = got["epj_id"][got["epj_off"][g]:got["epj_off"][g + 1]]
+        b = w.epj_id[w.epj_off[g]:w.epj_off[g + 1]]
+        assert np.array_equal(np.sort(a), np.sort(b))
+    mask = group_mask(w, sample)
+    out = gpu_density(f, w, cfg.gamma)
+    rho, pr2 = oracle.sph_density(w.posm, w.sph, got["grp_first"], got["grp_n"], got["epj_off"], got["epj_id"], cfg.gamma, sample)
+    check_density(out, rho, pr2, mask, label="device-built lists")
+    rho_all, pr2_all = oracle.sph_density(w.posm, w.sph, got["grp_first"], got["grp_n"], got["epj_off"], got["epj_id"], cfg.gamma)
+    orec = w.sph.copy()
+    orec[:, 2], orec[:, 3] = rho_all, pr2_all
+    f.set_sph(orec)
+    acc, scale = oracle.sph_hydro(w.posm, orec, got["grp_first"], got["grp_n"], got["epj_off"], got["epj_id"], sample)
+    check_hydro(gpu_hydro(f, w), acc, scale, w.posm, orec, mask, label="device-built lists")
+    f.close()
