@@ -374,10 +374,11 @@ def quad_leg(args, cfg, binding, device):
 def sph_leg(args, binding, device):
     """Short-range workload (NEXT-4): one list-reuse step of the SPH pair of passes -- upload particles, density over all
     groups, pressure-gradient acceleration over all groups, retrieve -- on the gas Plummer sphere `sph_plummer_4m`
-    (N = 2^22, neighbour lists with 10 % skin).  Both kernels are ALU-bound like k_force.  Flop convention (FMA = 2,
-    sqrt / rsqrt = 4 as in the paper's 23, max = 1): density 25 flop per list interaction (3 sub, mul + 2 fma, sqrt, 1 mul,
-    two clamped differences, two cubes, 1 fma, 1 fma), hydro 45 (3 sub, 3 fma, rsqrt, 3 mul, two clamped-difference
-    polynomials of 8, 2 mul + fma, 1 add, 2 mul, 3 fma).  Interactions counted as for gravity: sum n_i x n_list."""
+    (N = 2^22, neighbour lists with 10 % skin).  Both kernels are ALU-bound like k_force.  Flop convention: the arithmetic
+    of the formulas with FMA = 2, sqrt / rsqrt = 4 as in the paper's 23, max = 1: density 25 flop per list interaction (3 sub,
+    mul + 2 fma, sqrt, 1 mul, two clamped differences, two cubes, 1 fma, 1 fma), hydro 45 (3 sub, 3 fma, rsqrt, 3 mul, two
+    clamped-difference quadratics of 8, 2 mul + fma, 1 add, 2 mul, 3 fma); constant-operand FMAs the kernels use instead of
+    adds count as the adds.  Interactions counted as for gravity: sum n_i x n_list."""
     import torch
     import oracle
     from paper_1907_02290_b200.workload import SPH_CONFIGS, make_workload

@@ -36,22 +36,29 @@ __device__ __forceinline__ int2 ld_stream_int2(const int2* p) {
     return v;
 }
 __device__ __forceinline__ float2 f2(float a) { return make_float2(a, a); }
-// (c - q)+ for both halves
-__device__ __forceinline__ float2 clamp_sub(float c, float2 q) {
-    const float2 t = __fadd2_rn(f2(c), make_float2(-q.x, -q.y));
+// (c - s q)+ for both halves
+__device__ __forceinline__ float2 clamp_lin(float c, float s, float2 q) {
+    const float2 t = __ffma2_rn(q, f2(-s), f2(c));
     return make_float2(fmaxf(t.x, 0.f), fmaxf(t.y, 0.f));
 }
-// (2-q)+^P - 4 (1-q)+^P for P = 2 or 3
+// Both branches of the cubic spline in one branch-free polynomial of t2 = (2 - q)+ and a scaled (1 - q)+, arranged so that
+// the last operation has only two distinct register operands (a three-operand FFMA2 costs 3 pipe cycles):
+//   P = 2:  (2-q)+^2 - 4 (1-q)+^2 = t2^2 - u^2,      u = (2 - 2q)+            (exactly 2 (1-q)+)
+//   P = 3:  (2-q)+^3 - 4 (1-q)+^3 = t2^3 - u^3,      u = (k - k q)+, k = 4^(1/3)
 template <int P>
 __device__ __forceinline__ float2 spline_poly(float2 q) {
-    const float2 t2 = clamp_sub(2.f, q), t1 = clamp_sub(1.f, q);
+    const float2 t2 = clamp_lin(2.f, 1.f, q);
     float2 a = __fmul2_rn(t2, t2);
-    float2 b = __fmul2_rn(t1, f2(-4.f));
-    if constexpr (P == 3) {
+    if constexpr (P == 2) {
+        const float2 u = clamp_lin(2.f, 2.f, q);
+        return __ffma2_rn(make_float2(-u.x, -u.y), u, a);
+    } else {
+        constexpr float K = 1.58740105196819947475f;
+        const float2 u = clamp_lin(K, K, q);
         a = __fmul2_rn(a, t2);
-        b = __fmul2_rn(b, t1);
+        const float2 c = __fmul2_rn(u, u);
+        return __ffma2_rn(make_float2(-c.x, -c.y), u, a);
     }
-    return __ffma2_rn(b, t1, a);
 }
 
 struct ItemSetup {
