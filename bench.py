@@ -415,6 +415,18 @@ def sph_leg(args, binding, device):
             if it >= args.warmup:
                 ms["step"].append(e0.elapsed_time(e1)); ms["density"].append(t_d); ms["hydro"].append(f.last_dispatch_ms(0))
     launches = f.get_counters()["kernel_launches"]
+    # end to end through host buffers: pinned particles and records in, records and accelerations out (mwf_calc_sph_all)
+    src_host, rec_host, dst_host = f.pinned(w.n), f.pinned(w.n), f.pinned(w.n)
+    src_host.numpy()[:] = w.posm
+    e2e_ms = []
+    for it in range(args.warmup + args.steps):
+        rec_host.numpy()[:] = w.sph
+        torch.cuda.synchronize()
+        t = time.perf_counter()
+        f.begin_step(binding.REUSE_LIST)
+        f.calc_sph_all(src_host, rec_host, dst_host, cfg.gamma)
+        if it >= args.warmup:
+            e2e_ms.append((time.perf_counter() - t) * 1e3)
     f.close()
     # construction step on the device (mwf_build_neighbours) from particles in generator order, against the host builder
     from paper_1907_02290_b200.workload import build_tree_and_lists, make_particles, make_sph_fields
@@ -461,6 +473,9 @@ def sph_leg(args, binding, device):
                                  "interactions_per_pass": inter, "n_leaf": cfg.n_leaf, "n_grp": cfg.n_grp, "eta": cfg.eta, "skin": cfg.skin,
                                  "step": "list-reuse step: upload particles and records, density pass, hydro pass, retrieve (device-resident)"},
                       "kernels": kern, "peak_tflops": peak / 1e12, "gpu_launches": launches,
+                      "e2e": {"value": 2 * inter / (float(np.median(e2e_ms)) * 1e-3), "unit": "interactions/s", "ms_per_step": float(np.median(e2e_ms)),
+                              "h2d_bytes_per_step": 2 * 16 * w.n, "d2h_bytes_per_step": 2 * 16 * w.n,
+                              "what": "mwf_calc_sph_all with pinned host buffers (host wall clock around the blocking call)"},
                       "construction_step": {"device_ms": float(np.median(ms_build[1:])), "host_builder_s": t_host_build,
                                             "what": "mwf_build_neighbours: sort, tree, groups, neighbour-search walk (host wall clock around the blocking call)"}, "clocks": clk.summary(),
                       "cpu_baseline": {"value": n_cpu / t_cpu, "unit": "interactions/s", "cores": oracle.num_threads(), "kind": "oracle",

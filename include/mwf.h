@@ -203,6 +203,13 @@ int mwf_set_sph(mwf_ctx* c, const mwf_sph* src, int64_t first, int64_t n, int sr
 int mwf_get_sph(mwf_ctx* c, mwf_sph* dst, int64_t first, int64_t n, int dst_on_device);
 int mwf_dispatch_density(mwf_ctx* c, int32_t tag, int64_t g_begin, int64_t g_end, float gamma);
 int mwf_dispatch_hydro(mwf_ctx* c, int32_t tag, int64_t g_begin, int64_t g_end);
+/* One whole short-range evaluation for a step whose tree and neighbour lists are already on the device (the analogue of
+ * mwf_calc_force_all): upload all N particles (src HOST or DEVICE; NULL = keep the store) and all N records (rec: h and
+ * u are read), density pass over all groups, records back into rec (rho and P/rho^2 filled in), hydro pass over all
+ * groups, accelerations into dst.  With a host rec or dst the groups are split over the tags so that every tag's copy
+ * overlaps the other tags' kernels.  Blocking. */
+int mwf_calc_sph_all(mwf_ctx* c, const mwf_posm* src, int src_on_device, mwf_sph* rec, int rec_on_device, mwf_accp* dst, int dst_on_device,
+                     float gamma);
 
 /* (5) Copy acc+pot of the particles of every group dispatched under `tag` since its last retrieve into
  * dst and wait for it.  dst: base of an N-record array indexed by tree-order particle

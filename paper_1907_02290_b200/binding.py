@@ -25,7 +25,7 @@ SYMBOLS = (
     "mwf_last_dispatch_ms", "mwf_strerror", "mwf_last_cuda_error",
     "mwf_set_velocities", "mwf_get_velocities", "mwf_kick_drift", "mwf_kick", "mwf_step_reuse",
     "mwf_reserve_data_lists", "mwf_dispatch_data", "mwf_set_spj_order", "mwf_get_quadrupoles", "mwf_last_quad_ms",
-    "mwf_set_sph", "mwf_get_sph", "mwf_dispatch_density", "mwf_dispatch_hydro",
+    "mwf_set_sph", "mwf_get_sph", "mwf_dispatch_density", "mwf_dispatch_hydro", "mwf_calc_sph_all",
     "mwf_build", "mwf_build_neighbours", "mwf_get_build_sizes", "mwf_get_permutation", "mwf_get_tree", "mwf_get_groups", "mwf_get_lists",
 )
 
@@ -89,6 +89,7 @@ def load_library(path: str | None = None) -> ctypes.CDLL:
         "mwf_get_sph": [vp, vp, i64, i64, ci],
         "mwf_dispatch_density": [vp, i32, i64, i64, ctypes.c_float],
         "mwf_dispatch_hydro": [vp, i32, i64, i64],
+        "mwf_calc_sph_all": [vp, vp, ci, vp, ci, vp, ci, ctypes.c_float],
         "mwf_build": [vp, i64, i32, i32, ctypes.c_double, ci, vp],
         "mwf_build_neighbours": [vp, i64, i32, i32, ctypes.c_double, ci, vp],
         "mwf_get_build_sizes": [vp, P(i64), P(i64), P(i64), P(i64), P(i32)],
@@ -292,6 +293,16 @@ class MultiWalkForce:
 
     def build(self, n: int, n_leaf: int, n_grp: int, theta: float, mode: int = MAKE_LIST_FOR_REUSE, stream=None):
         self._ck(self._lib.mwf_build(self._h, int(n), int(n_leaf), int(n_grp), float(theta), int(mode), _stream_handle(stream)))
+
+    def calc_sph_all(self, src, rec, dst, gamma: float):
+        """One whole short-range evaluation: rec (h, u in; rho, P/rho^2 out) and dst (ax, ay, az, 0) are [N,4] float32."""
+        if src is None:
+            sp, s_dev = ctypes.c_void_p(None), 0
+        else:
+            sp, s_dev = _ptr(src, np.float32, "src")
+        rp, r_dev = _ptr(rec, np.float32, "rec")
+        dp, d_dev = _ptr(dst, np.float32, "dst")
+        self._ck(self._lib.mwf_calc_sph_all(self._h, sp, s_dev, rp, r_dev, dp, d_dev, float(gamma)))
 
     def build_neighbours(self, n: int, n_leaf: int, n_grp: int, skin: float, mode: int = MAKE_LIST_FOR_REUSE, stream=None):
         self._ck(self._lib.mwf_build_neighbours(self._h, int(n), int(n_leaf), int(n_grp), float(skin), int(mode), _stream_handle(stream)))

@@ -1168,6 +1168,37 @@ int mwf_dispatch_hydro(mwf_ctx* c, int32_t tag, int64_t g_begin, int64_t g_end) 
     return sph_dispatch(c, tag, g_begin, g_end, true, 0.f);
 }
 
+int mwf_calc_sph_all(mwf_ctx* c, const mwf_posm* src, int src_on_device, mwf_sph* rec, int rec_on_device, mwf_accp* dst, int dst_on_device, float gamma) {
+    if (!c || !rec || !dst) return MWF_EINVAL;
+    if (!c->have_tree || !c->have_lists) return MWF_ESTATE;
+    cudaStream_t s0 = c->tag_stream[0];
+    int rc;
+    if (src) {
+        rc = mwf_set_particles(c, src, 0, c->n_ptcl, src_on_device, s0);
+        if (rc) return rc;
+    }
+    rc = mwf_set_sph(c, rec, 0, c->n_ptcl, rec_on_device, s0);
+    if (rc) return rc;
+    // host destinations: one dispatch per tag so that each tag's copy overlaps the other tags' kernels
+    const int n_part = (rec_on_device && dst_on_device) ? 1 : c->p.n_tag;
+    for (int pass = 0; pass < 2; ++pass) {
+        bool used[MWF_MAX_TAG] = {false};
+        for (int t = 0; t < n_part; ++t) {
+            const int64_t gb = n_part == 1 ? 0 : c->h_split[(size_t)t], ge = n_part == 1 ? c->n_group : c->h_split[(size_t)t + 1];
+            if (ge == gb) continue;
+            rc = pass == 0 ? mwf_dispatch_density(c, t, gb, ge, gamma) : mwf_dispatch_hydro(c, t, gb, ge);
+            if (rc) return rc;
+            used[t] = true;
+        }
+        for (int t = 0; t < n_part; ++t) {
+            if (!used[t]) continue;
+            rc = pass == 0 ? mwf_retrieve(c, t, reinterpret_cast<mwf_accp*>(rec), rec_on_device) : mwf_retrieve(c, t, dst, dst_on_device);
+            if (rc) return rc;
+        }
+    }
+    return MWF_OK;
+}
+
 int mwf_set_spj_order(mwf_ctx* c, int order) {
     if (!c || (order != 1 && order != 2)) return MWF_EINVAL;
     for (int t = 0; t < c->p.n_tag; ++t)

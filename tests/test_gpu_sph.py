@@ -239,6 +239,25 @@ def test_sph_full_size_sampled_groups_with_reuse():
     f.close()
 
 
+def test_calc_sph_all_host_buffers_equals_the_single_dispatches():
+    """mwf_calc_sph_all through pinned host buffers (groups split over the tags, copies overlapped) gives bitwise what one
+    density dispatch and one hydro dispatch give."""
+    cfg = SPH_CONFIGS[0]
+    w = make_workload(cfg, n=30001)
+    f = make_ctx(w, n_tag=4)
+    rec1 = gpu_density(f, w, cfg.gamma)
+    acc1 = gpu_hydro(f, w)
+    src, rec, dst = f.pinned(w.n), f.pinned(w.n), f.pinned(w.n)
+    src.numpy()[:] = w.posm
+    rec.numpy()[:] = w.sph
+    dst.numpy()[:] = np.nan
+    f.begin_step(binding.REUSE_LIST)
+    f.calc_sph_all(src, rec, dst, cfg.gamma)
+    np.testing.assert_array_equal(rec.numpy(), rec1)
+    np.testing.assert_array_equal(dst.numpy(), acc1)
+    f.close()
+
+
 # ------------------------------------------------------------------ device-side construction of the neighbour lists
 def device_neighbour_build(posm, rec, n_leaf, n_grp, skin, max_entry=None):
     n = posm.shape[0]
