@@ -28,6 +28,10 @@ struct mwf_ctx {
     int32_t* parent = nullptr;    // [max_cell]
     int32_t* arrive = nullptr;    // [max_cell]
     double4* mom64 = nullptr;     // [max_cell]
+    int2* cell_lr = nullptr;      // [max_cell] range of leaf ranks of every cell (scan variant of the refresh)
+    double4* leaf_P = nullptr;    // [max_cell + 1] leaves' moments in rank order, scanned in place every refresh
+    double4* leaf_toff = nullptr; // [tiles] scanned tile totals
+    int64_t n_leaf_cells = 0;
     int32_t* grp_first = nullptr; // [max_group]
     int32_t* grp_n = nullptr;     // [max_group]
     uint8_t* grp_self = nullptr;  // [max_group]
@@ -181,6 +185,9 @@ Layout make_layout(const mwf_params& p) {
     L.add(walk_warps(p.max_group) * WALK_STACK * 4);    // 36 walk_stacks
     L.add(256);                                         // 37 walk_counter
     L.add((p.max_cell + 2) * 32);                       // 38 level_bounds (8 octant ends per cell of the level being split)
+    L.add(p.max_cell * 8);                              // 39 cell_lr
+    L.add((p.max_cell + 1) * 32);                       // 40 leaf_P
+    L.add((scan4_tiles(p.max_cell) + 1) * 32);          // 41 leaf_toff
     return L;
 }
 
@@ -261,6 +268,12 @@ void schedule_items(std::vector<int32_t>& order, int64_t b, int64_t e, const std
         const bool take_narrow = in < nn && (iw >= nw || (span > 0 ? in * span <= iw * nn : true) || iw >= span);
         order[(size_t)k++] = take_narrow ? narrow[in++] : wide[iw++];
     }
+}
+
+// MWF_REFRESH=climb in the environment: the bottom-up climb also for monopoles (A/B switch for the scan variant)
+bool use_scan_refresh() {
+    static const bool on = [] { const char* e = std::getenv("MWF_REFRESH"); return !(e && e[0] == 'c'); }();
+    return on;
 }
 
 // Host-side work plan of one set of lists: per-group list offsets (padded to tiles), work items, the two
@@ -446,6 +459,9 @@ int mwf_create(mwf_ctx** out, const mwf_params* p, void* arena, int64_t arena_by
     c->counters = (unsigned int*)(b + L.off[17]);
     c->err = (unsigned int*)(b + L.off[18]);
     c->vel = (float4*)(b + L.off[19]);
+    c->cell_lr = (int2*)(b + L.off[39]);
+    c->leaf_P = (double4*)(b + L.off[40]);
+    c->leaf_toff = (double4*)(b + L.off[41]);
     {
         BuildBuffers& q = c->bb;
         q.store = c->store; q.vel = c->vel; q.tmp16 = c->accp;
@@ -554,6 +570,14 @@ int mwf_set_tree(mwf_ctx* c, const mwf_cell* cells, int64_t n_cell, void* stream
     CU(c, cudaMemcpyAsync(c->cells, cells, (size_t)n_cell * sizeof(mwf_cell), cudaMemcpyHostToDevice, s));
     CU(c, launch_tree_prepare(c->cells, n_cell, c->p.max_ptcl, c->parent, c->arrive, c->err, s));
     ++c->n_launch;
+    {   // a tree that failed the validation must not be ranked (its ranges may point anywhere)
+        unsigned int e0 = 0;
+        rc = read_err_word(c, s, &e0);
+        if (rc) return rc;
+        if (e0) { after_store_op(c, s); return MWF_ERANGE; }
+    }
+    CU(c, launch_leaf_ranking(c->cells, n_cell, n, c->bb.mark, c->bb.scan_scratch, c->cell_lr, &c->n_leaf_cells, s));
+    c->n_launch += 5;
     // zero-mass dummy record behind the SPJ block: what list padding points at
     const float4 zero = make_float4(0.f, 0.f, 0.f, 0.f);
     CU(c, cudaMemcpyAsync(c->store + n + n_cell, &zero, 16, cudaMemcpyHostToDevice, s));
@@ -648,9 +672,14 @@ int mwf_refresh_monopoles(mwf_ctx* c, void* stream) {
     cudaStream_t s = static_cast<cudaStream_t>(stream);
     int rc = before_store_op(c, s);
     if (rc) return rc;
-    CU(c, launch_monopoles(c->cells, c->parent, c->n_cell, c->n_ptcl, c->store, c->mom64, c->arrive,
-                           c->spj_order == 2 ? c->quad64 : nullptr, c->spj_order == 2 ? c->quad : nullptr, s));
-    ++c->n_launch;
+    if (c->spj_order == 2 || !use_scan_refresh()) {  // the quadrupoles need the bottom-up pass (parallel-axis theorem)
+        CU(c, launch_monopoles(c->cells, c->parent, c->n_cell, c->n_ptcl, c->store, c->mom64, c->arrive,
+                               c->spj_order == 2 ? c->quad64 : nullptr, c->spj_order == 2 ? c->quad : nullptr, s));
+        ++c->n_launch;
+    } else {
+        CU(c, launch_monopoles_scan(c->cells, c->cell_lr, c->n_cell, c->n_ptcl, c->n_leaf_cells, c->store, c->leaf_P, c->leaf_toff, s));
+        c->n_launch += 4;
+    }
     c->mono_fresh = true;
     return after_store_op(c, s);
 }
@@ -901,8 +930,10 @@ static int build_impl(mwf_ctx* c, int64_t n, int32_t n_leaf, int32_t n_grp, doub
     rc = read_err_word(c, s, &e);
     if (rc) return rc;
     if (e) { after_store_op(c, s); return MWF_ENOMEM; }
-    // tree state as mwf_set_tree leaves it: arrival counters zero, dummy record behind the SPJ block
+    // tree state as mwf_set_tree leaves it: arrival counters zero, leaves ranked, dummy record behind the SPJ block
     CU(c, cudaMemsetAsync(c->arrive, 0, (size_t)n_cell * 4, s));
+    CU(c, launch_leaf_ranking(c->cells, n_cell, n, c->bb.mark, c->bb.scan_scratch, c->cell_lr, &c->n_leaf_cells, s));
+    c->n_launch += 5;
     const float4 zero = make_float4(0.f, 0.f, 0.f, 0.f);
     CU(c, cudaMemcpyAsync(c->store + n + n_cell, &zero, 16, cudaMemcpyHostToDevice, s));
     c->n_ptcl = n;
