@@ -191,13 +191,16 @@ __device__ __forceinline__ void run_item(const ForceArgs& a, const WorkItem it, 
     __syncwarp();  // the next item reuses the warp's tile buffers
 }
 
+// The block has blockDim.x / 32 warps (WARPS_PER_CTA for a whole-machine dispatch, fewer for a sub-wave one, see
+// launch_force); s_tiles is dynamic shared memory, two tiles per warp.
 template <bool INDEXED>
-__device__ __forceinline__ void force_body(const ForceArgs& a, float4 (*s_tiles)[2 * TILE_J]) {
+__device__ __forceinline__ void force_body(const ForceArgs& a, float4* s_tiles) {
     const int lane = threadIdx.x & 31;
     const int warp = threadIdx.x >> 5;
-    float4* sbuf = s_tiles[warp];
-    int64_t w = (int64_t)blockIdx.x * WARPS_PER_CTA + warp;  // first item: static
-    const int64_t n_warps = (int64_t)gridDim.x * WARPS_PER_CTA;
+    const int warps_per_cta = blockDim.x >> 5;
+    float4* sbuf = s_tiles + warp * (2 * TILE_J);
+    int64_t w = (int64_t)blockIdx.x * warps_per_cta + warp;  // first item: static
+    const int64_t n_warps = (int64_t)gridDim.x * warps_per_cta;
     while (w < a.n_items) {
         const int64_t pos = a.item_begin + w;
         const WorkItem it = a.items[a.order ? a.order[pos] : pos];
@@ -218,30 +221,37 @@ __device__ __forceinline__ void force_body(const ForceArgs& a, float4 (*s_tiles)
     }
 }
 
+extern __shared__ float4 s_force_tiles[];
+
 __global__ void __launch_bounds__(WARPS_PER_CTA * 32, MWF_MIN_CTAS) k_force(const ForceArgs a) {
-    __shared__ float4 s_tiles[WARPS_PER_CTA][2 * TILE_J];
-    force_body<true>(a, s_tiles);
+    force_body<true>(a, s_force_tiles);
 }
 
 // Method G1 of the paper (multiwalk without indirect addressing, Fig. 2): same items, same sweep, but
 // every group's list is a contiguous run of j RECORDS sent with the dispatch.  A/B variant.
 __global__ void __launch_bounds__(WARPS_PER_CTA * 32, MWF_MIN_CTAS) k_force_data(const ForceArgs a) {
-    __shared__ float4 s_tiles[WARPS_PER_CTA][2 * TILE_J];
-    force_body<false>(a, s_tiles);
+    force_body<false>(a, s_force_tiles);
 }
 
-cudaError_t launch_force(const ForceArgs& a, int grid, cudaStream_t s) {
+constexpr size_t FORCE_SMEM_PER_WARP = 2 * TILE_J * sizeof(float4);
+
+// warps = warps per block: WARPS_PER_CTA for a dispatch that fills the machine (persistent grid, items claimed dynamically);
+// a sub-wave dispatch (a batch of the multiwalk pipeline) is launched with small blocks, one item per warp, so
+// that a block gives its registers back as soon as its own items are done and the batches of the other tags' streams
+// pack beside it.
+cudaError_t launch_force(const ForceArgs& a, int grid, int warps, cudaStream_t s) {
     if (a.n_items <= 0 || grid <= 0) return cudaSuccess;
+    if (warps < 1 || warps > WARPS_PER_CTA) return cudaErrorInvalidValue;
     if (a.jdata)
-        k_force_data<<<grid, WARPS_PER_CTA * 32, 0, s>>>(a);
+        k_force_data<<<grid, warps * 32, warps * FORCE_SMEM_PER_WARP, s>>>(a);
     else
-        k_force<<<grid, WARPS_PER_CTA * 32, 0, s>>>(a);
+        k_force<<<grid, warps * 32, warps * FORCE_SMEM_PER_WARP, s>>>(a);
     return cudaGetLastError();
 }
 
 int force_max_ctas_per_sm() {
     int n = 0;
-    if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&n, k_force, WARPS_PER_CTA * 32, 0) != cudaSuccess) return 0;
+    if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&n, k_force, WARPS_PER_CTA * 32, WARPS_PER_CTA * FORCE_SMEM_PER_WARP) != cudaSuccess) return 0;
     return n;
 }
 

@@ -743,14 +743,17 @@ static int dispatch_launch(mwf_ctx* c, int32_t tag, int64_t g_begin, int64_t g_e
     }
     const int64_t resident = (int64_t)c->n_sm * c->ctas_per_sm;
     const int64_t want = (a.n_items + WARPS_PER_CTA - 1) / WARPS_PER_CTA;
-    const int grid = (int)std::min(want, resident);
+    int grid = (int)resident, warps = WARPS_PER_CTA;
     a.counter = nullptr;
     if (want > resident) {  // more items than resident warps: claim the rest dynamically
         a.counter = c->counters + (c->counter_seq++ % N_COUNTER);
         CU(c, cudaMemsetAsync(a.counter, 0, sizeof(unsigned int), s));
+    } else {  // sub-wave dispatch: one item per warp, small blocks (see launch_force)
+        warps = SMALL_CTA_WARPS;
+        grid = (int)((a.n_items + warps - 1) / warps);
     }
     CU(c, cudaEventRecord(c->ev_k0[tag], s));
-    CU(c, launch_force(a, grid, s));
+    CU(c, launch_force(a, grid, warps, s));
     c->tag_quad[tag] = false;
     if (c->spj_order == 2) {  // quadrupole terms of the SPJ entries, added behind the monopole kernel
         QuadArgs q;

@@ -12,6 +12,7 @@ namespace mwf {
 
 constexpr int TILE_J = 64;          // j entries staged per warp tile; merged lists are padded to this
 constexpr int WARPS_PER_CTA = 8;    // force kernel block = 256 threads
+constexpr int SMALL_CTA_WARPS = 2;  // block of a sub-wave dispatch (one item per warp)
 constexpr int CHUNK_I = 64;         // i-particles of a full work item (2 per lane)
 constexpr int MIN_WIDTH = 2;        // narrowest item: 2 lanes x 2 i-particles, 16 j-slices
 
@@ -101,7 +102,7 @@ cudaError_t launch_sph(const SphArgs& a, bool hydro, int grid, cudaStream_t s);
 int sph_max_ctas_per_sm(bool hydro);
 
 // kernels' host launchers (defined next to their kernels)
-cudaError_t launch_force(const ForceArgs& a, int grid, cudaStream_t s);
+cudaError_t launch_force(const ForceArgs& a, int grid, int warps_per_cta, cudaStream_t s);
 int force_max_ctas_per_sm();
 
 cudaError_t launch_tree_prepare(const mwf_cell* cells, int64_t n_cell, int64_t max_ptcl, int32_t* parent, int32_t* counter,
