@@ -197,3 +197,56 @@ def test_whole_loop_on_the_device():
     mom = oracle.monopoles(cells, p2)
     acc, pot = oracle.forces(p2, mom, gf, gn, eo, ei, so, si, cfg.eps)
     check_forces(out, acc, pot, "second construction")
+
+
+def test_more_than_2_31_list_entries():
+    """Maximum sizes: a construction whose lists hold more than 2^31 entries, so every list offset past the first
+    2^31 (merged-list offsets, SPJ offsets, the walk's output cursors) needs the 64-bit path (SURVEY.md 8(a) row a2:
+    "int32 ids, int64 offsets"; the paper's per-batch `int` offsets, would wrap here).  N = 2^21 with small
+    groups and a small opening angle; the forces of sampled groups from both ends of the list are compared with the
+    oracle run on the lists read back; then the same lists go through the host path of a second context."""
+    cfg = CONFIGS[1]
+    n, n_leaf, n_grp, theta = 1 << 21, 8, 32, 0.27
+    posm, _ = make_particles(cfg, n)
+    f = binding.MultiWalkForce(cfg.eps, 1.0, max_ptcl=n, max_cell=n, max_group=n // 2, max_entry=3_500_000_000, n_tag=2)
+    f.begin_step(binding.MAKE_LIST_FOR_REUSE)
+    f.set_particles(posm)
+    f.build(n, n_leaf, n_grp, theta, binding.MAKE_LIST_FOR_REUSE)
+    sz = f.get_build_sizes()
+    assert sz["n_spj"] > 2 ** 31 and sz["n_epj"] + sz["n_spj"] < 3_500_000_000, sz
+    ng = sz["n_group"]
+    f.refresh_monopoles()
+    f.dispatch(0, 0, ng)
+    out = np.zeros((n, 4), np.float32)
+    f.retrieve(0, out)
+    cells, _ = f.get_tree(sz["n_cell"], with_geom=False)
+    grp_first, grp_n = f.get_groups(ng)
+    epj_off, epj_id, spj_off, spj_id = f.get_lists(ng, sz["n_epj"], sz["n_spj"])
+    tree_posm = f.get_particles(0, n)
+    f.close()
+    assert epj_off[-1] == sz["n_epj"] and spj_off[-1] == sz["n_spj"]
+    assert np.all(np.diff(epj_off) >= 0) and np.all(np.diff(spj_off) > 0)
+    first_past = int(np.searchsorted(spj_off, 2 ** 31))           # first group whose SPJ list starts past 2^31
+    assert 0 < first_past < ng
+    rng = np.random.default_rng(11)
+    sample = np.unique(np.concatenate([rng.choice(first_past, 60, replace=False), [first_past - 1, first_past, ng - 1],
+                                       first_past + rng.choice(ng - first_past, 120, replace=False)])).astype(np.int64)
+    mom = oracle.monopoles(cells, tree_posm)
+    acc, pot = oracle.forces(tree_posm, mom, grp_first, grp_n, epj_off, epj_id, spj_off, spj_id, cfg.eps, 1.0, sample)
+    mask = np.zeros(n, bool)
+    for g in sample:
+        mask[grp_first[g]:grp_first[g] + grp_n[g]] = True
+    check_forces(out[mask], acc[mask], pot[mask], "E = %.2e entries, %d sampled groups" % (sz["n_epj"] + sz["n_spj"], len(sample)))
+    # the same lists through the host path (mwf_set_tree / mwf_set_lists: validation and merge kernels with 64-bit offsets)
+    f2 = binding.MultiWalkForce(cfg.eps, 1.0, max_ptcl=n, max_cell=sz["n_cell"], max_group=ng, max_entry=sz["n_epj"] + sz["n_spj"], n_tag=2)
+    f2.begin_step(binding.MAKE_LIST_FOR_REUSE)
+    f2.set_particles(tree_posm)
+    f2.set_tree(cells)
+    f2.set_lists(grp_first, grp_n, epj_off, epj_id, spj_off, spj_id, binding.MAKE_LIST_FOR_REUSE)
+    f2.refresh_monopoles()
+    f2.dispatch(0, 0, ng)
+    out2 = np.zeros((n, 4), np.float32)
+    f2.retrieve(0, out2)
+    f2.close()
+    check_forces(out2[mask], acc[mask], pot[mask], "host path, same lists")
+    assert np.array_equal(out2, out)                          # same lists in the same order: bitwise the same sums
