@@ -130,6 +130,8 @@ def run_reference(args, cfg, w, rank, world):
     if rank != 0:
         return
     import oracle
+    if world > 1:  # torchrun exports OMP_NUM_THREADS=1 to every rank; rank 0 alone works here, on all the host cores
+        oracle.set_num_threads(len(os.sched_getaffinity(0)))
     per_step_s = max(2.0, min(20.0, 150.0 / max(1, args.steps + args.warmup)))
     inter_tot, t_tot, groups = 0, 0.0, 0
     for s in range(args.warmup + args.steps):
