@@ -17,6 +17,7 @@ using namespace mwf;
 struct mwf_ctx {
     mwf_params p{};
     int n_sm = 0, ctas_per_sm = 0;
+    int64_t l2_bytes = 0;
     char* arena = nullptr;
     int64_t arena_bytes = 0;
     bool own_arena = false;
@@ -337,7 +338,26 @@ int make_plan(mwf_ctx* c, int64_t n_group, const int32_t* grp_first, const int32
     // ranges that mwf_calc_force_all uses for a host destination are made on first use (ensure_split_order)
     pl.order_full.resize((size_t)n_items);
     std::iota(pl.order_full.begin(), pl.order_full.end(), 0);
-    schedule_items(pl.order_full, 0, n_items, items, cost);
+    // A store that does not fit the L2 is walked in SCHED_WINDOWS windows of consecutive (Morton-ordered) items of equal
+    // modelled cost, each scheduled as above: the gathers of the items in flight then touch one stretch of the store at a
+    // time (config 4, 171 MB store: DRAM traffic 6.7 -> 3.1 GB per launch at the same kernel time; a store that fits loses
+    // 0.3-0.7 % to the less even mix of long and short items, so it keeps one window).
+    const int64_t store_bytes = (c->n_ptcl + c->n_cell + 1) * (int64_t)sizeof(float4);
+    const int n_win = store_bytes > c->l2_bytes ? SCHED_WINDOWS : 1;
+    if (n_win <= 1) {
+        schedule_items(pl.order_full, 0, n_items, items, cost);
+    } else {
+        int64_t tot = 0;
+        for (int64_t k = 0; k < n_items; ++k) tot += cost[(size_t)k];
+        int64_t b = 0, acc = 0;
+        for (int w = 1; w <= n_win && b < n_items; ++w) {
+            const int64_t want = tot / n_win * w;
+            int64_t e = b;
+            while (e < n_items && (acc < want || w == n_win)) acc += cost[(size_t)e++];
+            schedule_items(pl.order_full, b, e, items, cost);
+            b = e;
+        }
+    }
     pl.split.assign((size_t)c->p.n_tag + 1, 0);
     const int64_t total = pl.inter[(size_t)n_group];
     int64_t g = 0;
@@ -425,6 +445,7 @@ int mwf_create(mwf_ctx** out, const mwf_params* p, void* arena, int64_t arena_by
         return MWF_ECUDA;
     }
     c->n_sm = prop.multiProcessorCount;
+    c->l2_bytes = prop.l2CacheSize;
     c->ctas_per_sm = force_max_ctas_per_sm();
     if (c->ctas_per_sm < 1) { delete c; return MWF_ECUDA; }
     const Layout L = make_layout(*p);

@@ -13,6 +13,7 @@ namespace mwf {
 constexpr int TILE_J = 64;          // j entries staged per warp tile; merged lists are padded to this
 constexpr int WARPS_PER_CTA = 8;    // force kernel block = 256 threads
 constexpr int SMALL_CTA_WARPS = 2;  // block of a sub-wave dispatch (one item per warp)
+constexpr int SCHED_WINDOWS = 16;    // Morton windows of the work schedule when the store exceeds the L2
 constexpr int CHUNK_I = 64;         // i-particles of a full work item (2 per lane)
 constexpr int MIN_WIDTH = 2;        // narrowest item: 2 lanes x 2 i-particles, 16 j-slices
 
