@@ -222,6 +222,25 @@ int mwf_retrieve(mwf_ctx* c, int32_t tag, mwf_accp* dst, int dst_on_device);
  * the store), refresh, dispatch all groups split over the tags, retrieve everything into dst. */
 int mwf_calc_force_all(mwf_ctx* c, const mwf_posm* src, int src_on_device, mwf_accp* dst, int dst_on_device);
 
+/* ---- Pipelined host loop ("all of these can be overlapped", P:189 dispatch / retrieve split): the particles of the
+ * NEXT step are written into a second (shadow) store while the force kernels of the current step still read the current
+ * one, so that a host that integrates tag by tag hides the H2D copy of eq. 18's first term under the kernels:
+ *     for every tag t in dispatch order:  mwf_retrieve(t, dst)            results of step k of that tag's particles (D2H)
+ *                                         (the host integrates them)
+ *                                         mwf_set_particles_next(...)     their positions of step k+1 (H2D, own stream)
+ *     mwf_swap_store(); mwf_refresh_monopoles(); mwf_dispatch(t, ...) for every tag      step k+1
+ * mwf_set_particles_next: like mwf_set_particles, into the shadow store; asynchronous on `stream`, waits for nothing
+ *   (no kernel reads the shadow store); needs a tree (MWF_ESTATE), [first, first + n) inside [0, N) (MWF_ERANGE).
+ * mwf_swap_store: the shadow store becomes the store.  MWF_ESTATE unless the calls since the last swap wrote N particles
+ *   in total (the caller covers [0, N) exactly once) and no tag is in flight (every dispatched tag retrieved).  Everything
+ *   enqueued later on any stream through this library is ordered behind the shadow uploads.  The monopoles become
+ *   stale (mwf_refresh_monopoles must follow); velocities, results, tree and lists are not touched.
+ * mwf_get_tag_split: bounds[0 .. n_tag] = the group ranges [bounds[t], bounds[t+1]) of equal interaction count that
+ *   mwf_calc_force_all dispatches per tag (MWF_ESTATE without lists). */
+int mwf_set_particles_next(mwf_ctx* c, const mwf_posm* src, int64_t first, int64_t n, int src_on_device, void* stream);
+int mwf_swap_store(mwf_ctx* c, void* stream);
+int mwf_get_tag_split(mwf_ctx* c, int64_t* bounds);
+
 /* ---- Device-side construction step (paper P:149-172: root cell, Morton keys,
  * radix sort, reorder, cells linked level by level, one tree walk per i-group emitting an index list).  Works on
  * the particles [0, n) currently in the store, in ANY order: sorts them (and the velocities, when all n have been

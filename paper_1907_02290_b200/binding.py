@@ -27,6 +27,7 @@ SYMBOLS = (
     "mwf_reserve_data_lists", "mwf_dispatch_data", "mwf_set_spj_order", "mwf_get_quadrupoles", "mwf_last_quad_ms",
     "mwf_set_sph", "mwf_get_sph", "mwf_dispatch_density", "mwf_dispatch_hydro", "mwf_calc_sph_all",
     "mwf_build", "mwf_build_neighbours", "mwf_get_build_sizes", "mwf_get_permutation", "mwf_get_tree", "mwf_get_groups", "mwf_get_lists",
+    "mwf_set_particles_next", "mwf_swap_store", "mwf_get_tag_split",
 )
 
 
@@ -63,6 +64,9 @@ def load_library(path: str | None = None) -> ctypes.CDLL:
         "mwf_set_tag_stream": [vp, i32, vp],
         "mwf_set_particles": [vp, vp, i64, i64, ci, vp],
         "mwf_get_particles": [vp, vp, i64, i64, ci],
+        "mwf_set_particles_next": [vp, vp, i64, i64, ci, vp],
+        "mwf_swap_store": [vp, vp],
+        "mwf_get_tag_split": [vp, P(i64)],
         "mwf_set_tree": [vp, vp, i64, vp],
         "mwf_set_lists": [vp, i64, vp, vp, vp, vp, vp, vp, ci, vp],
         "mwf_begin_step": [vp, ci],
@@ -155,7 +159,11 @@ class MultiWalkForce:
             base = (self._arena.data_ptr() + 255) // 256 * 256
             self._h = ctypes.c_void_p(None)
             self._ck(self._lib.mwf_create(ctypes.byref(self._h), ctypes.byref(self.params), ctypes.c_void_p(base), self.arena_bytes), ctx=False)
-            self.streams = [torch.cuda.Stream(device=self.device) for _ in range(n_tag)]
+            # priorities fall with the tag (the library does the same for its own streams): tags dispatched together
+            # finish roughly in tag order, so a tag's retrieve overlaps the kernels of the tags behind it
+            least, greatest = torch.cuda.Stream.priority_range()
+            levels = least - greatest + 1
+            self.streams = [torch.cuda.Stream(device=self.device, priority=greatest + t * levels // n_tag) for t in range(n_tag)]
         for t, s in enumerate(self.streams):
             self._ck(self._lib.mwf_set_tag_stream(self._h, t, ctypes.c_void_p(int(s.cuda_stream))))
         self.n_tag = n_tag
@@ -193,6 +201,21 @@ class MultiWalkForce:
         if n is None:
             n = int(src.shape[0])
         self._ck(self._lib.mwf_set_particles(self._h, p, int(first), int(n), on_dev, _stream_handle(stream)))
+
+    def set_particles_next(self, src, first: int = 0, n: int | None = None, stream=None):
+        """Particles [first, first + n) of the NEXT step into the shadow store (pipelined host loop)."""
+        p, on_dev = _ptr(src, np.float32, "src")
+        if n is None:
+            n = int(src.shape[0])
+        self._ck(self._lib.mwf_set_particles_next(self._h, p, int(first), int(n), on_dev, _stream_handle(stream)))
+
+    def swap_store(self, stream=None):
+        self._ck(self._lib.mwf_swap_store(self._h, _stream_handle(stream)))
+
+    def get_tag_split(self) -> np.ndarray:
+        out = np.zeros(self.n_tag + 1, np.int64)
+        self._ck(self._lib.mwf_get_tag_split(self._h, out.ctypes.data_as(ctypes.POINTER(ctypes.c_int64))))
+        return out
 
     def get_particles(self, first: int, n: int) -> np.ndarray:
         out = np.empty((n, 4), np.float32)

@@ -23,6 +23,9 @@ struct mwf_ctx {
     bool own_arena = false;
     // carved device arrays
     float4* store = nullptr;      // [max_ptcl + max_cell + 1]
+    float4* store_next = nullptr; // same size: the shadow store of the pipelined host loop (mwf_set_particles_next / mwf_swap_store)
+    int64_t next_count = 0;       // particles written into the shadow store since the last swap
+    std::vector<cudaStream_t> next_streams;  // streams those uploads went to
     float4* accp = nullptr;       // [max_ptcl]
     float4* vel = nullptr;        // [max_ptcl] (vx, vy, vz, unused): device-resident integration
     mwf_cell* cells = nullptr;    // [max_cell]
@@ -69,6 +72,7 @@ struct mwf_ctx {
     cudaEvent_t ev_tag[MWF_MAX_TAG]{}, ev_k0[MWF_MAX_TAG]{}, ev_k1[MWF_MAX_TAG]{};
     bool tag_timed[MWF_MAX_TAG]{};
     cudaEvent_t ev_store{};
+    cudaEvent_t ev_next{};
     bool store_event_valid = false;
     std::vector<std::pair<int64_t, int64_t>> tag_ranges[MWF_MAX_TAG];  // particle ranges awaiting retrieve
     std::vector<int64_t> tag_groups;                                   // groups awaiting retrieve per tag
@@ -189,6 +193,7 @@ Layout make_layout(const mwf_params& p) {
     L.add(p.max_cell * 8);                              // 39 cell_lr
     L.add((p.max_cell + 1) * 32);                       // 40 leaf_P
     L.add((scan4_tiles(p.max_cell) + 1) * 32);          // 41 leaf_toff
+    L.add((p.max_ptcl + p.max_cell + 1) * 16);          // 42 store_next
     return L;
 }
 
@@ -461,6 +466,7 @@ int mwf_create(mwf_ctx** out, const mwf_params* p, void* arena, int64_t arena_by
     c->arena_bytes = L.total;
     char* b = c->arena;
     c->store = (float4*)(b + L.off[0]);
+    c->store_next = (float4*)(b + L.off[42]);
     c->accp = (float4*)(b + L.off[1]);
     c->cells = (mwf_cell*)(b + L.off[2]);
     c->parent = (int32_t*)(b + L.off[3]);
@@ -503,8 +509,14 @@ int mwf_create(mwf_ctx** out, const mwf_params* p, void* arena, int64_t arena_by
     c->max_items = max_items_of(*p);
     c->tag_groups.assign(MWF_MAX_TAG, 0);
     bool ok = true;
+    // Tag t's stream gets a priority that falls with t (the device has few levels: tags share them in order), so that the
+    // kernels of tags dispatched together finish roughly in tag order instead of all at the end: the retrieve of tag t (and,
+    // in the pipelined loop, the upload of its next particles) then overlaps the kernels of the tags behind it.
+    int prio_least = 0, prio_greatest = 0;
+    ok = ok && cudaDeviceGetStreamPriorityRange(&prio_least, &prio_greatest) == cudaSuccess;
+    const int prio_levels = prio_least - prio_greatest + 1;
     for (int t = 0; t < p->n_tag && ok; ++t) {
-        ok = ok && cudaStreamCreateWithFlags(&c->tag_stream[t], cudaStreamNonBlocking) == cudaSuccess;
+        ok = ok && cudaStreamCreateWithPriority(&c->tag_stream[t], cudaStreamNonBlocking, prio_greatest + t * prio_levels / p->n_tag) == cudaSuccess;
         c->tag_own[t] = ok;
         ok = ok && cudaEventCreateWithFlags(&c->ev_tag[t], cudaEventDisableTiming) == cudaSuccess;
         ok = ok && cudaEventCreate(&c->ev_k0[t]) == cudaSuccess;
@@ -512,6 +524,7 @@ int mwf_create(mwf_ctx** out, const mwf_params* p, void* arena, int64_t arena_by
         ok = ok && cudaEventCreate(&c->ev_kq[t]) == cudaSuccess;
     }
     ok = ok && cudaEventCreateWithFlags(&c->ev_store, cudaEventDisableTiming) == cudaSuccess;
+    ok = ok && cudaEventCreateWithFlags(&c->ev_next, cudaEventDisableTiming) == cudaSuccess;
     ok = ok && cudaMemset(c->counters, 0, N_COUNTER * 4) == cudaSuccess;
     ok = ok && cudaMemset(c->err, 0, 256) == cudaSuccess;
     if (!ok) { mwf_destroy(c); return MWF_ECUDA; }
@@ -533,6 +546,7 @@ int mwf_destroy(mwf_ctx* c) {
     if (c->quad64) cudaFree(c->quad64);
     if (c->quad) cudaFree(c->quad);
     if (c->ev_store) cudaEventDestroy(c->ev_store);
+    if (c->ev_next) cudaEventDestroy(c->ev_next);
     for (int t = 0; t < MWF_MAX_TAG; ++t) {
         if (c->data_buf[t]) cudaFree(c->data_buf[t]);
         if (c->data_off[t]) cudaFree(c->data_off[t]);
@@ -565,6 +579,49 @@ int mwf_set_particles(mwf_ctx* c, const mwf_posm* src, int64_t first, int64_t n,
     c->mono_fresh = false;
     c->acc_full = false;
     return after_store_op(c, s);
+}
+
+int mwf_set_particles_next(mwf_ctx* c, const mwf_posm* src, int64_t first, int64_t n, int src_on_device, void* stream) {
+    if (!c || !src || first < 0 || n < 0) return MWF_EINVAL;
+    if (!c->have_tree) return MWF_ESTATE;
+    if (first + n > c->n_ptcl) return MWF_ERANGE;
+    if (n == 0) return MWF_OK;
+    cudaStream_t s = static_cast<cudaStream_t>(stream);
+    // no kernel reads the shadow store: its last readers were retrieved before the swap that made it the shadow
+    CU(c, cudaMemcpyAsync(c->store_next + first, src, (size_t)n * 16, src_on_device ? cudaMemcpyDeviceToDevice : cudaMemcpyHostToDevice, s));
+    c->next_count += n;
+    if (std::find(c->next_streams.begin(), c->next_streams.end(), s) == c->next_streams.end()) c->next_streams.push_back(s);
+    return MWF_OK;
+}
+
+int mwf_swap_store(mwf_ctx* c, void* stream) {
+    if (!c) return MWF_EINVAL;
+    if (!c->have_tree || c->next_count != c->n_ptcl) return MWF_ESTATE;
+    for (int t = 0; t < c->p.n_tag; ++t)
+        if (c->tag_inflight[t] || !c->tag_ranges[t].empty()) return MWF_ESTATE;
+    cudaStream_t s = static_cast<cudaStream_t>(stream);
+    int rc = before_store_op(c, s);  // behind whatever still writes or reads the current store
+    if (rc) return rc;
+    for (cudaStream_t u : c->next_streams) {
+        if (u == s) continue;
+        CU(c, cudaEventRecord(c->ev_next, u));
+        CU(c, cudaStreamWaitEvent(s, c->ev_next, 0));
+    }
+    std::swap(c->store, c->store_next);
+    c->bb.store = c->store;
+    c->next_count = 0;
+    c->next_streams.clear();
+    c->ptcl_hi = c->n_ptcl;
+    c->mono_fresh = false;
+    c->acc_full = false;
+    return after_store_op(c, s);  // every later dispatch / store operation waits for this event, hence for the uploads
+}
+
+int mwf_get_tag_split(mwf_ctx* c, int64_t* bounds) {
+    if (!c || !bounds) return MWF_EINVAL;
+    if (!c->have_lists) return MWF_ESTATE;
+    for (int t = 0; t <= c->p.n_tag; ++t) bounds[t] = c->h_split[(size_t)t];
+    return MWF_OK;
 }
 
 int mwf_get_particles(mwf_ctx* c, mwf_posm* dst, int64_t first, int64_t n, int dst_on_device) {
@@ -602,6 +659,9 @@ int mwf_set_tree(mwf_ctx* c, const mwf_cell* cells, int64_t n_cell, void* stream
     // zero-mass dummy record behind the SPJ block: what list padding points at
     const float4 zero = make_float4(0.f, 0.f, 0.f, 0.f);
     CU(c, cudaMemcpyAsync(c->store + n + n_cell, &zero, 16, cudaMemcpyHostToDevice, s));
+    CU(c, cudaMemcpyAsync(c->store_next + n + n_cell, &zero, 16, cudaMemcpyHostToDevice, s));
+    c->next_count = 0;
+    c->next_streams.clear();
     unsigned int e = 0;
     rc = read_err_word(c, s, &e);
     if (rc) return rc;
@@ -960,6 +1020,9 @@ static int build_impl(mwf_ctx* c, int64_t n, int32_t n_leaf, int32_t n_grp, doub
     c->n_launch += 5;
     const float4 zero = make_float4(0.f, 0.f, 0.f, 0.f);
     CU(c, cudaMemcpyAsync(c->store + n + n_cell, &zero, 16, cudaMemcpyHostToDevice, s));
+    CU(c, cudaMemcpyAsync(c->store_next + n + n_cell, &zero, 16, cudaMemcpyHostToDevice, s));
+    c->next_count = 0;
+    c->next_streams.clear();
     c->n_ptcl = n;
     c->n_cell = n_cell;
     c->ptcl_hi = n;

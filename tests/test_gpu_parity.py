@@ -215,6 +215,75 @@ def test_calc_force_all_host_and_device_destinations():
     f.close()
 
 
+def test_pipelined_host_loop_equals_the_blocking_one():
+    """mwf_set_particles_next / mwf_swap_store: the next step's particles go into the shadow store tag
+    by tag, right behind the retrieve of that tag's results and while the other tags' kernels still read the current
+    store.  Every step must give bitwise the results of the blocking mwf_calc_force_all on the same particles, and the
+    oracle's on the last step."""
+    import torch
+    cfg = CONFIGS[4]
+    w = make_workload(cfg, 60000)
+    rng = np.random.default_rng(3)
+    steps = [w.posm.copy()]
+    for _ in range(3):                                           # moved particles, lists reused (tree order unchanged)
+        q = steps[-1].copy()
+        q[:, :3] += (1e-3 * rng.standard_normal((w.n, 3))).astype(np.float32)
+        steps.append(q)
+    n_tag = 4
+    ref = []
+    f = binding.MultiWalkForce.for_workload(w, n_tag=n_tag)
+    f.upload_workload(w, binding.MAKE_LIST_FOR_REUSE)
+    src, dst = f.pinned(w.n), f.pinned(w.n)
+    for q in steps:
+        src.numpy()[:] = q
+        f.begin_step(binding.REUSE_LIST)
+        f.calc_force_all(src, dst)
+        ref.append(dst.numpy().copy())
+    f.close()
+
+    f = binding.MultiWalkForce.for_workload(w, n_tag=n_tag)
+    f.upload_workload(w, binding.MAKE_LIST_FOR_REUSE)
+    split = f.get_tag_split()
+    assert split[0] == 0 and split[-1] == w.n_group and np.all(np.diff(split) >= 0)
+    first = [int(w.grp_first[split[t]]) if split[t] < w.n_group else w.n for t in range(n_tag)] + [w.n]
+    up = torch.cuda.Stream()
+    host_in = [f.pinned(w.n) for _ in steps]
+    for h, q in zip(host_in, steps):
+        h.numpy()[:] = q
+    out = f.pinned(w.n)
+
+    def dispatch_all():
+        f.refresh_monopoles()
+        for t in range(n_tag):
+            if split[t + 1] > split[t]:
+                f.dispatch(t, int(split[t]), int(split[t + 1]))
+
+    assert expect_code(f.swap_store) == binding.ESTATE            # nothing in the shadow store yet
+    assert expect_code(f.set_particles_next, host_in[0], w.n - 1, 2, up) == binding.ERANGE
+    dispatch_all()                                               # step 0 on the uploaded particles
+    for k in range(len(steps)):
+        nxt = host_in[(k + 1) % len(steps)]
+        for t in range(n_tag):
+            if split[t + 1] == split[t]:
+                continue
+            f.retrieve(t, out)                                   # results of step k for this tag's particles
+            if t == 0:
+                assert expect_code(f.swap_store) == binding.ESTATE   # not all N written, tags in flight
+            f.set_particles_next(nxt[first[t]:first[t + 1]], first[t], first[t + 1] - first[t], up)
+        assert np.array_equal(out.numpy(), ref[k]), "step %d" % k
+        f.swap_store()
+        assert expect_code(f.dispatch, 0, 0, 1) == binding.ESTATE   # monopoles stale after the swap
+        dispatch_all()
+    for t in range(n_tag):                                       # the loop wrapped around: step 0 again
+        if split[t + 1] > split[t]:
+            f.retrieve(t, out)
+    assert np.array_equal(out.numpy(), ref[0])
+    assert np.array_equal(f.get_particles(0, w.n), steps[0])
+    f.close()
+    acc, pot, _ = oracle_eval(w, cfg.eps, posm=steps[-1])
+    check(ref[-1], acc, pot, label="pipelined loop, last step")
+
+
 # ------------------------------------------------------------------ edge cases of the kernel mapping
 def synthetic_groups(n, sizes):
     """Consecutive groups of the given sizes over n particles with EVERY particle in every list
