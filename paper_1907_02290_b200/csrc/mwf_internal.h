@@ -33,7 +33,7 @@ struct WorkItem {
 #define MWF_COST_STAGE 40
 #endif
 #ifndef MWF_UNROLL_WIDE
-#define MWF_UNROLL_WIDE 16
+#define MWF_UNROLL_WIDE 32
 #endif
 #ifndef MWF_FLUSH_MIN
 #define MWF_FLUSH_MIN 2
