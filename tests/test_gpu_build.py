@@ -250,3 +250,35 @@ def test_more_than_2_31_list_entries():
     f2.close()
     check_forces(out2[mask], acc[mask], pot[mask], "host path, same lists")
     assert np.array_equal(out2, out)                          # same lists in the same order: bitwise the same sums
+
+
+def test_shadow_store_after_a_device_build():
+    """mwf_set_particles_next / mwf_swap_store on a tree and lists built on the device: the evaluation on the swapped-in
+    particles is bitwise the one mwf_set_particles gives, and the dummy record the padded list entries point at exists
+    in both stores (no NaN from the padding)."""
+    cfg = CONFIGS[4]
+    posm, _ = make_particles(cfg, 30000)
+    got, f = device_build(posm, cfg.n_leaf, cfg.n_grp, cfg.theta, eps=cfg.eps, keep=True)
+    n, ng = posm.shape[0], got["sizes"]["n_group"]
+    moved = got["posm"].copy()
+    moved[:, :3] += np.float32(1e-3) * np.random.default_rng(5).standard_normal((n, 3)).astype(np.float32)
+    out_a, out_b = np.zeros((n, 4), np.float32), np.zeros((n, 4), np.float32)
+    f.begin_step(binding.REUSE_LIST)
+    f.set_particles(moved)
+    f.refresh_monopoles()
+    f.dispatch(0, 0, ng)
+    f.retrieve(0, out_a)
+    f.set_particles(got["posm"])                                # back to the built positions in the current store
+    half = n // 2
+    f.set_particles_next(moved[:half], 0, half)
+    with pytest.raises(binding.MwfError) as e:
+        f.swap_store()
+    assert e.value.code == binding.ESTATE                       # only half of the particles written
+    f.set_particles_next(moved[half:], half, n - half)
+    f.swap_store()
+    assert np.array_equal(f.get_particles(0, n), moved)
+    f.refresh_monopoles()
+    f.dispatch(0, 0, ng)
+    f.retrieve(0, out_b)
+    f.close()
+    assert np.all(np.isfinite(out_b)) and np.array_equal(out_a, out_b)
