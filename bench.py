@@ -45,52 +45,105 @@ def log(*a):
 
 # ----------------------------------------------------------------------------- clocks
 class ClockSampler:
-    """nvidia-smi sampled every 200 ms during the timed region (B200_PROFILING.md clocks line)."""
+    """SM clock, power and throttle reasons sampled IN PROCESS through NVML every ~4 ms by a thread (>= 10 Hz
+    during the timed region).  mark_begin() / mark_end() bracket the timed region; summary() describes only the samples
+    taken between the two marks.  Falls back to `nvidia-smi -lms` when NVML cannot be loaded."""
     Q = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,clocks_event_reasons.hw_thermal_slowdown,"
          "clocks_event_reasons.sw_thermal_slowdown,clocks_event_reasons.sw_power_cap")
 
-    def __init__(self, index: int):
-        self.rows, self.proc, self.index = [], None, index
+    def __init__(self, index: int, period_s: float = 0.004):
+        self.rows, self.proc, self.index, self.period = [], None, index, period_s
+        self.t_begin, self.t_end, self.stop, self.thread, self.nvml, self.source = None, None, False, None, None, "none"
+
+    def _nvml_handle(self):
+        import pynvml
+        pynvml.nvmlInit()
+        try:
+            import torch
+            uuid = str(torch.cuda.get_device_properties(self.index).uuid)
+            return pynvml, pynvml.nvmlDeviceGetHandleByUUID(("GPU-" + uuid).encode())
+        except Exception:
+            vis = os.environ.get("CUDA_VISIBLE_DEVICES", "")
+            ids = [x for x in vis.split(",") if x.strip().isdigit()]
+            phys = int(ids[self.index]) if self.index < len(ids) else self.index
+            return pynvml, pynvml.nvmlDeviceGetHandleByIndex(phys)
 
     def __enter__(self):
         try:
-            self.proc = subprocess.Popen(["nvidia-smi", "-i", str(self.index), "--query-gpu=" + self.Q, "--format=csv,noheader,nounits", "-lms", "200"],
+            self.nvml, self.handle = self._nvml_handle()
+            self.max_mhz = float(self.nvml.nvmlDeviceGetMaxClockInfo(self.handle, self.nvml.NVML_CLOCK_SM))
+            self.source = "nvml in-process thread, %.0f ms period" % (1e3 * self.period)
+            self.thread = threading.Thread(target=self._poll_nvml, daemon=True)
+            self.thread.start()
+            return self
+        except Exception:
+            self.nvml = None
+        try:
+            self.proc = subprocess.Popen(["nvidia-smi", "-i", str(self.index), "--query-gpu=" + self.Q, "--format=csv,noheader,nounits", "-lms", "20"],
                                          stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
-            self.thread = threading.Thread(target=self._read, daemon=True)
+            self.source = "nvidia-smi -lms 20"
+            self.thread = threading.Thread(target=self._read_smi, daemon=True)
             self.thread.start()
         except OSError:
             self.proc = None
         return self
 
-    def _read(self):
+    def _poll_nvml(self):
+        n = self.nvml
+        bits = {"hw_slowdown": getattr(n, "nvmlClocksEventReasonHwSlowdown", 0x8), "hw_thermal_slowdown": getattr(n, "nvmlClocksEventReasonHwThermalSlowdown", 0x40),
+                "sw_thermal_slowdown": getattr(n, "nvmlClocksEventReasonSwThermalSlowdown", 0x20), "sw_power_cap": getattr(n, "nvmlClocksEventReasonSwPowerCap", 0x4)}
+        reasons_fn = getattr(n, "nvmlDeviceGetCurrentClocksEventReasons", None) or n.nvmlDeviceGetCurrentClocksThrottleReasons
+        while not self.stop:
+            try:
+                t = time.perf_counter()
+                sm = float(n.nvmlDeviceGetClockInfo(self.handle, n.NVML_CLOCK_SM))
+                pw = n.nvmlDeviceGetPowerUsage(self.handle) / 1e3
+                mask = int(reasons_fn(self.handle))
+                self.rows.append((t, sm, self.max_mhz, pw, [k for k, b in bits.items() if mask & b]))
+            except Exception:
+                pass
+            time.sleep(self.period)
+
+    def _read_smi(self):
         for line in self.proc.stdout:
             parts = [x.strip() for x in line.split(",")]
             if len(parts) >= 7:
-                self.rows.append(parts)
+                try:
+                    names = ("hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap")
+                    self.rows.append((time.perf_counter(), float(parts[0]), float(parts[1]), float(parts[2]),
+                                      [k for k, v in zip(names, parts[3:7]) if v.lower().startswith("active")]))
+                except ValueError:
+                    continue
+
+    def mark_begin(self):
+        self.t_begin = time.perf_counter()
+
+    def mark_end(self):
+        self.t_end = time.perf_counter()
 
     def __exit__(self, *exc):
+        self.stop = True
         if self.proc:
             self.proc.terminate()
             try:
                 self.proc.wait(timeout=5)
             except subprocess.TimeoutExpired:
                 self.proc.kill()
+        if self.thread is not None:
+            self.thread.join(timeout=2)
 
     def summary(self):
-        sm, mx, pw, reasons = [], [], [], set()
-        for r in self.rows:
-            try:
-                sm.append(float(r[0])); mx.append(float(r[1])); pw.append(float(r[2]))
-            except ValueError:
-                continue
-            for name, v in zip(("hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"), r[3:7]):
-                if v.lower().startswith("active"):
-                    reasons.add(name)
-        if not sm:
-            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": [], "samples": 0}
-        busy = [s for s, p in zip(sm, pw) if p >= 0.5 * max(pw)] or sm
-        return {"sm_mhz": float(np.median(busy)), "sm_max_mhz": float(max(mx)), "reasons": sorted(reasons),
-                "samples": len(sm), "power_w_max": float(max(pw))}
+        t0 = self.t_begin if self.t_begin is not None else -1e300
+        t1 = self.t_end if self.t_end is not None else 1e300
+        inside = [r for r in self.rows if t0 <= r[0] <= t1]
+        rows = inside or self.rows
+        if not rows:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": [], "samples": 0, "source": self.source}
+        sm = [r[1] for r in rows]
+        reasons = sorted({k for r in rows for k in r[4]})
+        return {"sm_mhz": float(np.median(sm)), "sm_min_mhz": float(min(sm)), "sm_max_mhz": float(max(r[2] for r in rows)), "reasons": reasons,
+                "samples": len(inside), "samples_outside_region": len(self.rows) - len(inside), "power_w_max": float(max(r[3] for r in rows)),
+                "region_s": None if self.t_begin is None or self.t_end is None else round(self.t_end - self.t_begin, 4), "source": self.source}
 
 
 def measured_peaks():
@@ -101,7 +154,7 @@ def measured_peaks():
 
 
 # ----------------------------------------------------------------------------- oracle legs
-def oracle_sample(w, cfg, target_s: float, seed: int = 12345):
+def oracle_sample(w, cfg, target_s: float, seed: int = 12345, want_result: bool = False):
     """Times the fp64 oracle (monopoles excluded: forces only, like the GPU kernel figure) on a seeded
     sample of groups sized for about `target_s` seconds.  Returns (interactions, seconds, n_groups)."""
     import oracle
@@ -122,9 +175,27 @@ def oracle_sample(w, cfg, target_s: float, seed: int = 12345):
     k = max(k0, min(k, w.n_group))
     sel = order[:k]
     t = time.perf_counter()
-    oracle.forces(*args, groups=sel)
+    acc, pot = oracle.forces(*args, groups=sel)
     dt = time.perf_counter() - t
+    if want_result:
+        return int(per_group[sel].sum()), dt, k, (sel, acc, pot)
     return int(per_group[sel].sum()), dt, k
+
+
+def parity_of(w, out, sel, acc, pot):
+    """GPU result `out` [N,4] against the oracle's (acc, pot) on every particle of the groups `sel` (the north_star's
+    norms: per-particle relative acceleration error, relative potential error)."""
+    mask = np.zeros(w.n, bool)
+    for g in sel:
+        mask[w.grp_first[g]:w.grp_first[g] + w.grp_n[g]] = True
+    a, p = out[mask, :3].astype(np.float64), out[mask, 3].astype(np.float64)
+    ea = np.linalg.norm(a - acc[mask], axis=1) / np.linalg.norm(acc[mask], axis=1)
+    ep = np.abs(p - pot[mask]) / np.abs(pot[mask])
+    res = {"acc_max": float(ea.max()), "acc_rms": float(np.sqrt(np.mean(ea ** 2))), "pot_max": float(ep.max()), "pot_rms": float(np.sqrt(np.mean(ep ** 2))),
+           "particles": int(mask.sum()), "of": int(w.n), "groups": int(len(sel)), "of_groups": int(w.n_group),
+           "tolerance": {"acc_max": 1e-4, "acc_rms": 2e-5, "pot_rms": 1e-5}}
+    res["ok"] = bool(res["acc_max"] <= 1e-4 and res["acc_rms"] <= 2e-5 and res["pot_rms"] <= 1e-5)
+    return res
 
 
 def run_reference(args, cfg, w, rank, world):
@@ -573,20 +644,21 @@ def main():
     replicas.barrier(world)
     kernel_ms = []
     with ClockSampler(local) as clocks:
-        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        ev = [torch.cuda.Event(enable_timing=True) for _ in range(args.steps + 1)]
+        time.sleep(0.05)                                  # lets the sampler thread take its first samples
         torch.cuda.synchronize()
-        e0.record(f.streams[0])
-        for _ in range(args.steps):
+        clocks.mark_begin()
+        ev[0].record(f.streams[0])
+        for k in range(args.steps):
             step_device()
             kernel_ms.append(f.last_dispatch_ms(0))
-        e1.record(f.streams[0])
+            ev[k + 1].record(f.streams[0])
         torch.cuda.synchronize()
-        ms_dev = e0.elapsed_time(e1)
+        clocks.mark_end()
+        ms_dev = ev[0].elapsed_time(ev[-1])
+        step_ms = [ev[k].elapsed_time(ev[k + 1]) for k in range(args.steps)]
         c1 = f.get_counters()
-        # keep the sampler alive long enough for at least a few samples under load
-        t_end = time.perf_counter() + max(0.0, 1.0 - ms_dev * 1e-3)
-        while time.perf_counter() < t_end:
-            step_device()
+    result_dev = dst_dev.cpu().numpy()                    # forces of w.posm, for the parity key below
     replicas.barrier(world)
     launches = (c1["kernel_launches"] - c0["kernel_launches"])
     units, ms_max = replicas.reduce_timing(inter * args.steps, ms_dev, world)
@@ -738,33 +810,38 @@ def main():
         peak_tflops = n_sm * 128 * 2 * sm_max_mhz * 1e6 / 1e12
         k_ms = float(np.mean(kernel_ms))
         achieved = N_OP * inter / (k_ms * 1e-3) / 1e12
-        traffic = None
+        # ncu dram__bytes_read.sum + dram__bytes_write.sum per k_force launch, from a separate `ncu --set full` capture of this
+        # command (a run under ncu is never a bench value): "config_name bytes # source" lines
+        traffic, traffic_source = None, None
         try:
-            # ncu dram__bytes_read.sum + dram__bytes_write.sum per k_force launch: "config_name bytes" lines
             for line in open(os.path.join(ROOT, "profiles", "force_kernel_traffic.txt")):
-                parts = line.split("#", 1)[0].split()
+                body, _, note = line.partition("#")
+                parts = body.split()
                 if len(parts) == 2 and parts[0] == cfg.name:
-                    traffic = float(parts[1])
+                    traffic, traffic_source = float(parts[1]), "ncu capture, not this run: " + note.strip()
         except (OSError, ValueError):
             pass
         roof = {"bound": "alu", "kernel": "mwf::k_force", "achieved": achieved, "peak": peak_tflops, "unit": "TFLOP/s",
-                "frac": achieved / peak_tflops, "traffic": traffic, "kernel_ms": k_ms,
+                "frac": achieved / peak_tflops, "traffic": traffic, "traffic_source": traffic_source, "kernel_ms": k_ms,
+                "kernel_ms_median": float(np.median(kernel_ms)), "kernel_ms_min": float(min(kernel_ms)),
                 "peak_source": "SMs x 128 FMA/clk x 2 x max SM clock (%d x 256 x %.0f MHz; clock from %s)" % (
                     n_sm, sm_max_mhz, "MEASURED_PEAKS.json" if peaks.get("sm_max_mhz") else "nvidia-smi"),
                 "flop_per_interaction": N_OP, "interactions_per_launch": inter}
         if clk.get("sm_mhz"):
             roof["frac_at_sustained_clock"] = achieved / (n_sm * 256 * clk["sm_mhz"] * 1e6 / 1e12)
         log("[bench] oracle cpu_baseline ...")
-        ci, cdt, ck = oracle_sample(w, cfg, args.cpu_baseline_seconds)
+        ci, cdt, ck, (sel, o_acc, o_pot) = oracle_sample(w, cfg, args.cpu_baseline_seconds, want_result=True)
+        parity = parity_of(w, result_dev, sel, o_acc, o_pot)
         import oracle
         cpu = {"value": ci / cdt, "unit": UNIT, "cores": oracle.num_threads(), "kind": "oracle",
                "sample": "%d of %d groups (seeded), %.3e interactions, forces only, %.1f s" % (ck, w.n_group, ci, cdt)}
         out = {
             "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
-            "ms_per_step": ms_max / args.steps, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+            "ms_per_step": ms_max / args.steps, "ms_per_step_median": float(np.median(step_ms)), "ms_per_step_min": float(min(step_ms)),
+            "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
             "dtype": "f32", "data": "synthetic", "config": workload_config(cfg, w),
             "gflops_at_23": value * N_OP / 1e9, "frac_fp32_peak_whole_step": value * N_OP / 1e12 / (peak_tflops * world),
-            "roofline": roof, "cpu_baseline": cpu,
+            "roofline": roof, "cpu_baseline": cpu, "parity": parity,
             "e2e": e2e_pipe,
             "e2e_blocking_call": {"value": e2e_value, "unit": UNIT, "h2d_bytes_per_step": 16 * w.n, "d2h_bytes_per_step": 16 * w.n,
                                   "ms_per_step": ms_e_max / args.steps,

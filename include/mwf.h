@@ -97,11 +97,13 @@ int mwf_set_tag_stream(mwf_ctx* c, int32_t tag, void* cuda_stream);
  * monopoles stale: mwf_refresh_monopoles() must follow before the next dispatch. */
 int mwf_set_particles(mwf_ctx* c, const mwf_posm* src, int64_t first, int64_t n, int src_on_device, void* stream);
 
-/* Read back particles [first, first + n) of the store (test / integration hook). dst HOST or DEVICE. Blocking. */
+/* Read back particles [first, first + n) of the store (test / integration hook). dst HOST or DEVICE. Blocking.
+ * MWF_ERANGE when the range reaches behind the particles (N once a tree is set, else what has been uploaded). */
 int mwf_get_particles(mwf_ctx* c, mwf_posm* dst, int64_t first, int64_t n, int dst_on_device);
 
 /* (2a) Upload the tree topology (construction step only).  cells: n_cell records, HOST.
- * Defines N = cells[0].n_ptcl.  Validated on the device (MWF_ERANGE).  Blocking. */
+ * Defines N = cells[0].n_ptcl.  Validated on the device (MWF_ERANGE): particle and child ranges in bounds, children
+ * partition their parent, every cell but the root is the child of exactly one cell.  Blocking. */
 int mwf_set_tree(mwf_ctx* c, const mwf_cell* cells, int64_t n_cell, void* stream);
 
 /* (2b) Upload the i-groups and their interaction lists as two CSR index lists (construction step only;
@@ -194,7 +196,8 @@ int mwf_last_quad_ms(mwf_ctx* c, int32_t tag, float* ms);
  *   the result array that mwf_retrieve() copies out.  Reads h and P/rho^2 of every listed particle: these must be
  *   current (from density dispatches over all groups, or uploaded); the library orders a hydro dispatch behind the
  *   density kernels in flight on every tag.
- * Both need the tree, the lists, particles and records for all N (MWF_ESTATE otherwise); no monopoles are involved.
+ * Both need the tree, the lists, particles and records for all N (MWF_ESTATE otherwise); no monopoles are involved,
+ * and lists that hold SPJ entries (gravity lists) are refused with MWF_ESTATE.
  * A tag holds one kind of result at a time: MWF_ESTATE when its previous results of the other kind (records vs
  * accelerations) have not been retrieved.  Lists set with MWF_MAKE_LIST stay until the next mwf_begin_step /
  * mwf_set_lists (a step needs them twice).  Artificial viscosity and the energy equation are not evaluated. */
@@ -231,8 +234,8 @@ int mwf_calc_force_all(mwf_ctx* c, const mwf_posm* src, int src_on_device, mwf_a
  *     mwf_swap_store(); mwf_refresh_monopoles(); mwf_dispatch(t, ...) for every tag      step k+1
  * mwf_set_particles_next: like mwf_set_particles, into the shadow store; asynchronous on `stream`, waits for nothing
  *   (no kernel reads the shadow store); needs a tree (MWF_ESTATE), [first, first + n) inside [0, N) (MWF_ERANGE).
- * mwf_swap_store: the shadow store becomes the store.  MWF_ESTATE unless the calls since the last swap wrote N particles
- *   in total (the caller covers [0, N) exactly once) and no tag is in flight (every dispatched tag retrieved).  Everything
+ * mwf_swap_store: the shadow store becomes the store.  MWF_ESTATE unless the ranges written since the last swap tile
+ *   [0, N) exactly (no hole, no overlap) and no tag is in flight (every dispatched tag retrieved).  Everything
  *   enqueued later on any stream through this library is ordered behind the shadow uploads.  The monopoles become
  *   stale (mwf_refresh_monopoles must follow); velocities, results, tree and lists are not touched.
  * mwf_get_tag_split: bounds[0 .. n_tag] = the group ranges [bounds[t], bounds[t+1]) of equal interaction count that
@@ -268,6 +271,12 @@ int mwf_get_permutation(mwf_ctx* c, int32_t* perm, int dst_on_device);
 int mwf_get_tree(mwf_ctx* c, mwf_cell* cells, double* geom4);
 int mwf_get_groups(mwf_ctx* c, int32_t* grp_first, int32_t* grp_n);
 int mwf_get_lists(mwf_ctx* c, int64_t* epj_off, int32_t* epj_id, int64_t* spj_off, int32_t* spj_id);
+/* The list buffers exactly as the force kernel reads them (pin P9 of SURVEY.md 8(c): "list buffers bit-identical before /
+ * after the reuse steps"): list_off[n_group + 1] (offsets in entries, multiples of 64) and the merged,
+ * padded index list (per group: EPJ ids, SPJ ids + N, the dummy index up to a whole tile).  *n_group, *n_entry = groups and
+ * entries in the merged list (also without destinations: call once to size them).  Destinations HOST or DEVICE, either may be NULL.
+ * MWF_ESTATE without lists.  Blocking. */
+int mwf_get_list_buffer(mwf_ctx* c, int64_t* list_off, int32_t* list, int64_t* n_group, int64_t* n_entry, int dst_on_device);
 
 /* ---- Device-resident reuse step (the paper's own conclusion, P:1171-1185:
  * with the lists resident the per-step host<->device transfers of particles and forces are what is left,

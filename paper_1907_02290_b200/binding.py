@@ -26,7 +26,7 @@ SYMBOLS = (
     "mwf_set_velocities", "mwf_get_velocities", "mwf_kick_drift", "mwf_kick", "mwf_step_reuse",
     "mwf_reserve_data_lists", "mwf_dispatch_data", "mwf_set_spj_order", "mwf_get_quadrupoles", "mwf_last_quad_ms",
     "mwf_set_sph", "mwf_get_sph", "mwf_dispatch_density", "mwf_dispatch_hydro", "mwf_calc_sph_all",
-    "mwf_build", "mwf_build_neighbours", "mwf_get_build_sizes", "mwf_get_permutation", "mwf_get_tree", "mwf_get_groups", "mwf_get_lists",
+    "mwf_build", "mwf_build_neighbours", "mwf_get_build_sizes", "mwf_get_permutation", "mwf_get_tree", "mwf_get_groups", "mwf_get_lists", "mwf_get_list_buffer",
     "mwf_set_particles_next", "mwf_swap_store", "mwf_get_tag_split",
 )
 
@@ -101,6 +101,7 @@ def load_library(path: str | None = None) -> ctypes.CDLL:
         "mwf_get_tree": [vp, vp, vp],
         "mwf_get_groups": [vp, vp, vp],
         "mwf_get_lists": [vp, vp, vp, vp, vp],
+        "mwf_get_list_buffer": [vp, vp, vp, P(i64), P(i64), ci],
     }
     for name, args in sig.items():
         fn = getattr(lib, name)
@@ -359,6 +360,20 @@ class MultiWalkForce:
         self._ck(self._lib.mwf_get_lists(self._h, _host_ptr(eo, np.int64, "epj_off"), _host_ptr(ei, np.int32, "epj_id"),
                                          _host_ptr(so, np.int64, "spj_off"), _host_ptr(si, np.int32, "spj_id")))
         return eo, ei[:n_epj], so, si[:n_spj]
+
+    def get_list_buffer(self, on_device: bool = False):
+        """(list_off, list) as the force kernel reads them: numpy arrays, or torch CUDA tensors when on_device."""
+        g, n = ctypes.c_int64(0), ctypes.c_int64(0)
+        self._ck(self._lib.mwf_get_list_buffer(self._h, None, None, ctypes.byref(g), ctypes.byref(n), 0))
+        if on_device:
+            t = self._torch
+            off = t.empty(g.value + 1, dtype=t.int64, device=self.device)
+            lst = t.empty(max(1, n.value), dtype=t.int32, device=self.device)
+            self._ck(self._lib.mwf_get_list_buffer(self._h, ctypes.c_void_p(off.data_ptr()), ctypes.c_void_p(lst.data_ptr()), None, None, 1))
+            return off, lst[:n.value]
+        off, lst = np.empty(g.value + 1, np.int64), np.empty(max(1, n.value), np.int32)
+        self._ck(self._lib.mwf_get_list_buffer(self._h, _host_ptr(off, np.int64, "list_off"), _host_ptr(lst, np.int32, "list"), None, None, 0))
+        return off, lst[:n.value]
 
     def get_monopoles(self, n_cell: int) -> np.ndarray:
         out = np.empty((n_cell, 4), np.float32)

@@ -13,10 +13,8 @@ import subprocess
 _HERE = os.path.dirname(os.path.abspath(__file__))
 _ROOT = os.path.dirname(_HERE)
 
-NVCC_FLAGS = [
-    "-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-lineinfo", "-std=c++17",
-    "-Xcompiler", "-fPIC", "-shared", "-cudart", "static",
-]
+NVCC_COMPILE = ["-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-lineinfo", "-std=c++17", "-Xcompiler", "-fPIC"]
+NVCC_LINK = ["-gencode", "arch=compute_100a,code=sm_100a", "-shared", "-cudart", "static"]
 
 
 def _stale(target: str, sources: list[str]) -> bool:
@@ -46,15 +44,27 @@ def mwf_sources() -> list[str]:
 
 
 def build_mwf(force: bool = False) -> str:
-    out = os.path.join(_HERE, "csrc", "libmwf.so")
+    """Every csrc/*.cu is compiled to its own object (in parallel, only when stale) and linked into libmwf.so."""
+    from concurrent.futures import ThreadPoolExecutor
+    csrc = os.path.join(_HERE, "csrc")
+    out = os.path.join(csrc, "libmwf.so")
     srcs = mwf_sources()
-    deps = srcs + [os.path.join(_HERE, "csrc", f) for f in os.listdir(os.path.join(_HERE, "csrc")) if f.endswith((".cuh", ".h"))]
-    deps.append(os.path.join(_ROOT, "include", "mwf.h"))
-    if force or _stale(out, deps):
-        nvcc = shutil.which("nvcc") or "/usr/local/cuda/bin/nvcc"
-        if not os.path.exists(nvcc):
-            raise RuntimeError("nvcc not found; cannot build libmwf.so")
-        _run([nvcc] + NVCC_FLAGS + ["-I", os.path.join(_ROOT, "include"), "-o", out] + srcs)
+    headers = [os.path.join(csrc, f) for f in os.listdir(csrc) if f.endswith((".cuh", ".h"))]
+    headers.append(os.path.join(_ROOT, "include", "mwf.h"))
+    nvcc = shutil.which("nvcc") or "/usr/local/cuda/bin/nvcc"
+    if not os.path.exists(nvcc):
+        if os.path.exists(out) and not force:
+            return out
+        raise RuntimeError("nvcc not found; cannot build libmwf.so")
+    objdir = os.path.join(csrc, "build")
+    os.makedirs(objdir, exist_ok=True)
+    objs = [os.path.join(objdir, os.path.basename(f)[:-3] + ".o") for f in srcs]
+    todo = [(f, o) for f, o in zip(srcs, objs) if force or _stale(o, [f] + headers)]
+    extra = os.environ.get("MWF_NVCC_EXTRA", "").split()
+    with ThreadPoolExecutor(max_workers=min(8, max(1, len(todo)))) as ex:
+        list(ex.map(lambda fo: _run([nvcc] + NVCC_COMPILE + extra + ["-I", os.path.join(_ROOT, "include"), "-c", "-o", fo[1], fo[0]]), todo))
+    if todo or force or _stale(out, objs):
+        _run([nvcc] + NVCC_LINK + ["-o", out] + objs)
     return out
 
 

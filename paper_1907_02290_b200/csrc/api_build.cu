@@ -1,0 +1,186 @@
+// Device-side construction step behind mwf_build / mwf_build_neighbours and its read-back hooks
+// (SURVEY.md section 8(f) NEXT-2).
+#include <cstring>
+
+#include "mwf_ctx.h"
+
+using namespace mwf;
+
+// The device-side construction step behind mwf_build (opening angle theta) and mwf_build_neighbours (search radii 2 (1 + skin) h).
+static int build_impl(mwf_ctx* c, int64_t n, int32_t n_leaf, int32_t n_grp, double theta, bool neighbours, double skin, int mode, void* stream) {
+    if (!c || n < 1 || n_leaf < 1 || n_grp < 1) return MWF_EINVAL;
+    if (neighbours ? !(skin >= 0.0) : (!(theta >= 0.0) || theta > 1.0)) return MWF_EINVAL;
+    if (mode != MWF_MAKE_LIST && mode != MWF_MAKE_LIST_FOR_REUSE) return MWF_EINVAL;
+    if (n > c->p.max_ptcl) return MWF_ENOMEM;
+    if (neighbours && (!c->sph || c->sph_hi < n)) return MWF_ESTATE;  // the smoothing lengths of particles [0, n) must have been uploaded
+    if (c->ptcl_hi < n && !(c->have_tree && c->n_ptcl >= n)) return MWF_ESTATE;  // particles [0, n) must have been uploaded
+    for (int t = 0; t < c->p.n_tag; ++t)
+        if (!c->tag_ranges[t].empty()) return MWF_ESTATE;  // tmp16 aliases the result array: retrieve first
+    cudaStream_t s = static_cast<cudaStream_t>(stream);
+    int rc = before_store_op(c, s);
+    if (rc) return rc;
+    c->have_tree = false;
+    c->built_on_device = false;
+    drop_lists(c);
+    c->mono_fresh = false;
+    CU(c, cudaMemsetAsync(c->err, 0, sizeof(unsigned int), s));
+    const bool with_vel = c->vel_hi >= n;
+    int64_t n_cell = 0, n_group = 0;
+    int n_level = 0;
+    PhaseTimer tm;
+    float4* sph = (c->sph && c->sph_hi >= n) ? c->sph : nullptr;
+    CU(c, build_tree_device(c->bb, n, n_leaf, n_grp, c->p.max_cell, c->p.max_group, with_vel, sph, &n_cell, &n_group, &n_level, s));
+    c->n_launch += 8 + 3 * 8 + 3 * n_level;
+    tm.lap("sort + tree + groups");
+    if (n_cell > c->p.max_cell || n_group > c->p.max_group) { after_store_op(c, s); return MWF_ENOMEM; }
+    unsigned int e = 0;
+    rc = read_err_word(c, s, &e);
+    if (rc) return rc;
+    if (e) { after_store_op(c, s); return MWF_ENOMEM; }
+    // tree state as mwf_set_tree leaves it: arrival counters zero, leaves ranked, dummy record behind the SPJ block
+    CU(c, cudaMemsetAsync(c->arrive, 0, (size_t)n_cell * 4, s));
+    CU(c, launch_leaf_ranking(c->cells, n_cell, n, c->bb.mark, c->bb.scan_scratch, c->cell_lr, &c->n_leaf_cells, s));
+    c->n_launch += 5;
+    const float4 zero = make_float4(0.f, 0.f, 0.f, 0.f);
+    CU(c, cudaMemcpyAsync(c->store + n + n_cell, &zero, 16, cudaMemcpyHostToDevice, s));
+    CU(c, cudaMemcpyAsync(c->store_next + n + n_cell, &zero, 16, cudaMemcpyHostToDevice, s));
+    c->next_ranges.clear();
+    c->next_streams.clear();
+    c->n_ptcl = n;
+    c->n_cell = n_cell;
+    c->ptcl_hi = n;
+    // lists: counting walk, offsets, capacity check, fill walk
+    int64_t padded = 0, e_epj = 0, e_spj = 0;
+    WalkRule rule;
+    rule.theta = theta;
+    if (neighbours) {  // per-cell and per-group search radii; level_cnt and mark are free once the tree and the groups exist
+        rule.neighbours = true;
+        rule.reach = 2.0 * (1.0 + skin);
+        rule.cell_h = reinterpret_cast<float*>(c->bb.level_cnt);
+        rule.grp_h = reinterpret_cast<float*>(c->bb.mark);
+        CU(c, build_smoothing_reach(c->bb, c->sph, n_cell, n_group, reinterpret_cast<float*>(c->bb.level_cnt), reinterpret_cast<float*>(c->bb.mark), s));
+        c->n_launch += 2;
+    }
+    CU(c, build_lists_count(c->bb, n_group, rule, c->walk_warps_n, &padded, &e_epj, &e_spj, s));
+    tm.lap("list walk: count + offsets");
+    if (e_epj + e_spj > c->p.max_entry) { after_store_op(c, s); return MWF_ENOMEM; }
+    // group sizes and list lengths come back for the host work plan; the fill walk runs meanwhile
+    std::vector<int32_t> h_first((size_t)n_group), h_n((size_t)n_group), h_ne((size_t)n_group), h_ns((size_t)n_group);
+    const auto D2H = cudaMemcpyDeviceToHost;
+    CU(c, cudaMemcpyAsync(h_first.data(), c->grp_first, (size_t)n_group * 4, D2H, s));
+    CU(c, cudaMemcpyAsync(h_n.data(), c->grp_n, (size_t)n_group * 4, D2H, s));
+    CU(c, cudaMemcpyAsync(h_ne.data(), c->bb.n_epj, (size_t)n_group * 4, D2H, s));
+    CU(c, cudaMemcpyAsync(h_ns.data(), c->bb.n_spj, (size_t)n_group * 4, D2H, s));
+    CU(c, cudaStreamSynchronize(s));
+    CU(c, build_lists_fill(c->bb, n_group, rule, c->walk_warps_n, n, n_cell, s));
+    CU(c, cudaMemsetAsync(c->grp_self, 1, (size_t)n_group, s));  // theta <= 1: a group's own cells are always opened
+    c->n_launch += 6;
+    std::vector<int64_t> n_list((size_t)n_group);
+    for (int64_t g = 0; g < n_group; ++g) n_list[(size_t)g] = (int64_t)h_ne[(size_t)g] + h_ns[(size_t)g];
+    Plan plan;
+    rc = make_plan(c, n_group, h_first.data(), h_n.data(), n_list.data(), plan);
+    tm.lap("host work plan | fill walk");
+    if (rc) { after_store_op(c, s); return rc; }
+    if (plan.list_off[(size_t)n_group] != padded) { after_store_op(c, s); return MWF_ERANGE; }  // host and device offsets must agree
+    const int64_t n_items = (int64_t)plan.items.size();
+    const auto H2D = cudaMemcpyHostToDevice;
+    CU(c, cudaMemcpyAsync(c->items, plan.items.data(), (size_t)n_items * sizeof(WorkItem), H2D, s));
+    CU(c, cudaMemcpyAsync(c->order_full, plan.order_full.data(), (size_t)n_items * 4, H2D, s));
+    CU(c, cudaStreamSynchronize(s));  // the plan's host vectors die with this call
+    tm.lap("plan upload");
+    rc = after_store_op(c, s);
+    if (rc) return rc;
+    c->have_tree = true;
+    c->built_on_device = true;
+    c->build_e_epj = e_epj;
+    c->build_e_spj = e_spj;
+    c->build_n_level = n_level;
+    adopt_plan(c, plan, n_group, h_first.data(), h_n.data(), mode);
+    return MWF_OK;
+}
+
+extern "C" {
+
+int mwf_build(mwf_ctx* c, int64_t n, int32_t n_leaf, int32_t n_grp, double theta, int mode, void* stream) {
+    MWF_ENTER(c);
+    return build_impl(c, n, n_leaf, n_grp, theta, false, 0.0, mode, stream);
+}
+
+int mwf_build_neighbours(mwf_ctx* c, int64_t n, int32_t n_leaf, int32_t n_grp, double skin, int mode, void* stream) {
+    MWF_ENTER(c);
+    return build_impl(c, n, n_leaf, n_grp, 0.0, true, skin, mode, stream);
+}
+
+int mwf_get_build_sizes(mwf_ctx* c, int64_t* n_cell, int64_t* n_group, int64_t* n_epj, int64_t* n_spj, int32_t* n_level) {
+    MWF_ENTER(c);
+    if (!c) return MWF_EINVAL;
+    if (!c->built_on_device || !c->have_lists) return MWF_ESTATE;
+    if (n_cell) *n_cell = c->n_cell;
+    if (n_group) *n_group = c->n_group;
+    if (n_epj) *n_epj = c->build_e_epj;
+    if (n_spj) *n_spj = c->build_e_spj;
+    if (n_level) *n_level = c->build_n_level;
+    return MWF_OK;
+}
+
+int mwf_get_permutation(mwf_ctx* c, int32_t* perm, int dst_on_device) {
+    MWF_ENTER(c);
+    if (!c || !perm) return MWF_EINVAL;
+    if (!c->built_on_device) return MWF_ESTATE;
+    CU(c, cudaDeviceSynchronize());
+    CU(c, cudaMemcpy(perm, c->bb.idx_a, (size_t)c->n_ptcl * 4, dst_on_device ? cudaMemcpyDeviceToDevice : cudaMemcpyDeviceToHost));
+    return MWF_OK;
+}
+
+int mwf_get_tree(mwf_ctx* c, mwf_cell* cells, double* geom4) {
+    MWF_ENTER(c);
+    if (!c || (!cells && !geom4)) return MWF_EINVAL;
+    if (!c->have_tree) return MWF_ESTATE;
+    if (geom4 && !c->built_on_device) return MWF_ESTATE;  // an uploaded tree carries no geometry
+    CU(c, cudaDeviceSynchronize());
+    if (cells) CU(c, cudaMemcpy(cells, c->cells, (size_t)c->n_cell * sizeof(mwf_cell), cudaMemcpyDeviceToHost));
+    if (geom4) CU(c, cudaMemcpy(geom4, c->bb.geom, (size_t)c->n_cell * 32, cudaMemcpyDeviceToHost));
+    return MWF_OK;
+}
+
+int mwf_get_groups(mwf_ctx* c, int32_t* grp_first, int32_t* grp_n) {
+    MWF_ENTER(c);
+    if (!c || !grp_first || !grp_n) return MWF_EINVAL;
+    if (!c->have_lists) return MWF_ESTATE;
+    std::memcpy(grp_first, c->h_grp_first.data(), (size_t)c->n_group * 4);
+    std::memcpy(grp_n, c->h_grp_n.data(), (size_t)c->n_group * 4);
+    return MWF_OK;
+}
+
+int mwf_get_lists(mwf_ctx* c, int64_t* epj_off, int32_t* epj_id, int64_t* spj_off, int32_t* spj_id) {
+    MWF_ENTER(c);
+    if (!c || !epj_off || !spj_off || !epj_id || !spj_id) return MWF_EINVAL;
+    if (!c->have_lists) return MWF_ESTATE;
+    CU(c, cudaDeviceSynchronize());
+    // un-merge into the staging area of the upload path, then two bulk copies
+    if (c->build_e_epj + c->build_e_spj > c->p.max_entry) return MWF_ENOMEM;
+    int32_t* d_epj = c->st_ids;
+    int32_t* d_spj = c->st_ids + c->build_e_epj;
+    CU(c, unmerge_lists(c->bb, c->n_group, c->n_ptcl, d_epj, d_spj, nullptr));
+    CU(c, cudaDeviceSynchronize());
+    CU(c, cudaMemcpy(epj_off, c->bb.epj_off, (size_t)(c->n_group + 1) * 8, cudaMemcpyDeviceToHost));
+    CU(c, cudaMemcpy(spj_off, c->bb.spj_off, (size_t)(c->n_group + 1) * 8, cudaMemcpyDeviceToHost));
+    if (c->build_e_epj) CU(c, cudaMemcpy(epj_id, d_epj, (size_t)c->build_e_epj * 4, cudaMemcpyDeviceToHost));
+    if (c->build_e_spj) CU(c, cudaMemcpy(spj_id, d_spj, (size_t)c->build_e_spj * 4, cudaMemcpyDeviceToHost));
+    return MWF_OK;
+}
+
+int mwf_get_list_buffer(mwf_ctx* c, int64_t* list_off, int32_t* list, int64_t* n_group, int64_t* n_entry, int dst_on_device) {
+    MWF_ENTER(c);
+    if (!c) return MWF_EINVAL;
+    if (!c->have_lists) return MWF_ESTATE;
+    if (n_group) *n_group = c->n_group;
+    if (n_entry) *n_entry = c->padded_entries;
+    CU(c, cudaDeviceSynchronize());
+    const auto kind = dst_on_device ? cudaMemcpyDeviceToDevice : cudaMemcpyDeviceToHost;
+    if (list_off) CU(c, cudaMemcpy(list_off, c->list_off, (size_t)(c->n_group + 1) * 8, kind));
+    if (list && c->padded_entries > 0) CU(c, cudaMemcpy(list, c->list, (size_t)c->padded_entries * 4, kind));
+    return MWF_OK;
+}
+
+}  // extern "C"

@@ -44,6 +44,24 @@ __global__ void k_tree_prepare(const mwf_cell* __restrict__ cells, int64_t n_cel
         }
     }
     if (e) atomicOr(err, e);
+    // number of child claims, for k_tree_check (a cell with a bad child range claims nothing)
+    unsigned claims = (cc.n_child > 0 && !(e & ERR_CHILD_RANGE)) ? (unsigned)cc.n_child : 0u;
+#pragma unroll
+    for (int d = 16; d > 0; d >>= 1) claims += __shfl_xor_sync(0xffffffffu, claims, d);
+    if ((threadIdx.x & 31) == 0 && claims) atomicAdd(err + 1, claims);
+}
+
+// Every cell but the root must have been claimed by exactly one parent: parent[] was preset to a negative mark, so an
+// orphan still carries it, and n_cell - 1 claims over n_cell - 1 claimed cells leave no cell claimed twice.  (The climb
+// variant of the refresh and the per-cell passes of the construction step follow parent[] without checks.)
+__global__ void k_tree_check(const int32_t* __restrict__ parent, int64_t n_cell, unsigned int* __restrict__ err) {
+    const int64_t c = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (c >= n_cell) return;
+    if (c == 0) {
+        if ((int64_t)err[1] != n_cell - 1) atomicOr(err, ERR_CHILD_PART);
+    } else if (parent[c] < 0) {
+        atomicOr(err, ERR_CHILD_RANGE);
+    }
 }
 
 __device__ __forceinline__ void store_moment(float4* __restrict__ store, double4* __restrict__ mom64, int64_t n_ptcl, int64_t c,
@@ -289,7 +307,12 @@ cudaError_t launch_tree_prepare(const mwf_cell* cells, int64_t n_cell, int64_t m
                                 unsigned int* err, cudaStream_t s) {
     const int block = 256;
     const int64_t grid = (n_cell + block - 1) / block;
+    cudaError_t e = cudaMemsetAsync(parent, 0xFE, (size_t)n_cell * 4, s);  // "unclaimed": negative
+    if (e != cudaSuccess) return e;
+    if ((e = cudaMemsetAsync(err + 1, 0, 4, s)) != cudaSuccess) return e;
     k_tree_prepare<<<(unsigned)grid, block, 0, s>>>(cells, n_cell, max_ptcl, parent, counter, err);
+    if ((e = cudaGetLastError()) != cudaSuccess) return e;
+    k_tree_check<<<(unsigned)grid, block, 0, s>>>(parent, n_cell, err);
     return cudaGetLastError();
 }
 

@@ -558,6 +558,23 @@ def test_state_machine_and_validation():
     cells = w.cells.copy()
     cells[1, 0] += 1
     assert expect_code(f.set_tree, cells) == binding.ERANGE
+    # a cell nobody claims (its parent's child range stops short of it) / a cell claimed by two parents
+    par = np.nonzero(w.cells[:, 3] >= 2)[0][-1]
+    cells = w.cells.copy()
+    last = cells[par, 2] + cells[par, 3] - 1
+    cells[par, 3] -= 1                                                         # orphan: `last`
+    cells[last - 1, 1] += cells[last, 1]                                       # keep the partition of the parent's range
+    assert expect_code(f.set_tree, cells) == binding.ERANGE
+    leaves = np.nonzero(w.cells[:, 3] == 0)[0]
+    cells = w.cells.copy()
+    victim = cells[par, 2]                                                     # first child of `par` ...
+    thief = leaves[leaves != victim][0]
+    if cells[thief, 1] == cells[victim, 1] and cells[thief, 0] == cells[victim, 0]:
+        thief = leaves[leaves != victim][1]
+    cells[thief, 2], cells[thief, 3] = victim, 1                               # ... also claimed by a leaf turned parent
+    assert expect_code(f.set_tree, cells) == binding.ERANGE
+    f.set_tree(w.cells)
+    assert expect_code(f.get_particles, w.n - 1, 2) == binding.ERANGE          # behind the particles: the SPJ block
     small = binding.MultiWalkForce(cfg.eps, max_ptcl=w.n, max_cell=w.n_cell, max_group=w.n_group, max_entry=10, n_tag=1)
     small.set_particles(w.posm)
     small.set_tree(w.cells)
@@ -579,7 +596,8 @@ def test_reuse_run_per_step():
     v = w.vel.copy()
     posm = w.posm.copy()
     host_in, host_out = f.pinned(w.n), f.pinned(w.n)
-    padded0, spj_prev, a = None, None, None
+    spj_prev, a = None, None
+    off0, list0 = f.get_list_buffer()                          # pin P9: the list buffers as the kernel reads them
     for step in range(cfg.n_reuse + 1):
         if step > 0:
             v += 0.5 * cfg.dt * a
@@ -598,9 +616,8 @@ def test_reuse_run_per_step():
         if spj_prev is not None:
             assert not np.array_equal(spj, spj_prev)           # moments follow the particles
         spj_prev = spj
-        c = f.get_counters()
-        padded0 = c["padded_entries"] if padded0 is None else padded0
-        assert c["padded_entries"] == padded0                  # lists untouched on reuse steps
+        off1, list1 = f.get_list_buffer()
+        assert np.array_equal(off0, off1) and np.array_equal(list0, list1)   # bit-identical on reuse steps
         a = out[:, :3].astype(np.float64)
         if step > 0:
             v += 0.5 * cfg.dt * a
@@ -626,6 +643,7 @@ def test_device_resident_reuse_run():
     f = binding.MultiWalkForce.for_workload(w, n_tag=2)
     f.upload_workload(w, binding.MAKE_LIST_FOR_REUSE)
     assert expect_code(f.step_reuse, dt) == binding.ESTATE          # no evaluation yet, no velocities
+    lists0 = f.get_list_buffer()
     f.refresh_monopoles()
     f.dispatch(0, 0, w.n_group)
     out = np.zeros((w.n, 4), np.float32)
@@ -653,6 +671,7 @@ def test_device_resident_reuse_run():
         spj = f.get_monopoles(w.n_cell)
         assert np.all(np.abs(spj[:, 3] - mom[:, 3]) <= 1e-6 * mom[:, 3])
         x_prev, v_prev, a_prev = x_now, v_now, out.copy()
+    assert np.array_equal(lists0[0], f.get_list_buffer()[0]) and np.array_equal(lists0[1], f.get_list_buffer()[1])   # pin P9
     assert expect_code(f.kick_drift, float("nan")) == binding.EINVAL
     f.set_particles(w.posm)                                         # positions changed: forces are stale
     assert expect_code(f.kick_drift, dt) == binding.ESTATE
