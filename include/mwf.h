@@ -273,7 +273,7 @@ int mwf_get_groups(mwf_ctx* c, int32_t* grp_first, int32_t* grp_n);
 int mwf_get_lists(mwf_ctx* c, int64_t* epj_off, int32_t* epj_id, int64_t* spj_off, int32_t* spj_id);
 /* The list buffers exactly as the force kernel reads them (pin P9 of SURVEY.md 8(c): "list buffers bit-identical before /
  * after the reuse steps"): list_off[n_group + 1] (offsets in entries, multiples of 64) and the merged,
- * padded index list (per group: EPJ ids, SPJ ids + N, the dummy index up to a whole tile).  *n_group, *n_entry = groups and
+ * padded index list (per group: EPJ ids, dummy indices up to a whole tile, SPJ ids + N, dummy indices up to a whole tile).  *n_group, *n_entry = groups and
  * entries in the merged list (also without destinations: call once to size them).  Destinations HOST or DEVICE, either may be NULL.
  * MWF_ESTATE without lists.  Blocking. */
 int mwf_get_list_buffer(mwf_ctx* c, int64_t* list_off, int32_t* list, int64_t* n_group, int64_t* n_entry, int dst_on_device);

@@ -44,6 +44,7 @@ static int build_impl(mwf_ctx* c, int64_t n, int32_t n_leaf, int32_t n_grp, doub
     const float4 zero = make_float4(0.f, 0.f, 0.f, 0.f);
     CU(c, cudaMemcpyAsync(c->store + n + n_cell, &zero, 16, cudaMemcpyHostToDevice, s));
     CU(c, cudaMemcpyAsync(c->store_next + n + n_cell, &zero, 16, cudaMemcpyHostToDevice, s));
+    CU(c, cudaMemsetAsync(c->spj_rec + 2 * n_cell, 0, 32, s));
     c->next_ranges.clear();
     c->next_streams.clear();
     c->n_ptcl = n;
@@ -75,10 +76,9 @@ static int build_impl(mwf_ctx* c, int64_t n, int32_t n_leaf, int32_t n_grp, doub
     CU(c, build_lists_fill(c->bb, n_group, rule, c->walk_warps_n, n, n_cell, s));
     CU(c, cudaMemsetAsync(c->grp_self, 1, (size_t)n_group, s));  // theta <= 1: a group's own cells are always opened
     c->n_launch += 6;
-    std::vector<int64_t> n_list((size_t)n_group);
-    for (int64_t g = 0; g < n_group; ++g) n_list[(size_t)g] = (int64_t)h_ne[(size_t)g] + h_ns[(size_t)g];
+    std::vector<int64_t> n_epj(h_ne.begin(), h_ne.end()), n_spj(h_ns.begin(), h_ns.end());
     Plan plan;
-    rc = make_plan(c, n_group, h_first.data(), h_n.data(), n_list.data(), plan);
+    rc = make_plan(c, n_group, h_first.data(), h_n.data(), n_epj.data(), n_spj.data(), plan);
     tm.lap("host work plan | fill walk");
     if (rc) { after_store_op(c, s); return rc; }
     if (plan.list_off[(size_t)n_group] != padded) { after_store_op(c, s); return MWF_ERANGE; }  // host and device offsets must agree

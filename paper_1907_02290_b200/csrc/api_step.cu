@@ -51,6 +51,11 @@ static int dispatch_launch(mwf_ctx* c, int32_t tag, int64_t g_begin, int64_t g_e
     cudaStream_t s = c->tag_stream[tag];
     ForceArgs a;
     a.store = c->store;
+    a.spj_rec = c->spj_rec;
+    a.n_ptcl = (int32_t)c->n_ptcl;
+    a.dummy = (int32_t)(c->n_ptcl + c->n_cell);
+    a.epj_off = c->st_epj_off;
+    a.spj_off = c->st_spj_off;
     a.list = c->list;
     a.list_off = c->list_off;
     a.grp_self = c->grp_self;
@@ -224,6 +229,7 @@ int mwf_set_tree(mwf_ctx* c, const mwf_cell* cells, int64_t n_cell, void* stream
     const float4 zero = make_float4(0.f, 0.f, 0.f, 0.f);
     CU(c, cudaMemcpyAsync(c->store + n + n_cell, &zero, 16, cudaMemcpyHostToDevice, s));
     CU(c, cudaMemcpyAsync(c->store_next + n + n_cell, &zero, 16, cudaMemcpyHostToDevice, s));
+    CU(c, cudaMemsetAsync(c->spj_rec + 2 * n_cell, 0, 32, s));
     c->next_ranges.clear();
     c->next_streams.clear();
     unsigned int e = 0;
@@ -252,15 +258,16 @@ int mwf_set_lists(mwf_ctx* c, int64_t n_group, const int32_t* grp_first, const i
     if ((e_epj > 0 && !epj_id) || (e_spj > 0 && !spj_id)) return MWF_EINVAL;
     if (e_epj + e_spj > c->p.max_entry) return MWF_ENOMEM;
     // host pass: offsets, items, schedule
-    std::vector<int64_t> n_list((size_t)n_group);
+    std::vector<int64_t> n_epj((size_t)n_group), n_spj((size_t)n_group);
     for (int64_t g = 0; g < n_group; ++g) {
         const int64_t ne = epj_off[g + 1] - epj_off[g], ns = spj_off[g + 1] - spj_off[g];
         if (ne < 0 || ns < 0) return MWF_ERANGE;
-        n_list[(size_t)g] = ne + ns;
+        n_epj[(size_t)g] = ne;
+        n_spj[(size_t)g] = ns;
     }
     Plan plan;
     {
-        const int prc = make_plan(c, n_group, grp_first, grp_n, n_list.data(), plan);
+        const int prc = make_plan(c, n_group, grp_first, grp_n, n_epj.data(), n_spj.data(), plan);
         if (prc) return prc;
     }
     const std::vector<int64_t>& list_off = plan.list_off;
@@ -323,11 +330,11 @@ int mwf_refresh_monopoles(mwf_ctx* c, void* stream) {
     int rc = before_store_op(c, s);
     if (rc) return rc;
     if (c->spj_order == 2 || !use_scan_refresh()) {  // the quadrupoles need the bottom-up pass (parallel-axis theorem)
-        CU(c, launch_monopoles(c->cells, c->parent, c->n_cell, c->n_ptcl, c->store, c->mom64, c->arrive,
+        CU(c, launch_monopoles(c->cells, c->parent, c->n_cell, c->n_ptcl, c->store, c->spj_rec, c->mom64, c->arrive,
                                c->spj_order == 2 ? c->quad64 : nullptr, c->spj_order == 2 ? c->quad : nullptr, s));
         ++c->n_launch;
     } else {
-        CU(c, launch_monopoles_scan(c->cells, c->cell_lr, c->n_cell, c->n_ptcl, c->n_leaf_cells, c->store, c->leaf_P, c->leaf_toff, s));
+        CU(c, launch_monopoles_scan(c->cells, c->cell_lr, c->n_cell, c->n_ptcl, c->n_leaf_cells, c->store, c->spj_rec, c->leaf_P, c->leaf_toff, s));
         c->n_launch += 4;
     }
     c->mono_fresh = true;

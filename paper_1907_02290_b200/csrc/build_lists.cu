@@ -12,7 +12,7 @@
 // compacts the three outcomes with ballots / warp prefix sums.  At most 256 cells of any one level are ever on
 // the stack, so 22 levels x 256 entries bound it.  The walk runs twice: a counting pass (n_epj, n_spj per group)
 // and, after the offsets have been scanned, a fill pass that writes the merged, padded list the force kernel
-// reads: EPJ ids, then SPJ ids + N, then the dummy index up to a multiple of 64 (P:441-477 layout).
+// reads: EPJ ids, then SPJ ids + N (P:441-477 layout), each run padded with the dummy index to a multiple of 64.
 #include "mwf_internal.h"
 #include "scan_sort.cuh"
 
@@ -46,7 +46,7 @@ __global__ void __launch_bounds__(256) k_walk(const mwf_cell* __restrict__ cells
         int64_t off_e = 0, off_s = 0;
         if (FILL) {
             off_e = list_off[g];
-            off_s = off_e + n_epj[g];
+            off_s = off_e + (n_epj[g] + TILE_J - 1) / TILE_J * TILE_J;  // each run in whole tiles
         }
         int ne = 0, ns = 0, sp = 1;
         if (lane == 0) stack[0] = 0;
@@ -132,9 +132,10 @@ __global__ void __launch_bounds__(256) k_walk(const mwf_cell* __restrict__ cells
             }
             __syncwarp();
         }
-        if (FILL) {  // pad to whole tiles with the zero-mass dummy record
+        if (FILL) {  // pad both runs to whole tiles with the zero-mass dummy record
             const int64_t end = list_off[g + 1];
-            for (int64_t k = off_e + ne + ns + lane; k < end; k += 32) list[k] = dummy;
+            for (int64_t k = off_e + ne + lane; k < off_s; k += 32) list[k] = dummy;
+            for (int64_t k = off_s + ns + lane; k < end; k += 32) list[k] = dummy;
         } else if (lane == 0) {
             n_epj[g] = ne;
             n_spj[g] = ns;
@@ -179,8 +180,7 @@ __global__ void __launch_bounds__(256) k_padded_len(const int32_t* __restrict__ 
     const int64_t g = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
     if (g > n_group) return;
     if (g == n_group) { list_off[g] = 0; epj_off[g] = 0; spj_off[g] = 0; return; }
-    const int64_t len = (int64_t)n_epj[g] + n_spj[g];
-    list_off[g] = (len + TILE_J - 1) / TILE_J * TILE_J;
+    list_off[g] = ((int64_t)n_epj[g] + TILE_J - 1) / TILE_J * TILE_J + ((int64_t)n_spj[g] + TILE_J - 1) / TILE_J * TILE_J;
     epj_off[g] = n_epj[g];
     spj_off[g] = n_spj[g];
 }
@@ -191,8 +191,9 @@ __global__ void __launch_bounds__(256) k_unmerge(const int32_t* __restrict__ lis
                                                  int32_t* __restrict__ spj_id) {
     for (int64_t g = blockIdx.x; g < n_group; g += gridDim.x) {
         const int64_t l0 = list_off[g], e0 = epj_off[g], ne = epj_off[g + 1] - e0, s0 = spj_off[g], ns = spj_off[g + 1] - s0;
+        const int64_t ne_pad = (ne + TILE_J - 1) / TILE_J * TILE_J;
         for (int64_t k = threadIdx.x; k < ne; k += blockDim.x) epj_id[e0 + k] = list[l0 + k];
-        for (int64_t k = threadIdx.x; k < ns; k += blockDim.x) spj_id[s0 + k] = list[l0 + ne + k] - n_ptcl;
+        for (int64_t k = threadIdx.x; k < ns; k += blockDim.x) spj_id[s0 + k] = list[l0 + ne_pad + k] - n_ptcl;
     }
 }
 

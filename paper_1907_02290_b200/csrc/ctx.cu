@@ -93,7 +93,7 @@ Layout make_layout(const mwf_params& p) {
     L.add((p.max_group + 1) * 8);                       // 10 st_epj_off
     L.add((p.max_group + 1) * 8);                       // 11 st_spj_off
     L.add(p.max_entry * 4);                             // 12 st_ids
-    L.add((p.max_entry + TILE_J * p.max_group) * 4);    // 13 list
+    L.add((p.max_entry + 2 * TILE_J * p.max_group) * 4);  // 13 list (each of a group's two runs padded to whole tiles)
     L.add(mi * (int64_t)sizeof(WorkItem));              // 14 items
     L.add(mi * 4);                                      // 15 order_full
     L.add(mi * 4);                                      // 16 order_split
@@ -126,6 +126,7 @@ Layout make_layout(const mwf_params& p) {
     L.add((p.max_cell + 1) * 32);                       // 40 leaf_P
     L.add((scan4_tiles(p.max_cell) + 1) * 32);          // 41 leaf_toff
     L.add((p.max_ptcl + p.max_cell + 1) * 16);          // 42 store_next
+    L.add((p.max_cell + 1) * 32);                       // 43 spj_rec
     return L;
 }
 
@@ -199,6 +200,7 @@ int mwf_create(mwf_ctx** out, const mwf_params* p, void* arena, int64_t arena_by
     char* b = c->arena;
     c->store = (float4*)(b + L.off[0]);
     c->store_next = (float4*)(b + L.off[42]);
+    c->spj_rec = (float4*)(b + L.off[43]);
     c->accp = (float4*)(b + L.off[1]);
     c->cells = (mwf_cell*)(b + L.off[2]);
     c->parent = (int32_t*)(b + L.off[3]);

@@ -19,6 +19,13 @@
 //   * accumulation is two-level: partial sums over 32 j-pairs are added into running totals (two
 //     independent sums per component from the j-pairing), which keeps the fp32 summation error far inside
 //     the tolerance.
+//   * two coordinate conventions, one per kind of list entry (reading S11b of DESIGN.md).  EPJ tiles run in the
+//     caller's coordinates: particle positions are exact fp32 inputs and d = fl(x_j - x_i) is good to half an ulp of the
+//     DIFFERENCE however small it is.  SPJ tiles run in item-centred coordinates, c = the item's first i-particle: a
+//     centre of mass is not an fp32 input -- on the fp32 grid it is up to 2^-25 |X| off, which for a cell 1e-3 away at
+//     coordinates of order 1 is the north_star's whole error budget -- so the refresh keeps its rounding remainder next
+//     to it (spj_rec: 32 B per cell) and the staged position (hi - c) + lo carries 24 bits of the DISTANCE to the item;
+//     the i-side switches by adding c to -x_i.  The two runs of a group's list are padded to whole tiles separately.
 //   * the self term (an i-particle meets itself in its own EPJ list) contributes exactly 0 to acc and
 //     m_i * rsqrt(eps^2) to the potential sum; the same value is subtracted up front (reading S2).
 #include "mwf_internal.h"
@@ -117,6 +124,10 @@ __device__ __forceinline__ void run_item(const ForceArgs& a, const WorkItem it, 
         const float4 p = __ldg(J + it.i_first + (valid[k] ? off : 0));
         nx[k] = -p.x; ny[k] = -p.y; nz[k] = -p.z; mi[k] = p.w;
     }
+    if constexpr (INDEXED) {  // origin of the SPJ tiles
+        if (lane == 0) sbuf[2 * TILE_J] = __ldg(J + it.i_first);
+        __syncwarp();
+    }
     const float self_rinv = rsqrt_approx(a.eps2);  // what the sweep computes for d = 0
     const bool self_in = a.grp_self[it.group] != 0;
 
@@ -128,25 +139,38 @@ __device__ __forceinline__ void run_item(const ForceArgs& a, const WorkItem it, 
     for (int k = 0; k < 2; ++k) acc.p[k].x = (self_in && sl == 0) ? -mi[k] * self_rinv : 0.f;
 
     int64_t l0, n_list = 0;
-    int n_tiles;
+    int n_tiles, te;  // tiles [0, te) hold EPJ entries, [te, n_tiles) SPJ entries
     if constexpr (INDEXED) {
         l0 = a.list_off[it.group];
         n_tiles = (int)((a.list_off[it.group + 1] - l0) / TILE_J);
+        te = (int)((a.epj_off[it.group + 1] - a.epj_off[it.group] + TILE_J - 1) / TILE_J);
     } else {
         l0 = a.joff[it.group - a.g_base];
         n_list = a.joff[it.group - a.g_base + 1] - l0;
         n_tiles = (int)((n_list + TILE_J - 1) / TILE_J);
+        te = n_tiles;  // the records of a data list are all fp32: one convention
     }
     const int2* __restrict__ lst = reinterpret_cast<const int2*>(a.list + (INDEXED ? l0 : 0));
     const float4* __restrict__ jd = a.jdata + (INDEXED ? 0 : l0);
 
+    // SPJ entries are cell index + N: their 32-byte records (float4 record, float4 remainder) are gathered from here
+    const float4* __restrict__ R = a.spj_rec - 2 * (int64_t)a.n_ptcl;
     int2 idn = make_int2(0, 0);
-    float4 j0 = make_float4(0.f, 0.f, 0.f, 0.f), j1 = j0;
-    if (n_tiles > 0) {
-        if constexpr (INDEXED) {
-            const int2 id = ld_stream_int2(lst + lane);
+    float4 j0 = make_float4(0.f, 0.f, 0.f, 0.f), j1 = j0, q0 = j0, q1 = j0;
+    auto gather = [&](int t, const int2 id) {
+        if (t < te) {
             j0 = __ldg(J + id.x);
             j1 = __ldg(J + id.y);
+        } else {
+            j0 = __ldg(R + 2 * id.x);
+            q0 = __ldg(R + 2 * id.x + 1);
+            j1 = __ldg(R + 2 * id.y);
+            q1 = __ldg(R + 2 * id.y + 1);
+        }
+    };
+    if (n_tiles > 0) {
+        if constexpr (INDEXED) {
+            gather(0, ld_stream_int2(lst + lane));
             if (n_tiles > 1) idn = ld_stream_int2(lst + 32 + lane);
         } else {
             ld_data_pair(jd, n_list, 0, lane, j0, j1);
@@ -155,13 +179,22 @@ __device__ __forceinline__ void run_item(const ForceArgs& a, const WorkItem it, 
     for (int t = 0; t < n_tiles; ++t) {
         float4* sA = sbuf + (t & 1) * TILE_J;
         float4* sB = sA + TILE_J / 2;
-        sA[lane] = make_float4(j0.x, j1.x, j0.y, j1.y);
-        sB[lane] = make_float4(j0.z, j1.z, j0.w, j1.w);
+        if (!INDEXED || t < te) {
+            sA[lane] = make_float4(j0.x, j1.x, j0.y, j1.y);
+            sB[lane] = make_float4(j0.z, j1.z, j0.w, j1.w);
+        } else {
+            const float4 c = sbuf[2 * TILE_J];  // the item's origin (kept in shared memory, not in registers across the sweep)
+            if (t == te) {
+#pragma unroll
+                for (int k = 0; k < 2; ++k) { nx[k] += c.x; ny[k] += c.y; nz[k] += c.z; }
+            }
+            sA[lane] = make_float4((j0.x - c.x) + q0.x, (j1.x - c.x) + q1.x, (j0.y - c.y) + q0.y, (j1.y - c.y) + q1.y);
+            sB[lane] = make_float4((j0.z - c.z) + q0.z, (j1.z - c.z) + q1.z, j0.w, j1.w);
+        }
         __syncwarp();
         if (t + 1 < n_tiles) {
             if constexpr (INDEXED) {
-                j0 = __ldg(J + idn.x);
-                j1 = __ldg(J + idn.y);
+                gather(t + 1, idn);
                 if (t + 2 < n_tiles) idn = ld_stream_int2(lst + (int64_t)(t + 2) * 32 + lane);
             } else {
                 ld_data_pair(jd, n_list, t + 1, lane, j0, j1);
@@ -198,7 +231,7 @@ __device__ __forceinline__ void force_body(const ForceArgs& a, float4* s_tiles) 
     const int lane = threadIdx.x & 31;
     const int warp = threadIdx.x >> 5;
     const int warps_per_cta = blockDim.x >> 5;
-    float4* sbuf = s_tiles + warp * (2 * TILE_J);
+    float4* sbuf = s_tiles + warp * (2 * TILE_J + 1);
     int64_t w = (int64_t)blockIdx.x * warps_per_cta + warp;  // first item: static
     const int64_t n_warps = (int64_t)gridDim.x * warps_per_cta;
     while (w < a.n_items) {
@@ -233,7 +266,7 @@ __global__ void __launch_bounds__(WARPS_PER_CTA * 32, MWF_MIN_CTAS) k_force_data
     force_body<false>(a, s_force_tiles);
 }
 
-constexpr size_t FORCE_SMEM_PER_WARP = 2 * TILE_J * sizeof(float4);
+constexpr size_t FORCE_SMEM_PER_WARP = (2 * TILE_J + 1) * sizeof(float4);  // two tiles and the item's origin
 
 // warps = warps per block: WARPS_PER_CTA for a dispatch that fills the machine (persistent grid, items claimed dynamically);
 // a sub-wave dispatch (a batch of the multiwalk pipeline) is launched with small blocks, one item per warp, so

@@ -1,8 +1,9 @@
 // Construction-step re-encoding of the uploaded CSR index lists.
 // The two lists of a group (EPJ particle indices, SPJ cell indices) become ONE list of indices into the
-// combined store -- EPJ ids, then SPJ ids + N -- exactly the paper's layout ("id_epj ... id_spj + n_epj_tot",
-// P:441-477), padded to a whole number of 64-entry tiles with the index of a zero-mass dummy record
-// (the paper pads with a sentinel walk whose list is empty).  Indices are validated
+// combined store -- EPJ ids, then SPJ ids + N -- the paper's layout ("id_epj ... id_spj + n_epj_tot"),
+// with EACH of the two runs padded to a whole number of 64-entry tiles with the index of a zero-mass dummy record
+// (the paper pads with a sentinel walk whose list is empty): the force kernel sweeps EPJ tiles
+// and SPJ tiles in different coordinate conventions (reading S11b), so no tile may hold both kinds.  Indices are validated
 // here, once; the force kernel then runs check-free on every reuse step.
 #include "mwf_internal.h"
 
@@ -21,6 +22,7 @@ __global__ void __launch_bounds__(256) k_merge_lists(int64_t n_group, const int3
         const int64_t e0 = epj_off[g], ne = epj_off[g + 1] - e0;
         const int64_t s0 = spj_off[g], ns = spj_off[g + 1] - s0;
         const int64_t o0 = list_off[g], padded = list_off[g + 1] - o0;
+        const int64_t ne_pad = (ne + TILE_J - 1) / TILE_J * TILE_J;  // the SPJ run starts on a tile boundary
         const int32_t gf = grp_first[g], gn = grp_n[g];
         unsigned int e = 0;
         int self = 0;
@@ -35,9 +37,10 @@ __global__ void __launch_bounds__(256) k_merge_lists(int64_t n_group, const int3
             const int32_t id = spj_id[s0 + k];
             int64_t v = n_ptcl + id;
             if (id < 0 || id >= n_cell) { e |= ERR_SPJ_INDEX; v = n_ptcl + n_cell; }
-            list[o0 + ne + k] = (int32_t)v;
+            list[o0 + ne_pad + k] = (int32_t)v;
         }
-        for (int64_t k = ne + ns + threadIdx.x; k < padded; k += blockDim.x) list[o0 + k] = (int32_t)(n_ptcl + n_cell);
+        for (int64_t k = ne + threadIdx.x; k < ne_pad; k += blockDim.x) list[o0 + k] = (int32_t)(n_ptcl + n_cell);
+        for (int64_t k = ne_pad + ns + threadIdx.x; k < padded; k += blockDim.x) list[o0 + k] = (int32_t)(n_ptcl + n_cell);
         if (self) atomicAdd(&s_self, self);
         __syncthreads();
         if (threadIdx.x == 0) {

@@ -23,6 +23,7 @@ struct mwf_ctx {
     float4* store_next = nullptr; // same size: the shadow store of the pipelined host loop (mwf_set_particles_next / mwf_swap_store)
     std::vector<std::pair<int64_t, int64_t>> next_ranges;  // particle ranges written into the shadow store since the last swap
     std::vector<cudaStream_t> next_streams;  // streams those uploads went to
+    float4* spj_rec = nullptr;    // [2 (max_cell + 1)] per cell: SPJ record + rounding remainder of its centre of mass (reading S11b)
     float4* accp = nullptr;       // [max_ptcl]
     float4* vel = nullptr;        // [max_ptcl] (vx, vy, vz, unused): device-resident integration
     mwf_cell* cells = nullptr;    // [max_cell]
@@ -138,7 +139,7 @@ struct Plan {
     std::vector<int64_t> cost;
     std::vector<int32_t> order_full;
 };
-int make_plan(mwf_ctx* c, int64_t n_group, const int32_t* grp_first, const int32_t* grp_n, const int64_t* n_list_of, Plan& pl);
+int make_plan(mwf_ctx* c, int64_t n_group, const int32_t* grp_first, const int32_t* grp_n, const int64_t* n_epj_of, const int64_t* n_spj_of, Plan& pl);
 void adopt_plan(mwf_ctx* c, Plan& pl, int64_t n_group, const int32_t* grp_first, const int32_t* grp_n, int mode);
 int ensure_split_order(mwf_ctx* c, cudaStream_t s);
 

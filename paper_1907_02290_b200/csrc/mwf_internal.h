@@ -47,6 +47,11 @@ inline int64_t item_cost_per_tile(int width) { return COST_STAGE + COST_PAIR * w
 
 struct ForceArgs {
     const float4* store;        // particles then SPJ then one zero-mass dummy
+    const float4* spj_rec;      // [2 (n_cell + 1)] per cell: the SPJ record and the rounding remainder of its centre of mass (entry n_cell: zero)
+    int32_t n_ptcl;             // list indices >= n_ptcl are SPJ entries
+    int32_t dummy;              // index of the zero-mass record (n_ptcl + n_cell)
+    const int64_t* epj_off;     // scanned EPJ / SPJ counts per group: entries [0, ne) of a group's list are EPJ,
+    const int64_t* spj_off;     //   [ne, ne + ns) SPJ, the rest of its last tile padding
     const int32_t* list;        // merged, padded lists
     const int64_t* list_off;    // per group, in entries (multiples of TILE_J)
     const uint8_t* grp_self;    // 1: the group's own particles are in its EPJ list
@@ -109,14 +114,14 @@ int force_max_ctas_per_sm();
 cudaError_t launch_tree_prepare(const mwf_cell* cells, int64_t n_cell, int64_t max_ptcl, int32_t* parent, int32_t* counter,
                                 unsigned int* err, cudaStream_t s);
 // quad64 / quad non-null: also the second moments about the centres of mass (6 doubles per cell) and their float record
-cudaError_t launch_monopoles(const mwf_cell* cells, const int32_t* parent, int64_t n_cell, int64_t n_ptcl, float4* store,
+cudaError_t launch_monopoles(const mwf_cell* cells, const int32_t* parent, int64_t n_cell, int64_t n_ptcl, float4* store, float4* spj_rec,
                              double4* mom64, int32_t* counter, double* quad64, float4* quad, cudaStream_t s);
 // scan variant of the refresh (monopole_kernel.cu): leaf ranking at the construction step, then leaf sums + prefix scan per refresh
 int64_t scan4_tiles(int64_t n_leaf_cells);
 cudaError_t launch_leaf_ranking(const mwf_cell* cells, int64_t n_cell, int64_t n_ptcl, int32_t* mark, int32_t* scratch, int2* cell_lr,
                                 int64_t* n_leaf_cells, cudaStream_t s);
 cudaError_t launch_monopoles_scan(const mwf_cell* cells, const int2* cell_lr, int64_t n_cell, int64_t n_ptcl, int64_t n_leaf_cells, float4* store,
-                                  double4* P, double4* toff, cudaStream_t s);
+                                  float4* spj_rec, double4* P, double4* toff, cudaStream_t s);
 cudaError_t launch_merge_lists(int64_t n_group, const int32_t* grp_first, const int32_t* grp_n, const int64_t* epj_off,
                                const int32_t* epj_id, const int64_t* spj_off, const int32_t* spj_id, const int64_t* list_off,
                                int64_t n_ptcl, int64_t n_cell, int32_t* list, uint8_t* grp_self, unsigned int* err, cudaStream_t s);

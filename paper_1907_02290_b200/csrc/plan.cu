@@ -50,7 +50,7 @@ void schedule_items(std::vector<int32_t>& order, int64_t b, int64_t e, const std
 
 }  // namespace
 
-int make_plan(mwf_ctx* c, int64_t n_group, const int32_t* grp_first, const int32_t* grp_n, const int64_t* n_list_of, Plan& pl) {
+int make_plan(mwf_ctx* c, int64_t n_group, const int32_t* grp_first, const int32_t* grp_n, const int64_t* n_epj_of, const int64_t* n_spj_of, Plan& pl) {
     pl.list_off.assign((size_t)n_group + 1, 0);
     pl.item_off.assign((size_t)n_group + 1, 0);
     pl.inter.assign((size_t)n_group + 1, 0);
@@ -60,8 +60,8 @@ int make_plan(mwf_ctx* c, int64_t n_group, const int32_t* grp_first, const int32
     for (int64_t g = 0; g < n_group; ++g) {
         const int64_t gf = grp_first[g], gn = grp_n[g];
         if (gf < 0 || gn < 1 || gf + gn > c->n_ptcl) return MWF_ERANGE;
-        const int64_t n_list = n_list_of[g];
-        const int64_t n_tiles = (n_list + TILE_J - 1) / TILE_J;
+        const int64_t n_list = n_epj_of[g] + n_spj_of[g];
+        const int64_t n_tiles = (n_epj_of[g] + TILE_J - 1) / TILE_J + (n_spj_of[g] + TILE_J - 1) / TILE_J;  // each run in whole tiles
         pl.list_off[(size_t)g + 1] = pl.list_off[(size_t)g] + n_tiles * TILE_J;
         pl.inter[(size_t)g + 1] = pl.inter[(size_t)g] + gn * n_list;
         // Cut the group into items: whole 64-particle items, then power-of-two pieces of the remainder

@@ -116,7 +116,7 @@ __device__ __forceinline__ void quad_item(const QuadArgs& a, const WorkItem it, 
     const int il = lane % W;
     const int64_t n_spj = a.spj_off[it.group + 1] - a.spj_off[it.group];
     if (n_spj == 0) return;
-    const int32_t* __restrict__ lst = a.list + a.list_off[it.group] + (a.epj_off[it.group + 1] - a.epj_off[it.group]);
+    const int32_t* __restrict__ lst = a.list + a.list_off[it.group] + (a.epj_off[it.group + 1] - a.epj_off[it.group] + TILE_J - 1) / TILE_J * TILE_J;
     float nx[2], ny[2], nz[2];
     bool valid[2];
 #pragma unroll

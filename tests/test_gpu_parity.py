@@ -373,8 +373,10 @@ def test_coincident_particles():
 # ------------------------------------------------------------------ method G1: data lists (NEXT-3; Fig. 2)
 def test_data_lists_equal_index_lists():
     """The paper's method G1 (the lists carry j records, sent with every dispatch) against its method G2 (indices into
-    the device store) on the same lists: same sweep and summation order, so the results are bitwise equal; and both
-    match the oracle."""
+    the device store) on the same lists: same items, sweep and summation order.  The 16-byte records of G1 hold
+    the SPJ centres rounded to fp32, the index path also reads their rounding remainders (reading S11b), so the two agree
+    bitwise on lists without SPJ entries and to the oracle's tolerance otherwise; G1 is bitwise the same however it is
+    batched."""
     cfg = CONFIGS[1]
     w = make_workload(cfg, 60001)
     out_idx, f = gpu_eval(w, cfg.eps, keep=True)
@@ -395,9 +397,10 @@ def test_data_lists_equal_index_lists():
         tag = (tag + 1) % f.n_tag
     for t in pending:
         f.retrieve(t, out)
-    assert np.array_equal(out, out_idx)
     acc, pot, _ = oracle_eval(w, cfg.eps)
     check(out, acc, pot, label="G1 data lists")
+    check(out_idx, acc, pot, label="G2 index lists")
+    assert np.abs(out - out_idx).max() <= 1e-4 * np.abs(out_idx).max()
     # device-resident records, one dispatch over everything
     import torch
     rec, joff = pack_data_lists(w, 0, w.n_group, w.posm, spj)
@@ -406,13 +409,24 @@ def test_data_lists_equal_index_lists():
     f.dispatch_data(1, 0, w.n_group, torch.from_numpy(rec).cuda(), joff)
     assert expect_code(f.dispatch_data, 1, 0, 1, rec, joff[:2].copy()) == binding.ESTATE              # tag still in flight
     f.retrieve(1, out2)
-    assert np.array_equal(out2, out_idx)
+    assert np.array_equal(out2, out)
     bad = joff.copy()
     bad[1] += 1
     assert expect_code(f.dispatch_data, 0, 0, w.n_group, rec, bad) == binding.ERANGE                  # run length != list length
     f.reserve_data_lists(10)
     assert expect_code(f.dispatch_data, 0, 0, w.n_group, rec, joff) == binding.ENOMEM
     f.close()
+    # lists without SPJ entries (theta = 0: every particle is an EPJ of every group): bitwise the index path
+    w0 = make_workload(cfg, 3000, theta=0.0)
+    assert w0.spj_id.size == 0
+    idx0, f = gpu_eval(w0, cfg.eps, keep=True)
+    rec, joff = pack_data_lists(w0, 0, w0.n_group, w0.posm, np.zeros((w0.n_cell, 4), np.float32))
+    f.reserve_data_lists(rec.shape[0])
+    dat0 = np.full((w0.n, 4), np.nan, np.float32)
+    f.dispatch_data(0, 0, w0.n_group, rec, joff)
+    f.retrieve(0, dat0)
+    f.close()
+    assert np.array_equal(idx0, dat0)
 
 
 # ------------------------------------------------------------------ quadrupole SPJ (NEXT-3, reading S22)
