@@ -802,6 +802,47 @@ def main():
     except binding.MwfError as ex:
         dev_build = {"error": str(ex)}
 
+    # ---- the whole run in the paper's sense (its 27 % of peak is the WHOLE step averaged over the reuse interval;
+    # construction step 0.42 s, reuse step 0.095 s): from unsorted particles and velocities resident on the device,
+    # one device-side construction step (sort, tree, groups, lists) + its evaluation, then n_reuse device-resident reuse
+    # steps, all inside one timed region; nothing crosses the host link.
+    whole_run = None
+    if w.vel is not None and cfg.dt > 0 and cfg.n_reuse > 0 and dev_build and "error" not in dev_build:
+        try:
+            from paper_1907_02290_b200.workload import make_particles
+            posm0, vel0 = make_particles(cfg, args.n)
+            p_dev = torch.from_numpy(posm0).to(f.device)
+            v4 = np.zeros((w.n, 4), np.float32)
+            v4[:, :3] = vel0
+            v_dev = torch.from_numpy(v4).to(f.device)
+            s0 = f.streams[0]
+            runs = []
+            for rep in range(4):
+                f.begin_step(binding.MAKE_LIST_FOR_REUSE)
+                f.set_particles(p_dev, 0, w.n, s0)
+                f.set_velocities(v_dev, 0, w.n, s0)
+                torch.cuda.synchronize()
+                t0 = time.perf_counter()
+                f.build(w.n, cfg.n_leaf, cfg.n_grp, cfg.theta, binding.MAKE_LIST_FOR_REUSE, s0)
+                t1 = time.perf_counter()
+                f.refresh_monopoles(s0)
+                f.dispatch(0, 0, w.n_group)
+                for _ in range(cfg.n_reuse):
+                    f.step_reuse(cfg.dt)
+                f.retrieve(0, None)
+                torch.cuda.synchronize()
+                t2 = time.perf_counter()
+                if rep > 0:
+                    runs.append((t2 - t0, t1 - t0))
+            tot = float(np.median([r[0] for r in runs]))
+            n_eval = cfg.n_reuse + 1
+            whole_run = {"evaluations": n_eval, "n_reuse": cfg.n_reuse, "total_ms": 1e3 * tot, "construction_ms": 1e3 * float(np.median([r[1] for r in runs])),
+                         "ms_per_step": 1e3 * tot / n_eval, "value": inter * n_eval / tot, "unit": UNIT,
+                         "timing": "host wall clock around the whole run, median of 3 after one warm-up; inputs resident in HBM, no host transfer",
+                         "what": "mwf_build from unsorted particles + evaluation, then %d x mwf_step_reuse (kick-drift, refresh, force, kick)" % cfg.n_reuse}
+        except binding.MwfError as ex:
+            whole_run = {"error": str(ex)}
+
     if rank == 0:
         peaks = measured_peaks()
         clk = clocks.summary()
@@ -821,6 +862,9 @@ def main():
                     traffic, traffic_source = float(parts[1]), "ncu capture, not this run: " + note.strip()
         except (OSError, ValueError):
             pass
+        if whole_run and "error" not in whole_run:
+            whole_run["frac_fp32_peak"] = whole_run["value"] * N_OP / 1e12 / peak_tflops
+            whole_run["context"] = "paper: 27 % of peak for the whole step on a TITAN V (P:673), construction 0.42 s vs reuse 0.095 s (P:716)"
         roof = {"bound": "alu", "kernel": "mwf::k_force", "achieved": achieved, "peak": peak_tflops, "unit": "TFLOP/s",
                 "frac": achieved / peak_tflops, "traffic": traffic, "traffic_source": traffic_source, "kernel_ms": k_ms,
                 "kernel_ms_median": float(np.median(kernel_ms)), "kernel_ms_min": float(min(kernel_ms)),
@@ -847,6 +891,7 @@ def main():
                                   "ms_per_step": ms_e_max / args.steps,
                                   "what": "one blocking mwf_calc_force_all per step, pinned host source and destination (the H2D cannot overlap the kernels)"},
             "gpu_launches": launches, "clocks": clk, "phases": phases, "device_resident_step": dev_res, "batched_dispatch": batched,
+            "run_n_reuse_%d" % max(cfg.n_reuse, 0): whole_run,
             "construction_step": {"host_tree_and_lists_s": round(t_build, 3), "upload_tree_and_lists_s": round(t_upload, 3), "on_device": dev_build},
             "context": {"paper_fraction_of_peak": 0.27, "paper_hardware": "TITAN V (P:673), whole step"},
         }

@@ -117,8 +117,12 @@ int mwf_step_reuse(mwf_ctx* c, float dt) {
     c->groups_outstanding -= c->tag_groups[0];
     c->tag_groups[0] = 0;
     c->tag_ranges[0].clear();
+    const bool fused = c->spj_order == 1;  // the closing kick rides in the force kernel's epilogue (with quadrupoles a second
+    c->fuse_kick_h = fused ? 0.5f * dt : 0.f;  // kernel still adds to the result, so the kick stays a pass of its own)
     rc = mwf_dispatch(c, 0, 0, c->n_group);
+    c->fuse_kick_h = 0.f;
     if (rc) return rc;
+    if (fused) return MWF_OK;
     return mwf_kick(c, dt, s0);
 }
 

@@ -68,6 +68,8 @@ static int dispatch_launch(mwf_ctx* c, int32_t tag, int64_t g_begin, int64_t g_e
     a.n_items = c->h_item_off[(size_t)g_end] - a.item_begin;
     a.eps2 = c->p.eps * c->p.eps;
     a.G = c->p.G;
+    a.vel = (c->fuse_kick_h != 0.f && !jdata && c->spj_order == 1) ? c->vel : nullptr;
+    a.kick_h = c->fuse_kick_h;
     {
         const int rc = pick_order(c, g_begin, g_end, s, &a.order);
         if (rc) return rc;

@@ -218,8 +218,16 @@ __device__ __forceinline__ void run_item(const ForceArgs& a, const WorkItem it, 
             rz += __shfl_xor_sync(0xffffffffu, rz, m);
             rp += __shfl_xor_sync(0xffffffffu, rp, m);
         }
-        if (valid[k] && sl == 0)
-            a.accp[it.i_first + il + W * k] = make_float4(a.G * rx, a.G * ry, a.G * rz, -a.G * rp);
+        if (valid[k] && sl == 0) {
+            const int64_t i = it.i_first + il + W * k;
+            const float4 r = make_float4(a.G * rx, a.G * ry, a.G * rz, -a.G * rp);
+            a.accp[i] = r;
+            if (a.vel) {  // device-resident step: the closing kick of the leapfrog, the arithmetic of k_kick bit for bit
+                float4 v = a.vel[i];
+                v.x = fmaf(r.x, a.kick_h, v.x); v.y = fmaf(r.y, a.kick_h, v.y); v.z = fmaf(r.z, a.kick_h, v.z);
+                a.vel[i] = v;
+            }
+        }
     }
     __syncwarp();  // the next item reuses the warp's tile buffers
 }

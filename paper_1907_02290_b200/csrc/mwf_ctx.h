@@ -33,6 +33,7 @@ struct mwf_ctx {
     int2* cell_lr = nullptr;      // [max_cell] range of leaf ranks of every cell (scan variant of the refresh)
     double4* leaf_P = nullptr;    // [max_cell + 1] leaves' moments in rank order, scanned in place every refresh
     double4* leaf_toff = nullptr; // [tiles] scanned tile totals
+    float fuse_kick_h = 0.f;      // mwf_step_reuse: the closing kick rides in the force kernel's epilogue (0: no kick)
     int64_t n_leaf_cells = 0;
     int32_t* grp_first = nullptr; // [max_group]
     int32_t* grp_n = nullptr;     // [max_group]

@@ -66,6 +66,8 @@ struct ForceArgs {
     int64_t n_items;
     float eps2;
     float G;
+    float4* vel;                // non-null: the closing kick of the leapfrog in the epilogue, v += acc * kick_h (NEXT-1)
+    float kick_h;
 };
 
 // Quadrupole correction of the SPJ entries (NEXT-3, quad_kernel.cu): same items and schedule as the force kernel.
