@@ -252,8 +252,10 @@ int mwf_get_tag_split(mwf_ctx* c, int64_t* bounds);
  * builder's): cube root cell padded by 2^-10, 21 key bits per axis, leaf = at most n_leaf particles, group =
  * first cell on a root path with at most n_grp particles, open iff cell side > theta x distance from the cell
  * centre to the group's particle bounding box.  theta in [0, 1].  Results of the previous step must have been
- * retrieved (MWF_ESTATE otherwise).  MWF_ENOMEM when max_cell / max_group / max_entry are too small.  Blocking
- * (a few stream synchronisations to size the levels and the lists). */
+ * retrieved (MWF_ESTATE otherwise).  MWF_ENOMEM when max_cell / max_group / max_entry are too small; the particles
+ * (velocities, SPH records) have then already been sorted in place, so they count as not uploaded any more: upload them
+ * again before the next attempt.  Blocking (stream synchronisations to size the tree levels, after the counting walk and
+ * at the end; the host cuts and schedules the work items while the device walks the tree). */
 int mwf_build(mwf_ctx* c, int64_t n, int32_t n_leaf, int32_t n_grp, double theta, int mode, void* stream);
 /* The same construction step for the short-range workload (NEXT-4): the list walk uses the neighbour-search criterion
  * of reading S24 instead of the opening angle -- a cell is opened iff the gap between its cube and the group's particle

@@ -7,6 +7,15 @@
 using namespace mwf;
 
 // The device-side construction step behind mwf_build (opening angle theta) and mwf_build_neighbours (search radii 2 (1 + skin) h).
+// The construction step failed after the particles (and velocities, SPH records) were sorted in place: what the store
+// holds is a permutation the caller cannot name, so it counts as not uploaded (the caller uploads again before retrying).
+static int build_failed(mwf_ctx* c, cudaStream_t s, int code) {
+    after_store_op(c, s);
+    c->ptcl_hi = c->vel_hi = c->sph_hi = 0;
+    c->n_ptcl = 0;
+    return code;
+}
+
 static int build_impl(mwf_ctx* c, int64_t n, int32_t n_leaf, int32_t n_grp, double theta, bool neighbours, double skin, int mode, void* stream) {
     if (!c || n < 1 || n_leaf < 1 || n_grp < 1) return MWF_EINVAL;
     if (neighbours ? !(skin >= 0.0) : (!(theta >= 0.0) || theta > 1.0)) return MWF_EINVAL;
@@ -32,18 +41,24 @@ static int build_impl(mwf_ctx* c, int64_t n, int32_t n_leaf, int32_t n_grp, doub
     CU(c, build_tree_device(c->bb, n, n_leaf, n_grp, c->p.max_cell, c->p.max_group, with_vel, sph, &n_cell, &n_group, &n_level, s));
     c->n_launch += 8 + 3 * 8 + 3 * n_level;
     tm.lap("sort + tree + groups");
-    if (n_cell > c->p.max_cell || n_group > c->p.max_group) { after_store_op(c, s); return MWF_ENOMEM; }
-    unsigned int e = 0;
-    rc = read_err_word(c, s, &e);
-    if (rc) return rc;
-    if (e) { after_store_op(c, s); return MWF_ENOMEM; }
+    if (n_cell > c->p.max_cell || n_group > c->p.max_group) return build_failed(c, s, MWF_ENOMEM);
+    // Everything up to the counting walk is enqueued without a host synchronisation; small results travel to pinned host
+    // memory on the stream.  The group ranges come first, so that the host cuts the groups into work items while the
+    // device ranks the leaves and walks the tree.
+    const auto D2H = cudaMemcpyDeviceToHost;
+    int32_t *h_first = c->h_groups, *h_n = h_first + n_group, *h_ne = h_n + n_group, *h_ns = h_ne + n_group;
+    int64_t* totals = c->h_scalars;                                          // [0..2] padded, EPJ, SPJ entries
+    int32_t* n_leaf_pinned = reinterpret_cast<int32_t*>(c->h_scalars + 4);
+    unsigned int* err_pinned = reinterpret_cast<unsigned int*>(c->h_scalars + 5);
+    CU(c, cudaMemcpyAsync(h_first, c->grp_first, (size_t)n_group * 4, D2H, s));
+    CU(c, cudaMemcpyAsync(h_n, c->grp_n, (size_t)n_group * 4, D2H, s));
+    CU(c, cudaEventRecord(c->ev_groups, s));
     // tree state as mwf_set_tree leaves it: arrival counters zero, leaves ranked, dummy record behind the SPJ block
     CU(c, cudaMemsetAsync(c->arrive, 0, (size_t)n_cell * 4, s));
-    CU(c, launch_leaf_ranking(c->cells, n_cell, n, c->bb.mark, c->bb.scan_scratch, c->cell_lr, &c->n_leaf_cells, s));
+    CU(c, launch_leaf_ranking(c->cells, n_cell, n, c->bb.mark, c->bb.scan_scratch, c->cell_lr, n_leaf_pinned, s));
     c->n_launch += 5;
-    const float4 zero = make_float4(0.f, 0.f, 0.f, 0.f);
-    CU(c, cudaMemcpyAsync(c->store + n + n_cell, &zero, 16, cudaMemcpyHostToDevice, s));
-    CU(c, cudaMemcpyAsync(c->store_next + n + n_cell, &zero, 16, cudaMemcpyHostToDevice, s));
+    CU(c, cudaMemsetAsync(c->store + n + n_cell, 0, 16, s));
+    CU(c, cudaMemsetAsync(c->store_next + n + n_cell, 0, 16, s));
     CU(c, cudaMemsetAsync(c->spj_rec + 2 * n_cell, 0, 32, s));
     c->next_ranges.clear();
     c->next_streams.clear();
@@ -51,7 +66,6 @@ static int build_impl(mwf_ctx* c, int64_t n, int32_t n_leaf, int32_t n_grp, doub
     c->n_cell = n_cell;
     c->ptcl_hi = n;
     // lists: counting walk, offsets, capacity check, fill walk
-    int64_t padded = 0, e_epj = 0, e_spj = 0;
     WalkRule rule;
     rule.theta = theta;
     if (neighbours) {  // per-cell and per-group search radii; level_cnt and mark are free once the tree and the groups exist
@@ -62,32 +76,36 @@ static int build_impl(mwf_ctx* c, int64_t n, int32_t n_leaf, int32_t n_grp, doub
         CU(c, build_smoothing_reach(c->bb, c->sph, n_cell, n_group, reinterpret_cast<float*>(c->bb.level_cnt), reinterpret_cast<float*>(c->bb.mark), s));
         c->n_launch += 2;
     }
-    CU(c, build_lists_count(c->bb, n_group, rule, c->walk_warps_n, &padded, &e_epj, &e_spj, s));
-    tm.lap("list walk: count + offsets");
-    if (e_epj + e_spj > c->p.max_entry) { after_store_op(c, s); return MWF_ENOMEM; }
-    // group sizes and list lengths come back for the host work plan; the fill walk runs meanwhile
-    std::vector<int32_t> h_first((size_t)n_group), h_n((size_t)n_group), h_ne((size_t)n_group), h_ns((size_t)n_group);
-    const auto D2H = cudaMemcpyDeviceToHost;
-    CU(c, cudaMemcpyAsync(h_first.data(), c->grp_first, (size_t)n_group * 4, D2H, s));
-    CU(c, cudaMemcpyAsync(h_n.data(), c->grp_n, (size_t)n_group * 4, D2H, s));
-    CU(c, cudaMemcpyAsync(h_ne.data(), c->bb.n_epj, (size_t)n_group * 4, D2H, s));
-    CU(c, cudaMemcpyAsync(h_ns.data(), c->bb.n_spj, (size_t)n_group * 4, D2H, s));
+    CU(c, build_lists_count(c->bb, n_group, rule, c->walk_warps_n, totals, s));
+    CU(c, cudaMemcpyAsync(h_ne, c->bb.n_epj, (size_t)n_group * 4, D2H, s));
+    CU(c, cudaMemcpyAsync(h_ns, c->bb.n_spj, (size_t)n_group * 4, D2H, s));
+    CU(c, cudaMemcpyAsync(err_pinned, c->err, sizeof(unsigned int), D2H, s));
+    // host, meanwhile: the work items
+    Plan plan;
+    CU(c, cudaEventSynchronize(c->ev_groups));
+    rc = plan_cut(c, n_group, h_first, h_n, plan);
+    tm.lap("host: cutting | leaf ranking + counting walk");
     CU(c, cudaStreamSynchronize(s));
+    tm.lap("counting walk: rest");
+    c->n_leaf_cells = *n_leaf_pinned;
+    if (rc) return build_failed(c, s, rc);
+    if (*err_pinned) return build_failed(c, s, MWF_ENOMEM);
+    const int64_t padded = totals[0], e_epj = totals[1], e_spj = totals[2];
+    if (e_epj + e_spj > c->p.max_entry) return build_failed(c, s, MWF_ENOMEM);
     CU(c, build_lists_fill(c->bb, n_group, rule, c->walk_warps_n, n, n_cell, s));
     CU(c, cudaMemsetAsync(c->grp_self, 1, (size_t)n_group, s));  // theta <= 1: a group's own cells are always opened
     c->n_launch += 6;
-    std::vector<int64_t> n_epj(h_ne.begin(), h_ne.end()), n_spj(h_ns.begin(), h_ns.end());
-    Plan plan;
-    rc = make_plan(c, n_group, h_first.data(), h_n.data(), n_epj.data(), n_spj.data(), plan);
-    tm.lap("host work plan | fill walk");
-    if (rc) { after_store_op(c, s); return rc; }
-    if (plan.list_off[(size_t)n_group] != padded) { after_store_op(c, s); return MWF_ERANGE; }  // host and device offsets must agree
+    // host, meanwhile: costs and schedules
+    rc = plan_finish(c, n_group, h_n, h_ne, h_ns, plan);
+    tm.lap("host: schedule | fill walk");
+    if (rc) return build_failed(c, s, rc);
+    if (plan.list_off[(size_t)n_group] != padded) return build_failed(c, s, MWF_ERANGE);  // host and device offsets must agree
     const int64_t n_items = (int64_t)plan.items.size();
     const auto H2D = cudaMemcpyHostToDevice;
     CU(c, cudaMemcpyAsync(c->items, plan.items.data(), (size_t)n_items * sizeof(WorkItem), H2D, s));
     CU(c, cudaMemcpyAsync(c->order_full, plan.order_full.data(), (size_t)n_items * 4, H2D, s));
     CU(c, cudaStreamSynchronize(s));  // the plan's host vectors die with this call
-    tm.lap("plan upload");
+    tm.lap("fill walk: rest + plan upload");
     rc = after_store_op(c, s);
     if (rc) return rc;
     c->have_tree = true;
@@ -95,7 +113,7 @@ static int build_impl(mwf_ctx* c, int64_t n, int32_t n_leaf, int32_t n_grp, doub
     c->build_e_epj = e_epj;
     c->build_e_spj = e_spj;
     c->build_n_level = n_level;
-    adopt_plan(c, plan, n_group, h_first.data(), h_n.data(), mode);
+    adopt_plan(c, plan, n_group, h_first, h_n, mode);
     return MWF_OK;
 }
 

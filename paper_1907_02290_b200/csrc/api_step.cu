@@ -225,7 +225,8 @@ int mwf_set_tree(mwf_ctx* c, const mwf_cell* cells, int64_t n_cell, void* stream
         if (rc) return rc;
         if (e0) { after_store_op(c, s); return MWF_ERANGE; }
     }
-    CU(c, launch_leaf_ranking(c->cells, n_cell, n, c->bb.mark, c->bb.scan_scratch, c->cell_lr, &c->n_leaf_cells, s));
+    int32_t* n_leaf_pinned = reinterpret_cast<int32_t*>(c->h_scalars);
+    CU(c, launch_leaf_ranking(c->cells, n_cell, n, c->bb.mark, c->bb.scan_scratch, c->cell_lr, n_leaf_pinned, s));
     c->n_launch += 5;
     // zero-mass dummy record behind the SPJ block: what list padding points at
     const float4 zero = make_float4(0.f, 0.f, 0.f, 0.f);
@@ -235,8 +236,9 @@ int mwf_set_tree(mwf_ctx* c, const mwf_cell* cells, int64_t n_cell, void* stream
     c->next_ranges.clear();
     c->next_streams.clear();
     unsigned int e = 0;
-    rc = read_err_word(c, s, &e);
+    rc = read_err_word(c, s, &e);  // synchronises the stream: the number of leaves has arrived too
     if (rc) return rc;
+    c->n_leaf_cells = *n_leaf_pinned;
     rc = after_store_op(c, s);
     if (rc) return rc;
     if (e) return MWF_ERANGE;
@@ -260,12 +262,12 @@ int mwf_set_lists(mwf_ctx* c, int64_t n_group, const int32_t* grp_first, const i
     if ((e_epj > 0 && !epj_id) || (e_spj > 0 && !spj_id)) return MWF_EINVAL;
     if (e_epj + e_spj > c->p.max_entry) return MWF_ENOMEM;
     // host pass: offsets, items, schedule
-    std::vector<int64_t> n_epj((size_t)n_group), n_spj((size_t)n_group);
+    std::vector<int32_t> n_epj((size_t)n_group), n_spj((size_t)n_group);
     for (int64_t g = 0; g < n_group; ++g) {
         const int64_t ne = epj_off[g + 1] - epj_off[g], ns = spj_off[g + 1] - spj_off[g];
-        if (ne < 0 || ns < 0) return MWF_ERANGE;
-        n_epj[(size_t)g] = ne;
-        n_spj[(size_t)g] = ns;
+        if (ne < 0 || ns < 0 || ne > INT32_MAX || ns > INT32_MAX) return MWF_ERANGE;
+        n_epj[(size_t)g] = (int32_t)ne;
+        n_spj[(size_t)g] = (int32_t)ns;
     }
     Plan plan;
     {

@@ -210,8 +210,8 @@ int64_t walk_warps(int64_t max_group) {
     return max_group < cap ? (max_group < 8 ? 8 : (max_group + 7) / 8 * 8) : cap;
 }
 
-// Counting pass + offsets.  Leaves list_off / epj_off / spj_off scanned (n_group + 1 entries each) and returns the
-// totals through *padded / *e_epj / *e_spj (one stream synchronisation).
+// Counting pass + offsets.  Leaves list_off / epj_off / spj_off scanned (n_group + 1 entries each); the totals go to pinned
+// host memory on the stream (no synchronisation here).
 cudaError_t build_smoothing_reach(const BuildBuffers& b, const float4* sph, int64_t n_cell, int64_t n_group, float* cell_h, float* grp_h, cudaStream_t s) {
     BL(cudaMemsetAsync(cell_h, 0, (size_t)n_cell * 4, s));
     k_cell_hmax<<<(unsigned)((n_cell + 255) / 256), 256, 0, s>>>(b.cells, b.parent, sph, n_cell, reinterpret_cast<int*>(cell_h));
@@ -220,8 +220,7 @@ cudaError_t build_smoothing_reach(const BuildBuffers& b, const float4* sph, int6
     return cudaGetLastError();
 }
 
-cudaError_t build_lists_count(const BuildBuffers& b, int64_t n_group, const WalkRule& rule, int64_t n_warps, int64_t* padded, int64_t* e_epj, int64_t* e_spj,
-                              cudaStream_t s) {
+cudaError_t build_lists_count(const BuildBuffers& b, int64_t n_group, const WalkRule& rule, int64_t n_warps, int64_t* totals_pinned, cudaStream_t s) {
     const double th2 = rule.theta * rule.theta;
     BL(cudaMemsetAsync(b.walk_counter, 0, 4, s));
     if (rule.neighbours)
@@ -236,14 +235,9 @@ cudaError_t build_lists_count(const BuildBuffers& b, int64_t n_group, const Walk
     BL(scan_exclusive<int64_t>(b.list_off, n_group + 1, b.scan_scratch64, s));
     BL(scan_exclusive<int64_t>(b.epj_off, n_group + 1, b.scan_scratch64, s));
     BL(scan_exclusive<int64_t>(b.spj_off, n_group + 1, b.scan_scratch64, s));
-    int64_t h[3] = {0, 0, 0};
-    BL(cudaMemcpyAsync(&h[0], b.list_off + n_group, 8, cudaMemcpyDeviceToHost, s));
-    BL(cudaMemcpyAsync(&h[1], b.epj_off + n_group, 8, cudaMemcpyDeviceToHost, s));
-    BL(cudaMemcpyAsync(&h[2], b.spj_off + n_group, 8, cudaMemcpyDeviceToHost, s));
-    BL(cudaStreamSynchronize(s));
-    *padded = h[0];
-    *e_epj = h[1];
-    *e_spj = h[2];
+    BL(cudaMemcpyAsync(totals_pinned + 0, b.list_off + n_group, 8, cudaMemcpyDeviceToHost, s));
+    BL(cudaMemcpyAsync(totals_pinned + 1, b.epj_off + n_group, 8, cudaMemcpyDeviceToHost, s));
+    BL(cudaMemcpyAsync(totals_pinned + 2, b.spj_off + n_group, 8, cudaMemcpyDeviceToHost, s));
     return cudaSuccess;
 }
 

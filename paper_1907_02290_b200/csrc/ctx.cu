@@ -261,6 +261,9 @@ int mwf_create(mwf_ctx** out, const mwf_params* p, void* arena, int64_t arena_by
     ok = ok && cudaEventCreateWithFlags(&c->ev_next, cudaEventDisableTiming) == cudaSuccess;
     ok = ok && cudaMemset(c->counters, 0, N_COUNTER * 4) == cudaSuccess;
     ok = ok && cudaMemset(c->err, 0, 256) == cudaSuccess;
+    ok = ok && cudaHostAlloc(reinterpret_cast<void**>(&c->h_scalars), 16 * sizeof(int64_t), cudaHostAllocDefault) == cudaSuccess;
+    ok = ok && cudaHostAlloc(reinterpret_cast<void**>(&c->h_groups), (size_t)p->max_group * 4 * sizeof(int32_t), cudaHostAllocDefault) == cudaSuccess;
+    ok = ok && cudaEventCreateWithFlags(&c->ev_groups, cudaEventDisableTiming) == cudaSuccess;
     if (!ok) { mwf_destroy(c); return MWF_ECUDA; }
     *out = c;
     return MWF_OK;
@@ -278,6 +281,9 @@ int mwf_destroy(mwf_ctx* c) {
         if (c->ev_k1[t]) cudaEventDestroy(c->ev_k1[t]);
         if (c->ev_kq[t]) cudaEventDestroy(c->ev_kq[t]);
     }
+    if (c->h_scalars) cudaFreeHost(c->h_scalars);
+    if (c->h_groups) cudaFreeHost(c->h_groups);
+    if (c->ev_groups) cudaEventDestroy(c->ev_groups);
     if (c->quad64) cudaFree(c->quad64);
     if (c->quad) cudaFree(c->quad);
     if (c->ev_store) cudaEventDestroy(c->ev_store);

@@ -336,9 +336,10 @@ namespace mwf {
 int64_t scan4_tiles(int64_t n_leaf_cells) { return (n_leaf_cells + 1 + SCAN4_TILE - 1) / SCAN4_TILE; }
 
 // Construction step: rank the leaves in Morton order and give every cell its range of leaf ranks.  mark: n_ptcl + 1
-// ints of scratch (left holding the ranks), scratch: scan scratch for n_ptcl + 1 ints.  *n_leaf_cells through a stream sync.
+// ints of scratch (left holding the ranks), scratch: scan scratch for n_ptcl + 1 ints.  The number of leaves is copied to
+// *n_leaf_pinned (pinned host memory) on the stream: valid once the caller has synchronised it.
 cudaError_t launch_leaf_ranking(const mwf_cell* cells, int64_t n_cell, int64_t n_ptcl, int32_t* mark, int32_t* scratch, int2* cell_lr,
-                                int64_t* n_leaf_cells, cudaStream_t s) {
+                                int32_t* n_leaf_pinned, cudaStream_t s) {
     cudaError_t e = cudaMemsetAsync(mark, 0, (size_t)(n_ptcl + 1) * 4, s);
     if (e != cudaSuccess) return e;
     k_leaf_mark<<<(unsigned)((n_cell + 255) / 256), 256, 0, s>>>(cells, n_cell, mark);
@@ -346,11 +347,7 @@ cudaError_t launch_leaf_ranking(const mwf_cell* cells, int64_t n_cell, int64_t n
     if ((e = scan_exclusive<int32_t>(mark, n_ptcl + 1, scratch, s)) != cudaSuccess) return e;
     k_leaf_ranges<<<(unsigned)((n_cell + 255) / 256), 256, 0, s>>>(cells, n_cell, mark, cell_lr);
     if ((e = cudaGetLastError()) != cudaSuccess) return e;
-    int32_t nl = 0;
-    if ((e = cudaMemcpyAsync(&nl, mark + n_ptcl, 4, cudaMemcpyDeviceToHost, s)) != cudaSuccess) return e;
-    if ((e = cudaStreamSynchronize(s)) != cudaSuccess) return e;
-    *n_leaf_cells = nl;
-    return cudaSuccess;
+    return cudaMemcpyAsync(n_leaf_pinned, mark + n_ptcl, 4, cudaMemcpyDeviceToHost, s);
 }
 
 cudaError_t launch_monopoles_scan(const mwf_cell* cells, const int2* cell_lr, int64_t n_cell, int64_t n_ptcl, int64_t n_leaf_cells, float4* store,

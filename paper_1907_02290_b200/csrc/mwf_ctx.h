@@ -33,6 +33,9 @@ struct mwf_ctx {
     int2* cell_lr = nullptr;      // [max_cell] range of leaf ranks of every cell (scan variant of the refresh)
     double4* leaf_P = nullptr;    // [max_cell + 1] leaves' moments in rank order, scanned in place every refresh
     double4* leaf_toff = nullptr; // [tiles] scanned tile totals
+    int64_t* h_scalars = nullptr; // pinned: small results of the construction step (counts, totals, validation word)
+    int32_t* h_groups = nullptr;  // pinned [4 x max_group]: group ranges and list lengths on their way to the host work plan
+    cudaEvent_t ev_groups{};      // the group ranges have arrived
     float fuse_kick_h = 0.f;      // mwf_step_reuse: the closing kick rides in the force kernel's epilogue (0: no kick)
     int64_t n_leaf_cells = 0;
     int32_t* grp_first = nullptr; // [max_group]
@@ -140,7 +143,9 @@ struct Plan {
     std::vector<int64_t> cost;
     std::vector<int32_t> order_full;
 };
-int make_plan(mwf_ctx* c, int64_t n_group, const int32_t* grp_first, const int32_t* grp_n, const int64_t* n_epj_of, const int64_t* n_spj_of, Plan& pl);
+int plan_cut(mwf_ctx* c, int64_t n_group, const int32_t* grp_first, const int32_t* grp_n, Plan& pl);
+int plan_finish(mwf_ctx* c, int64_t n_group, const int32_t* grp_n, const int32_t* n_epj_of, const int32_t* n_spj_of, Plan& pl);
+int make_plan(mwf_ctx* c, int64_t n_group, const int32_t* grp_first, const int32_t* grp_n, const int32_t* n_epj_of, const int32_t* n_spj_of, Plan& pl);
 void adopt_plan(mwf_ctx* c, Plan& pl, int64_t n_group, const int32_t* grp_first, const int32_t* grp_n, int mode);
 int ensure_split_order(mwf_ctx* c, cudaStream_t s);
 

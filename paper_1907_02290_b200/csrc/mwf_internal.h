@@ -121,7 +121,7 @@ cudaError_t launch_monopoles(const mwf_cell* cells, const int32_t* parent, int64
 // scan variant of the refresh (monopole_kernel.cu): leaf ranking at the construction step, then leaf sums + prefix scan per refresh
 int64_t scan4_tiles(int64_t n_leaf_cells);
 cudaError_t launch_leaf_ranking(const mwf_cell* cells, int64_t n_cell, int64_t n_ptcl, int32_t* mark, int32_t* scratch, int2* cell_lr,
-                                int64_t* n_leaf_cells, cudaStream_t s);
+                                int32_t* n_leaf_pinned, cudaStream_t s);
 cudaError_t launch_monopoles_scan(const mwf_cell* cells, const int2* cell_lr, int64_t n_cell, int64_t n_ptcl, int64_t n_leaf_cells, float4* store,
                                   float4* spj_rec, double4* P, double4* toff, cudaStream_t s);
 cudaError_t launch_merge_lists(int64_t n_group, const int32_t* grp_first, const int32_t* grp_n, const int64_t* epj_off,
@@ -154,8 +154,8 @@ struct WalkRule {
     const float* cell_h = nullptr;  // [n_cell] largest h among the cell's particles
     const float* grp_h = nullptr;   // [n_group]
 };
-cudaError_t build_lists_count(const BuildBuffers& b, int64_t n_group, const WalkRule& rule, int64_t n_warps, int64_t* padded, int64_t* e_epj, int64_t* e_spj,
-                              cudaStream_t s);
+// totals_pinned[0..2] (pinned host memory) = padded entries, EPJ entries, SPJ entries, valid once the stream has been synchronised
+cudaError_t build_lists_count(const BuildBuffers& b, int64_t n_group, const WalkRule& rule, int64_t n_warps, int64_t* totals_pinned, cudaStream_t s);
 cudaError_t build_lists_fill(const BuildBuffers& b, int64_t n_group, const WalkRule& rule, int64_t n_warps, int64_t n_ptcl, int64_t n_cell, cudaStream_t s);
 // cell_h / grp_h of a WalkRule from the h field of the SPH records (tree order)
 cudaError_t build_smoothing_reach(const BuildBuffers& b, const float4* sph, int64_t n_cell, int64_t n_group, float* cell_h, float* grp_h, cudaStream_t s);

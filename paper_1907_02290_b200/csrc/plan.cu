@@ -50,32 +50,48 @@ void schedule_items(std::vector<int32_t>& order, int64_t b, int64_t e, const std
 
 }  // namespace
 
-int make_plan(mwf_ctx* c, int64_t n_group, const int32_t* grp_first, const int32_t* grp_n, const int64_t* n_epj_of, const int64_t* n_spj_of, Plan& pl) {
-    pl.list_off.assign((size_t)n_group + 1, 0);
+// How a remainder of rem < 64 particles is cut: the widths of its pieces, widest first (0-terminated).  The remainder is
+// padded to a multiple of a quantum q and cut into power-of-two pieces; q is the quantum whose modelled cost is lowest (a
+// coarser quantum wastes lanes, a finer one re-stages the list for one more narrow item).  A table: the rule only depends
+// on rem.
+struct RemainderCut { int8_t width[6]; };
+static const RemainderCut* remainder_table() {
+    static RemainderCut table[CHUNK_I];
+    static const bool made = [] {
+        for (int64_t rem = 0; rem < CHUNK_I; ++rem) {
+            RemainderCut& rc = table[rem];
+            for (int8_t& w : rc.width) w = 0;
+            if (rem == 0) continue;
+            int64_t best_q = CHUNK_I, best_cost = INT64_MAX;
+            for (int64_t q = 2 * MIN_WIDTH; q <= CHUNK_I; q *= 2) {
+                const int64_t padded = (rem + q - 1) / q * q;
+                int64_t cst = 0;
+                for (int64_t piece = CHUNK_I; piece >= 2 * MIN_WIDTH; piece /= 2)
+                    if (padded & piece) cst += item_cost_per_tile((int)(piece / 2));
+                if (cst < best_cost) { best_cost = cst; best_q = q; }
+            }
+            const int64_t padded = (rem + best_q - 1) / best_q * best_q;
+            int k = 0;
+            for (int64_t piece = CHUNK_I; piece >= 2 * MIN_WIDTH; piece /= 2)
+                if (padded & piece) rc.width[k++] = (int8_t)(piece / 2);
+        }
+        return true;
+    }();
+    (void)made;
+    return table;
+}
+
+// First half of the plan: cutting every group into work items.  Needs the group ranges only, so a device-side construction
+// step runs it while its counting walk is still under way.
+int plan_cut(mwf_ctx* c, int64_t n_group, const int32_t* grp_first, const int32_t* grp_n, Plan& pl) {
     pl.item_off.assign((size_t)n_group + 1, 0);
-    pl.inter.assign((size_t)n_group + 1, 0);
     std::vector<WorkItem>& items = pl.items;
-    std::vector<int64_t>& cost = pl.cost;
+    items.clear();
     items.reserve((size_t)(c->n_ptcl / CHUNK_I + 3 * n_group));
+    const RemainderCut* cut = remainder_table();
     for (int64_t g = 0; g < n_group; ++g) {
         const int64_t gf = grp_first[g], gn = grp_n[g];
         if (gf < 0 || gn < 1 || gf + gn > c->n_ptcl) return MWF_ERANGE;
-        const int64_t n_list = n_epj_of[g] + n_spj_of[g];
-        const int64_t n_tiles = (n_epj_of[g] + TILE_J - 1) / TILE_J + (n_spj_of[g] + TILE_J - 1) / TILE_J;  // each run in whole tiles
-        pl.list_off[(size_t)g + 1] = pl.list_off[(size_t)g] + n_tiles * TILE_J;
-        pl.inter[(size_t)g + 1] = pl.inter[(size_t)g] + gn * n_list;
-        // Cut the group into items: whole 64-particle items, then power-of-two pieces of the remainder
-        // padded to a multiple of q; q is the quantum whose modelled cost is lowest (a coarser quantum
-        // wastes lanes, a finer one re-stages the list for one more narrow item).
-        const int64_t n_full = gn / CHUNK_I, rem = gn % CHUNK_I;
-        int64_t best_q = CHUNK_I, best_cost = INT64_MAX;
-        for (int64_t q = 2 * MIN_WIDTH; q <= CHUNK_I && rem > 0; q *= 2) {
-            const int64_t padded = (rem + q - 1) / q * q;
-            int64_t cst = 0;
-            for (int64_t piece = CHUNK_I; piece >= 2 * MIN_WIDTH; piece /= 2)
-                if (padded & piece) cst += item_cost_per_tile((int)(piece / 2));
-            if (cst < best_cost) { best_cost = cst; best_q = q; }
-        }
         int64_t done = 0;
         auto emit = [&](int64_t n_i, int width) {
             WorkItem it;
@@ -85,18 +101,32 @@ int make_plan(mwf_ctx* c, int64_t n_group, const int32_t* grp_first, const int32
             it.width = width;
             done += n_i;
             items.push_back(it);
-            cost.push_back(n_tiles * item_cost_per_tile(width));
         };
-        for (int64_t k = 0; k < n_full; ++k) emit(CHUNK_I, CHUNK_I / 2);
-        if (rem > 0) {
-            const int64_t padded = (rem + best_q - 1) / best_q * best_q;
-            for (int64_t piece = CHUNK_I; piece >= 2 * MIN_WIDTH; piece /= 2)
-                if (padded & piece) emit(std::min(piece, gn - done), (int)(piece / 2));
-        }
+        for (int64_t k = 0; k < gn / CHUNK_I; ++k) emit(CHUNK_I, CHUNK_I / 2);
+        const RemainderCut& rc = cut[gn % CHUNK_I];
+        for (int k = 0; rc.width[k]; ++k) emit(std::min<int64_t>(2 * rc.width[k], gn - done), rc.width[k]);
         pl.item_off[(size_t)g + 1] = (int64_t)items.size();
     }
+    if ((int64_t)items.size() > c->max_items) return MWF_ENOMEM;
+    return MWF_OK;
+}
+
+// Second half: list offsets, interaction counts, the items' modelled costs, the schedules.  Needs the list lengths.
+int plan_finish(mwf_ctx* c, int64_t n_group, const int32_t* grp_n, const int32_t* n_epj_of, const int32_t* n_spj_of, Plan& pl) {
+    pl.list_off.assign((size_t)n_group + 1, 0);
+    pl.inter.assign((size_t)n_group + 1, 0);
+    std::vector<WorkItem>& items = pl.items;
+    std::vector<int64_t>& cost = pl.cost;
+    cost.resize(items.size());
+    for (int64_t g = 0; g < n_group; ++g) {
+        const int64_t n_list = (int64_t)n_epj_of[g] + n_spj_of[g];
+        const int64_t n_tiles = ((int64_t)n_epj_of[g] + TILE_J - 1) / TILE_J + ((int64_t)n_spj_of[g] + TILE_J - 1) / TILE_J;  // each run in whole tiles
+        pl.list_off[(size_t)g + 1] = pl.list_off[(size_t)g] + n_tiles * TILE_J;
+        pl.inter[(size_t)g + 1] = pl.inter[(size_t)g] + (int64_t)grp_n[g] * n_list;
+        for (int64_t k = pl.item_off[(size_t)g]; k < pl.item_off[(size_t)g + 1]; ++k) cost[(size_t)k] = n_tiles * item_cost_per_tile(items[(size_t)k].width);
+    }
     const int64_t n_items = (int64_t)items.size();
-    if (n_items > c->max_items) return MWF_ENOMEM;
+
     // work schedule over everything (see schedule_items); the schedules inside the n_tag interaction-balanced group
     // ranges that mwf_calc_force_all uses for a host destination are made on first use (ensure_split_order)
     pl.order_full.resize((size_t)n_items);
@@ -131,6 +161,11 @@ int make_plan(mwf_ctx* c, int64_t n_group, const int32_t* grp_first, const int32
     }
     pl.split[(size_t)c->p.n_tag] = n_group;
     return MWF_OK;
+}
+
+int make_plan(mwf_ctx* c, int64_t n_group, const int32_t* grp_first, const int32_t* grp_n, const int32_t* n_epj_of, const int32_t* n_spj_of, Plan& pl) {
+    const int rc = plan_cut(c, n_group, grp_first, grp_n, pl);
+    return rc ? rc : plan_finish(c, n_group, grp_n, n_epj_of, n_spj_of, pl);
 }
 
 // Adopt a plan as the ctx's current lists (after the device side is in place).

@@ -96,6 +96,9 @@ def test_device_build_errors():
     with pytest.raises(binding.MwfError) as e:
         f.dispatch(0, 0, 1)
     assert e.value.code == binding.ESTATE                       # a failed build leaves no lists
+    with pytest.raises(binding.MwfError) as e:
+        f.build(3000, 8, 64, 0.5)
+    assert e.value.code == binding.ESTATE                       # ... and the particles in an order nobody knows: upload again
     f.close()
 
 
