@@ -46,7 +46,7 @@ static int build_impl(mwf_ctx* c, int64_t n, int32_t n_leaf, int32_t n_grp, doub
     // memory on the stream.  The group ranges come first, so that the host cuts the groups into work items while the
     // device ranks the leaves and walks the tree.
     const auto D2H = cudaMemcpyDeviceToHost;
-    int32_t *h_first = c->h_groups, *h_n = h_first + n_group, *h_ne = h_n + n_group, *h_ns = h_ne + n_group;
+    int32_t *h_first = c->h_groups, *h_n = h_first + n_group, *h_ne = h_n + n_group, *h_ns = h_ne + n_group, *h_nf = h_ns + n_group;
     int64_t* totals = c->h_scalars;                                          // [0..2] padded, EPJ, SPJ entries
     int32_t* n_leaf_pinned = reinterpret_cast<int32_t*>(c->h_scalars + 4);
     unsigned int* err_pinned = reinterpret_cast<unsigned int*>(c->h_scalars + 5);
@@ -59,7 +59,7 @@ static int build_impl(mwf_ctx* c, int64_t n, int32_t n_leaf, int32_t n_grp, doub
     c->n_launch += 5;
     CU(c, cudaMemsetAsync(c->store + n + n_cell, 0, 16, s));
     CU(c, cudaMemsetAsync(c->store_next + n + n_cell, 0, 16, s));
-    CU(c, cudaMemsetAsync(c->spj_rec + 2 * n_cell, 0, 32, s));
+    CU(c, cudaMemsetAsync(c->spj_lo + n_cell, 0, 16, s));
     c->next_ranges.clear();
     c->next_streams.clear();
     c->n_ptcl = n;
@@ -79,6 +79,7 @@ static int build_impl(mwf_ctx* c, int64_t n, int32_t n_leaf, int32_t n_grp, doub
     CU(c, build_lists_count(c->bb, n_group, rule, c->walk_warps_n, totals, s));
     CU(c, cudaMemcpyAsync(h_ne, c->bb.n_epj, (size_t)n_group * 4, D2H, s));
     CU(c, cudaMemcpyAsync(h_ns, c->bb.n_spj, (size_t)n_group * 4, D2H, s));
+    CU(c, cudaMemcpyAsync(h_nf, c->bb.n_far, (size_t)n_group * 4, D2H, s));
     CU(c, cudaMemcpyAsync(err_pinned, c->err, sizeof(unsigned int), D2H, s));
     // host, meanwhile: the work items
     Plan plan;
@@ -96,6 +97,10 @@ static int build_impl(mwf_ctx* c, int64_t n, int32_t n_leaf, int32_t n_grp, doub
     CU(c, cudaMemsetAsync(c->grp_self, 1, (size_t)n_group, s));  // theta <= 1: a group's own cells are always opened
     c->n_launch += 6;
     // host, meanwhile: costs and schedules
+    for (int64_t g = 0; g < n_group; ++g) {  // the two runs of every list: EPJ + far SPJ, near SPJ
+        h_ne[g] += h_nf[g];
+        h_ns[g] -= h_nf[g];
+    }
     rc = plan_finish(c, n_group, h_n, h_ne, h_ns, plan);
     tm.lap("host: schedule | fill walk");
     if (rc) return build_failed(c, s, rc);

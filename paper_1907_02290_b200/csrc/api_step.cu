@@ -51,11 +51,10 @@ static int dispatch_launch(mwf_ctx* c, int32_t tag, int64_t g_begin, int64_t g_e
     cudaStream_t s = c->tag_stream[tag];
     ForceArgs a;
     a.store = c->store;
-    a.spj_rec = c->spj_rec;
+    a.spj_lo = c->spj_lo;
     a.n_ptcl = (int32_t)c->n_ptcl;
     a.dummy = (int32_t)(c->n_ptcl + c->n_cell);
-    a.epj_off = c->st_epj_off;
-    a.spj_off = c->st_spj_off;
+    a.run1_len = c->grp_run1;
     a.list = c->list;
     a.list_off = c->list_off;
     a.grp_self = c->grp_self;
@@ -91,7 +90,7 @@ static int dispatch_launch(mwf_ctx* c, int32_t tag, int64_t g_begin, int64_t g_e
     if (c->spj_order == 2) {  // quadrupole terms of the SPJ entries, added behind the monopole kernel
         QuadArgs q;
         q.store = c->store; q.quad = c->quad; q.list = c->list; q.list_off = c->list_off;
-        q.epj_off = c->st_epj_off; q.spj_off = c->st_spj_off;
+        q.epj_off = c->st_epj_off; q.spj_off = c->st_spj_off; q.n_far = c->grp_nfar;
         q.items = c->items; q.order = a.order; q.accp = c->accp;
         q.item_begin = a.item_begin; q.n_items = a.n_items; q.n_ptcl = c->n_ptcl; q.eps2 = a.eps2; q.G = a.G;
         const int64_t qres = (int64_t)c->n_sm * c->quad_ctas_per_sm;
@@ -232,7 +231,7 @@ int mwf_set_tree(mwf_ctx* c, const mwf_cell* cells, int64_t n_cell, void* stream
     const float4 zero = make_float4(0.f, 0.f, 0.f, 0.f);
     CU(c, cudaMemcpyAsync(c->store + n + n_cell, &zero, 16, cudaMemcpyHostToDevice, s));
     CU(c, cudaMemcpyAsync(c->store_next + n + n_cell, &zero, 16, cudaMemcpyHostToDevice, s));
-    CU(c, cudaMemsetAsync(c->spj_rec + 2 * n_cell, 0, 32, s));
+    CU(c, cudaMemsetAsync(c->spj_lo + n_cell, 0, 16, s));
     c->next_ranges.clear();
     c->next_streams.clear();
     unsigned int e = 0;
@@ -269,15 +268,6 @@ int mwf_set_lists(mwf_ctx* c, int64_t n_group, const int32_t* grp_first, const i
         n_epj[(size_t)g] = (int32_t)ne;
         n_spj[(size_t)g] = (int32_t)ns;
     }
-    Plan plan;
-    {
-        const int prc = make_plan(c, n_group, grp_first, grp_n, n_epj.data(), n_spj.data(), plan);
-        if (prc) return prc;
-    }
-    const std::vector<int64_t>& list_off = plan.list_off;
-    const std::vector<WorkItem>& items = plan.items;
-    const std::vector<int32_t>& order_full = plan.order_full;
-    const int64_t n_items = (int64_t)items.size();
     cudaStream_t s = static_cast<cudaStream_t>(stream);
     int rc = before_store_op(c, s);
     if (rc) return rc;
@@ -290,11 +280,38 @@ int mwf_set_lists(mwf_ctx* c, int64_t n_group, const int32_t* grp_first, const i
     CU(c, cudaMemcpyAsync(c->st_spj_off, spj_off, (size_t)(n_group + 1) * 8, H2D, s));
     if (e_epj) CU(c, cudaMemcpyAsync(c->st_ids, epj_id, (size_t)e_epj * 4, H2D, s));
     if (e_spj) CU(c, cudaMemcpyAsync(c->st_ids + e_epj, spj_id, (size_t)e_spj * 4, H2D, s));
+    // which SPJ entries are far enough to be swept like particles (run 1); their number per group sizes the two runs
+    CU(c, launch_classify_spj(n_group, c->grp_first, c->grp_n, c->st_spj_off, c->st_ids + e_epj, c->cells, c->store, c->n_ptcl, c->n_cell,
+                              c->ptcl_hi >= c->n_ptcl, c->grp_nfar, s));
+    ++c->n_launch;
+    std::vector<int32_t> n_far((size_t)n_group);
+    CU(c, cudaMemcpyAsync(n_far.data(), c->grp_nfar, (size_t)n_group * 4, cudaMemcpyDeviceToHost, s));
+    CU(c, cudaStreamSynchronize(s));
+    for (int64_t g = 0; g < n_group; ++g) {  // run 1 = EPJ + far SPJ, run 2 = near SPJ
+        if (n_far[(size_t)g] < 0 || n_far[(size_t)g] > n_spj[(size_t)g]) { after_store_op(c, s); return cuda_fail(c, cudaErrorUnknown, "SPJ classification"); }
+        n_epj[(size_t)g] += n_far[(size_t)g];
+        n_spj[(size_t)g] -= n_far[(size_t)g];
+    }
+    if (trace_on()) {
+        int64_t nf = 0;
+        for (int64_t g = 0; g < n_group; ++g) nf += n_far[(size_t)g];
+        fprintf(stderr, "[mwf trace] far SPJ entries: %lld of %lld\n", (long long)nf, (long long)e_spj);
+    }
+    // host pass: offsets, items, schedule
+    Plan plan;
+    {
+        const int prc = make_plan(c, n_group, grp_first, grp_n, n_epj.data(), n_spj.data(), plan);
+        if (prc) { after_store_op(c, s); return prc; }
+    }
+    const std::vector<int64_t>& list_off = plan.list_off;
+    const std::vector<WorkItem>& items = plan.items;
+    const std::vector<int32_t>& order_full = plan.order_full;
+    const int64_t n_items = (int64_t)items.size();
     CU(c, cudaMemcpyAsync(c->list_off, list_off.data(), (size_t)(n_group + 1) * 8, H2D, s));
     CU(c, cudaMemcpyAsync(c->items, items.data(), (size_t)n_items * sizeof(WorkItem), H2D, s));
     CU(c, cudaMemcpyAsync(c->order_full, order_full.data(), (size_t)n_items * 4, H2D, s));
     CU(c, launch_merge_lists(n_group, c->grp_first, c->grp_n, c->st_epj_off, c->st_ids, c->st_spj_off, c->st_ids + e_epj, c->list_off,
-                             c->n_ptcl, c->n_cell, c->list, c->grp_self, c->err, s));
+                             c->grp_nfar, c->grp_run1, c->n_ptcl, c->n_cell, c->list, c->grp_self, c->err, s));
     ++c->n_launch;
     unsigned int e = 0;
     rc = read_err_word(c, s, &e);  // also makes the host vectors above safe to free
@@ -334,11 +351,11 @@ int mwf_refresh_monopoles(mwf_ctx* c, void* stream) {
     int rc = before_store_op(c, s);
     if (rc) return rc;
     if (c->spj_order == 2 || !use_scan_refresh()) {  // the quadrupoles need the bottom-up pass (parallel-axis theorem)
-        CU(c, launch_monopoles(c->cells, c->parent, c->n_cell, c->n_ptcl, c->store, c->spj_rec, c->mom64, c->arrive,
+        CU(c, launch_monopoles(c->cells, c->parent, c->n_cell, c->n_ptcl, c->store, c->spj_lo, c->mom64, c->arrive,
                                c->spj_order == 2 ? c->quad64 : nullptr, c->spj_order == 2 ? c->quad : nullptr, s));
         ++c->n_launch;
     } else {
-        CU(c, launch_monopoles_scan(c->cells, c->cell_lr, c->n_cell, c->n_ptcl, c->n_leaf_cells, c->store, c->spj_rec, c->leaf_P, c->leaf_toff, s));
+        CU(c, launch_monopoles_scan(c->cells, c->cell_lr, c->n_cell, c->n_ptcl, c->n_leaf_cells, c->store, c->spj_lo, c->leaf_P, c->leaf_toff, s));
         c->n_launch += 4;
     }
     c->mono_fresh = true;

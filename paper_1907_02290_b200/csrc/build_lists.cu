@@ -24,8 +24,8 @@ template <bool FILL, bool NEIGH>
 __global__ void __launch_bounds__(256) k_walk(const mwf_cell* __restrict__ cells, const double4* __restrict__ geom, const float* __restrict__ grp_box,
                                               int64_t n_group, double th2, double reach, const float* __restrict__ cell_h, const float* __restrict__ grp_h,
                                               int32_t* __restrict__ stacks, unsigned int* __restrict__ counter,
-                                              int32_t* __restrict__ n_epj, int32_t* __restrict__ n_spj, const int64_t* __restrict__ list_off,
-                                              int32_t* __restrict__ list, int32_t n_ptcl, int32_t dummy) {
+                                              int32_t* __restrict__ n_epj, int32_t* __restrict__ n_spj, int32_t* __restrict__ n_far,
+                                              const int64_t* __restrict__ list_off, int32_t* __restrict__ list, int32_t n_ptcl, int32_t dummy) {
     const int lane = threadIdx.x & 31;
     const unsigned lt = (1u << lane) - 1u;
     const int64_t warp_global = ((int64_t)blockIdx.x * blockDim.x + threadIdx.x) >> 5;
@@ -43,12 +43,13 @@ __global__ void __launch_bounds__(256) k_walk(const mwf_cell* __restrict__ cells
         }
         double rg = 0.0;
         if constexpr (NEIGH) rg = __dmul_rn(reach, (double)grp_h[g]);
-        int64_t off_e = 0, off_s = 0;
+        int64_t off_e = 0, off_f = 0, off_s = 0;  // where the group's EPJ, far SPJ and near SPJ entries go
         if (FILL) {
             off_e = list_off[g];
-            off_s = off_e + (n_epj[g] + TILE_J - 1) / TILE_J * TILE_J;  // each run in whole tiles
+            off_f = off_e + n_epj[g];                                                    // run 1: EPJ, then far SPJ
+            off_s = off_e + (n_epj[g] + n_far[g] + TILE_J - 1) / TILE_J * TILE_J;        // run 2 starts on a tile boundary
         }
-        int ne = 0, ns = 0, sp = 1;
+        int ne = 0, ns = 0, nf = 0, sp = 1;  // ns: near SPJ, nf: far SPJ
         if (lane == 0) stack[0] = 0;
         __syncwarp();
         while (sp > 0) {
@@ -57,6 +58,7 @@ __global__ void __launch_bounds__(256) k_walk(const mwf_cell* __restrict__ cells
             const int c = lane < take ? stack[sp + lane] : -1;
             __syncwarp();
             int kind = 0;  // 1: SPJ, 2: opened internal cell, 3: opened leaf
+            bool far = false;
             mwf_cell cc = {0, 0, 0, 0};
             if (c >= 0) {
                 cc = cells[c];
@@ -86,11 +88,21 @@ __global__ void __launch_bounds__(256) k_walk(const mwf_cell* __restrict__ cells
                     }
                     const bool open = __dmul_rn(gm.w, gm.w) > __dmul_rn(th2, d2);
                     kind = !open ? 1 : (cc.n_child == 0 ? 3 : 2);
+                    if (!open) {  // far or near (SPJ_FAR_KAPPA): the centre of mass lies within the cell's cube
+                        const double half = 0.5 * gm.w;
+                        const double amax = fmax(fmax(fabs(s3[0]), fabs(s3[1])), fabs(s3[2])) + half;
+                        far = amax <= (double)SPJ_FAR_KAPPA * fmax(0.0, sqrt(d2) - 1.7320508075688772 * half);
+                    }
                 }
             }
-            // SPJ entries
-            const unsigned m_s = __ballot_sync(0xffffffffu, kind == 1);
-            if (FILL && kind == 1) list[off_s + ns + __popc(m_s & lt)] = n_ptcl + c;
+            // SPJ entries: far ones behind the EPJ entries of run 1, near ones in run 2
+            const unsigned m_f = __ballot_sync(0xffffffffu, kind == 1 && far);
+            const unsigned m_s = __ballot_sync(0xffffffffu, kind == 1 && !far);
+            if (FILL && kind == 1) {
+                if (far) list[off_f + nf + __popc(m_f & lt)] = n_ptcl + c;
+                else list[off_s + ns + __popc(m_s & lt)] = n_ptcl + c;
+            }
+            nf += __popc(m_f);
             ns += __popc(m_s);
             // opened leaves: their particles
             const unsigned m_l = __ballot_sync(0xffffffffu, kind == 3);
@@ -134,11 +146,12 @@ __global__ void __launch_bounds__(256) k_walk(const mwf_cell* __restrict__ cells
         }
         if (FILL) {  // pad both runs to whole tiles with the zero-mass dummy record
             const int64_t end = list_off[g + 1];
-            for (int64_t k = off_e + ne + lane; k < off_s; k += 32) list[k] = dummy;
+            for (int64_t k = off_f + nf + lane; k < off_s; k += 32) list[k] = dummy;
             for (int64_t k = off_s + ns + lane; k < end; k += 32) list[k] = dummy;
         } else if (lane == 0) {
             n_epj[g] = ne;
-            n_spj[g] = ns;
+            n_spj[g] = ns + nf;
+            n_far[g] = nf;
         }
     }
 }
@@ -175,25 +188,28 @@ __global__ void __launch_bounds__(256) k_group_hmax(const float4* __restrict__ s
 }
 
 // list_off[g] (to be scanned) = padded length of group g's merged list
-__global__ void __launch_bounds__(256) k_padded_len(const int32_t* __restrict__ n_epj, const int32_t* __restrict__ n_spj, int64_t n_group,
-                                                    int64_t* __restrict__ list_off, int64_t* __restrict__ epj_off, int64_t* __restrict__ spj_off) {
+__global__ void __launch_bounds__(256) k_padded_len(const int32_t* __restrict__ n_epj, const int32_t* __restrict__ n_spj, const int32_t* __restrict__ n_far,
+                                                    int64_t n_group, int32_t* __restrict__ run1_len, int64_t* __restrict__ list_off,
+                                                    int64_t* __restrict__ epj_off, int64_t* __restrict__ spj_off) {
     const int64_t g = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
     if (g > n_group) return;
     if (g == n_group) { list_off[g] = 0; epj_off[g] = 0; spj_off[g] = 0; return; }
-    list_off[g] = ((int64_t)n_epj[g] + TILE_J - 1) / TILE_J * TILE_J + ((int64_t)n_spj[g] + TILE_J - 1) / TILE_J * TILE_J;
+    const int64_t n1 = (int64_t)n_epj[g] + n_far[g], n2 = (int64_t)n_spj[g] - n_far[g];  // run 1: EPJ + far SPJ, run 2: near SPJ
+    run1_len[g] = (int32_t)n1;
+    list_off[g] = (n1 + TILE_J - 1) / TILE_J * TILE_J + (n2 + TILE_J - 1) / TILE_J * TILE_J;
     epj_off[g] = n_epj[g];
     spj_off[g] = n_spj[g];
 }
 
 // merged list -> the two CSR id arrays of the upload interface (read-back hook)
 __global__ void __launch_bounds__(256) k_unmerge(const int32_t* __restrict__ list, const int64_t* __restrict__ list_off, const int64_t* __restrict__ epj_off,
-                                                 const int64_t* __restrict__ spj_off, int64_t n_group, int32_t n_ptcl, int32_t* __restrict__ epj_id,
-                                                 int32_t* __restrict__ spj_id) {
+                                                 const int64_t* __restrict__ spj_off, const int32_t* __restrict__ n_far, int64_t n_group, int32_t n_ptcl,
+                                                 int32_t* __restrict__ epj_id, int32_t* __restrict__ spj_id) {
     for (int64_t g = blockIdx.x; g < n_group; g += gridDim.x) {
         const int64_t l0 = list_off[g], e0 = epj_off[g], ne = epj_off[g + 1] - e0, s0 = spj_off[g], ns = spj_off[g + 1] - s0;
-        const int64_t ne_pad = (ne + TILE_J - 1) / TILE_J * TILE_J;
+        const int64_t nf = n_far[g], n1_pad = (ne + nf + TILE_J - 1) / TILE_J * TILE_J;  // far SPJ behind the EPJ, near SPJ in run 2
         for (int64_t k = threadIdx.x; k < ne; k += blockDim.x) epj_id[e0 + k] = list[l0 + k];
-        for (int64_t k = threadIdx.x; k < ns; k += blockDim.x) spj_id[s0 + k] = list[l0 + ne_pad + k] - n_ptcl;
+        for (int64_t k = threadIdx.x; k < ns; k += blockDim.x) spj_id[s0 + k] = list[k < nf ? l0 + ne + k : l0 + n1_pad + (k - nf)] - n_ptcl;
     }
 }
 
@@ -225,12 +241,12 @@ cudaError_t build_lists_count(const BuildBuffers& b, int64_t n_group, const Walk
     BL(cudaMemsetAsync(b.walk_counter, 0, 4, s));
     if (rule.neighbours)
         k_walk<false, true><<<(unsigned)(n_warps / 8), 256, 0, s>>>(b.cells, b.geom, b.grp_box, n_group, th2, rule.reach, rule.cell_h, rule.grp_h, b.walk_stacks,
-                                                                    b.walk_counter, b.n_epj, b.n_spj, nullptr, nullptr, 0, 0);
+                                                                    b.walk_counter, b.n_epj, b.n_spj, b.n_far, nullptr, nullptr, 0, 0);
     else
         k_walk<false, false><<<(unsigned)(n_warps / 8), 256, 0, s>>>(b.cells, b.geom, b.grp_box, n_group, th2, 0.0, nullptr, nullptr, b.walk_stacks,
-                                                                     b.walk_counter, b.n_epj, b.n_spj, nullptr, nullptr, 0, 0);
+                                                                     b.walk_counter, b.n_epj, b.n_spj, b.n_far, nullptr, nullptr, 0, 0);
     BL(cudaGetLastError());
-    k_padded_len<<<(unsigned)((n_group + 1 + 255) / 256), 256, 0, s>>>(b.n_epj, b.n_spj, n_group, b.list_off, b.epj_off, b.spj_off);
+    k_padded_len<<<(unsigned)((n_group + 1 + 255) / 256), 256, 0, s>>>(b.n_epj, b.n_spj, b.n_far, n_group, b.run1_len, b.list_off, b.epj_off, b.spj_off);
     BL(cudaGetLastError());
     BL(scan_exclusive<int64_t>(b.list_off, n_group + 1, b.scan_scratch64, s));
     BL(scan_exclusive<int64_t>(b.epj_off, n_group + 1, b.scan_scratch64, s));
@@ -246,17 +262,17 @@ cudaError_t build_lists_fill(const BuildBuffers& b, int64_t n_group, const WalkR
     BL(cudaMemsetAsync(b.walk_counter, 0, 4, s));
     if (rule.neighbours)
         k_walk<true, true><<<(unsigned)(n_warps / 8), 256, 0, s>>>(b.cells, b.geom, b.grp_box, n_group, th2, rule.reach, rule.cell_h, rule.grp_h, b.walk_stacks,
-                                                                   b.walk_counter, b.n_epj, b.n_spj, b.list_off, b.list, (int32_t)n_ptcl, (int32_t)(n_ptcl + n_cell));
+                                                                   b.walk_counter, b.n_epj, b.n_spj, b.n_far, b.list_off, b.list, (int32_t)n_ptcl, (int32_t)(n_ptcl + n_cell));
     else
         k_walk<true, false><<<(unsigned)(n_warps / 8), 256, 0, s>>>(b.cells, b.geom, b.grp_box, n_group, th2, 0.0, nullptr, nullptr, b.walk_stacks,
-                                                                    b.walk_counter, b.n_epj, b.n_spj, b.list_off, b.list, (int32_t)n_ptcl, (int32_t)(n_ptcl + n_cell));
+                                                                    b.walk_counter, b.n_epj, b.n_spj, b.n_far, b.list_off, b.list, (int32_t)n_ptcl, (int32_t)(n_ptcl + n_cell));
     return cudaGetLastError();
 }
 
 cudaError_t unmerge_lists(const BuildBuffers& b, int64_t n_group, int64_t n_ptcl, int32_t* epj_id, int32_t* spj_id, cudaStream_t s) {
     if (n_group <= 0) return cudaSuccess;
     const int64_t grid = n_group < 148 * 16 ? n_group : 148 * 16;
-    k_unmerge<<<(unsigned)grid, 256, 0, s>>>(b.list, b.list_off, b.epj_off, b.spj_off, n_group, (int32_t)n_ptcl, epj_id, spj_id);
+    k_unmerge<<<(unsigned)grid, 256, 0, s>>>(b.list, b.list_off, b.epj_off, b.spj_off, b.n_far, n_group, (int32_t)n_ptcl, epj_id, spj_id);
     return cudaGetLastError();
 }
 

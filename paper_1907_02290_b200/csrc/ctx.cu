@@ -126,7 +126,9 @@ Layout make_layout(const mwf_params& p) {
     L.add((p.max_cell + 1) * 32);                       // 40 leaf_P
     L.add((scan4_tiles(p.max_cell) + 1) * 32);          // 41 leaf_toff
     L.add((p.max_ptcl + p.max_cell + 1) * 16);          // 42 store_next
-    L.add((p.max_cell + 1) * 32);                       // 43 spj_rec
+    L.add((p.max_cell + 1) * 16);                       // 43 spj_lo
+    L.add(p.max_group * 4);                             // 44 grp_nfar
+    L.add(p.max_group * 4);                             // 45 grp_run1
     return L;
 }
 
@@ -136,6 +138,7 @@ bool params_ok(const mwf_params* p) {
     if (!(p->G == p->G)) return false;
     if (p->max_ptcl < 1 || p->max_cell < 1 || p->max_group < 1 || p->max_entry < 1) return false;
     if (p->max_ptcl + p->max_cell + 1 > 0x7fffffffLL) return false;  // 32-bit list indices
+    if (p->max_cell >= 0x40000000LL) return false;                   // one bit of a cell index is borrowed while lists are re-encoded
     if (p->n_tag < 1 || p->n_tag > MWF_MAX_TAG) return false;
     if (p->device < 0) return false;
     return true;
@@ -200,7 +203,9 @@ int mwf_create(mwf_ctx** out, const mwf_params* p, void* arena, int64_t arena_by
     char* b = c->arena;
     c->store = (float4*)(b + L.off[0]);
     c->store_next = (float4*)(b + L.off[42]);
-    c->spj_rec = (float4*)(b + L.off[43]);
+    c->spj_lo = (float4*)(b + L.off[43]);
+    c->grp_nfar = (int32_t*)(b + L.off[44]);
+    c->grp_run1 = (int32_t*)(b + L.off[45]);
     c->accp = (float4*)(b + L.off[1]);
     c->cells = (mwf_cell*)(b + L.off[2]);
     c->parent = (int32_t*)(b + L.off[3]);
@@ -235,6 +240,7 @@ int mwf_create(mwf_ctx** out, const mwf_params* p, void* arena, int64_t arena_by
         q.mark = (int32_t*)(b + L.off[31]); q.grp_cell = (int32_t*)(b + L.off[32]);
         q.grp_first = c->grp_first; q.grp_n = c->grp_n; q.grp_box = (float*)(b + L.off[33]);
         q.n_epj = (int32_t*)(b + L.off[34]); q.n_spj = (int32_t*)(b + L.off[35]);
+        q.n_far = c->grp_nfar; q.run1_len = c->grp_run1;
         q.list_off = c->list_off; q.epj_off = c->st_epj_off; q.spj_off = c->st_spj_off; q.list = c->list;
         q.walk_stacks = (int32_t*)(b + L.off[36]); q.walk_counter = (unsigned int*)(b + L.off[37]); q.err = c->err;
         q.level_bounds = (int32_t*)(b + L.off[38]);
@@ -262,7 +268,7 @@ int mwf_create(mwf_ctx** out, const mwf_params* p, void* arena, int64_t arena_by
     ok = ok && cudaMemset(c->counters, 0, N_COUNTER * 4) == cudaSuccess;
     ok = ok && cudaMemset(c->err, 0, 256) == cudaSuccess;
     ok = ok && cudaHostAlloc(reinterpret_cast<void**>(&c->h_scalars), 16 * sizeof(int64_t), cudaHostAllocDefault) == cudaSuccess;
-    ok = ok && cudaHostAlloc(reinterpret_cast<void**>(&c->h_groups), (size_t)p->max_group * 4 * sizeof(int32_t), cudaHostAllocDefault) == cudaSuccess;
+    ok = ok && cudaHostAlloc(reinterpret_cast<void**>(&c->h_groups), (size_t)p->max_group * 5 * sizeof(int32_t), cudaHostAllocDefault) == cudaSuccess;
     ok = ok && cudaEventCreateWithFlags(&c->ev_groups, cudaEventDisableTiming) == cudaSuccess;
     if (!ok) { mwf_destroy(c); return MWF_ECUDA; }
     *out = c;

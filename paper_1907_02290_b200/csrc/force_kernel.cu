@@ -19,13 +19,15 @@
 //   * accumulation is two-level: partial sums over 32 j-pairs are added into running totals (two
 //     independent sums per component from the j-pairing), which keeps the fp32 summation error far inside
 //     the tolerance.
-//   * two coordinate conventions, one per kind of list entry (reading S11b of DESIGN.md).  EPJ tiles run in the
-//     caller's coordinates: particle positions are exact fp32 inputs and d = fl(x_j - x_i) is good to half an ulp of the
-//     DIFFERENCE however small it is.  SPJ tiles run in item-centred coordinates, c = the item's first i-particle: a
-//     centre of mass is not an fp32 input -- on the fp32 grid it is up to 2^-25 |X| off, which for a cell 1e-3 away at
-//     coordinates of order 1 is the north_star's whole error budget -- so the refresh keeps its rounding remainder next
-//     to it (spj_rec: 32 B per cell) and the staged position (hi - c) + lo carries 24 bits of the DISTANCE to the item;
-//     the i-side switches by adding c to -x_i.  The two runs of a group's list are padded to whole tiles separately.
+//   * two coordinate conventions (reading S11b of DESIGN.md).  The tiles of a list's run 1 -- every EPJ entry and every
+//     FAR SPJ entry -- are swept in the caller's coordinates: particle positions are exact fp32 inputs and
+//     d = fl(x_j - x_i) is good to half an ulp of the DIFFERENCE however small it is; a cell at least a quarter of its
+//     own coordinates away from the group (SPJ_FAR_KAPPA) is placed well enough by its fp32 record.  The tiles of run 2,
+//     the NEAR SPJ entries, are swept in item-centred coordinates, c = the item's first i-particle: a centre of mass is
+//     not an fp32 input -- on the fp32 grid it is up to 2^-25 |X| off, which for a cell 1e-3 away at coordinates of
+//     order 1 is the north_star's whole error budget -- so the refresh keeps its rounding remainder (spj_lo) and the
+//     staged position (hi - c) + lo carries 24 bits of the DISTANCE to the item; the i-side switches by adding c to -x_i.
+//     The two runs of a group's list are padded to whole tiles separately.
 //   * the self term (an i-particle meets itself in its own EPJ list) contributes exactly 0 to acc and
 //     m_i * rsqrt(eps^2) to the potential sum; the same value is subtracted up front (reading S2).
 #include "mwf_internal.h"
@@ -43,6 +45,13 @@ __device__ __forceinline__ int2 ld_stream_int2(const int2* p) {
     asm volatile("ld.global.nc.L1::no_allocate.v2.s32 {%0, %1}, [%2];" : "=r"(v.x), "=r"(v.y) : "l"(p));
     return v;
 }
+
+// 16-byte asynchronous copy global -> shared (LDGSTS), through L1 like the plain gathers
+__device__ __forceinline__ void cp_async16(float4* smem, const float4* gmem) {
+    asm volatile("cp.async.ca.shared.global [%0], [%1], 16;" ::"r"((unsigned)__cvta_generic_to_shared(smem)), "l"(gmem) : "memory");
+}
+__device__ __forceinline__ void cp_async_commit() { asm volatile("cp.async.commit_group;" ::: "memory"); }
+__device__ __forceinline__ void cp_async_wait_all() { asm volatile("cp.async.wait_all;" ::: "memory"); }
 
 struct Acc2 {  // sums for the two i-particles of a lane; .x / .y halves are the two j of a pair
     float2 x[2], y[2], z[2], p[2];
@@ -108,6 +117,9 @@ __device__ __forceinline__ void ld_data_pair(const float4* __restrict__ jd, int6
     j1 = e + 1 < n_list ? __ldg(jd + e + 1) : zero;
 }
 
+// per warp: two tiles in pair layout, the item's origin and a zero, the remainders of the tile in flight
+constexpr int FORCE_SMEM_FLOAT4_PER_WARP = 2 * TILE_J + 2 + TILE_J + 2;
+
 template <int W, bool INDEXED>
 __device__ __forceinline__ void run_item(const ForceArgs& a, const WorkItem it, float4* __restrict__ sbuf, int lane) {
     constexpr int S = 32 / W;
@@ -124,8 +136,12 @@ __device__ __forceinline__ void run_item(const ForceArgs& a, const WorkItem it, 
         const float4 p = __ldg(J + it.i_first + (valid[k] ? off : 0));
         nx[k] = -p.x; ny[k] = -p.y; nz[k] = -p.z; mi[k] = p.w;
     }
-    if constexpr (INDEXED) {  // origin of the SPJ tiles
+    if constexpr (INDEXED) {  // origin of the tiles of run 2, a zero for those of run 1, no remainders yet
+        const float4 zero = make_float4(0.f, 0.f, 0.f, 0.f);
         if (lane == 0) sbuf[2 * TILE_J] = __ldg(J + it.i_first);
+        if (lane == 1) sbuf[2 * TILE_J + 1] = zero;
+        sbuf[2 * TILE_J + 2 + lane] = zero;
+        sbuf[2 * TILE_J + 2 + 32 + lane] = zero;
         __syncwarp();
     }
     const float self_rinv = rsqrt_approx(a.eps2);  // what the sweep computes for d = 0
@@ -139,11 +155,12 @@ __device__ __forceinline__ void run_item(const ForceArgs& a, const WorkItem it, 
     for (int k = 0; k < 2; ++k) acc.p[k].x = (self_in && sl == 0) ? -mi[k] * self_rinv : 0.f;
 
     int64_t l0, n_list = 0;
-    int n_tiles, te;  // tiles [0, te) hold EPJ entries, [te, n_tiles) SPJ entries
+    int n_tiles, te;  // tiles [0, te): run 1 (EPJ and far SPJ entries), [te, n_tiles): run 2 (near SPJ entries)
     if constexpr (INDEXED) {
         l0 = a.list_off[it.group];
         n_tiles = (int)((a.list_off[it.group + 1] - l0) / TILE_J);
-        te = (int)((a.epj_off[it.group + 1] - a.epj_off[it.group] + TILE_J - 1) / TILE_J);
+        te = (a.run1_len[it.group] + TILE_J - 1) / TILE_J;
+
     } else {
         l0 = a.joff[it.group - a.g_base];
         n_list = a.joff[it.group - a.g_base + 1] - l0;
@@ -153,19 +170,23 @@ __device__ __forceinline__ void run_item(const ForceArgs& a, const WorkItem it, 
     const int2* __restrict__ lst = reinterpret_cast<const int2*>(a.list + (INDEXED ? l0 : 0));
     const float4* __restrict__ jd = a.jdata + (INDEXED ? 0 : l0);
 
-    // SPJ entries are cell index + N: their 32-byte records (float4 record, float4 remainder) are gathered from here
-    const float4* __restrict__ R = a.spj_rec - 2 * (int64_t)a.n_ptcl;
+    // Every tile is staged by the same instructions: the lane's two records come from the store through their indices
+    // (particles and SPJ records alike), are moved to the tile's origin and get their remainders added, (x - c) + q.  For
+    // the tiles of run 1 both c and q are zero, which leaves x as it is; for the tiles of run 2 c is the item's origin
+    // and q the remainder of the centre of mass, brought in by cp.async one tile ahead (registers held across the sweep
+    // are what its schedule is most sensitive to).  sbuf[ORIGIN] = c, sbuf[ORIGIN + 1] = 0, lo_raw = 64 remainders.
+    constexpr int ORIGIN = 2 * TILE_J;
+    float4* lo_raw = sbuf + ORIGIN + 2;
+    const float4* __restrict__ LO = a.spj_lo - a.n_ptcl;  // SPJ entries are cell index + N
     int2 idn = make_int2(0, 0);
-    float4 j0 = make_float4(0.f, 0.f, 0.f, 0.f), j1 = j0, q0 = j0, q1 = j0;
+    float4 j0 = make_float4(0.f, 0.f, 0.f, 0.f), j1 = j0;
     auto gather = [&](int t, const int2 id) {
-        if (t < te) {
-            j0 = __ldg(J + id.x);
-            j1 = __ldg(J + id.y);
-        } else {
-            j0 = __ldg(R + 2 * id.x);
-            q0 = __ldg(R + 2 * id.x + 1);
-            j1 = __ldg(R + 2 * id.y);
-            q1 = __ldg(R + 2 * id.y + 1);
+        j0 = __ldg(J + id.x);
+        j1 = __ldg(J + id.y);
+        if (t >= te) {
+            cp_async16(lo_raw + lane, LO + id.x);
+            cp_async16(lo_raw + 32 + lane, LO + id.y);
+            cp_async_commit();
         }
     };
     if (n_tiles > 0) {
@@ -179,17 +200,19 @@ __device__ __forceinline__ void run_item(const ForceArgs& a, const WorkItem it, 
     for (int t = 0; t < n_tiles; ++t) {
         float4* sA = sbuf + (t & 1) * TILE_J;
         float4* sB = sA + TILE_J / 2;
-        if (!INDEXED || t < te) {
-            sA[lane] = make_float4(j0.x, j1.x, j0.y, j1.y);
-            sB[lane] = make_float4(j0.z, j1.z, j0.w, j1.w);
-        } else {
-            const float4 c = sbuf[2 * TILE_J];  // the item's origin (kept in shared memory, not in registers across the sweep)
-            if (t == te) {
+        if constexpr (INDEXED) {
+            const float4 c = sbuf[ORIGIN + (t < te ? 1 : 0)];
+            cp_async_wait_all();  // the lane's own two remainders, if any are under way
+            const float4 q0 = lo_raw[lane], q1 = lo_raw[32 + lane];
+            if (t == te) {  // from here on: item-centred
 #pragma unroll
                 for (int k = 0; k < 2; ++k) { nx[k] += c.x; ny[k] += c.y; nz[k] += c.z; }
             }
             sA[lane] = make_float4((j0.x - c.x) + q0.x, (j1.x - c.x) + q1.x, (j0.y - c.y) + q0.y, (j1.y - c.y) + q1.y);
             sB[lane] = make_float4((j0.z - c.z) + q0.z, (j1.z - c.z) + q1.z, j0.w, j1.w);
+        } else {
+            sA[lane] = make_float4(j0.x, j1.x, j0.y, j1.y);
+            sB[lane] = make_float4(j0.z, j1.z, j0.w, j1.w);
         }
         __syncwarp();
         if (t + 1 < n_tiles) {
@@ -239,7 +262,7 @@ __device__ __forceinline__ void force_body(const ForceArgs& a, float4* s_tiles) 
     const int lane = threadIdx.x & 31;
     const int warp = threadIdx.x >> 5;
     const int warps_per_cta = blockDim.x >> 5;
-    float4* sbuf = s_tiles + warp * (2 * TILE_J + 1);
+    float4* sbuf = s_tiles + warp * FORCE_SMEM_FLOAT4_PER_WARP;
     int64_t w = (int64_t)blockIdx.x * warps_per_cta + warp;  // first item: static
     const int64_t n_warps = (int64_t)gridDim.x * warps_per_cta;
     while (w < a.n_items) {
@@ -274,7 +297,7 @@ __global__ void __launch_bounds__(WARPS_PER_CTA * 32, MWF_MIN_CTAS) k_force_data
     force_body<false>(a, s_force_tiles);
 }
 
-constexpr size_t FORCE_SMEM_PER_WARP = (2 * TILE_J + 1) * sizeof(float4);  // two tiles and the item's origin
+constexpr size_t FORCE_SMEM_PER_WARP = FORCE_SMEM_FLOAT4_PER_WARP * sizeof(float4);
 
 // warps = warps per block: WARPS_PER_CTA for a dispatch that fills the machine (persistent grid, items claimed dynamically);
 // a sub-wave dispatch (a batch of the multiwalk pipeline) is launched with small blocks, one item per warp, so

@@ -65,11 +65,11 @@ __global__ void k_tree_check(const int32_t* __restrict__ parent, int64_t n_cell,
 }
 
 // The SPJ record of cell c: centre of mass and mass rounded to the float4 the force kernel gathers at store[N + c], plus
-// the rounding remainder of the centre, spj_rec[c] = X - (double)float(X) rounded to float (reading S11b of DESIGN.md: a
+// the rounding remainder of the centre, spj_lo[c] = X - (double)float(X) rounded to float (reading S11b of DESIGN.md: a
 // centre of mass is not an fp32 input, and on the fp32 grid of coordinates of order 1 it would be 3e-8 off -- 1e-4 of the
 // force of a cell 1e-3 away, which is the north_star's whole error budget).  The force kernel adds the remainder after it
 // has moved the record into group-centred coordinates.
-__device__ __forceinline__ void write_spj(float4* __restrict__ store, float4* __restrict__ spj_rec, int64_t n_ptcl, int64_t c,
+__device__ __forceinline__ void write_spj(float4* __restrict__ store, float4* __restrict__ spj_lo, int64_t n_ptcl, int64_t c,
                                           double sx, double sy, double sz, double m, float fx, float fy, float fz) {
     float4 r, lo = make_float4(0.f, 0.f, 0.f, 0.f);
     if (m > 0.0) {
@@ -80,15 +80,14 @@ __device__ __forceinline__ void write_spj(float4* __restrict__ store, float4* __
     } else {  // massless cell: exerts nothing; keep a finite position
         r = make_float4(fx, fy, fz, 0.f);
     }
-    store[n_ptcl + c] = r;   // SPJ behind the EPJ: what mwf_get_monopoles, the quadrupole kernel and method G1 read
-    spj_rec[2 * c] = r;      // the force kernel's copy, next to its remainder: one 32-byte sector per gather
-    spj_rec[2 * c + 1] = lo;
+    store[n_ptcl + c] = r;   // SPJ behind the EPJ
+    spj_lo[c] = lo;
 }
 
-__device__ __forceinline__ void store_moment(float4* __restrict__ store, float4* __restrict__ spj_rec, double4* __restrict__ mom64, int64_t n_ptcl,
+__device__ __forceinline__ void store_moment(float4* __restrict__ store, float4* __restrict__ spj_lo, double4* __restrict__ mom64, int64_t n_ptcl,
                                              int64_t c, double sx, double sy, double sz, double m, float fx, float fy, float fz) {
     mom64[c] = make_double4(sx, sy, sz, m);  // mass-weighted position sums and mass
-    write_spj(store, spj_rec, n_ptcl, c, sx, sy, sz, m, fx, fy, fz);
+    write_spj(store, spj_lo, n_ptcl, c, sx, sy, sz, m, fx, fy, fz);
 }
 
 // Second moments about the centre of mass (NEXT-3, quadrupole SPJ): quad64[6c..6c+5] = (Qxx Qyy Qzz Qxy Qxz Qyz) in fp64
@@ -102,7 +101,7 @@ __device__ __forceinline__ void store_quad(double* __restrict__ quad64, float4* 
 
 template <bool QUAD>
 __global__ void __launch_bounds__(128) k_monopoles(const mwf_cell* __restrict__ cells, const int32_t* __restrict__ parent,
-                                                   int64_t n_cell, int64_t n_ptcl, float4* __restrict__ store, float4* __restrict__ spj_rec,
+                                                   int64_t n_cell, int64_t n_ptcl, float4* __restrict__ store, float4* __restrict__ spj_lo,
                                                    double4* __restrict__ mom64, int32_t* __restrict__ counter,
                                                    double* __restrict__ quad64, float4* __restrict__ quad) {
     const int64_t c0 = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
@@ -120,7 +119,7 @@ __global__ void __launch_bounds__(128) k_monopoles(const mwf_cell* __restrict__ 
         sz += mq * (double)q.z;
     }
     const float4 f = p[0];
-    store_moment(store, spj_rec, mom64, n_ptcl, c0, sx, sy, sz, m, f.x, f.y, f.z);
+    store_moment(store, spj_lo, mom64, n_ptcl, c0, sx, sy, sz, m, f.x, f.y, f.z);
     if constexpr (QUAD) {  // second pass over the leaf's particles, about its centre of mass
         double q[6] = {0.0, 0.0, 0.0, 0.0, 0.0, 0.0};
         if (m > 0.0) {
@@ -151,7 +150,7 @@ __global__ void __launch_bounds__(128) k_monopoles(const mwf_cell* __restrict__ 
             sx += lo.x; sy += lo.y; sz += hi.x; m += hi.y;
         }
         const float4 g = store[pc.first_ptcl];
-        store_moment(store, spj_rec, mom64, n_ptcl, par, sx, sy, sz, m, g.x, g.y, g.z);
+        store_moment(store, spj_lo, mom64, n_ptcl, par, sx, sy, sz, m, g.x, g.y, g.z);
         if constexpr (QUAD) {  // parallel-axis theorem: Q = sum over children of Q_child + M_child d d^T, d = X_child - X
             double q[6] = {0.0, 0.0, 0.0, 0.0, 0.0, 0.0};
             if (m > 0.0) {
@@ -202,7 +201,7 @@ __global__ void __launch_bounds__(256) k_leaf_ranges(const mwf_cell* __restrict_
 }
 
 __global__ void __launch_bounds__(256) k_leaf_moments(const mwf_cell* __restrict__ cells, const int2* __restrict__ cell_lr, int64_t n_cell,
-                                                      int64_t n_ptcl, int64_t n_leaf_cells, float4* __restrict__ store, float4* __restrict__ spj_rec,
+                                                      int64_t n_ptcl, int64_t n_leaf_cells, float4* __restrict__ store, float4* __restrict__ spj_lo,
                                                       double4* __restrict__ P) {
     const int64_t c = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
     if (c == 0) P[n_leaf_cells] = make_double4(0.0, 0.0, 0.0, 0.0);  // the scan turns this entry into the grand total
@@ -222,7 +221,7 @@ __global__ void __launch_bounds__(256) k_leaf_moments(const mwf_cell* __restrict
         sz += mq * (double)q.z;
     }
     P[cell_lr[c].x] = make_double4(sx, sy, sz, m);
-    write_spj(store, spj_rec, n_ptcl, c, sx, sy, sz, m, f.x, f.y, f.z);
+    write_spj(store, spj_lo, n_ptcl, c, sx, sy, sz, m, f.x, f.y, f.z);
 }
 
 constexpr int SCAN4_THREADS = 256, SCAN4_ITEMS = 4, SCAN4_TILE = SCAN4_THREADS * SCAN4_ITEMS;
@@ -291,7 +290,7 @@ __global__ void __launch_bounds__(1024) k_scan4_totals(double4* __restrict__ tsu
 }
 
 __global__ void __launch_bounds__(256) k_cells_from_prefix(const mwf_cell* __restrict__ cells, const int2* __restrict__ cell_lr, int64_t n_cell,
-                                                           int64_t n_ptcl, float4* __restrict__ store, float4* __restrict__ spj_rec,
+                                                           int64_t n_ptcl, float4* __restrict__ store, float4* __restrict__ spj_lo,
                                                            const double4* __restrict__ P, const double4* __restrict__ toff) {
     const int64_t c = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
     if (c >= n_cell) return;
@@ -302,7 +301,7 @@ __global__ void __launch_bounds__(256) k_cells_from_prefix(const mwf_cell* __res
     const double sx = hi.x - lo.x, sy = hi.y - lo.y, sz = hi.z - lo.z, m = hi.w - lo.w;
     float4 f = make_float4(0.f, 0.f, 0.f, 0.f);
     if (!(m > 0.0)) f = store[cc.first_ptcl];
-    write_spj(store, spj_rec, n_ptcl, c, sx, sy, sz, m, f.x, f.y, f.z);
+    write_spj(store, spj_lo, n_ptcl, c, sx, sy, sz, m, f.x, f.y, f.z);
 }
 
 cudaError_t launch_tree_prepare(const mwf_cell* cells, int64_t n_cell, int64_t max_ptcl, int32_t* parent, int32_t* counter,
@@ -318,14 +317,14 @@ cudaError_t launch_tree_prepare(const mwf_cell* cells, int64_t n_cell, int64_t m
     return cudaGetLastError();
 }
 
-cudaError_t launch_monopoles(const mwf_cell* cells, const int32_t* parent, int64_t n_cell, int64_t n_ptcl, float4* store, float4* spj_rec,
+cudaError_t launch_monopoles(const mwf_cell* cells, const int32_t* parent, int64_t n_cell, int64_t n_ptcl, float4* store, float4* spj_lo,
                              double4* mom64, int32_t* counter, double* quad64, float4* quad, cudaStream_t s) {
     const int block = 128;
     const int64_t grid = (n_cell + block - 1) / block;
     if (quad64 && quad)
-        k_monopoles<true><<<(unsigned)grid, block, 0, s>>>(cells, parent, n_cell, n_ptcl, store, spj_rec, mom64, counter, quad64, quad);
+        k_monopoles<true><<<(unsigned)grid, block, 0, s>>>(cells, parent, n_cell, n_ptcl, store, spj_lo, mom64, counter, quad64, quad);
     else
-        k_monopoles<false><<<(unsigned)grid, block, 0, s>>>(cells, parent, n_cell, n_ptcl, store, spj_rec, mom64, counter, nullptr, nullptr);
+        k_monopoles<false><<<(unsigned)grid, block, 0, s>>>(cells, parent, n_cell, n_ptcl, store, spj_lo, mom64, counter, nullptr, nullptr);
     return cudaGetLastError();
 }
 
@@ -351,9 +350,9 @@ cudaError_t launch_leaf_ranking(const mwf_cell* cells, int64_t n_cell, int64_t n
 }
 
 cudaError_t launch_monopoles_scan(const mwf_cell* cells, const int2* cell_lr, int64_t n_cell, int64_t n_ptcl, int64_t n_leaf_cells, float4* store,
-                                  float4* spj_rec, double4* P, double4* toff, cudaStream_t s) {
+                                  float4* spj_lo, double4* P, double4* toff, cudaStream_t s) {
     const unsigned grid = (unsigned)((n_cell + 255) / 256);
-    k_leaf_moments<<<grid, 256, 0, s>>>(cells, cell_lr, n_cell, n_ptcl, n_leaf_cells, store, spj_rec, P);
+    k_leaf_moments<<<grid, 256, 0, s>>>(cells, cell_lr, n_cell, n_ptcl, n_leaf_cells, store, spj_lo, P);
     cudaError_t e = cudaGetLastError();
     if (e != cudaSuccess) return e;
     const int64_t nt = scan4_tiles(n_leaf_cells);
@@ -361,7 +360,7 @@ cudaError_t launch_monopoles_scan(const mwf_cell* cells, const int2* cell_lr, in
     if ((e = cudaGetLastError()) != cudaSuccess) return e;
     k_scan4_totals<<<1, 1024, 0, s>>>(toff, nt);
     if ((e = cudaGetLastError()) != cudaSuccess) return e;
-    k_cells_from_prefix<<<grid, 256, 0, s>>>(cells, cell_lr, n_cell, n_ptcl, store, spj_rec, P, toff);
+    k_cells_from_prefix<<<grid, 256, 0, s>>>(cells, cell_lr, n_cell, n_ptcl, store, spj_lo, P, toff);
     return cudaGetLastError();
 }
 

@@ -23,7 +23,7 @@ struct mwf_ctx {
     float4* store_next = nullptr; // same size: the shadow store of the pipelined host loop (mwf_set_particles_next / mwf_swap_store)
     std::vector<std::pair<int64_t, int64_t>> next_ranges;  // particle ranges written into the shadow store since the last swap
     std::vector<cudaStream_t> next_streams;  // streams those uploads went to
-    float4* spj_rec = nullptr;    // [2 (max_cell + 1)] per cell: SPJ record + rounding remainder of its centre of mass (reading S11b)
+    float4* spj_lo = nullptr;     // [max_cell + 1] per cell: rounding remainder of the SPJ record's centre of mass (reading S11b)
     float4* accp = nullptr;       // [max_ptcl]
     float4* vel = nullptr;        // [max_ptcl] (vx, vy, vz, unused): device-resident integration
     mwf_cell* cells = nullptr;    // [max_cell]
@@ -34,13 +34,15 @@ struct mwf_ctx {
     double4* leaf_P = nullptr;    // [max_cell + 1] leaves' moments in rank order, scanned in place every refresh
     double4* leaf_toff = nullptr; // [tiles] scanned tile totals
     int64_t* h_scalars = nullptr; // pinned: small results of the construction step (counts, totals, validation word)
-    int32_t* h_groups = nullptr;  // pinned [4 x max_group]: group ranges and list lengths on their way to the host work plan
+    int32_t* h_groups = nullptr;  // pinned [5 x max_group]: group ranges and list lengths on their way to the host work plan
     cudaEvent_t ev_groups{};      // the group ranges have arrived
     float fuse_kick_h = 0.f;      // mwf_step_reuse: the closing kick rides in the force kernel's epilogue (0: no kick)
     int64_t n_leaf_cells = 0;
     int32_t* grp_first = nullptr; // [max_group]
     int32_t* grp_n = nullptr;     // [max_group]
     uint8_t* grp_self = nullptr;  // [max_group]
+    int32_t* grp_nfar = nullptr;  // [max_group] far SPJ entries of every group (swept like particles, see SPJ_FAR_KAPPA)
+    int32_t* grp_run1 = nullptr;  // [max_group] entries of run 1 = EPJ + far SPJ
     int64_t* list_off = nullptr;  // [max_group + 1]
     int64_t* st_epj_off = nullptr, *st_spj_off = nullptr;  // [max_group + 1] staging
     int32_t* st_ids = nullptr;    // [max_entry] staging of the uploaded ids

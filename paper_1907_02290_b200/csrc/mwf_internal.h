@@ -11,11 +11,19 @@
 namespace mwf {
 
 constexpr int TILE_J = 64;          // j entries staged per warp tile; merged lists are padded to this
-constexpr int WARPS_PER_CTA = 8;    // force kernel block = 256 threads
+#ifndef MWF_WARPS_PER_CTA
+#define MWF_WARPS_PER_CTA 8
+#endif
+constexpr int WARPS_PER_CTA = MWF_WARPS_PER_CTA;    // force kernel block
 constexpr int SMALL_CTA_WARPS = 2;  // block of a sub-wave dispatch (one item per warp)
 constexpr int SCHED_WINDOWS = 16;    // Morton windows of the work schedule when the store exceeds the L2
 constexpr int CHUNK_I = 64;         // i-particles of a full work item (2 per lane)
 constexpr int MIN_WIDTH = 2;        // narrowest item: 2 lanes x 2 i-particles, 16 j-slices
+// An SPJ entry is FAR when the cell's coordinates are at most this many times its distance from the group: the fp32
+// rounding of its centre of mass, 2^-25 of the coordinate, is then within 2^-23 of the separation (a couple of ulps, like
+// the difference of two particle positions), and the entry is swept like a particle, from its 16-byte record in the
+// caller's coordinates.  NEAR entries are swept in item-centred coordinates with the rounding remainder (reading S11b).
+constexpr float SPJ_FAR_KAPPA = 4.f;
 
 // One unit of work for one warp: n_i <= 2 * width consecutive i-particles of one group against the
 // group's whole list.  width = 32, 16, 8, 4 or 2 lanes hold the i-particles (2 per lane); the warp is
@@ -47,11 +55,11 @@ inline int64_t item_cost_per_tile(int width) { return COST_STAGE + COST_PAIR * w
 
 struct ForceArgs {
     const float4* store;        // particles then SPJ then one zero-mass dummy
-    const float4* spj_rec;      // [2 (n_cell + 1)] per cell: the SPJ record and the rounding remainder of its centre of mass (entry n_cell: zero)
+    const float4* spj_lo;       // [n_cell + 1] per cell: the rounding remainder of the SPJ record's centre of mass (entry n_cell: zero)
     int32_t n_ptcl;             // list indices >= n_ptcl are SPJ entries
     int32_t dummy;              // index of the zero-mass record (n_ptcl + n_cell)
-    const int64_t* epj_off;     // scanned EPJ / SPJ counts per group: entries [0, ne) of a group's list are EPJ,
-    const int64_t* spj_off;     //   [ne, ne + ns) SPJ, the rest of its last tile padding
+    const int32_t* run1_len;    // per group: entries of run 1 (EPJ + far SPJ; 16-byte records, caller's coordinates); run 2
+                                //   (near SPJ; 32-byte records, item-centred) starts at the next tile boundary
     const int32_t* list;        // merged, padded lists
     const int64_t* list_off;    // per group, in entries (multiples of TILE_J)
     const uint8_t* grp_self;    // 1: the group's own particles are in its EPJ list
@@ -76,8 +84,9 @@ struct QuadArgs {
     const float4* quad;         // two float4 per cell: (Qxx Qyy Qzz Qxy) (Qxz Qyz tr(Q)/2 0)
     const int32_t* list;
     const int64_t* list_off;
-    const int64_t* epj_off;     // scanned EPJ / SPJ counts per group: the SPJ part of group g starts at
-    const int64_t* spj_off;     //   list_off[g] + epj_off[g+1] - epj_off[g] and has spj_off[g+1] - spj_off[g] entries
+    const int64_t* epj_off;     // scanned EPJ / SPJ counts per group; the SPJ entries of group g are its n_far[g] far ones at
+    const int64_t* spj_off;     //   list_off[g] + ne and the near ones from the next tile boundary behind them
+    const int32_t* n_far;
     const WorkItem* items;
     const int32_t* order;
     float4* accp;
@@ -116,17 +125,21 @@ int force_max_ctas_per_sm();
 cudaError_t launch_tree_prepare(const mwf_cell* cells, int64_t n_cell, int64_t max_ptcl, int32_t* parent, int32_t* counter,
                                 unsigned int* err, cudaStream_t s);
 // quad64 / quad non-null: also the second moments about the centres of mass (6 doubles per cell) and their float record
-cudaError_t launch_monopoles(const mwf_cell* cells, const int32_t* parent, int64_t n_cell, int64_t n_ptcl, float4* store, float4* spj_rec,
+cudaError_t launch_monopoles(const mwf_cell* cells, const int32_t* parent, int64_t n_cell, int64_t n_ptcl, float4* store, float4* spj_lo,
                              double4* mom64, int32_t* counter, double* quad64, float4* quad, cudaStream_t s);
 // scan variant of the refresh (monopole_kernel.cu): leaf ranking at the construction step, then leaf sums + prefix scan per refresh
 int64_t scan4_tiles(int64_t n_leaf_cells);
 cudaError_t launch_leaf_ranking(const mwf_cell* cells, int64_t n_cell, int64_t n_ptcl, int32_t* mark, int32_t* scratch, int2* cell_lr,
                                 int32_t* n_leaf_pinned, cudaStream_t s);
 cudaError_t launch_monopoles_scan(const mwf_cell* cells, const int2* cell_lr, int64_t n_cell, int64_t n_ptcl, int64_t n_leaf_cells, float4* store,
-                                  float4* spj_rec, double4* P, double4* toff, cudaStream_t s);
+                                  float4* spj_lo, double4* P, double4* toff, cudaStream_t s);
+cudaError_t launch_classify_spj(int64_t n_group, const int32_t* grp_first, const int32_t* grp_n, const int64_t* spj_off, int32_t* spj_id,
+                                const mwf_cell* cells, const float4* store, int64_t n_ptcl, int64_t n_cell, bool have_ptcl, int32_t* n_far,
+                                cudaStream_t s);
 cudaError_t launch_merge_lists(int64_t n_group, const int32_t* grp_first, const int32_t* grp_n, const int64_t* epj_off,
                                const int32_t* epj_id, const int64_t* spj_off, const int32_t* spj_id, const int64_t* list_off,
-                               int64_t n_ptcl, int64_t n_cell, int32_t* list, uint8_t* grp_self, unsigned int* err, cudaStream_t s);
+                               const int32_t* n_far, int32_t* run1_len, int64_t n_ptcl, int64_t n_cell, int32_t* list, uint8_t* grp_self,
+                               unsigned int* err, cudaStream_t s);
 
 // ---- device-side construction step (NEXT-2): buffers carved from the arena, see build_tree.cu / build_lists.cu
 constexpr int WALK_STACK = 6144;  // >= 22 levels x 256 cells (bound derived in build_lists.cu)
@@ -138,7 +151,7 @@ struct BuildBuffers {
     float* bbox_part; double* root;
     mwf_cell* cells; double4* geom; int32_t* parent; int32_t* level_cnt; int32_t* level_bounds; int64_t level_cap;
     int32_t* mark; int32_t* grp_cell; int32_t* grp_first; int32_t* grp_n; float* grp_box;
-    int32_t* n_epj; int32_t* n_spj; int64_t* list_off; int64_t* epj_off; int64_t* spj_off; int32_t* list;
+    int32_t* n_epj; int32_t* n_spj; int32_t* n_far; int32_t* run1_len; int64_t* list_off; int64_t* epj_off; int64_t* spj_off; int32_t* list;
     int32_t* walk_stacks; unsigned int* walk_counter; unsigned int* err;
 };
 

@@ -97,11 +97,13 @@ struct CellRec {
     float4 xm, q0, q1;
 };
 
-__device__ __forceinline__ CellRec ld_cell(const QuadArgs& a, const int32_t* __restrict__ lst, int64_t e, int64_t n_spj) {
+// SPJ entry e of a group: the first n_far of them sit behind the EPJ entries in run 1 (lst_far), the others in run 2 (lst_near)
+__device__ __forceinline__ CellRec ld_cell(const QuadArgs& a, const int32_t* __restrict__ lst_far, const int32_t* __restrict__ lst_near, int64_t n_far,
+                                           int64_t e, int64_t n_spj) {
     CellRec r;
     r.xm = r.q0 = r.q1 = make_float4(0.f, 0.f, 0.f, 0.f);  // past the end: a cell without moments
     if (e < n_spj) {
-        const int32_t id = __ldg(lst + e);  // index into the store: n_ptcl + cell
+        const int32_t id = __ldg(e < n_far ? lst_far + e : lst_near + (e - n_far));  // index into the store: n_ptcl + cell
         r.xm = __ldg(a.store + id);
         const float4* q = a.quad + 2 * (int64_t)(id - a.n_ptcl);
         r.q0 = __ldg(q);
@@ -116,7 +118,9 @@ __device__ __forceinline__ void quad_item(const QuadArgs& a, const WorkItem it, 
     const int il = lane % W;
     const int64_t n_spj = a.spj_off[it.group + 1] - a.spj_off[it.group];
     if (n_spj == 0) return;
-    const int32_t* __restrict__ lst = a.list + a.list_off[it.group] + (a.epj_off[it.group + 1] - a.epj_off[it.group] + TILE_J - 1) / TILE_J * TILE_J;
+    const int64_t n_epj = a.epj_off[it.group + 1] - a.epj_off[it.group], n_far = a.n_far[it.group];
+    const int32_t* __restrict__ lst_far = a.list + a.list_off[it.group] + n_epj;
+    const int32_t* __restrict__ lst_near = a.list + a.list_off[it.group] + (n_epj + n_far + TILE_J - 1) / TILE_J * TILE_J;
     float nx[2], ny[2], nz[2];
     bool valid[2];
 #pragma unroll
@@ -130,7 +134,7 @@ __device__ __forceinline__ void quad_item(const QuadArgs& a, const WorkItem it, 
 #pragma unroll
     for (int k = 0; k < 2; ++k) acc.x[k] = acc.y[k] = acc.z[k] = acc.p[k] = make_float2(0.f, 0.f);
     const int n_tiles = (int)((n_spj + TILE_J - 1) / TILE_J);
-    CellRec c0 = ld_cell(a, lst, 2 * lane, n_spj), c1 = ld_cell(a, lst, 2 * lane + 1, n_spj);
+    CellRec c0 = ld_cell(a, lst_far, lst_near, n_far, 2 * lane, n_spj), c1 = ld_cell(a, lst_far, lst_near, n_far, 2 * lane + 1, n_spj);
     for (int t = 0; t < n_tiles; ++t) {
         float4* tile = sbuf + (t & 1) * (QT * 32);
         tile[lane] = make_float4(c0.xm.x, c1.xm.x, c0.xm.y, c1.xm.y);
@@ -141,8 +145,8 @@ __device__ __forceinline__ void quad_item(const QuadArgs& a, const WorkItem it, 
         __syncwarp();
         if (t + 1 < n_tiles) {
             const int64_t e = (int64_t)(t + 1) * TILE_J + 2 * lane;
-            c0 = ld_cell(a, lst, e, n_spj);
-            c1 = ld_cell(a, lst, e + 1, n_spj);
+            c0 = ld_cell(a, lst_far, lst_near, n_far, e, n_spj);
+            c1 = ld_cell(a, lst_far, lst_near, n_far, e + 1, n_spj);
         }
         quad_sweep<W>(tile, sl, nx, ny, nz, a.eps2, acc);
     }

@@ -252,7 +252,10 @@ def test_more_than_2_31_list_entries():
     f2.retrieve(0, out2)
     f2.close()
     check_forces(out2[mask], acc[mask], pot[mask], "host path, same lists")
-    assert np.array_equal(out2, out)                          # same lists in the same order: bitwise the same sums
+    # same lists in the same order; which SPJ entries count as far (swept like particles) is decided from the cell geometry by
+    # the device builder and from the particles by the upload path, so the two sums agree to rounding, not bit for bit
+    da = np.linalg.norm(out2[:, :3].astype(np.float64) - out[:, :3], axis=1) / np.linalg.norm(out[:, :3].astype(np.float64), axis=1)
+    assert da.max() <= 2e-5 and np.sqrt(np.mean(da ** 2)) <= 1e-6
 
 
 def test_shadow_store_after_a_device_build():
