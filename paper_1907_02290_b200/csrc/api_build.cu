@@ -96,21 +96,25 @@ static int build_impl(mwf_ctx* c, int64_t n, int32_t n_leaf, int32_t n_grp, doub
     CU(c, build_lists_fill(c->bb, n_group, rule, c->walk_warps_n, n, n_cell, s));
     CU(c, cudaMemsetAsync(c->grp_self, 1, (size_t)n_group, s));  // theta <= 1: a group's own cells are always opened
     c->n_launch += 6;
-    // host, meanwhile: costs and schedules
+    // beside the fill walk, on a stream of its own: the work items go up and are scheduled (the list offsets they need were
+    // made by the counting pass, which the host has just waited for)
+    const int64_t n_items = (int64_t)plan.items.size();
+    CU(c, cudaMemcpyAsync(c->items, plan.items.data(), (size_t)n_items * sizeof(WorkItem), cudaMemcpyHostToDevice, c->aux_stream));
+    rc = schedule_full(c, n_items, c->aux_stream);
+    if (rc) return build_failed(c, s, rc);
+    CU(c, cudaEventRecord(c->ev_aux, c->aux_stream));
+    CU(c, cudaStreamWaitEvent(s, c->ev_aux, 0));
+    // host, meanwhile: list offsets and interaction counts per group, the tags' group ranges
     for (int64_t g = 0; g < n_group; ++g) {  // the two runs of every list: EPJ + far SPJ, near SPJ
         h_ne[g] += h_nf[g];
         h_ns[g] -= h_nf[g];
     }
     rc = plan_finish(c, n_group, h_n, h_ne, h_ns, plan);
-    tm.lap("host: schedule | fill walk");
+    tm.lap("host: offsets | fill walk, schedule");
     if (rc) return build_failed(c, s, rc);
     if (plan.list_off[(size_t)n_group] != padded) return build_failed(c, s, MWF_ERANGE);  // host and device offsets must agree
-    const int64_t n_items = (int64_t)plan.items.size();
-    const auto H2D = cudaMemcpyHostToDevice;
-    CU(c, cudaMemcpyAsync(c->items, plan.items.data(), (size_t)n_items * sizeof(WorkItem), H2D, s));
-    CU(c, cudaMemcpyAsync(c->order_full, plan.order_full.data(), (size_t)n_items * 4, H2D, s));
     CU(c, cudaStreamSynchronize(s));  // the plan's host vectors die with this call
-    tm.lap("fill walk: rest + plan upload");
+    tm.lap("fill walk, schedule: rest");
     rc = after_store_op(c, s);
     if (rc) return rc;
     c->have_tree = true;

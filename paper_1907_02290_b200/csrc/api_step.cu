@@ -305,13 +305,13 @@ int mwf_set_lists(mwf_ctx* c, int64_t n_group, const int32_t* grp_first, const i
     }
     const std::vector<int64_t>& list_off = plan.list_off;
     const std::vector<WorkItem>& items = plan.items;
-    const std::vector<int32_t>& order_full = plan.order_full;
     const int64_t n_items = (int64_t)items.size();
     CU(c, cudaMemcpyAsync(c->list_off, list_off.data(), (size_t)(n_group + 1) * 8, H2D, s));
     CU(c, cudaMemcpyAsync(c->items, items.data(), (size_t)n_items * sizeof(WorkItem), H2D, s));
-    CU(c, cudaMemcpyAsync(c->order_full, order_full.data(), (size_t)n_items * 4, H2D, s));
     CU(c, launch_merge_lists(n_group, c->grp_first, c->grp_n, c->st_epj_off, c->st_ids, c->st_spj_off, c->st_ids + e_epj, c->list_off,
                              c->grp_nfar, c->grp_run1, c->n_ptcl, c->n_cell, c->list, c->grp_self, c->err, s));
+    rc = schedule_full(c, n_items, s);
+    if (rc) return rc;
     ++c->n_launch;
     unsigned int e = 0;
     rc = read_err_word(c, s, &e);  // also makes the host vectors above safe to free

@@ -47,14 +47,20 @@ __global__ void __launch_bounds__(256) k_bbox_partial(const float4* __restrict__
 
 // root[0..2] = centre, root[3] = side, root[4..6] = lower corner (all fp64, rounded like the host's)
 __global__ void k_root(const float* __restrict__ part, int n_part, double* __restrict__ root) {
-    if (threadIdx.x != 0 || blockIdx.x != 0) return;
-    double lo[3], hi[3];
-    for (int a = 0; a < 3; ++a) { lo[a] = (double)part[a]; hi[a] = (double)part[3 + a]; }
-    for (int b = 1; b < n_part; ++b)
+    // one warp: min / max are exact, so the order in which the partial boxes are combined does not matter
+    if (blockIdx.x != 0 || threadIdx.x >= 32) return;
+    double lo[3] = {INFINITY, INFINITY, INFINITY}, hi[3] = {-INFINITY, -INFINITY, -INFINITY};
+    for (int b = threadIdx.x; b < n_part; b += 32)
         for (int a = 0; a < 3; ++a) {
             lo[a] = fmin(lo[a], (double)part[6 * b + a]);
             hi[a] = fmax(hi[a], (double)part[6 * b + 3 + a]);
         }
+    for (int a = 0; a < 3; ++a)
+        for (int d = 16; d > 0; d >>= 1) {
+            lo[a] = fmin(lo[a], __shfl_xor_sync(0xffffffffu, lo[a], d));
+            hi[a] = fmax(hi[a], __shfl_xor_sync(0xffffffffu, hi[a], d));
+        }
+    if (threadIdx.x != 0) return;
     double ext = 0.0;
     for (int a = 0; a < 3; ++a) {
         root[a] = __dmul_rn(0.5, __dadd_rn(lo[a], hi[a]));

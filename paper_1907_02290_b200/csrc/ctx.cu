@@ -65,7 +65,7 @@ namespace {
 inline int64_t up(int64_t x, int64_t a) { return (x + a - 1) / a * a; }
 
 struct Layout {
-    int64_t off[48];
+    int64_t off[64];
     int n = 0;
     int64_t total = 0;
     int64_t add(int64_t bytes) {
@@ -101,7 +101,7 @@ Layout make_layout(const mwf_params& p) {
     L.add(256);                                         // 18 err
     L.add(p.max_ptcl * 16);                             // 19 vel
     // device-side construction step (NEXT-2)
-    const int64_t nsb = sort_blocks(p.max_ptcl);
+    const int64_t nsb = sort_blocks(std::max<int64_t>(p.max_ptcl, mi));  // the sort of the particles' keys and that of the work items' share the scratch
     const int64_t scan_n = std::max<int64_t>(std::max<int64_t>(256 * nsb + 1, p.max_ptcl + 2), p.max_cell + 2);
     L.add(p.max_ptcl * 8);                              // 20 key_a
     L.add(p.max_ptcl * 8);                              // 21 key_b
@@ -109,7 +109,7 @@ Layout make_layout(const mwf_params& p) {
     L.add(p.max_ptcl * 4);                              // 23 idx_b
     L.add((256 * nsb + 1) * 4);                         // 24 hist
     L.add(scan_scratch_elems(scan_n) * 4);              // 25 scan_scratch (int32)
-    L.add(scan_scratch_elems(p.max_group + 2) * 8);     // 26 scan_scratch64
+    L.add(scan_scratch_elems(std::max<int64_t>(p.max_group + 2, mi + 2)) * 8);  // 26 scan_scratch64
     L.add(148 * 4 * 6 * 4);                             // 27 bbox_part
     L.add(8 * 8);                                       // 28 root
     L.add(p.max_cell * 32);                             // 29 geom
@@ -129,6 +129,13 @@ Layout make_layout(const mwf_params& p) {
     L.add((p.max_cell + 1) * 16);                       // 43 spj_lo
     L.add(p.max_group * 4);                             // 44 grp_nfar
     L.add(p.max_group * 4);                             // 45 grp_run1
+    L.add((mi + 1) * 8);                                // 46 sched cost
+    L.add((mi + 1) * 8);                                // 47 sched cum
+    L.add(mi * 8);                                      // 48 sched key_a
+    L.add(mi * 8);                                      // 49 sched key_b
+    L.add(mi * 4);                                      // 50 sched idx_a
+    L.add(mi * 4);                                      // 51 sched idx_b
+    L.add(256);                                         // 52 sched seg (2 x max(SCHED_WINDOWS, MWF_MAX_TAG) + 1 ints)
     return L;
 }
 
@@ -246,6 +253,11 @@ int mwf_create(mwf_ctx** out, const mwf_params* p, void* arena, int64_t arena_by
         q.level_bounds = (int32_t*)(b + L.off[38]);
         c->walk_warps_n = walk_warps(p->max_group);
     }
+    c->sched.cost = (int64_t*)(b + L.off[46]); c->sched.cum = (int64_t*)(b + L.off[47]);
+    c->sched.key_a = (uint64_t*)(b + L.off[48]); c->sched.key_b = (uint64_t*)(b + L.off[49]);
+    c->sched.idx_a = (int32_t*)(b + L.off[50]); c->sched.idx_b = (int32_t*)(b + L.off[51]);
+    c->sched.seg = (int32_t*)(b + L.off[52]);
+    c->sched.hist = c->bb.hist; c->sched.scan_scratch = c->bb.scan_scratch; c->sched.scan_scratch64 = c->bb.scan_scratch64;
     c->max_items = max_items_of(*p);
     c->tag_groups.assign(MWF_MAX_TAG, 0);
     bool ok = true;
@@ -270,6 +282,8 @@ int mwf_create(mwf_ctx** out, const mwf_params* p, void* arena, int64_t arena_by
     ok = ok && cudaHostAlloc(reinterpret_cast<void**>(&c->h_scalars), 16 * sizeof(int64_t), cudaHostAllocDefault) == cudaSuccess;
     ok = ok && cudaHostAlloc(reinterpret_cast<void**>(&c->h_groups), (size_t)p->max_group * 5 * sizeof(int32_t), cudaHostAllocDefault) == cudaSuccess;
     ok = ok && cudaEventCreateWithFlags(&c->ev_groups, cudaEventDisableTiming) == cudaSuccess;
+    ok = ok && cudaStreamCreateWithFlags(&c->aux_stream, cudaStreamNonBlocking) == cudaSuccess;
+    ok = ok && cudaEventCreateWithFlags(&c->ev_aux, cudaEventDisableTiming) == cudaSuccess;
     if (!ok) { mwf_destroy(c); return MWF_ECUDA; }
     *out = c;
     return MWF_OK;
@@ -290,6 +304,8 @@ int mwf_destroy(mwf_ctx* c) {
     if (c->h_scalars) cudaFreeHost(c->h_scalars);
     if (c->h_groups) cudaFreeHost(c->h_groups);
     if (c->ev_groups) cudaEventDestroy(c->ev_groups);
+    if (c->aux_stream) cudaStreamDestroy(c->aux_stream);
+    if (c->ev_aux) cudaEventDestroy(c->ev_aux);
     if (c->quad64) cudaFree(c->quad64);
     if (c->quad) cudaFree(c->quad);
     if (c->ev_store) cudaEventDestroy(c->ev_store);

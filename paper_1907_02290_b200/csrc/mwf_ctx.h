@@ -36,6 +36,8 @@ struct mwf_ctx {
     int64_t* h_scalars = nullptr; // pinned: small results of the construction step (counts, totals, validation word)
     int32_t* h_groups = nullptr;  // pinned [5 x max_group]: group ranges and list lengths on their way to the host work plan
     cudaEvent_t ev_groups{};      // the group ranges have arrived
+    cudaStream_t aux_stream{};    // construction step: the work schedule is made here while the fill walk runs on the caller's stream
+    cudaEvent_t ev_aux{};
     float fuse_kick_h = 0.f;      // mwf_step_reuse: the closing kick rides in the force kernel's epilogue (0: no kick)
     int64_t n_leaf_cells = 0;
     int32_t* grp_first = nullptr; // [max_group]
@@ -64,8 +66,7 @@ struct mwf_ctx {
     int64_t vel_hi = 0;      // velocities [0, vel_hi) have been uploaded
     std::vector<int64_t> h_item_off, h_inter, h_split;  // per group prefix of items / interactions; split group bounds
     std::vector<int32_t> h_grp_first, h_grp_n;
-    std::vector<mwf::WorkItem> h_items;   // kept for the per-tag schedule, which is made on first use
-    std::vector<int64_t> h_cost;
+    mwf::SchedBuffers sched{};            // scratch of the device-side work schedule
     bool split_ready = false;
     int64_t groups_outstanding = 0;  // MAKE_LIST: groups dispatched and not yet retrieved
     int64_t groups_dispatched = 0;
@@ -142,14 +143,14 @@ bool use_scan_refresh();
 struct Plan {
     std::vector<int64_t> list_off, item_off, inter, split;
     std::vector<WorkItem> items;
-    std::vector<int64_t> cost;
-    std::vector<int32_t> order_full;
 };
 int plan_cut(mwf_ctx* c, int64_t n_group, const int32_t* grp_first, const int32_t* grp_n, Plan& pl);
 int plan_finish(mwf_ctx* c, int64_t n_group, const int32_t* grp_n, const int32_t* n_epj_of, const int32_t* n_spj_of, Plan& pl);
 int make_plan(mwf_ctx* c, int64_t n_group, const int32_t* grp_first, const int32_t* grp_n, const int32_t* n_epj_of, const int32_t* n_spj_of, Plan& pl);
 void adopt_plan(mwf_ctx* c, Plan& pl, int64_t n_group, const int32_t* grp_first, const int32_t* grp_n, int mode);
 int ensure_split_order(mwf_ctx* c, cudaStream_t s);
+// order_full of the items now on the device (behind their upload on the stream); no host synchronisation
+int schedule_full(mwf_ctx* c, int64_t n_items, cudaStream_t s);
 
 // dispatch plumbing shared by the gravity and the short-range dispatches (api_step.cu)
 int pick_order(mwf_ctx* c, int64_t g_begin, int64_t g_end, cudaStream_t s, const int32_t** order);

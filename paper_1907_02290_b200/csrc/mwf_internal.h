@@ -141,6 +141,21 @@ cudaError_t launch_merge_lists(int64_t n_group, const int32_t* grp_first, const 
                                const int32_t* n_far, int32_t* run1_len, int64_t n_ptcl, int64_t n_cell, int32_t* list, uint8_t* grp_self,
                                unsigned int* err, cudaStream_t s);
 
+// ---- work schedule on the device (sched_kernel.cu)
+struct SchedBuffers {
+    int64_t* cost; int64_t* cum;                 // [max_items + 1]
+    uint64_t* key_a; uint64_t* key_b;            // [max_items]
+    int32_t* idx_a; int32_t* idx_b;              // [max_items]
+    int32_t* seg;                                // [2 * max windows + 1]
+    int32_t* hist; int32_t* scan_scratch; int64_t* scan_scratch64;  // scratch of the sort and the scans
+};
+struct SchedTags {                               // one window per tag: bound[t] = first group of tag t (n_tag = 0: not by tag)
+    int32_t n_tag;
+    int32_t bound[MWF_MAX_TAG + 1];
+};
+cudaError_t launch_schedule(const SchedBuffers& b, const WorkItem* items, int64_t n_items, const int64_t* list_off, int n_win, const SchedTags& tags,
+                            int32_t* order, cudaStream_t s);
+
 // ---- device-side construction step (NEXT-2): buffers carved from the arena, see build_tree.cu / build_lists.cu
 constexpr int WALK_STACK = 6144;  // >= 22 levels x 256 cells (bound derived in build_lists.cu)
 

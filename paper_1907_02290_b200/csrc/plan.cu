@@ -1,54 +1,11 @@
-// Host-side work plan: cutting groups into warp-sized work items and ordering them.
+// Host side of the work plan: cutting groups into warp-sized work items, list offsets, interaction counts (DESIGN.md
+// section 6.1).  The order in which the items are worked on is made on the device (sched_kernel.cu).
 #include <climits>
 #include <numeric>
 
 #include "mwf_ctx.h"
 
 namespace mwf {
-
-namespace {
-
-// Work order of items [b, e) of `order`: longest first (so the tail of the launch is made of short items),
-// except that the NARROW items (width <= 8: few j-pairs per staged tile, so they wait on the gathers rather
-// than on the FP32 pipe) are spread evenly over the first 7/8 of the schedule, where the wide items of the
-// other warps of the SM keep the pipe busy meanwhile.
-// Stable LSD radix sort (11-bit digits) of item indices by DESCENDING cost: O(n), ties keep item order.
-void sort_longest_first(std::vector<int32_t>& v, const std::vector<int64_t>& cost, std::vector<int32_t>& tmp) {
-    const size_t n = v.size();
-    if (n < 2) return;
-    int64_t cmax = 0;
-    for (int32_t it : v) cmax = std::max(cmax, cost[(size_t)it]);
-    tmp.resize(n);
-    for (int shift = 0; shift < 63 && (cmax >> shift) > 0; shift += 11) {
-        size_t count[2049] = {0};
-        for (int32_t it : v) ++count[(size_t)(((cmax - cost[(size_t)it]) >> shift) & 2047) + 1];
-        for (int d = 0; d < 2048; ++d) count[d + 1] += count[d];
-        for (int32_t it : v) tmp[count[(size_t)(((cmax - cost[(size_t)it]) >> shift) & 2047)]++] = it;
-        v.swap(tmp);
-    }
-}
-
-void schedule_items(std::vector<int32_t>& order, int64_t b, int64_t e, const std::vector<WorkItem>& items, const std::vector<int64_t>& cost) {
-    std::vector<int32_t> wide, narrow, tmp;
-    wide.reserve((size_t)(e - b));
-    for (int64_t k = b; k < e; ++k) {
-        const int32_t it = order[(size_t)k];
-        (items[(size_t)it].width > 8 ? wide : narrow).push_back(it);
-    }
-    sort_longest_first(wide, cost, tmp);
-    sort_longest_first(narrow, cost, tmp);
-    const size_t nw = wide.size(), nn = narrow.size();
-    const size_t span = nw - nw / 8;  // narrow items go between the first `span` wide items
-    size_t iw = 0, in = 0;
-    int64_t k = b;
-    while (iw < nw || in < nn) {
-        // keep in / nn ~ iw / span
-        const bool take_narrow = in < nn && (iw >= nw || (span > 0 ? in * span <= iw * nn : true) || iw >= span);
-        order[(size_t)k++] = take_narrow ? narrow[in++] : wide[iw++];
-    }
-}
-
-}  // namespace
 
 // How a remainder of rem < 64 particles is cut: the widths of its pieces, widest first (0-terminated).  The remainder is
 // padded to a multiple of a quantum q and cut into power-of-two pieces; q is the quantum whose modelled cost is lowest (a
@@ -115,42 +72,13 @@ int plan_cut(mwf_ctx* c, int64_t n_group, const int32_t* grp_first, const int32_
 int plan_finish(mwf_ctx* c, int64_t n_group, const int32_t* grp_n, const int32_t* n_epj_of, const int32_t* n_spj_of, Plan& pl) {
     pl.list_off.assign((size_t)n_group + 1, 0);
     pl.inter.assign((size_t)n_group + 1, 0);
-    std::vector<WorkItem>& items = pl.items;
-    std::vector<int64_t>& cost = pl.cost;
-    cost.resize(items.size());
     for (int64_t g = 0; g < n_group; ++g) {
         const int64_t n_list = (int64_t)n_epj_of[g] + n_spj_of[g];
         const int64_t n_tiles = ((int64_t)n_epj_of[g] + TILE_J - 1) / TILE_J + ((int64_t)n_spj_of[g] + TILE_J - 1) / TILE_J;  // each run in whole tiles
         pl.list_off[(size_t)g + 1] = pl.list_off[(size_t)g] + n_tiles * TILE_J;
         pl.inter[(size_t)g + 1] = pl.inter[(size_t)g] + (int64_t)grp_n[g] * n_list;
-        for (int64_t k = pl.item_off[(size_t)g]; k < pl.item_off[(size_t)g + 1]; ++k) cost[(size_t)k] = n_tiles * item_cost_per_tile(items[(size_t)k].width);
     }
-    const int64_t n_items = (int64_t)items.size();
-
-    // work schedule over everything (see schedule_items); the schedules inside the n_tag interaction-balanced group
-    // ranges that mwf_calc_force_all uses for a host destination are made on first use (ensure_split_order)
-    pl.order_full.resize((size_t)n_items);
-    std::iota(pl.order_full.begin(), pl.order_full.end(), 0);
-    // A store that does not fit the L2 is walked in SCHED_WINDOWS windows of consecutive (Morton-ordered) items of equal
-    // modelled cost, each scheduled as above: the gathers of the items in flight then touch one stretch of the store at a
-    // time (config 4, 171 MB store: DRAM traffic 6.7 -> 3.1 GB per launch at the same kernel time; a store that fits loses
-    // 0.3-0.7 % to the less even mix of long and short items, so it keeps one window).
-    const int64_t store_bytes = (c->n_ptcl + c->n_cell + 1) * (int64_t)sizeof(float4);
-    const int n_win = store_bytes > c->l2_bytes ? SCHED_WINDOWS : 1;
-    if (n_win <= 1) {
-        schedule_items(pl.order_full, 0, n_items, items, cost);
-    } else {
-        int64_t tot = 0;
-        for (int64_t k = 0; k < n_items; ++k) tot += cost[(size_t)k];
-        int64_t b = 0, acc = 0;
-        for (int w = 1; w <= n_win && b < n_items; ++w) {
-            const int64_t want = tot / n_win * w;
-            int64_t e = b;
-            while (e < n_items && (acc < want || w == n_win)) acc += cost[(size_t)e++];
-            schedule_items(pl.order_full, b, e, items, cost);
-            b = e;
-        }
-    }
+    // the group ranges of equal interaction count that mwf_calc_force_all dispatches per tag for a host destination
     pl.split.assign((size_t)c->p.n_tag + 1, 0);
     const int64_t total = pl.inter[(size_t)n_group];
     int64_t g = 0;
@@ -170,34 +98,42 @@ int make_plan(mwf_ctx* c, int64_t n_group, const int32_t* grp_first, const int32
 
 // Adopt a plan as the ctx's current lists (after the device side is in place).
 void adopt_plan(mwf_ctx* c, Plan& pl, int64_t n_group, const int32_t* grp_first, const int32_t* grp_n, int mode) {
+    c->n_items = (int64_t)pl.items.size();
+    c->padded_entries = pl.list_off[(size_t)n_group];
     c->h_item_off.swap(pl.item_off);
     c->h_inter.swap(pl.inter);
     c->h_split.swap(pl.split);
-    c->h_items.swap(pl.items);
-    c->h_cost.swap(pl.cost);
     c->split_ready = false;
     c->h_grp_first.assign(grp_first, grp_first + n_group);
     c->h_grp_n.assign(grp_n, grp_n + n_group);
     c->n_group = n_group;
-    c->n_items = (int64_t)c->h_items.size();
-    c->padded_entries = pl.list_off[(size_t)n_group];
     c->have_lists = true;
     c->lists_for_reuse = (mode == MWF_MAKE_LIST_FOR_REUSE);
     c->groups_dispatched = 0;
     c->groups_outstanding = 0;
 }
 
-// Per-tag schedules: made and uploaded the first time a dispatch covers exactly one of the balanced ranges.
+// The schedule over everything (sched_kernel.cu).  A store that does not fit the L2 is walked in SCHED_WINDOWS windows of
+// consecutive (Morton-ordered) items of equal modelled cost: the gathers of the items in flight then touch one stretch of
+// the store at a time (config 4, 171 MB store: DRAM traffic 6.7 -> 3.1 GB per launch at the same kernel time; a store that
+// fits loses 0.3-0.7 % to the less even mix of long and short items, so it keeps one window).
+int schedule_full(mwf_ctx* c, int64_t n_items, cudaStream_t s) {
+    const int64_t store_bytes = (c->n_ptcl + c->n_cell + 1) * (int64_t)sizeof(float4);
+    SchedTags none{};
+    CU(c, launch_schedule(c->sched, c->items, n_items, c->list_off, store_bytes > c->l2_bytes ? SCHED_WINDOWS : 1, none, c->order_full, s));
+    c->n_launch += 8;
+    return MWF_OK;
+}
+
+// Per-tag schedules: made the first time a dispatch covers exactly one of the balanced ranges.
 int ensure_split_order(mwf_ctx* c, cudaStream_t s) {
     if (c->split_ready) return MWF_OK;
-    std::vector<int32_t> order((size_t)c->n_items);
-    std::iota(order.begin(), order.end(), 0);
-    for (int t = 0; t < c->p.n_tag; ++t) {
-        const int64_t b = c->h_item_off[(size_t)c->h_split[(size_t)t]], e = c->h_item_off[(size_t)c->h_split[(size_t)t + 1]];
-        schedule_items(order, b, e, c->h_items, c->h_cost);
-    }
-    CU(c, cudaMemcpyAsync(c->order_split, order.data(), (size_t)c->n_items * 4, cudaMemcpyHostToDevice, s));
-    CU(c, cudaStreamSynchronize(s));
+    SchedTags tags{};
+    tags.n_tag = c->p.n_tag;
+    for (int t = 0; t <= c->p.n_tag; ++t) tags.bound[t] = (int32_t)c->h_split[(size_t)t];
+    CU(c, launch_schedule(c->sched, c->items, c->n_items, c->list_off, 1, tags, c->order_split, s));
+    CU(c, cudaStreamSynchronize(s));  // the other tags' streams read it too
+    c->n_launch += 8;
     c->split_ready = true;
     return MWF_OK;
 }
