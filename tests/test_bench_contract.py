@@ -58,5 +58,9 @@ def test_cuda_arm_line():
     assert roof["bound"] == "alu" and roof["unit"] == "TFLOP/s" and roof["kernel"] == "mwf::k_force"
     assert abs(roof["frac"] - roof["achieved"] / roof["peak"]) < 1e-12 and 0 < roof["frac"] < 1
     assert "traffic" in roof
+    assert "traffic_source" in roof and roof["kernel_ms_min"] <= roof["kernel_ms_median"]
     clk = d["clocks"]
-    assert set(("sm_mhz", "sm_max_mhz", "reasons")) <= set(clk)
+    assert set(("sm_mhz", "sm_max_mhz", "reasons", "samples", "source")) <= set(clk)
+    assert d["ms_per_step_min"] <= d["ms_per_step_median"]
+    par = d["parity"]                                   # the oracle pass of the cpu_baseline leg, compared with the GPU's result
+    assert par["ok"] and par["acc_max"] <= 1e-4 and par["acc_rms"] <= 2e-5 and par["pot_rms"] <= 1e-5 and par["particles"] > 0

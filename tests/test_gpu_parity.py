@@ -638,6 +638,50 @@ def test_reuse_run_per_step():
     f.close()
 
 
+def test_energy_over_the_reuse_run():
+    """Sanity band P11: over config 5's 8 kick-drift-kick steps with reused lists the total energy
+    E = sum m v^2 / 2 + sum m pot / 2 barely moves, and it moves the same way whether the orbit is driven by the GPU's
+    forces or by the oracle's (reduced N; the harness integrates in fp64 and uploads fp32 positions, reading O7)."""
+    cfg = CONFIGS[4]
+    w = make_workload(cfg, 40000)
+    m = w.posm[:, 3].astype(np.float64)
+    f = binding.MultiWalkForce.for_workload(w, n_tag=2)
+    f.upload_workload(w, binding.MAKE_LIST_FOR_REUSE)
+    host_in, host_out = f.pinned(w.n), f.pinned(w.n)
+
+    def gpu_forces(posm):
+        host_in.numpy()[:] = posm
+        f.begin_step(binding.REUSE_LIST)
+        f.calc_force_all(host_in, host_out)
+        out = host_out.numpy()
+        return out[:, :3].astype(np.float64), out[:, 3].astype(np.float64)
+
+    def oracle_forces(posm):
+        acc, pot, _ = oracle_eval(w, cfg.eps, posm=posm)
+        return acc, pot
+
+    energies = {}
+    for name, forces in (("gpu", gpu_forces), ("oracle", oracle_forces)):
+        x, v, posm = w.posm[:, :3].astype(np.float64), w.vel.copy(), w.posm.copy()
+        a, pot = forces(posm)
+        e = [0.5 * np.sum(m * (v * v).sum(1)) + 0.5 * np.sum(m * pot)]
+        for _ in range(cfg.n_reuse):
+            v += 0.5 * cfg.dt * a
+            x += cfg.dt * v
+            posm[:, :3] = x.astype(np.float32)
+            a, pot = forces(posm)
+            v += 0.5 * cfg.dt * a
+            e.append(0.5 * np.sum(m * (v * v).sum(1)) + 0.5 * np.sum(m * pot))
+        energies[name] = np.array(e)
+    f.close()
+    eg, eo = energies["gpu"], energies["oracle"]
+    print("energy: E0 %.6f, drift over %d steps gpu %.2e oracle %.2e, |gpu - oracle| max %.2e (relative)" % (
+        eo[0], cfg.n_reuse, (eg[-1] - eg[0]) / abs(eg[0]), (eo[-1] - eo[0]) / abs(eo[0]), np.abs(eg - eo).max() / abs(eo[0])))
+    assert abs(eo[0] / (0.5 * -3 * np.pi / 32 * 1.0055) - 1) < 0.2   # virial equilibrium: E = W / 2, W of pin P6
+    assert abs(eg[-1] - eg[0]) <= 1e-4 * abs(eg[0]) and abs(eo[-1] - eo[0]) <= 1e-4 * abs(eo[0])
+    assert np.abs(eg - eo).max() <= 1e-6 * abs(eo[0])
+
+
 # ------------------------------------------------------------------ NEXT-1: device-resident reuse steps
 def _vel4(v):
     out = np.zeros((v.shape[0], 4), np.float32)

@@ -177,3 +177,25 @@ def test_pack_data_lists_is_a_plain_gather():
         c = w.spj_id[w.spj_off[g]:w.spj_off[g + 1]]
         want = np.concatenate([w.posm[e], spj[c]])
         assert np.array_equal(rec[joff[g - g0]:joff[g - g0 + 1]], want)
+
+
+@pytest.mark.parametrize("kind,n,lo,hi", [("uniform", 60000, 0.45, 1.2), ("plummer", 65536, 0.8, 1.9)])
+def test_list_length_follows_the_papers_model(golden, kind, n, lo, hi):
+    """Sanity band P10: the particle-weighted mean list length of the harness against the paper's
+    geometric model, eq. 30, evaluated at the group-mean <n_i>.  The model counts cube surfaces in a uniform
+    medium, so a uniform sphere sits somewhat below it and a centrally concentrated one above; a band, not a pin."""
+    theta, n_grp = 0.5, 256
+    if kind == "uniform":
+        rng = np.random.default_rng(9)
+        p = rng.normal(size=(n, 3))
+        p *= (rng.uniform(0, 1, n) ** (1 / 3) / np.linalg.norm(p, axis=1))[:, None]
+        posm = np.concatenate([p, np.full((n, 1), 1.0 / n)], axis=1).astype(np.float32)
+    else:
+        posm, _ = make_particles(CONFIGS[1], n)
+    w = build_tree_and_lists(posm, 16, n_grp, theta)
+    ni = n / w.n_group
+    model = (ni + golden["nlist_c1"] * ni ** (2 / 3) / theta + golden["nlist_c2"] * np.pi * ni ** (1 / 3) / theta ** 2
+             + golden["nlist_c3"] * np.pi / (3 * theta ** 3) * np.log2(theta / golden["nlist_c4"] * (n ** (1 / 3) - ni ** (1 / 3))))
+    measured = w.interactions / n                      # sum n_i n_list / n
+    print("%s: <n_i> %.1f, <n_list> measured %.0f, eq. 30 %.0f, ratio %.2f" % (kind, ni, measured, model, measured / model))
+    assert lo < measured / model < hi
