@@ -52,8 +52,8 @@ class ClockSampler:
          "clocks_event_reasons.sw_thermal_slowdown,clocks_event_reasons.sw_power_cap")
 
     def __init__(self, index: int, period_s: float = 0.004):
-        self.rows, self.proc, self.index, self.period = [], None, index, period_s
-        self.t_begin, self.t_end, self.stop, self.thread, self.nvml, self.source = None, None, False, None, None, "none"
+        self.rows, self.rows_smi, self.proc, self.index, self.period = [], [], None, index, period_s
+        self.t_begin, self.t_end, self.stop, self.thread, self.thread_smi, self.nvml = None, None, False, None, None, None
 
     def _nvml_handle(self):
         import pynvml
@@ -69,21 +69,21 @@ class ClockSampler:
             return pynvml, pynvml.nvmlDeviceGetHandleByIndex(phys)
 
     def __enter__(self):
+        # two independent sources: an NVML thread in this process and an nvidia-smi child process (its own NVML session,
+        # untouched by this interpreter's GIL or by a slow driver call behind a busy context); summary() uses whichever
+        # put more samples inside the timed region and says how many each one had
         try:
             self.nvml, self.handle = self._nvml_handle()
             self.max_mhz = float(self.nvml.nvmlDeviceGetMaxClockInfo(self.handle, self.nvml.NVML_CLOCK_SM))
-            self.source = "nvml in-process thread, %.0f ms period" % (1e3 * self.period)
             self.thread = threading.Thread(target=self._poll_nvml, daemon=True)
             self.thread.start()
-            return self
         except Exception:
             self.nvml = None
         try:
             self.proc = subprocess.Popen(["nvidia-smi", "-i", str(self.index), "--query-gpu=" + self.Q, "--format=csv,noheader,nounits", "-lms", "20"],
-                                         stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
-            self.source = "nvidia-smi -lms 20"
-            self.thread = threading.Thread(target=self._read_smi, daemon=True)
-            self.thread.start()
+                                         stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True, bufsize=1)
+            self.thread_smi = threading.Thread(target=self._read_smi, daemon=True)
+            self.thread_smi.start()
         except OSError:
             self.proc = None
         return self
@@ -110,7 +110,7 @@ class ClockSampler:
             if len(parts) >= 7:
                 try:
                     names = ("hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap")
-                    self.rows.append((time.perf_counter(), float(parts[0]), float(parts[1]), float(parts[2]),
+                    self.rows_smi.append((time.perf_counter(), float(parts[0]), float(parts[1]), float(parts[2]),
                                       [k for k, v in zip(names, parts[3:7]) if v.lower().startswith("active")]))
                 except ValueError:
                     continue
@@ -129,21 +129,26 @@ class ClockSampler:
                 self.proc.wait(timeout=5)
             except subprocess.TimeoutExpired:
                 self.proc.kill()
-        if self.thread is not None:
-            self.thread.join(timeout=2)
+        for th in (self.thread, self.thread_smi):
+            if th is not None:
+                th.join(timeout=2)
 
     def summary(self):
         t0 = self.t_begin if self.t_begin is not None else -1e300
         t1 = self.t_end if self.t_end is not None else 1e300
-        inside = [r for r in self.rows if t0 <= r[0] <= t1]
-        rows = inside or self.rows
+        src = {"nvml in-process thread, %.0f ms period" % (1e3 * self.period): self.rows, "nvidia-smi -lms 20 (child process)": self.rows_smi}
+        inside = {k: [r for r in v if t0 <= r[0] <= t1] for k, v in src.items()}
+        best = max(src, key=lambda k: (len(inside[k]), len(src[k])))
+        rows_in, rows_all = inside[best], src[best]
+        rows = rows_in or rows_all
         if not rows:
-            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": [], "samples": 0, "source": self.source}
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": [], "samples": 0, "source": "none"}
         sm = [r[1] for r in rows]
-        reasons = sorted({k for r in rows for k in r[4]})
+        reasons = sorted({k for v in inside.values() for r in v for k in r[4]} | {k for r in rows for k in r[4]})
         return {"sm_mhz": float(np.median(sm)), "sm_min_mhz": float(min(sm)), "sm_max_mhz": float(max(r[2] for r in rows)), "reasons": reasons,
-                "samples": len(inside), "samples_outside_region": len(self.rows) - len(inside), "power_w_max": float(max(r[3] for r in rows)),
-                "region_s": None if self.t_begin is None or self.t_end is None else round(self.t_end - self.t_begin, 4), "source": self.source}
+                "samples": len(rows_in), "samples_outside_region": len(rows_all) - len(rows_in), "power_w_max": float(max(r[3] for r in rows)),
+                "region_s": None if self.t_begin is None or self.t_end is None else round(self.t_end - self.t_begin, 4), "source": best,
+                "samples_in_region_by_source": {k: len(v) for k, v in inside.items()}}
 
 
 def measured_peaks():

@@ -21,7 +21,7 @@
 //     the tolerance.
 //   * two coordinate conventions (reading S11b of DESIGN.md).  The tiles of a list's run 1 -- every EPJ entry and every
 //     FAR SPJ entry -- are swept in the caller's coordinates: particle positions are exact fp32 inputs and
-//     d = fl(x_j - x_i) is good to half an ulp of the DIFFERENCE however small it is; a cell at least a quarter of its
+//     d = fl(x_j - x_i) is good to half an ulp of the DIFFERENCE however small it is; a cell at least 1/32 of its
 //     own coordinates away from the group (SPJ_FAR_KAPPA) is placed well enough by its fp32 record.  The tiles of run 2,
 //     the NEAR SPJ entries, are swept in item-centred coordinates, c = the item's first i-particle: a centre of mass is
 //     not an fp32 input -- on the fp32 grid it is up to 2^-25 |X| off, which for a cell 1e-3 away at coordinates of
@@ -73,12 +73,12 @@ __device__ __forceinline__ void add_into(Acc2& a, const Acc2& t) {
 }
 
 // Sweep one staged tile: the lane belongs to slice `sl` of S and takes pairs sl, sl + S, ... (W = 32 / S of them).
-template <int W>
+template <int W, int UNROLL_CAP = MWF_UNROLL_WIDE>
 __device__ __forceinline__ void sweep_tile(const float4* __restrict__ sA, const float4* __restrict__ sB, int sl,
                                            const float (&nx)[2], const float (&ny)[2], const float (&nz)[2], float eps2, Acc2& t) {
     constexpr int S = 32 / W;
     const float2 e2 = make_float2(eps2, eps2);
-    constexpr int UNROLL = W < MWF_UNROLL_WIDE ? W : MWF_UNROLL_WIDE;
+    constexpr int UNROLL = W < UNROLL_CAP ? W : UNROLL_CAP;
 #pragma unroll UNROLL
     for (int pp = 0; pp < W; ++pp) {
         const int p = pp * S + sl;
@@ -117,120 +117,36 @@ __device__ __forceinline__ void ld_data_pair(const float4* __restrict__ jd, int6
     j1 = e + 1 < n_list ? __ldg(jd + e + 1) : zero;
 }
 
-// per warp: two tiles in pair layout, the item's origin and a zero, the remainders of the tile in flight
-constexpr int FORCE_SMEM_FLOAT4_PER_WARP = 2 * TILE_J + 2 + TILE_J + 2;
+// per warp: two tiles in pair layout, the remainders of the near tile in flight
+constexpr int FORCE_SMEM_FLOAT4_PER_WARP = 2 * TILE_J + TILE_J;
 
-template <int W, bool INDEXED>
-__device__ __forceinline__ void run_item(const ForceArgs& a, const WorkItem it, float4* __restrict__ sbuf, int lane) {
-    constexpr int S = 32 / W;
-    const int sl = lane / W;
-    const int il = lane % W;
-    const float4* __restrict__ J = a.store;
+#ifndef MWF_NEAR_UNROLL
+#define MWF_NEAR_UNROLL 4
+#endif
 
-    float nx[2], ny[2], nz[2], mi[2];
-    bool valid[2];
+// The lane's two i-particles (negated positions), the running totals started at minus the self term (slice 0 only:
+// the slices are added later).
+template <int W>
+__device__ __forceinline__ void item_begin(const ForceArgs& a, const WorkItem& it, int lane, float (&nx)[2], float (&ny)[2], float (&nz)[2],
+                                           bool (&valid)[2], Acc2& acc) {
+    const int sl = lane / W, il = lane % W;
+    const float self_rinv = rsqrt_approx(a.eps2);  // what the sweep computes for d = 0
+    const bool self_in = a.grp_self[it.group] != 0;
+    zero(acc);
 #pragma unroll
     for (int k = 0; k < 2; ++k) {
         const int off = il + W * k;
         valid[k] = off < it.n_i;
-        const float4 p = __ldg(J + it.i_first + (valid[k] ? off : 0));
-        nx[k] = -p.x; ny[k] = -p.y; nz[k] = -p.z; mi[k] = p.w;
+        const float4 p = __ldg(a.store + it.i_first + (valid[k] ? off : 0));
+        nx[k] = -p.x; ny[k] = -p.y; nz[k] = -p.z;
+        acc.p[k].x = (self_in && sl == 0) ? -p.w * self_rinv : 0.f;
     }
-    if constexpr (INDEXED) {  // origin of the tiles of run 2, a zero for those of run 1, no remainders yet
-        const float4 zero = make_float4(0.f, 0.f, 0.f, 0.f);
-        if (lane == 0) sbuf[2 * TILE_J] = __ldg(J + it.i_first);
-        if (lane == 1) sbuf[2 * TILE_J + 1] = zero;
-        sbuf[2 * TILE_J + 2 + lane] = zero;
-        sbuf[2 * TILE_J + 2 + 32 + lane] = zero;
-        __syncwarp();
-    }
-    const float self_rinv = rsqrt_approx(a.eps2);  // what the sweep computes for d = 0
-    const bool self_in = a.grp_self[it.group] != 0;
+}
 
-    Acc2 acc, part;
-    zero(acc);
-    zero(part);
-    // start the potential sum at minus the self term (slice 0 only: the slices are added later)
-#pragma unroll
-    for (int k = 0; k < 2; ++k) acc.p[k].x = (self_in && sl == 0) ? -mi[k] * self_rinv : 0.f;
-
-    int64_t l0, n_list = 0;
-    int n_tiles, te;  // tiles [0, te): run 1 (EPJ and far SPJ entries), [te, n_tiles): run 2 (near SPJ entries)
-    if constexpr (INDEXED) {
-        l0 = a.list_off[it.group];
-        n_tiles = (int)((a.list_off[it.group + 1] - l0) / TILE_J);
-        te = (a.run1_len[it.group] + TILE_J - 1) / TILE_J;
-
-    } else {
-        l0 = a.joff[it.group - a.g_base];
-        n_list = a.joff[it.group - a.g_base + 1] - l0;
-        n_tiles = (int)((n_list + TILE_J - 1) / TILE_J);
-        te = n_tiles;  // the records of a data list are all fp32: one convention
-    }
-    const int2* __restrict__ lst = reinterpret_cast<const int2*>(a.list + (INDEXED ? l0 : 0));
-    const float4* __restrict__ jd = a.jdata + (INDEXED ? 0 : l0);
-
-    // Every tile is staged by the same instructions: the lane's two records come from the store through their indices
-    // (particles and SPJ records alike), are moved to the tile's origin and get their remainders added, (x - c) + q.  For
-    // the tiles of run 1 both c and q are zero, which leaves x as it is; for the tiles of run 2 c is the item's origin
-    // and q the remainder of the centre of mass, brought in by cp.async one tile ahead (registers held across the sweep
-    // are what its schedule is most sensitive to).  sbuf[ORIGIN] = c, sbuf[ORIGIN + 1] = 0, lo_raw = 64 remainders.
-    constexpr int ORIGIN = 2 * TILE_J;
-    float4* lo_raw = sbuf + ORIGIN + 2;
-    const float4* __restrict__ LO = a.spj_lo - a.n_ptcl;  // SPJ entries are cell index + N
-    int2 idn = make_int2(0, 0);
-    float4 j0 = make_float4(0.f, 0.f, 0.f, 0.f), j1 = j0;
-    auto gather = [&](int t, const int2 id) {
-        j0 = __ldg(J + id.x);
-        j1 = __ldg(J + id.y);
-        if (t >= te) {
-            cp_async16(lo_raw + lane, LO + id.x);
-            cp_async16(lo_raw + 32 + lane, LO + id.y);
-            cp_async_commit();
-        }
-    };
-    if (n_tiles > 0) {
-        if constexpr (INDEXED) {
-            gather(0, ld_stream_int2(lst + lane));
-            if (n_tiles > 1) idn = ld_stream_int2(lst + 32 + lane);
-        } else {
-            ld_data_pair(jd, n_list, 0, lane, j0, j1);
-        }
-    }
-    for (int t = 0; t < n_tiles; ++t) {
-        float4* sA = sbuf + (t & 1) * TILE_J;
-        float4* sB = sA + TILE_J / 2;
-        if constexpr (INDEXED) {
-            const float4 c = sbuf[ORIGIN + (t < te ? 1 : 0)];
-            cp_async_wait_all();  // the lane's own two remainders, if any are under way
-            const float4 q0 = lo_raw[lane], q1 = lo_raw[32 + lane];
-            if (t == te) {  // from here on: item-centred
-#pragma unroll
-                for (int k = 0; k < 2; ++k) { nx[k] += c.x; ny[k] += c.y; nz[k] += c.z; }
-            }
-            sA[lane] = make_float4((j0.x - c.x) + q0.x, (j1.x - c.x) + q1.x, (j0.y - c.y) + q0.y, (j1.y - c.y) + q1.y);
-            sB[lane] = make_float4((j0.z - c.z) + q0.z, (j1.z - c.z) + q1.z, j0.w, j1.w);
-        } else {
-            sA[lane] = make_float4(j0.x, j1.x, j0.y, j1.y);
-            sB[lane] = make_float4(j0.z, j1.z, j0.w, j1.w);
-        }
-        __syncwarp();
-        if (t + 1 < n_tiles) {
-            if constexpr (INDEXED) {
-                gather(t + 1, idn);
-                if (t + 2 < n_tiles) idn = ld_stream_int2(lst + (int64_t)(t + 2) * 32 + lane);
-            } else {
-                ld_data_pair(jd, n_list, t + 1, lane, j0, j1);
-            }
-        }
-        sweep_tile<W>(sA, sB, sl, nx, ny, nz, a.eps2, part);
-        constexpr int FLUSH = S > MWF_FLUSH_MIN ? S : MWF_FLUSH_MIN;
-        if ((t & (FLUSH - 1)) == FLUSH - 1) {  // every partial sum covers 32 j-pairs whatever the slice count
-            add_into(acc, part);
-            zero(part);
-        }
-    }
-    add_into(acc, part);
+// Slices combined by shuffles; slice 0 writes (ax, ay, az, pot) and, in the device-resident step, the closing kick.
+template <int W>
+__device__ __forceinline__ void item_end(const ForceArgs& a, const WorkItem& it, int lane, const bool (&valid)[2], const Acc2& acc) {
+    const int sl = lane / W, il = lane % W;
 #pragma unroll
     for (int k = 0; k < 2; ++k) {
         float rx = acc.x[k].x + acc.x[k].y, ry = acc.y[k].x + acc.y[k].y, rz = acc.z[k].x + acc.z[k].y, rp = acc.p[k].x + acc.p[k].y;
@@ -255,6 +171,137 @@ __device__ __forceinline__ void run_item(const ForceArgs& a, const WorkItem it, 
     __syncwarp();  // the next item reuses the warp's tile buffers
 }
 
+// every partial sum covers 32 j-pairs per lane whatever the slice count (MWF_FLUSH_MIN tiles at least)
+template <int W>
+__device__ __forceinline__ void flush_partial(int t, Acc2& acc, Acc2& part) {
+    constexpr int S = 32 / W;
+    constexpr int FLUSH = S > MWF_FLUSH_MIN ? S : MWF_FLUSH_MIN;
+    if ((t & (FLUSH - 1)) == FLUSH - 1) {
+        add_into(acc, part);
+        zero(part);
+    }
+}
+
+// Index lists (method G2, the hot path), one tile loop per run.  Loop 1 (run 1: EPJ and far SPJ entries, caller's
+// coordinates) knows nothing of run 2: its staging is a plain transpose of the two gathered records.  The remainders of the
+// FIRST tile of run 2 are requested (cp.async) in the item's prologue, so that they arrive behind loop 1; between the
+// loops the i-side moves to item-centred coordinates; loop 2 stages (x - c) + q with the remainders of tile t + 1 under
+// way during the sweep of tile t.  One loop with both stagings costs 5 % on the tiles of run 1, whether a list has a run 2
+// or not (profiles/r02_kforce_variants.md); the sweep of loop 2 is unrolled less (MWF_NEAR_UNROLL) to keep the kernel small.
+template <int W>
+__device__ __forceinline__ void run_item(const ForceArgs& a, const WorkItem it, float4* __restrict__ sbuf, int lane) {
+    const int sl = lane / W;
+    const float4* __restrict__ J = a.store;
+    float4* lo_raw = sbuf + 2 * TILE_J;
+    const float4* __restrict__ LO = a.spj_lo - a.n_ptcl;  // SPJ entries are cell index + N
+
+    const int64_t l0 = a.list_off[it.group];
+    const int n_tiles = (int)((a.list_off[it.group + 1] - l0) / TILE_J);
+    // tiles [0, te): run 1 (EPJ and far SPJ entries), [te, n_tiles): run 2 (near SPJ entries)
+    const int te = (a.run1_len[it.group] + TILE_J - 1) / TILE_J;
+    const int2* __restrict__ lst = reinterpret_cast<const int2*>(a.list + l0);
+
+    int2 idn = make_int2(0, 0);
+    float4 j0 = make_float4(0.f, 0.f, 0.f, 0.f), j1 = j0;
+    if (n_tiles > 0) {
+        const int2 id = ld_stream_int2(lst + lane);
+        if (te < n_tiles) {  // remainders of the first near tile: under way while run 1 is swept
+            const int2 ide = te == 0 ? id : ld_stream_int2(lst + (int64_t)te * 32 + lane);
+            cp_async16(lo_raw + lane, LO + ide.x);
+            cp_async16(lo_raw + 32 + lane, LO + ide.y);
+            cp_async_commit();
+        }
+        j0 = __ldg(J + id.x);
+        j1 = __ldg(J + id.y);
+        if (n_tiles > 1) idn = ld_stream_int2(lst + 32 + lane);
+    }
+
+    float nx[2], ny[2], nz[2];
+    bool valid[2];
+    Acc2 acc, part;
+    item_begin<W>(a, it, lane, nx, ny, nz, valid, acc);
+    zero(part);
+
+    int t = 0;
+    for (; t < te; ++t) {
+        float4* sA = sbuf + (t & 1) * TILE_J;
+        float4* sB = sA + TILE_J / 2;
+        sA[lane] = make_float4(j0.x, j1.x, j0.y, j1.y);
+        sB[lane] = make_float4(j0.z, j1.z, j0.w, j1.w);
+        __syncwarp();
+        if (t + 1 < n_tiles) {
+            j0 = __ldg(J + idn.x);
+            j1 = __ldg(J + idn.y);
+            if (t + 2 < n_tiles) idn = ld_stream_int2(lst + (int64_t)(t + 2) * 32 + lane);
+        }
+        sweep_tile<W>(sA, sB, sl, nx, ny, nz, a.eps2, part);
+        flush_partial<W>(t, acc, part);
+    }
+    if (t < n_tiles) {
+        const float4 c = __ldg(J + it.i_first);  // from here on: item-centred
+#pragma unroll
+        for (int k = 0; k < 2; ++k) { nx[k] += c.x; ny[k] += c.y; nz[k] += c.z; }
+        for (; t < n_tiles; ++t) {
+            float4* sA = sbuf + (t & 1) * TILE_J;
+            float4* sB = sA + TILE_J / 2;
+            cp_async_wait_all();  // the lane's own two remainders
+            const float4 q0 = lo_raw[lane], q1 = lo_raw[32 + lane];
+            sA[lane] = make_float4((j0.x - c.x) + q0.x, (j1.x - c.x) + q1.x, (j0.y - c.y) + q0.y, (j1.y - c.y) + q1.y);
+            sB[lane] = make_float4((j0.z - c.z) + q0.z, (j1.z - c.z) + q1.z, j0.w, j1.w);
+            __syncwarp();
+            if (t + 1 < n_tiles) {
+                j0 = __ldg(J + idn.x);
+                j1 = __ldg(J + idn.y);
+                cp_async16(lo_raw + lane, LO + idn.x);
+                cp_async16(lo_raw + 32 + lane, LO + idn.y);
+                cp_async_commit();
+                if (t + 2 < n_tiles) idn = ld_stream_int2(lst + (int64_t)(t + 2) * 32 + lane);
+            }
+            sweep_tile<W, MWF_NEAR_UNROLL>(sA, sB, sl, nx, ny, nz, a.eps2, part);
+            flush_partial<W>(t, acc, part);
+        }
+    }
+    add_into(acc, part);
+    item_end<W>(a, it, lane, valid, acc);
+}
+
+// Data lists (method G1 of the paper, A/B variant): the group's list is a contiguous run of j RECORDS sent with the
+// dispatch; same items, same sweep, one coordinate convention (the records are all fp32).
+template <int W>
+__device__ __forceinline__ void run_item_data(const ForceArgs& a, const WorkItem it, float4* __restrict__ sbuf, int lane) {
+    const int sl = lane / W;
+    const int64_t l0 = a.joff[it.group - a.g_base];
+    const int64_t n_list = a.joff[it.group - a.g_base + 1] - l0;
+    const int n_tiles = (int)((n_list + TILE_J - 1) / TILE_J);
+    const float4* __restrict__ jd = a.jdata + l0;
+    float4 j0 = make_float4(0.f, 0.f, 0.f, 0.f), j1 = j0;
+    if (n_tiles > 0) ld_data_pair(jd, n_list, 0, lane, j0, j1);
+
+    float nx[2], ny[2], nz[2];
+    bool valid[2];
+    Acc2 acc, part;
+    item_begin<W>(a, it, lane, nx, ny, nz, valid, acc);
+    zero(part);
+    for (int t = 0; t < n_tiles; ++t) {
+        float4* sA = sbuf + (t & 1) * TILE_J;
+        float4* sB = sA + TILE_J / 2;
+        sA[lane] = make_float4(j0.x, j1.x, j0.y, j1.y);
+        sB[lane] = make_float4(j0.z, j1.z, j0.w, j1.w);
+        __syncwarp();
+        if (t + 1 < n_tiles) ld_data_pair(jd, n_list, t + 1, lane, j0, j1);
+        sweep_tile<W>(sA, sB, sl, nx, ny, nz, a.eps2, part);
+        flush_partial<W>(t, acc, part);
+    }
+    add_into(acc, part);
+    item_end<W>(a, it, lane, valid, acc);
+}
+
+template <int W, bool INDEXED>
+__device__ __forceinline__ void run_item_any(const ForceArgs& a, const WorkItem it, float4* __restrict__ sbuf, int lane) {
+    if constexpr (INDEXED) run_item<W>(a, it, sbuf, lane);
+    else run_item_data<W>(a, it, sbuf, lane);
+}
+
 // The block has blockDim.x / 32 warps (WARPS_PER_CTA for a whole-machine dispatch, fewer for a sub-wave one, see
 // launch_force); s_tiles is dynamic shared memory, two tiles per warp.
 template <bool INDEXED>
@@ -269,11 +316,11 @@ __device__ __forceinline__ void force_body(const ForceArgs& a, float4* s_tiles) 
         const int64_t pos = a.item_begin + w;
         const WorkItem it = a.items[a.order ? a.order[pos] : pos];
         switch (it.width) {
-            case 32: run_item<32, INDEXED>(a, it, sbuf, lane); break;
-            case 16: run_item<16, INDEXED>(a, it, sbuf, lane); break;
-            case 8: run_item<8, INDEXED>(a, it, sbuf, lane); break;
-            case 4: run_item<4, INDEXED>(a, it, sbuf, lane); break;
-            default: run_item<2, INDEXED>(a, it, sbuf, lane); break;
+            case 32: run_item_any<32, INDEXED>(a, it, sbuf, lane); break;
+            case 16: run_item_any<16, INDEXED>(a, it, sbuf, lane); break;
+            case 8: run_item_any<8, INDEXED>(a, it, sbuf, lane); break;
+            case 4: run_item_any<4, INDEXED>(a, it, sbuf, lane); break;
+            default: run_item_any<2, INDEXED>(a, it, sbuf, lane); break;
         }
         if (a.counter) {  // dynamic: next unclaimed item
             unsigned int nxt = 0;

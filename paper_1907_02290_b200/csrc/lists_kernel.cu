@@ -5,8 +5,8 @@
 // (the paper pads with a sentinel walk whose list is empty):
 //   run 1  entries the force kernel sweeps in the caller's coordinates with 16-byte records: every EPJ entry, and
 //          every FAR SPJ entry -- a cell whose coordinates are no larger than SPJ_FAR_KAPPA times its distance from
-//          the group, so that the fp32 rounding of its centre of mass (2^-25 of the coordinate) stays within a
-//          couple of ulps of the separation;
+//          the group, so that the fp32 rounding of its centre of mass (2^-24 of the coordinate) stays within
+//          2e-6 of the separation;
 //   run 2  the NEAR SPJ entries, swept in item-centred coordinates with the rounding remainder of the centre
 //          (reading S11b of DESIGN.md).
 // Indices are validated here, once; the force kernel then runs check-free on every reuse step.

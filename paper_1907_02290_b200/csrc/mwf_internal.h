@@ -20,10 +20,15 @@ constexpr int SCHED_WINDOWS = 16;    // Morton windows of the work schedule when
 constexpr int CHUNK_I = 64;         // i-particles of a full work item (2 per lane)
 constexpr int MIN_WIDTH = 2;        // narrowest item: 2 lanes x 2 i-particles, 16 j-slices
 // An SPJ entry is FAR when the cell's coordinates are at most this many times its distance from the group: the fp32
-// rounding of its centre of mass, 2^-25 of the coordinate, is then within 2^-23 of the separation (a couple of ulps, like
-// the difference of two particle positions), and the entry is swept like a particle, from its 16-byte record in the
-// caller's coordinates.  NEAR entries are swept in item-centred coordinates with the rounding remainder (reading S11b).
-constexpr float SPJ_FAR_KAPPA = 4.f;
+// rounding of its centre of mass, at most 2^-24 of the coordinate, is then within 32 * 2^-24 = 1.9e-6 of the separation, i.e.
+// at most 6e-6 of that entry's term and of the order of the kernel's other rounding errors (the north_star bound is 1e-4 on
+// the whole acceleration; measured maxima per config: profiles/r02_acceptance.md), and the entry is swept like a particle,
+// from its 16-byte record in the caller's coordinates.  NEAR entries are swept in item-centred coordinates with the
+// rounding remainder (reading S11b).  kappa = 4 costs 3.5 % on config 5 (31 % of the SPJ entries near instead of none).
+#ifndef MWF_KAPPA
+#define MWF_KAPPA 32.f
+#endif
+constexpr float SPJ_FAR_KAPPA = MWF_KAPPA;
 
 // One unit of work for one warp: n_i <= 2 * width consecutive i-particles of one group against the
 // group's whole list.  width = 32, 16, 8, 4 or 2 lanes hold the i-particles (2 per lane); the warp is
@@ -41,7 +46,7 @@ struct WorkItem {
 #define MWF_COST_STAGE 40
 #endif
 #ifndef MWF_UNROLL_WIDE
-#define MWF_UNROLL_WIDE 32
+#define MWF_UNROLL_WIDE 16
 #endif
 #ifndef MWF_FLUSH_MIN
 #define MWF_FLUSH_MIN 2
