@@ -3,7 +3,13 @@
 #include <climits>
 #include <numeric>
 
+#include <algorithm>
+
 #include "mwf_ctx.h"
+
+#ifndef MWF_TAPER
+#define MWF_TAPER 1
+#endif
 
 namespace mwf {
 
@@ -78,16 +84,25 @@ int plan_finish(mwf_ctx* c, int64_t n_group, const int32_t* grp_n, const int32_t
         pl.list_off[(size_t)g + 1] = pl.list_off[(size_t)g] + n_tiles * TILE_J;
         pl.inter[(size_t)g + 1] = pl.inter[(size_t)g] + (int64_t)grp_n[g] * n_list;
     }
-    // the group ranges of equal interaction count that mwf_calc_force_all dispatches per tag for a host destination
-    pl.split.assign((size_t)c->p.n_tag + 1, 0);
+    // The group ranges that mwf_calc_force_all dispatches per tag for a host destination, by interaction count: equal
+    // shares for the first half of the tags, then tapering to an eighth of a share.  The tags finish in order (stream
+    // priorities), the copies of tag t hide behind the kernels of the tags after it, and what nothing hides -- the D2H
+    // (and, in the pipelined loop, the H2D) of the LAST tag -- shrinks with its share.
+    const int n_tag = c->p.n_tag;
+    pl.split.assign((size_t)n_tag + 1, 0);
     const int64_t total = pl.inter[(size_t)n_group];
+    std::vector<double> share((size_t)n_tag);
+    double sum = 0.0;
+    for (int t = 0; t < n_tag; ++t) sum += share[(size_t)t] = MWF_TAPER ? std::min(1.0, 2.0 * (n_tag - t - 0.5) / n_tag) : 1.0;
     int64_t g = 0;
-    for (int t = 1; t < c->p.n_tag; ++t) {
-        const int64_t want = total / c->p.n_tag * t;
+    double acc = 0.0;
+    for (int t = 1; t < n_tag; ++t) {
+        acc += share[(size_t)t - 1];
+        const int64_t want = (int64_t)((double)total * (acc / sum));
         while (g < n_group && pl.inter[(size_t)g] < want) ++g;
         pl.split[(size_t)t] = g;
     }
-    pl.split[(size_t)c->p.n_tag] = n_group;
+    pl.split[(size_t)n_tag] = n_group;
     return MWF_OK;
 }
 
