@@ -407,12 +407,13 @@ def g1_leg(args, cfg, binding, device):
 
 
 def quad_leg(args, cfg, binding, device):
-    """Quadrupole SPJ (NEXT-3): the list-reuse step with order 2 -- refresh of monopoles AND quadrupoles, force kernel,
-    quadrupole correction kernel -- device-resident source and destination.  k_quad is ALU-bound like k_force: 36 packed
-    FP32 operations + 2 MUFU per i per j-pair = 60 flop per SPJ correction (FMA = 2, rsqrt = 4, the paper's counting)."""
+    """Quadrupole SPJ (NEXT-3): the list-reuse step with order 2 -- refresh of monopoles AND quadrupoles, then the order-2
+    force kernel (Q terms of the SPJ entries in the same sweep) -- device-resident source and destination.  ALU-bound like
+    k_force: 40 packed FP32 operations + 2 MUFU per i per j-pair of SPJ entries = 64 flop per SPJ interaction (FMA = 2,
+    rsqrt = 4, the paper's counting), 23 per EPJ interaction."""
     import torch
     from paper_1907_02290_b200.workload import make_workload
-    N_OP_QUAD = 60
+    N_OP_QUAD = 64   # 4 add + 14 mul + 21 fma x 2 + rsqrt counted 4, the counting that gives 23 for the monopole interaction
     w = make_workload(cfg, args.n)
     f = binding.MultiWalkForce.for_workload(w, n_tag=args.n_tag, device=device)
     f.upload_workload(w, binding.MAKE_LIST_FOR_REUSE)
@@ -425,7 +426,7 @@ def quad_leg(args, cfg, binding, device):
     res = {}
     for order in (1, 2):
         f.set_spj_order(order)
-        ms_step, ms_force, ms_quad, ms_ref = [], [], [], []
+        ms_step, ms_force, ms_ref = [], [], []
         s0 = f.streams[0]
         for it in range(args.warmup + args.steps):
             ev = [torch.cuda.Event(enable_timing=True) for _ in range(4)]
@@ -436,13 +437,13 @@ def quad_leg(args, cfg, binding, device):
             ev[3].record(s0); torch.cuda.synchronize()
             if it >= args.warmup:
                 ms_step.append(ev[0].elapsed_time(ev[3])); ms_ref.append(ev[1].elapsed_time(ev[2]))
-                q = f.last_quad_ms(0) if order == 2 else 0.0
-                ms_quad.append(q); ms_force.append(f.last_dispatch_ms(0) - q)
+                ms_force.append(f.last_dispatch_ms(0))
         r = {"ms_per_step": float(np.median(ms_step)), "refresh_ms": float(np.median(ms_ref)), "k_force_ms": float(np.median(ms_force))}
-        if order == 2:
-            tq = float(np.median(ms_quad)) * 1e-3
-            r.update({"k_quad_ms": tq * 1e3, "spj_interactions": inter_spj, "flop_per_correction": N_OP_QUAD,
-                      "k_quad_tflops": N_OP_QUAD * inter_spj / tq / 1e12, "k_quad_frac_fp32_peak": N_OP_QUAD * inter_spj / tq / peak})
+        if order == 2:  # one kernel: 23 flop per EPJ interaction, N_OP_QUAD per SPJ interaction (monopole + Q terms from one distance)
+            tq = r["k_force_ms"] * 1e-3
+            flop = 23.0 * (inter - inter_spj) + N_OP_QUAD * inter_spj
+            r.update({"kernel": "mwf::k_force_quad", "spj_interactions": inter_spj, "flop_per_spj_interaction": N_OP_QUAD,
+                      "tflops": flop / tq / 1e12, "frac_fp32_peak": flop / tq / peak})
         res["order_%d" % order] = r
     f.close()
     print(json.dumps({"leg": "quad", "config": workload_config(cfg, w), "steps": args.steps, "warmup": args.warmup,
@@ -793,6 +794,31 @@ def main():
     except binding.MwfError as ex:
         batched = {"error": str(ex)}
 
+    # ---- NEXT-3: the same list-reuse step with quadrupole SPJ (order 2: Q terms of the SPJ entries in the same sweep)
+    order2 = None
+    try:
+        inter_spj = int(np.sum(w.grp_n.astype(np.int64) * np.diff(w.spj_off)))
+        f.set_spj_order(2)
+        ms2, s0 = [], f.streams[0]
+        for it in range(2 + 3):
+            f.begin_step(binding.REUSE_LIST)
+            f.set_particles(src_dev, 0, w.n, s0)
+            f.refresh_monopoles(s0)
+            f.dispatch(0, 0, w.n_group)
+            f.retrieve(0, dst_dev)
+            torch.cuda.synchronize()
+            if it >= 2:
+                ms2.append(f.last_dispatch_ms(0))
+        t2 = float(np.median(ms2)) * 1e-3
+        n_sm2 = torch.cuda.get_device_properties(local).multi_processor_count
+        peak2 = n_sm2 * 256 * (measured_peaks().get("sm_max_mhz") or 1965.0) * 1e6
+        order2 = {"kernel": "mwf::k_force_quad", "kernel_ms": t2 * 1e3, "spj_interactions": inter_spj, "flop": "23 per EPJ interaction, 64 per SPJ interaction",
+                  "frac_fp32_peak": (23.0 * (inter - inter_spj) + 64.0 * inter_spj) / t2 / peak2,
+                  "what": "mwf_set_spj_order(2): refresh of monopoles and quadrupoles, one kernel (median of 3 launches, CUDA events)"}
+        f.set_spj_order(1)
+    except binding.MwfError as ex:
+        order2 = {"error": str(ex)}
+
     # ---- NEXT-1: device-resident reuse steps (kick-drift, refresh, force, kick; no host transfer)
     dev_res = None
     if w.vel is not None and cfg.dt > 0:
@@ -926,7 +952,7 @@ def main():
             "e2e_blocking_call": {"value": e2e_value, "unit": UNIT, "h2d_bytes_per_step": 16 * w.n, "d2h_bytes_per_step": 16 * w.n,
                                   "ms_per_step": ms_e_max / args.steps,
                                   "what": "one blocking mwf_calc_force_all per step, pinned host source and destination (the H2D cannot overlap the kernels)"},
-            "gpu_launches": launches, "clocks": clk, "phases": phases, "device_resident_step": dev_res, "batched_dispatch": batched,
+            "gpu_launches": launches, "clocks": clk, "phases": phases, "device_resident_step": dev_res, "batched_dispatch": batched, "order2_step": order2,
             "run_n_reuse_%d" % max(cfg.n_reuse, 0): whole_run,
             "construction_step": {"host_tree_and_lists_s": round(t_build, 3), "upload_tree_and_lists_s": round(t_upload, 3), "on_device": dev_build},
             "context": {"paper_fraction_of_peak": 0.27, "paper_hardware": "TITAN V (P:673), whole step"},

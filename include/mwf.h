@@ -163,14 +163,13 @@ int mwf_dispatch_data(mwf_ctx* c, int32_t tag, int64_t g_begin, int64_t g_end, c
  *     pot_i -= G [ M/s - tr(Q)/(2 s^3) + 3 (R.Q.R)/(2 s^5) ]
  *     acc_i += G [ M R/s^3 - 3 tr(Q) R/(2 s^5) - 3 (Q R)/s^5 + 15 (R.Q.R) R/(2 s^7) ]
  * mwf_refresh_monopoles() then also computes Q bottom-up (parallel-axis theorem, fp64), and every mwf_dispatch()
- * runs a second kernel behind the force kernel that adds the Q terms of the SPJ part of each group's list.
+ * runs the order-2 force kernel: the same sweep over the same lists, with the Q terms of the SPJ entries evaluated
+ * from the same distances and reciprocal square roots as their monopole terms (one kernel, one pass over the lists).
  * Allocates 80 B per max_cell with cudaMalloc on first use (MWF_ENOMEM); marks the moments stale when the order
  * changes; MWF_ESTATE while a tag is in flight or unretrieved.  mwf_dispatch_data() supports order 1 only. */
 int mwf_set_spj_order(mwf_ctx* c, int order);
 /* Test hook: 8 floats per cell (Qxx Qyy Qzz Qxy Qxz Qyz tr(Q)/2 0) as the refresh stored them.  dst HOST or DEVICE. */
 int mwf_get_quadrupoles(mwf_ctx* c, float* dst, int dst_on_device);
-/* Timing hook: ms of the quadrupole kernel of the last mwf_dispatch on `tag` (mwf_last_dispatch_ms covers both kernels). */
-int mwf_last_quad_ms(mwf_ctx* c, int32_t tag, float* ms);
 
 /* ---- Short-range workload through the same index lists (paper P:79: "In the case of
  * short-range interaction such as SPH interaction between particles, we still use treewalk but with cell-opening

@@ -24,7 +24,7 @@ SYMBOLS = (
     "mwf_calc_force_all", "mwf_get_monopoles", "mwf_device_pointers", "mwf_sync", "mwf_get_counters",
     "mwf_last_dispatch_ms", "mwf_strerror", "mwf_last_cuda_error",
     "mwf_set_velocities", "mwf_get_velocities", "mwf_kick_drift", "mwf_kick", "mwf_step_reuse",
-    "mwf_reserve_data_lists", "mwf_dispatch_data", "mwf_set_spj_order", "mwf_get_quadrupoles", "mwf_last_quad_ms",
+    "mwf_reserve_data_lists", "mwf_dispatch_data", "mwf_set_spj_order", "mwf_get_quadrupoles",
     "mwf_set_sph", "mwf_get_sph", "mwf_dispatch_density", "mwf_dispatch_hydro", "mwf_calc_sph_all",
     "mwf_build", "mwf_build_neighbours", "mwf_get_build_sizes", "mwf_get_permutation", "mwf_get_tree", "mwf_get_groups", "mwf_get_lists", "mwf_get_list_buffer",
     "mwf_set_particles_next", "mwf_swap_store", "mwf_get_tag_split",
@@ -86,7 +86,6 @@ def load_library(path: str | None = None) -> ctypes.CDLL:
         "mwf_step_reuse": [vp, ctypes.c_float],
         "mwf_set_spj_order": [vp, ci],
         "mwf_get_quadrupoles": [vp, vp, ci],
-        "mwf_last_quad_ms": [vp, i32, P(ctypes.c_float)],
         "mwf_reserve_data_lists": [vp, i64],
         "mwf_dispatch_data": [vp, i32, i64, i64, vp, vp, ci],
         "mwf_set_sph": [vp, vp, i64, i64, ci, vp],
@@ -248,11 +247,6 @@ class MultiWalkForce:
         out = np.empty((n_cell, 8), np.float32)
         self._ck(self._lib.mwf_get_quadrupoles(self._h, _host_ptr(out, np.float32, "dst"), 0))
         return out
-
-    def last_quad_ms(self, tag: int) -> float:
-        ms = ctypes.c_float(0)
-        self._ck(self._lib.mwf_last_quad_ms(self._h, int(tag), ctypes.byref(ms)))
-        return float(ms.value)
 
     def reserve_data_lists(self, max_entry_per_tag: int):
         self._ck(self._lib.mwf_reserve_data_lists(self._h, int(max_entry_per_tag)))

@@ -46,7 +46,6 @@ static int sph_dispatch(mwf_ctx* c, int32_t tag, int64_t g_begin, int64_t g_end,
     CU(c, cudaEventRecord(c->ev_k1[tag], s));
     CU(c, cudaEventRecord(c->ev_tag[tag], s));
     c->tag_timed[tag] = true;
-    c->tag_quad[tag] = false;
     book_dispatch(c, tag, g_begin, g_end);
     return MWF_OK;
 }
@@ -117,13 +116,10 @@ int mwf_step_reuse(mwf_ctx* c, float dt) {
     c->groups_outstanding -= c->tag_groups[0];
     c->tag_groups[0] = 0;
     c->tag_ranges[0].clear();
-    const bool fused = c->spj_order == 1;  // the closing kick rides in the force kernel's epilogue (with quadrupoles a second
-    c->fuse_kick_h = fused ? 0.5f * dt : 0.f;  // kernel still adds to the result, so the kick stays a pass of its own)
+    c->fuse_kick_h = 0.5f * dt;  // the closing kick rides in the force kernel's epilogue
     rc = mwf_dispatch(c, 0, 0, c->n_group);
     c->fuse_kick_h = 0.f;
-    if (rc) return rc;
-    if (fused) return MWF_OK;
-    return mwf_kick(c, dt, s0);
+    return rc;
 }
 
 // ---- short-range workload (NEXT-4)
@@ -214,7 +210,7 @@ int mwf_set_spj_order(mwf_ctx* c, int order) {
         }
         c->quad64 = static_cast<double*>(a);
         c->quad = static_cast<float4*>(b);
-        c->quad_ctas_per_sm = quad_max_ctas_per_sm();
+        c->quad_ctas_per_sm = force_quad_max_ctas_per_sm();
         if (c->quad_ctas_per_sm < 1) return MWF_ECUDA;
     }
     if (order != c->spj_order) {
@@ -231,15 +227,6 @@ int mwf_get_quadrupoles(mwf_ctx* c, float* dst, int dst_on_device) {
     if (!c->have_tree || !c->mono_fresh || c->spj_order != 2) return MWF_ESTATE;
     CU(c, cudaDeviceSynchronize());
     CU(c, cudaMemcpy(dst, c->quad, (size_t)c->n_cell * 32, dst_on_device ? cudaMemcpyDeviceToDevice : cudaMemcpyDeviceToHost));
-    return MWF_OK;
-}
-
-int mwf_last_quad_ms(mwf_ctx* c, int32_t tag, float* ms) {
-    MWF_ENTER(c);
-    if (!c || tag < 0 || tag >= c->p.n_tag || !ms) return MWF_EINVAL;
-    if (!c->tag_timed[tag] || !c->tag_quad[tag]) return MWF_ESTATE;
-    CU(c, cudaEventSynchronize(c->ev_k1[tag]));
-    CU(c, cudaEventElapsedTime(ms, c->ev_kq[tag], c->ev_k1[tag]));
     return MWF_OK;
 }
 

@@ -67,13 +67,16 @@ static int dispatch_launch(mwf_ctx* c, int32_t tag, int64_t g_begin, int64_t g_e
     a.n_items = c->h_item_off[(size_t)g_end] - a.item_begin;
     a.eps2 = c->p.eps * c->p.eps;
     a.G = c->p.G;
-    a.vel = (c->fuse_kick_h != 0.f && !jdata && c->spj_order == 1) ? c->vel : nullptr;
+    a.quad = (c->spj_order == 2 && !jdata) ? c->quad : nullptr;  // order 2: the Q terms of the SPJ entries in the same sweep
+    a.n_far = c->grp_nfar;
+    a.n_cell = (int32_t)c->n_cell;
+    a.vel = (c->fuse_kick_h != 0.f && !jdata) ? c->vel : nullptr;
     a.kick_h = c->fuse_kick_h;
     {
         const int rc = pick_order(c, g_begin, g_end, s, &a.order);
         if (rc) return rc;
     }
-    const int64_t resident = (int64_t)c->n_sm * c->ctas_per_sm;
+    const int64_t resident = (int64_t)c->n_sm * (a.quad ? c->quad_ctas_per_sm : c->ctas_per_sm);
     const int64_t want = (a.n_items + WARPS_PER_CTA - 1) / WARPS_PER_CTA;
     int grid = (int)resident, warps = WARPS_PER_CTA;
     a.counter = nullptr;
@@ -86,25 +89,6 @@ static int dispatch_launch(mwf_ctx* c, int32_t tag, int64_t g_begin, int64_t g_e
     }
     CU(c, cudaEventRecord(c->ev_k0[tag], s));
     CU(c, launch_force(a, grid, warps, s));
-    c->tag_quad[tag] = false;
-    if (c->spj_order == 2) {  // quadrupole terms of the SPJ entries, added behind the monopole kernel
-        QuadArgs q;
-        q.store = c->store; q.quad = c->quad; q.list = c->list; q.list_off = c->list_off;
-        q.epj_off = c->st_epj_off; q.spj_off = c->st_spj_off; q.n_far = c->grp_nfar;
-        q.items = c->items; q.order = a.order; q.accp = c->accp;
-        q.item_begin = a.item_begin; q.n_items = a.n_items; q.n_ptcl = c->n_ptcl; q.eps2 = a.eps2; q.G = a.G;
-        const int64_t qres = (int64_t)c->n_sm * c->quad_ctas_per_sm;
-        const int qgrid = (int)std::min(want, qres);
-        q.counter = nullptr;
-        if (want > qres) {
-            q.counter = c->counters + (c->counter_seq++ % N_COUNTER);
-            CU(c, cudaMemsetAsync(q.counter, 0, sizeof(unsigned int), s));
-        }
-        CU(c, cudaEventRecord(c->ev_kq[tag], s));
-        CU(c, launch_quad(q, qgrid, s));
-        c->tag_quad[tag] = true;
-        ++c->n_launch;
-    }
     CU(c, cudaEventRecord(c->ev_k1[tag], s));
     CU(c, cudaEventRecord(c->ev_tag[tag], s));
     c->tag_timed[tag] = true;

@@ -273,7 +273,6 @@ int mwf_create(mwf_ctx** out, const mwf_params* p, void* arena, int64_t arena_by
         ok = ok && cudaEventCreateWithFlags(&c->ev_tag[t], cudaEventDisableTiming) == cudaSuccess;
         ok = ok && cudaEventCreate(&c->ev_k0[t]) == cudaSuccess;
         ok = ok && cudaEventCreate(&c->ev_k1[t]) == cudaSuccess;
-        ok = ok && cudaEventCreate(&c->ev_kq[t]) == cudaSuccess;
     }
     ok = ok && cudaEventCreateWithFlags(&c->ev_store, cudaEventDisableTiming) == cudaSuccess;
     ok = ok && cudaEventCreateWithFlags(&c->ev_next, cudaEventDisableTiming) == cudaSuccess;
@@ -299,7 +298,6 @@ int mwf_destroy(mwf_ctx* c) {
         if (c->ev_tag[t]) cudaEventDestroy(c->ev_tag[t]);
         if (c->ev_k0[t]) cudaEventDestroy(c->ev_k0[t]);
         if (c->ev_k1[t]) cudaEventDestroy(c->ev_k1[t]);
-        if (c->ev_kq[t]) cudaEventDestroy(c->ev_kq[t]);
     }
     if (c->h_scalars) cudaFreeHost(c->h_scalars);
     if (c->h_groups) cudaFreeHost(c->h_groups);

@@ -50,6 +50,10 @@ __device__ __forceinline__ int2 ld_stream_int2(const int2* p) {
 __device__ __forceinline__ void cp_async16(float4* smem, const float4* gmem) {
     asm volatile("cp.async.ca.shared.global [%0], [%1], 16;" ::"r"((unsigned)__cvta_generic_to_shared(smem)), "l"(gmem) : "memory");
 }
+// the same with src_bytes (0 or 16) read and the rest of the 16 bytes zero-filled
+__device__ __forceinline__ void cp_async16_zfill(float4* smem, const float4* gmem, int src_bytes) {
+    asm volatile("cp.async.ca.shared.global [%0], [%1], 16, %2;" ::"r"((unsigned)__cvta_generic_to_shared(smem)), "l"(gmem), "r"(src_bytes) : "memory");
+}
 __device__ __forceinline__ void cp_async_commit() { asm volatile("cp.async.commit_group;" ::: "memory"); }
 __device__ __forceinline__ void cp_async_wait_all() { asm volatile("cp.async.wait_all;" ::: "memory"); }
 
@@ -122,6 +126,9 @@ constexpr int FORCE_SMEM_FLOAT4_PER_WARP = 2 * TILE_J + TILE_J;
 
 #ifndef MWF_NEAR_UNROLL
 #define MWF_NEAR_UNROLL 4
+#endif
+#ifndef MWF_QUAD_UNROLL
+#define MWF_QUAD_UNROLL 4
 #endif
 
 // The lane's two i-particles (negated positions), the running totals started at minus the self term (slice 0 only:
@@ -296,6 +303,186 @@ __device__ __forceinline__ void run_item_data(const ForceArgs& a, const WorkItem
     item_end<W>(a, it, lane, valid, acc);
 }
 
+// ---- order 2 (NEXT-3, reading S22): the quadrupole terms of the SPJ entries in the same sweep ---------------------------
+// A quad tile carries, per j-pair, the two tile rows of the monopole sweep and Q of the two cells: [qxx qyy] [qzz qxy]
+// [qxz qyz] and -tr(Q)/2 (zero for particles and padding).  With R = X - x_i, s^2 = |R|^2 + eps^2 (include/mwf.h):
+//     potential sum  += m/s - (tr/2)/s^3 + (3/2) (R.Q.R)/s^5
+//     acceleration   += [ m/s^3 - 3 (tr/2)/s^5 + (15/2) (R.Q.R)/s^7 ] R - 3 (Q R)/s^5
+// 40 packed FP32 operations + 2 MUFU per i per j-pair; distances, r^2, rsqrt and the gathers are those of the monopole
+// interaction and are not done twice (a separate correction kernel behind k_force cost 36 + 13 operations and a second
+// pass over the lists).
+constexpr int QUAD_TILE_FLOAT4 = 5 * 32 + 16;                                    // five rows of 32 pairs + 32 float2
+#ifndef MWF_QUAD_ASYNC
+#define MWF_QUAD_ASYNC 1
+#endif
+// + remainders of the near tile in flight + (MWF_QUAD_ASYNC) the Q records of the tile in flight, as gathered
+constexpr int QUAD_SMEM_FLOAT4_PER_WARP = 2 * QUAD_TILE_FLOAT4 + TILE_J + (MWF_QUAD_ASYNC ? 2 * TILE_J : 0);
+
+template <int W>
+__device__ __forceinline__ void sweep_tile_quad(const float4* __restrict__ T, int sl, const float (&nx)[2], const float (&ny)[2],
+                                                const float (&nz)[2], float eps2, Acc2& t) {
+    constexpr int S = 32 / W;
+    const float2 e2 = make_float2(eps2, eps2);
+    const float2 p15 = make_float2(1.5f, 1.5f), p75 = make_float2(7.5f, 7.5f), p3 = make_float2(3.f, 3.f), m3 = make_float2(-3.f, -3.f);
+    const float2* __restrict__ H = reinterpret_cast<const float2*>(T + 160);
+    constexpr int UNROLL = W < MWF_QUAD_UNROLL ? W : MWF_QUAD_UNROLL;
+#pragma unroll UNROLL
+    for (int pp = 0; pp < W; ++pp) {
+        const int p = pp * S + sl;
+        const float4 A = T[p], B = T[32 + p], C = T[64 + p], D = T[96 + p], E = T[128 + p];
+        const float2 nh = H[p];
+        const float2 jx = make_float2(A.x, A.y), jy = make_float2(A.z, A.w), jz = make_float2(B.x, B.y), jm = make_float2(B.z, B.w);
+        const float2 qxx = make_float2(C.x, C.y), qyy = make_float2(C.z, C.w), qzz = make_float2(D.x, D.y), qxy = make_float2(D.z, D.w);
+        const float2 qxz = make_float2(E.x, E.y), qyz = make_float2(E.z, E.w);
+#pragma unroll
+        for (int k = 0; k < 2; ++k) {
+            const float2 dx = __fadd2_rn(jx, make_float2(nx[k], nx[k]));
+            const float2 dy = __fadd2_rn(jy, make_float2(ny[k], ny[k]));
+            const float2 dz = __fadd2_rn(jz, make_float2(nz[k], nz[k]));
+            float2 r2 = __ffma2_rn(dx, dx, e2);
+            r2 = __ffma2_rn(dy, dy, r2);
+            r2 = __ffma2_rn(dz, dz, r2);
+            float2 ri;
+            ri.x = rsqrt_approx(r2.x);
+            ri.y = rsqrt_approx(r2.y);
+            const float2 mr = __fmul2_rn(jm, ri);
+            const float2 ri2 = __fmul2_rn(ri, ri);
+            const float2 mr3 = __fmul2_rn(mr, ri2);
+            const float2 ri3 = __fmul2_rn(ri2, ri);
+            const float2 ri5 = __fmul2_rn(ri3, ri2);
+            const float2 ri7 = __fmul2_rn(ri5, ri2);
+            float2 Qx = __fmul2_rn(qxx, dx);
+            Qx = __ffma2_rn(qxy, dy, Qx);
+            Qx = __ffma2_rn(qxz, dz, Qx);
+            float2 Qy = __fmul2_rn(qxy, dx);
+            Qy = __ffma2_rn(qyy, dy, Qy);
+            Qy = __ffma2_rn(qyz, dz, Qy);
+            float2 Qz = __fmul2_rn(qxz, dx);
+            Qz = __ffma2_rn(qyz, dy, Qz);
+            Qz = __ffma2_rn(qzz, dz, Qz);
+            float2 dQd = __fmul2_rn(dx, Qx);
+            dQd = __ffma2_rn(dy, Qy, dQd);
+            dQd = __ffma2_rn(dz, Qz, dQd);
+            t.p[k] = __fadd2_rn(t.p[k], mr);
+            t.p[k] = __ffma2_rn(nh, ri3, t.p[k]);
+            const float2 u = __fmul2_rn(dQd, ri5);
+            t.p[k] = __ffma2_rn(p15, u, t.p[k]);
+            const float2 v = __fmul2_rn(nh, ri5);
+            float2 c1 = __ffma2_rn(p3, v, mr3);
+            const float2 w = __fmul2_rn(dQd, ri7);
+            c1 = __ffma2_rn(p75, w, c1);
+            const float2 c2 = __fmul2_rn(m3, ri5);
+            t.x[k] = __ffma2_rn(c1, dx, t.x[k]);
+            t.y[k] = __ffma2_rn(c1, dy, t.y[k]);
+            t.z[k] = __ffma2_rn(c1, dz, t.z[k]);
+            t.x[k] = __ffma2_rn(c2, Qx, t.x[k]);
+            t.y[k] = __ffma2_rn(c2, Qy, t.y[k]);
+            t.z[k] = __ffma2_rn(c2, Qz, t.z[k]);
+        }
+    }
+}
+
+struct QuadRec {
+    float4 a, b;  // (Qxx Qyy Qzz Qxy) (Qxz Qyz tr/2 0)
+};
+
+template <int W>
+__device__ __forceinline__ void run_item_quad(const ForceArgs& a, const WorkItem it, float4* __restrict__ sbuf, int lane) {
+    const int sl = lane / W;
+    const float4* __restrict__ J = a.store;
+    float4* lo_raw = sbuf + 2 * QUAD_TILE_FLOAT4;
+    float4* q_raw = lo_raw + TILE_J;
+    const float4* __restrict__ LO = a.spj_lo - a.n_ptcl;
+
+    const int64_t l0 = a.list_off[it.group];
+    const int n_tiles = (int)((a.list_off[it.group + 1] - l0) / TILE_J);
+    const int run1 = a.run1_len[it.group];
+    const int te = (run1 + TILE_J - 1) / TILE_J;                  // first tile of run 2
+    const int ts = (run1 - a.n_far[it.group]) / TILE_J;           // first tile with an SPJ entry (whole EPJ tiles before it)
+    const int2* __restrict__ lst = reinterpret_cast<const int2*>(a.list + l0);
+
+    int2 idn = make_int2(0, 0);
+    float4 j0 = make_float4(0.f, 0.f, 0.f, 0.f), j1 = j0;
+    QuadRec q0, q1;
+    q0.a = q0.b = q1.a = q1.b = j0;
+    // records of the lane's two entries of tile t; from tile ts on with Q (zero for particles and the padding), from te on
+    // also the remainders of the centres of mass (cp.async into lo_raw)
+    auto gather = [&](int t, const int2 id) {
+        j0 = __ldg(J + id.x);
+        j1 = __ldg(J + id.y);
+        if (t >= ts) {
+            const unsigned c0 = (unsigned)(id.x - a.n_ptcl), c1 = (unsigned)(id.y - a.n_ptcl);
+            const bool v0 = c0 < (unsigned)a.n_cell, v1 = c1 < (unsigned)a.n_cell;
+#if MWF_QUAD_ASYNC
+            const float4* g0 = a.quad + (v0 ? 2 * (size_t)c0 : 0), *g1 = a.quad + (v1 ? 2 * (size_t)c1 : 0);
+            cp_async16_zfill(q_raw + lane, g0, v0 ? 16 : 0);
+            cp_async16_zfill(q_raw + 32 + lane, g0 + 1, v0 ? 16 : 0);
+            cp_async16_zfill(q_raw + 64 + lane, g1, v1 ? 16 : 0);
+            cp_async16_zfill(q_raw + 96 + lane, g1 + 1, v1 ? 16 : 0);
+#else
+            const float4 z = make_float4(0.f, 0.f, 0.f, 0.f);
+            q0.a = v0 ? __ldg(a.quad + 2 * (size_t)c0) : z;
+            q0.b = v0 ? __ldg(a.quad + 2 * (size_t)c0 + 1) : z;
+            q1.a = v1 ? __ldg(a.quad + 2 * (size_t)c1) : z;
+            q1.b = v1 ? __ldg(a.quad + 2 * (size_t)c1 + 1) : z;
+#endif
+        }
+        if (t >= te) {
+            cp_async16(lo_raw + lane, LO + id.x);
+            cp_async16(lo_raw + 32 + lane, LO + id.y);
+        }
+        if (t >= ts) cp_async_commit();
+    };
+    if (n_tiles > 0) {
+        gather(0, ld_stream_int2(lst + lane));
+        if (n_tiles > 1) idn = ld_stream_int2(lst + 32 + lane);
+    }
+
+    float nx[2], ny[2], nz[2];
+    bool valid[2];
+    Acc2 acc, part;
+    item_begin<W>(a, it, lane, nx, ny, nz, valid, acc);
+    zero(part);
+    const float4 c = __ldg(J + it.i_first);  // origin of the tiles of run 2
+
+    for (int t = 0; t < n_tiles; ++t) {
+        float4* T = sbuf + (t & 1) * QUAD_TILE_FLOAT4;
+        if (t < te) {
+            T[lane] = make_float4(j0.x, j1.x, j0.y, j1.y);
+            T[32 + lane] = make_float4(j0.z, j1.z, j0.w, j1.w);
+        } else {
+            if (t == te) {  // from here on: item-centred
+#pragma unroll
+                for (int k = 0; k < 2; ++k) { nx[k] += c.x; ny[k] += c.y; nz[k] += c.z; }
+            }
+            cp_async_wait_all();  // the lane's own remainders (and Q records)
+            const float4 r0 = lo_raw[lane], r1 = lo_raw[32 + lane];
+            T[lane] = make_float4((j0.x - c.x) + r0.x, (j1.x - c.x) + r1.x, (j0.y - c.y) + r0.y, (j1.y - c.y) + r1.y);
+            T[32 + lane] = make_float4((j0.z - c.z) + r0.z, (j1.z - c.z) + r1.z, j0.w, j1.w);
+        }
+        if (t >= ts) {
+#if MWF_QUAD_ASYNC
+            cp_async_wait_all();
+            q0.a = q_raw[lane]; q0.b = q_raw[32 + lane]; q1.a = q_raw[64 + lane]; q1.b = q_raw[96 + lane];
+#endif
+            T[64 + lane] = make_float4(q0.a.x, q1.a.x, q0.a.y, q1.a.y);
+            T[96 + lane] = make_float4(q0.a.z, q1.a.z, q0.a.w, q1.a.w);
+            T[128 + lane] = make_float4(q0.b.x, q1.b.x, q0.b.y, q1.b.y);
+            reinterpret_cast<float2*>(T + 160)[lane] = make_float2(-q0.b.z, -q1.b.z);
+        }
+        __syncwarp();
+        if (t + 1 < n_tiles) {
+            gather(t + 1, idn);
+            if (t + 2 < n_tiles) idn = ld_stream_int2(lst + (int64_t)(t + 2) * 32 + lane);
+        }
+        if (t < ts) sweep_tile<W, MWF_NEAR_UNROLL>(T, T + 32, sl, nx, ny, nz, a.eps2, part);
+        else sweep_tile_quad<W>(T, sl, nx, ny, nz, a.eps2, part);
+        flush_partial<W>(t, acc, part);
+    }
+    add_into(acc, part);
+    item_end<W>(a, it, lane, valid, acc);
+}
+
 template <int W, bool INDEXED>
 __device__ __forceinline__ void run_item_any(const ForceArgs& a, const WorkItem it, float4* __restrict__ sbuf, int lane) {
     if constexpr (INDEXED) run_item<W>(a, it, sbuf, lane);
@@ -344,7 +531,36 @@ __global__ void __launch_bounds__(WARPS_PER_CTA * 32, MWF_MIN_CTAS) k_force_data
     force_body<false>(a, s_force_tiles);
 }
 
+// Order 2: the same items and schedule, quadrupole terms of the SPJ entries in the sweep (NEXT-3).
+__global__ void __launch_bounds__(WARPS_PER_CTA * 32, MWF_MIN_CTAS) k_force_quad(const ForceArgs a) {
+    const int lane = threadIdx.x & 31;
+    const int warp = threadIdx.x >> 5;
+    const int warps_per_cta = blockDim.x >> 5;
+    float4* sbuf = s_force_tiles + warp * QUAD_SMEM_FLOAT4_PER_WARP;
+    int64_t w = (int64_t)blockIdx.x * warps_per_cta + warp;
+    const int64_t n_warps = (int64_t)gridDim.x * warps_per_cta;
+    while (w < a.n_items) {
+        const int64_t pos = a.item_begin + w;
+        const WorkItem it = a.items[a.order ? a.order[pos] : pos];
+        switch (it.width) {
+            case 32: run_item_quad<32>(a, it, sbuf, lane); break;
+            case 16: run_item_quad<16>(a, it, sbuf, lane); break;
+            case 8: run_item_quad<8>(a, it, sbuf, lane); break;
+            case 4: run_item_quad<4>(a, it, sbuf, lane); break;
+            default: run_item_quad<2>(a, it, sbuf, lane); break;
+        }
+        if (a.counter) {
+            unsigned int nxt = 0;
+            if (lane == 0) nxt = atomicAdd(a.counter, 1u);
+            w = n_warps + (int64_t)__shfl_sync(0xffffffffu, nxt, 0);
+        } else {
+            w += n_warps;
+        }
+    }
+}
+
 constexpr size_t FORCE_SMEM_PER_WARP = FORCE_SMEM_FLOAT4_PER_WARP * sizeof(float4);
+constexpr size_t QUAD_SMEM_PER_WARP = QUAD_SMEM_FLOAT4_PER_WARP * sizeof(float4);
 
 // warps = warps per block: WARPS_PER_CTA for a dispatch that fills the machine (persistent grid, items claimed dynamically);
 // a sub-wave dispatch (a batch of the multiwalk pipeline) is launched with small blocks, one item per warp, so
@@ -353,11 +569,27 @@ constexpr size_t FORCE_SMEM_PER_WARP = FORCE_SMEM_FLOAT4_PER_WARP * sizeof(float
 cudaError_t launch_force(const ForceArgs& a, int grid, int warps, cudaStream_t s) {
     if (a.n_items <= 0 || grid <= 0) return cudaSuccess;
     if (warps < 1 || warps > WARPS_PER_CTA) return cudaErrorInvalidValue;
-    if (a.jdata)
+    if (a.quad) {
+        if (a.jdata) return cudaErrorInvalidValue;
+        static bool optin = false;  // 53 KB of dynamic shared memory per block
+        if (!optin) {
+            const cudaError_t e = cudaFuncSetAttribute(k_force_quad, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)(WARPS_PER_CTA * QUAD_SMEM_PER_WARP));
+            if (e != cudaSuccess) return e;
+            optin = true;
+        }
+        k_force_quad<<<grid, warps * 32, warps * QUAD_SMEM_PER_WARP, s>>>(a);
+    } else if (a.jdata)
         k_force_data<<<grid, warps * 32, warps * FORCE_SMEM_PER_WARP, s>>>(a);
     else
         k_force<<<grid, warps * 32, warps * FORCE_SMEM_PER_WARP, s>>>(a);
     return cudaGetLastError();
+}
+
+int force_quad_max_ctas_per_sm() {
+    int n = 0;
+    if (cudaFuncSetAttribute(k_force_quad, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)(WARPS_PER_CTA * QUAD_SMEM_PER_WARP)) != cudaSuccess) return 0;
+    if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&n, k_force_quad, WARPS_PER_CTA * 32, WARPS_PER_CTA * QUAD_SMEM_PER_WARP) != cudaSuccess) return 0;
+    return n;
 }
 
 int force_max_ctas_per_sm() {

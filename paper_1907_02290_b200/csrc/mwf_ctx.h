@@ -90,8 +90,6 @@ struct mwf_ctx {
     double* quad64 = nullptr;   // [6 * max_cell]
     float4* quad = nullptr;     // [2 * max_cell]
     int quad_ctas_per_sm = 0;
-    cudaEvent_t ev_kq[MWF_MAX_TAG]{};
-    bool tag_quad[MWF_MAX_TAG]{};
     // short-range workload (NEXT-4): per-particle SPH record, cudaMalloc'ed when mwf_set_sph() is first called
     float4* sph = nullptr;      // [max_ptcl] (h, u, rho, P/rho^2)
     int64_t sph_hi = 0;         // records [0, sph_hi) have been uploaded

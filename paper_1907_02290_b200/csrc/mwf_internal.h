@@ -79,31 +79,12 @@ struct ForceArgs {
     int64_t n_items;
     float eps2;
     float G;
+    const float4* quad;         // order 2 (NEXT-3): two float4 per cell (Qxx Qyy Qzz Qxy) (Qxz Qyz tr(Q)/2 0), else nullptr
+    const int32_t* n_far;       // order 2: per group, the far SPJ entries of run 1 (the EPJ entries are run1_len - n_far)
+    int32_t n_cell;
     float4* vel;                // non-null: the closing kick of the leapfrog in the epilogue, v += acc * kick_h (NEXT-1)
     float kick_h;
 };
-
-// Quadrupole correction of the SPJ entries (NEXT-3, quad_kernel.cu): same items and schedule as the force kernel.
-struct QuadArgs {
-    const float4* store;
-    const float4* quad;         // two float4 per cell: (Qxx Qyy Qzz Qxy) (Qxz Qyz tr(Q)/2 0)
-    const int32_t* list;
-    const int64_t* list_off;
-    const int64_t* epj_off;     // scanned EPJ / SPJ counts per group; the SPJ entries of group g are its n_far[g] far ones at
-    const int64_t* spj_off;     //   list_off[g] + ne and the near ones from the next tile boundary behind them
-    const int32_t* n_far;
-    const WorkItem* items;
-    const int32_t* order;
-    float4* accp;
-    unsigned int* counter;
-    int64_t item_begin;
-    int64_t n_items;
-    int64_t n_ptcl;
-    float eps2;
-    float G;
-};
-cudaError_t launch_quad(const QuadArgs& a, int grid, cudaStream_t s);
-int quad_max_ctas_per_sm();
 
 // Short-range workload (NEXT-4, sph_kernel.cu): same lists, items and schedule as the force kernel.
 struct SphArgs {
@@ -126,6 +107,7 @@ int sph_max_ctas_per_sm(bool hydro);
 // kernels' host launchers (defined next to their kernels)
 cudaError_t launch_force(const ForceArgs& a, int grid, int warps_per_cta, cudaStream_t s);
 int force_max_ctas_per_sm();
+int force_quad_max_ctas_per_sm();
 
 cudaError_t launch_tree_prepare(const mwf_cell* cells, int64_t n_cell, int64_t max_ptcl, int32_t* parent, int32_t* counter,
                                 unsigned int* err, cudaStream_t s);
