@@ -143,7 +143,7 @@ class MultiWalkForce:
     """One mwf_ctx.  Device memory is one torch uint8 arena; tags run on torch streams."""
 
     def __init__(self, eps: float, G: float = 1.0, *, max_ptcl: int, max_cell: int, max_group: int, max_entry: int,
-                 n_tag: int = 8, device: int = 0):
+                 n_tag: int = 8, device: int = 0, tag_priorities: bool = True):
         import torch
         if not torch.cuda.is_available():
             raise RuntimeError("MultiWalkForce needs a CUDA device (sm_100a); there is no CPU path")
@@ -161,19 +161,22 @@ class MultiWalkForce:
             self._ck(self._lib.mwf_create(ctypes.byref(self._h), ctypes.byref(self.params), ctypes.c_void_p(base), self.arena_bytes), ctx=False)
             # priorities fall with the tag (the library does the same for its own streams): tags dispatched together
             # finish roughly in tag order, so a tag's retrieve overlaps the kernels of the tags behind it
+            # (tag_priorities=False: equal priorities, for callers that cycle through the tags many times per step --
+            # the batched multiwalk pipeline -- where the oldest batch, not the lowest tag, should finish first)
             least, greatest = torch.cuda.Stream.priority_range()
             levels = least - greatest + 1
-            self.streams = [torch.cuda.Stream(device=self.device, priority=greatest + t * levels // n_tag) for t in range(n_tag)]
+            self.streams = [torch.cuda.Stream(device=self.device, priority=(greatest + t * levels // n_tag) if tag_priorities else least)
+                            for t in range(n_tag)]
         for t, s in enumerate(self.streams):
             self._ck(self._lib.mwf_set_tag_stream(self._h, t, ctypes.c_void_p(int(s.cuda_stream))))
         self.n_tag = n_tag
 
     @classmethod
-    def for_workload(cls, w, eps: float | None = None, G: float = 1.0, n_tag: int = 8, device: int = 0):
+    def for_workload(cls, w, eps: float | None = None, G: float = 1.0, n_tag: int = 8, device: int = 0, tag_priorities: bool = True):
         if eps is None:
             eps = w.cfg.eps if w.cfg.eps > 0 else 1.0   # short-range workloads have no softening; the ctx still wants one
         return cls(eps, G, max_ptcl=w.n, max_cell=w.n_cell, max_group=w.n_group,
-                   max_entry=max(1, w.n_entry), n_tag=n_tag, device=device)
+                   max_entry=max(1, w.n_entry), n_tag=n_tag, device=device, tag_priorities=tag_priorities)
 
     # -- error handling
     def _ck(self, rc: int, ctx: bool = True):

@@ -100,6 +100,7 @@ static int build_impl(mwf_ctx* c, int64_t n, int32_t n_leaf, int32_t n_grp, doub
     // made by the counting pass, which the host has just waited for)
     const int64_t n_items = (int64_t)plan.items.size();
     CU(c, cudaMemcpyAsync(c->items, plan.items.data(), (size_t)n_items * sizeof(WorkItem), cudaMemcpyHostToDevice, c->aux_stream));
+    CU(c, cudaMemcpyAsync(c->order_cls, plan.order_cls.data(), (size_t)n_items * 4, cudaMemcpyHostToDevice, c->aux_stream));
     rc = schedule_full(c, n_items, c->aux_stream);
     if (rc) return build_failed(c, s, rc);
     CU(c, cudaEventRecord(c->ev_aux, c->aux_stream));

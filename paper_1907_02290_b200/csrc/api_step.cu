@@ -76,6 +76,17 @@ static int dispatch_launch(mwf_ctx* c, int32_t tag, int64_t g_begin, int64_t g_e
         const int rc = pick_order(c, g_begin, g_end, s, &a.order);
         if (rc) return rc;
     }
+    a.n_seg = 0;
+    if (!a.order && !jdata) {  // any other group range: its items widest first, from the class-sorted permutation
+        a.order = c->order_cls;
+        a.n_seg = N_WIDTH_CLASS;
+        a.seg_cum[0] = 0;
+        for (int k = 0; k < N_WIDTH_CLASS; ++k) {
+            const int64_t lo = c->h_cls_off[k][(size_t)g_begin], hi = c->h_cls_off[k][(size_t)g_end];
+            a.seg_begin[k] = c->h_cls_base[k] + lo;
+            a.seg_cum[k + 1] = a.seg_cum[k] + (hi - lo);
+        }
+    }
     const int64_t resident = (int64_t)c->n_sm * (a.quad ? c->quad_ctas_per_sm : c->ctas_per_sm);
     const int64_t want = (a.n_items + WARPS_PER_CTA - 1) / WARPS_PER_CTA;
     int grid = (int)resident, warps = WARPS_PER_CTA;
@@ -292,6 +303,7 @@ int mwf_set_lists(mwf_ctx* c, int64_t n_group, const int32_t* grp_first, const i
     const int64_t n_items = (int64_t)items.size();
     CU(c, cudaMemcpyAsync(c->list_off, list_off.data(), (size_t)(n_group + 1) * 8, H2D, s));
     CU(c, cudaMemcpyAsync(c->items, items.data(), (size_t)n_items * sizeof(WorkItem), H2D, s));
+    CU(c, cudaMemcpyAsync(c->order_cls, plan.order_cls.data(), (size_t)n_items * 4, H2D, s));
     CU(c, launch_merge_lists(n_group, c->grp_first, c->grp_n, c->st_epj_off, c->st_ids, c->st_spj_off, c->st_ids + e_epj, c->list_off,
                              c->grp_nfar, c->grp_run1, c->n_ptcl, c->n_cell, c->list, c->grp_self, c->err, s));
     rc = schedule_full(c, n_items, s);

@@ -136,6 +136,7 @@ Layout make_layout(const mwf_params& p) {
     L.add(mi * 4);                                      // 50 sched idx_a
     L.add(mi * 4);                                      // 51 sched idx_b
     L.add(256);                                         // 52 sched seg (2 x max(SCHED_WINDOWS, MWF_MAX_TAG) + 1 ints)
+    L.add(mi * 4);                                      // 53 order_cls
     return L;
 }
 
@@ -229,6 +230,7 @@ int mwf_create(mwf_ctx** out, const mwf_params* p, void* arena, int64_t arena_by
     c->items = (WorkItem*)(b + L.off[14]);
     c->order_full = (int32_t*)(b + L.off[15]);
     c->order_split = (int32_t*)(b + L.off[16]);
+    c->order_cls = (int32_t*)(b + L.off[53]);
     c->counters = (unsigned int*)(b + L.off[17]);
     c->err = (unsigned int*)(b + L.off[18]);
     c->vel = (float4*)(b + L.off[19]);

@@ -489,6 +489,14 @@ __device__ __forceinline__ void run_item_any(const ForceArgs& a, const WorkItem 
     else run_item_data<W>(a, it, sbuf, lane);
 }
 
+// work index -> position in the class-sorted permutation (ForceArgs::n_seg)
+__device__ __forceinline__ int64_t seg_position(const ForceArgs& a, int64_t w) {
+    int k = 0;
+#pragma unroll
+    for (int q = 1; q < N_WIDTH_CLASS; ++q) k += w >= a.seg_cum[q] ? 1 : 0;
+    return a.seg_begin[k] + (w - a.seg_cum[k]);
+}
+
 // The block has blockDim.x / 32 warps (WARPS_PER_CTA for a whole-machine dispatch, fewer for a sub-wave one, see
 // launch_force); s_tiles is dynamic shared memory, two tiles per warp.
 template <bool INDEXED>
@@ -500,7 +508,7 @@ __device__ __forceinline__ void force_body(const ForceArgs& a, float4* s_tiles) 
     int64_t w = (int64_t)blockIdx.x * warps_per_cta + warp;  // first item: static
     const int64_t n_warps = (int64_t)gridDim.x * warps_per_cta;
     while (w < a.n_items) {
-        const int64_t pos = a.item_begin + w;
+        const int64_t pos = a.n_seg ? seg_position(a, w) : a.item_begin + w;
         const WorkItem it = a.items[a.order ? a.order[pos] : pos];
         switch (it.width) {
             case 32: run_item_any<32, INDEXED>(a, it, sbuf, lane); break;
@@ -540,7 +548,7 @@ __global__ void __launch_bounds__(WARPS_PER_CTA * 32, MWF_MIN_CTAS) k_force_quad
     int64_t w = (int64_t)blockIdx.x * warps_per_cta + warp;
     const int64_t n_warps = (int64_t)gridDim.x * warps_per_cta;
     while (w < a.n_items) {
-        const int64_t pos = a.item_begin + w;
+        const int64_t pos = a.n_seg ? seg_position(a, w) : a.item_begin + w;
         const WorkItem it = a.items[a.order ? a.order[pos] : pos];
         switch (it.width) {
             case 32: run_item_quad<32>(a, it, sbuf, lane); break;

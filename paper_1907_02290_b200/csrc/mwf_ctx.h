@@ -51,6 +51,11 @@ struct mwf_ctx {
     int32_t* list = nullptr;      // [max_entry + TILE_J * max_group] merged, padded
     mwf::WorkItem* items = nullptr;    // [max_items]
     int32_t* order_full = nullptr, *order_split = nullptr;  // [max_items]
+    // items sorted by width class (32, 16, 8, 4, 2), group order inside a class: any contiguous group range then has its
+    // items widest-first as five contiguous runs (h_cls_off[k][g] = items of class k in the groups before g)
+    int32_t* order_cls = nullptr;                            // [max_items]
+    std::vector<int32_t> h_cls_off[mwf::N_WIDTH_CLASS];
+    int64_t h_cls_base[mwf::N_WIDTH_CLASS + 1]{};
     unsigned int* counters = nullptr;  // [N_COUNTER]
     unsigned int* err = nullptr;
     int64_t max_items = 0;
@@ -141,6 +146,8 @@ bool use_scan_refresh();
 struct Plan {
     std::vector<int64_t> list_off, item_off, inter, split;
     std::vector<WorkItem> items;
+    std::vector<int32_t> order_cls, cls_off[N_WIDTH_CLASS];
+    int64_t cls_base[N_WIDTH_CLASS + 1]{};
 };
 int plan_cut(mwf_ctx* c, int64_t n_group, const int32_t* grp_first, const int32_t* grp_n, Plan& pl);
 int plan_finish(mwf_ctx* c, int64_t n_group, const int32_t* grp_n, const int32_t* n_epj_of, const int32_t* n_spj_of, Plan& pl);

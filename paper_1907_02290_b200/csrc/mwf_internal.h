@@ -19,6 +19,8 @@ constexpr int SMALL_CTA_WARPS = 2;  // block of a sub-wave dispatch (one item pe
 constexpr int SCHED_WINDOWS = 16;    // Morton windows of the work schedule when the store exceeds the L2
 constexpr int CHUNK_I = 64;         // i-particles of a full work item (2 per lane)
 constexpr int MIN_WIDTH = 2;        // narrowest item: 2 lanes x 2 i-particles, 16 j-slices
+constexpr int N_WIDTH_CLASS = 5;    // widths 32, 16, 8, 4, 2
+inline int width_class(int width) { return width >= 32 ? 0 : width >= 16 ? 1 : width >= 8 ? 2 : width >= 4 ? 3 : 4; }
 // An SPJ entry is FAR when the cell's coordinates are at most this many times its distance from the group: the fp32
 // rounding of its centre of mass, at most 2^-24 of the coordinate, is then within 32 * 2^-24 = 1.9e-6 of the separation, i.e.
 // at most 6e-6 of that entry's term and of the order of the kernel's other rounding errors (the north_star bound is 1e-4 on
@@ -70,6 +72,9 @@ struct ForceArgs {
     const uint8_t* grp_self;    // 1: the group's own particles are in its EPJ list
     const WorkItem* items;
     const int32_t* order;       // cost-sorted permutation of item indices, or nullptr = identity
+    int32_t n_seg;              // > 0: the dispatch is n_seg runs of `order` (the class-sorted permutation), widest items first:
+    int64_t seg_begin[N_WIDTH_CLASS];      //   work index w in [seg_cum[k], seg_cum[k + 1]) is order[seg_begin[k] + w - seg_cum[k]]
+    int64_t seg_cum[N_WIDTH_CLASS + 1];
     const float4* jdata;        // method G1 (data lists): j records of groups [g_base, ...), else nullptr
     const int64_t* joff;        // G1: offsets of those groups' runs in jdata, in records
     int64_t g_base;

@@ -71,6 +71,20 @@ int plan_cut(mwf_ctx* c, int64_t n_group, const int32_t* grp_first, const int32_
         pl.item_off[(size_t)g + 1] = (int64_t)items.size();
     }
     if ((int64_t)items.size() > c->max_items) return MWF_ENOMEM;
+    // the items by width class, group order inside a class (a stable counting sort), and the per-group prefix counts
+    for (int k = 0; k < N_WIDTH_CLASS; ++k) pl.cls_off[k].assign((size_t)n_group + 1, 0);
+    for (const WorkItem& it : items) ++pl.cls_off[width_class(it.width)][(size_t)it.group + 1];
+    pl.cls_base[0] = 0;
+    for (int k = 0; k < N_WIDTH_CLASS; ++k) {
+        for (int64_t g = 0; g < n_group; ++g) pl.cls_off[k][(size_t)g + 1] += pl.cls_off[k][(size_t)g];
+        pl.cls_base[k + 1] = pl.cls_base[k] + pl.cls_off[k][(size_t)n_group];
+    }
+    pl.order_cls.resize(items.size());
+    {
+        int64_t fill[N_WIDTH_CLASS];
+        for (int k = 0; k < N_WIDTH_CLASS; ++k) fill[k] = pl.cls_base[k];
+        for (size_t i = 0; i < items.size(); ++i) pl.order_cls[(size_t)fill[width_class(items[i].width)]++] = (int32_t)i;
+    }
     return MWF_OK;
 }
 
@@ -118,6 +132,8 @@ void adopt_plan(mwf_ctx* c, Plan& pl, int64_t n_group, const int32_t* grp_first,
     c->h_item_off.swap(pl.item_off);
     c->h_inter.swap(pl.inter);
     c->h_split.swap(pl.split);
+    for (int k = 0; k < N_WIDTH_CLASS; ++k) c->h_cls_off[k].swap(pl.cls_off[k]);
+    for (int k = 0; k <= N_WIDTH_CLASS; ++k) c->h_cls_base[k] = pl.cls_base[k];
     c->split_ready = false;
     c->h_grp_first.assign(grp_first, grp_first + n_group);
     c->h_grp_n.assign(grp_n, grp_n + n_group);
