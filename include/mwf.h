@@ -237,8 +237,10 @@ int mwf_calc_force_all(mwf_ctx* c, const mwf_posm* src, int src_on_device, mwf_a
  *   [0, N) exactly (no hole, no overlap) and no tag is in flight (every dispatched tag retrieved).  Everything
  *   enqueued later on any stream through this library is ordered behind the shadow uploads.  The monopoles become
  *   stale (mwf_refresh_monopoles must follow); velocities, results, tree and lists are not touched.
- * mwf_get_tag_split: bounds[0 .. n_tag] = the group ranges [bounds[t], bounds[t+1]) of equal interaction count that
- *   mwf_calc_force_all dispatches per tag (MWF_ESTATE without lists). */
+ * mwf_get_tag_split: bounds[0 .. n_tag] = the group ranges [bounds[t], bounds[t+1]) that mwf_calc_force_all dispatches
+ *   per tag (MWF_ESTATE without lists): by interaction count, equal shares for the first half of the tags, then shares
+ *   falling linearly to an eighth for the last tag -- the tags finish in order, the copies of a tag hide behind the
+ *   kernels of the tags after it, and the copies of the last tag, which nothing hides, are small. */
 int mwf_set_particles_next(mwf_ctx* c, const mwf_posm* src, int64_t first, int64_t n, int src_on_device, void* stream);
 int mwf_swap_store(mwf_ctx* c, void* stream);
 int mwf_get_tag_split(mwf_ctx* c, int64_t* bounds);
