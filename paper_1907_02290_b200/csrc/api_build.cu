@@ -100,12 +100,11 @@ static int build_impl(mwf_ctx* c, int64_t n, int32_t n_leaf, int32_t n_grp, doub
     // made by the counting pass, which the host has just waited for)
     const int64_t n_items = (int64_t)plan.items.size();
     CU(c, cudaMemcpyAsync(c->items, plan.items.data(), (size_t)n_items * sizeof(WorkItem), cudaMemcpyHostToDevice, c->aux_stream));
-    CU(c, cudaMemcpyAsync(c->order_cls, plan.order_cls.data(), (size_t)n_items * 4, cudaMemcpyHostToDevice, c->aux_stream));
     rc = schedule_full(c, n_items, c->aux_stream);
     if (rc) return build_failed(c, s, rc);
+    // host, meanwhile: list offsets and interaction counts per group, the tags' group ranges
     CU(c, cudaEventRecord(c->ev_aux, c->aux_stream));
     CU(c, cudaStreamWaitEvent(s, c->ev_aux, 0));
-    // host, meanwhile: list offsets and interaction counts per group, the tags' group ranges
     for (int64_t g = 0; g < n_group; ++g) {  // the two runs of every list: EPJ + far SPJ, near SPJ
         h_ne[g] += h_nf[g];
         h_ns[g] -= h_nf[g];

@@ -78,6 +78,8 @@ static int dispatch_launch(mwf_ctx* c, int32_t tag, int64_t g_begin, int64_t g_e
     }
     a.n_seg = 0;
     if (!a.order && !jdata) {  // any other group range: its items widest first, from the class-sorted permutation
+        const int rc = ensure_class_order(c, s);
+        if (rc) return rc;
         a.order = c->order_cls;
         a.n_seg = N_WIDTH_CLASS;
         a.seg_cum[0] = 0;
@@ -303,7 +305,6 @@ int mwf_set_lists(mwf_ctx* c, int64_t n_group, const int32_t* grp_first, const i
     const int64_t n_items = (int64_t)items.size();
     CU(c, cudaMemcpyAsync(c->list_off, list_off.data(), (size_t)(n_group + 1) * 8, H2D, s));
     CU(c, cudaMemcpyAsync(c->items, items.data(), (size_t)n_items * sizeof(WorkItem), H2D, s));
-    CU(c, cudaMemcpyAsync(c->order_cls, plan.order_cls.data(), (size_t)n_items * 4, H2D, s));
     CU(c, launch_merge_lists(n_group, c->grp_first, c->grp_n, c->st_epj_off, c->st_ids, c->st_spj_off, c->st_ids + e_epj, c->list_off,
                              c->grp_nfar, c->grp_run1, c->n_ptcl, c->n_cell, c->list, c->grp_self, c->err, s));
     rc = schedule_full(c, n_items, s);

@@ -281,6 +281,7 @@ int mwf_create(mwf_ctx** out, const mwf_params* p, void* arena, int64_t arena_by
     ok = ok && cudaMemset(c->counters, 0, N_COUNTER * 4) == cudaSuccess;
     ok = ok && cudaMemset(c->err, 0, 256) == cudaSuccess;
     ok = ok && cudaHostAlloc(reinterpret_cast<void**>(&c->h_scalars), 16 * sizeof(int64_t), cudaHostAllocDefault) == cudaSuccess;
+    ok = ok && cudaHostAlloc(reinterpret_cast<void**>(&c->h_order_cls), (size_t)c->max_items * sizeof(int32_t), cudaHostAllocDefault) == cudaSuccess;
     ok = ok && cudaHostAlloc(reinterpret_cast<void**>(&c->h_groups), (size_t)p->max_group * 5 * sizeof(int32_t), cudaHostAllocDefault) == cudaSuccess;
     ok = ok && cudaEventCreateWithFlags(&c->ev_groups, cudaEventDisableTiming) == cudaSuccess;
     ok = ok && cudaStreamCreateWithFlags(&c->aux_stream, cudaStreamNonBlocking) == cudaSuccess;
@@ -303,6 +304,7 @@ int mwf_destroy(mwf_ctx* c) {
     }
     if (c->h_scalars) cudaFreeHost(c->h_scalars);
     if (c->h_groups) cudaFreeHost(c->h_groups);
+    if (c->h_order_cls) cudaFreeHost(c->h_order_cls);
     if (c->ev_groups) cudaEventDestroy(c->ev_groups);
     if (c->aux_stream) cudaStreamDestroy(c->aux_stream);
     if (c->ev_aux) cudaEventDestroy(c->ev_aux);

@@ -34,6 +34,7 @@ struct mwf_ctx {
     double4* leaf_P = nullptr;    // [max_cell + 1] leaves' moments in rank order, scanned in place every refresh
     double4* leaf_toff = nullptr; // [tiles] scanned tile totals
     int64_t* h_scalars = nullptr; // pinned: small results of the construction step (counts, totals, validation word)
+    int32_t* h_order_cls = nullptr;  // pinned [max_items]: the class-sorted permutation on its way to the device
     int32_t* h_groups = nullptr;  // pinned [5 x max_group]: group ranges and list lengths on their way to the host work plan
     cudaEvent_t ev_groups{};      // the group ranges have arrived
     cudaStream_t aux_stream{};    // construction step: the work schedule is made here while the fill walk runs on the caller's stream
@@ -53,7 +54,9 @@ struct mwf_ctx {
     int32_t* order_full = nullptr, *order_split = nullptr;  // [max_items]
     // items sorted by width class (32, 16, 8, 4, 2), group order inside a class: any contiguous group range then has its
     // items widest-first as five contiguous runs (h_cls_off[k][g] = items of class k in the groups before g)
-    int32_t* order_cls = nullptr;                            // [max_items]
+    int32_t* order_cls = nullptr;                            // [max_items]; made on first use (ensure_class_order)
+    bool cls_ready = false;
+    std::vector<mwf::WorkItem> h_items;                      // the work items as cut (host copy)
     std::vector<int32_t> h_cls_off[mwf::N_WIDTH_CLASS];
     int64_t h_cls_base[mwf::N_WIDTH_CLASS + 1]{};
     unsigned int* counters = nullptr;  // [N_COUNTER]
@@ -146,14 +149,13 @@ bool use_scan_refresh();
 struct Plan {
     std::vector<int64_t> list_off, item_off, inter, split;
     std::vector<WorkItem> items;
-    std::vector<int32_t> order_cls, cls_off[N_WIDTH_CLASS];
-    int64_t cls_base[N_WIDTH_CLASS + 1]{};
 };
 int plan_cut(mwf_ctx* c, int64_t n_group, const int32_t* grp_first, const int32_t* grp_n, Plan& pl);
 int plan_finish(mwf_ctx* c, int64_t n_group, const int32_t* grp_n, const int32_t* n_epj_of, const int32_t* n_spj_of, Plan& pl);
 int make_plan(mwf_ctx* c, int64_t n_group, const int32_t* grp_first, const int32_t* grp_n, const int32_t* n_epj_of, const int32_t* n_spj_of, Plan& pl);
 void adopt_plan(mwf_ctx* c, Plan& pl, int64_t n_group, const int32_t* grp_first, const int32_t* grp_n, int mode);
 int ensure_split_order(mwf_ctx* c, cudaStream_t s);
+int ensure_class_order(mwf_ctx* c, cudaStream_t s);
 // order_full of the items now on the device (behind their upload on the stream); no host synchronisation
 int schedule_full(mwf_ctx* c, int64_t n_items, cudaStream_t s);
 

@@ -71,20 +71,29 @@ int plan_cut(mwf_ctx* c, int64_t n_group, const int32_t* grp_first, const int32_
         pl.item_off[(size_t)g + 1] = (int64_t)items.size();
     }
     if ((int64_t)items.size() > c->max_items) return MWF_ENOMEM;
-    // the items by width class, group order inside a class (a stable counting sort), and the per-group prefix counts
-    for (int k = 0; k < N_WIDTH_CLASS; ++k) pl.cls_off[k].assign((size_t)n_group + 1, 0);
-    for (const WorkItem& it : items) ++pl.cls_off[width_class(it.width)][(size_t)it.group + 1];
-    pl.cls_base[0] = 0;
+    return MWF_OK;
+}
+
+// The items by width class, group order inside a class (a stable counting sort), and the per-group prefix counts: made
+// the first time a dispatch covers a group range that has no sorted schedule of its own (1 ms of host time for 1.4e5 items,
+// which a device-side construction step followed by whole-workload dispatches never needs).
+int ensure_class_order(mwf_ctx* c, cudaStream_t s) {
+    if (c->cls_ready) return MWF_OK;
+    const std::vector<WorkItem>& items = c->h_items;
+    const int64_t n_group = c->n_group;
+    for (int k = 0; k < N_WIDTH_CLASS; ++k) c->h_cls_off[k].assign((size_t)n_group + 1, 0);
+    for (const WorkItem& it : items) ++c->h_cls_off[width_class(it.width)][(size_t)it.group + 1];
+    c->h_cls_base[0] = 0;
     for (int k = 0; k < N_WIDTH_CLASS; ++k) {
-        for (int64_t g = 0; g < n_group; ++g) pl.cls_off[k][(size_t)g + 1] += pl.cls_off[k][(size_t)g];
-        pl.cls_base[k + 1] = pl.cls_base[k] + pl.cls_off[k][(size_t)n_group];
+        for (int64_t g = 0; g < n_group; ++g) c->h_cls_off[k][(size_t)g + 1] += c->h_cls_off[k][(size_t)g];
+        c->h_cls_base[k + 1] = c->h_cls_base[k] + c->h_cls_off[k][(size_t)n_group];
     }
-    pl.order_cls.resize(items.size());
-    {
-        int64_t fill[N_WIDTH_CLASS];
-        for (int k = 0; k < N_WIDTH_CLASS; ++k) fill[k] = pl.cls_base[k];
-        for (size_t i = 0; i < items.size(); ++i) pl.order_cls[(size_t)fill[width_class(items[i].width)]++] = (int32_t)i;
-    }
+    int64_t fill[N_WIDTH_CLASS];
+    for (int k = 0; k < N_WIDTH_CLASS; ++k) fill[k] = c->h_cls_base[k];
+    for (size_t i = 0; i < items.size(); ++i) c->h_order_cls[fill[width_class(items[i].width)]++] = (int32_t)i;
+    CU(c, cudaMemcpyAsync(c->order_cls, c->h_order_cls, items.size() * sizeof(int32_t), cudaMemcpyHostToDevice, s));
+    CU(c, cudaStreamSynchronize(s));  // the other tags' streams read it too
+    c->cls_ready = true;
     return MWF_OK;
 }
 
@@ -121,8 +130,9 @@ int plan_finish(mwf_ctx* c, int64_t n_group, const int32_t* grp_n, const int32_t
 }
 
 int make_plan(mwf_ctx* c, int64_t n_group, const int32_t* grp_first, const int32_t* grp_n, const int32_t* n_epj_of, const int32_t* n_spj_of, Plan& pl) {
-    const int rc = plan_cut(c, n_group, grp_first, grp_n, pl);
-    return rc ? rc : plan_finish(c, n_group, grp_n, n_epj_of, n_spj_of, pl);
+    int rc = plan_cut(c, n_group, grp_first, grp_n, pl);
+    if (rc) return rc;
+    return plan_finish(c, n_group, grp_n, n_epj_of, n_spj_of, pl);
 }
 
 // Adopt a plan as the ctx's current lists (after the device side is in place).
@@ -132,8 +142,8 @@ void adopt_plan(mwf_ctx* c, Plan& pl, int64_t n_group, const int32_t* grp_first,
     c->h_item_off.swap(pl.item_off);
     c->h_inter.swap(pl.inter);
     c->h_split.swap(pl.split);
-    for (int k = 0; k < N_WIDTH_CLASS; ++k) c->h_cls_off[k].swap(pl.cls_off[k]);
-    for (int k = 0; k <= N_WIDTH_CLASS; ++k) c->h_cls_base[k] = pl.cls_base[k];
+    c->h_items.swap(pl.items);
+    c->cls_ready = false;
     c->split_ready = false;
     c->h_grp_first.assign(grp_first, grp_first + n_group);
     c->h_grp_n.assign(grp_n, grp_n + n_group);
