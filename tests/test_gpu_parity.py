@@ -245,6 +245,12 @@ def test_pipelined_host_loop_equals_the_blocking_one():
     f.upload_workload(w, binding.MAKE_LIST_FOR_REUSE)
     split = f.get_tag_split()
     assert split[0] == 0 and split[-1] == w.n_group and np.all(np.diff(split) >= 0)
+    # shares of the interactions per tag: equal over the first half of the tags, tapering to an eighth for the last one
+    per_group = w.grp_n.astype(np.int64) * w.n_list
+    share = np.array([per_group[split[t]:split[t + 1]].sum() for t in range(n_tag)], np.float64)
+    share /= share[0]
+    want = np.minimum(1.0, 2.0 * (n_tag - np.arange(n_tag) - 0.5) / n_tag)
+    assert np.all(np.abs(share - want) <= 0.02 + 2.0 * per_group.max() / (per_group.sum() / n_tag))
     first = [int(w.grp_first[split[t]]) if split[t] < w.n_group else w.n for t in range(n_tag)] + [w.n]
     up = torch.cuda.Stream()
     host_in = [f.pinned(w.n) for _ in steps]
