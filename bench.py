@@ -604,6 +604,53 @@ def batched_leg(binding, f, w, cfg, src_dev, dst_dev, steps):
             "value": w.interactions / (res["batched"] * 1e-3), "unit": UNIT, "timing": "host wall clock, device-resident source and destination"}
 
 
+def sph_summary(binding, device, steps=3):
+    """NEXT-4 for the default line: the short-range workload sph_plummer_4m with the neighbour lists built on the device
+    (mwf_build_neighbours), then the density and the pressure-gradient pass over all groups; kernel times from CUDA events
+    (median of `steps` after 2 warm-ups), flop convention of sph_leg."""
+    import torch
+    from paper_1907_02290_b200.workload import SPH_CONFIGS, make_particles, make_sph_fields
+    cfg = SPH_CONFIGS[2]
+    posm0, _ = make_particles(cfg, None)
+    rec0 = make_sph_fields(cfg, posm0)
+    n = posm0.shape[0]
+    f = binding.MultiWalkForce(1.0, 1.0, max_ptcl=n, max_cell=n, max_group=n // 8, max_entry=48 * n, n_tag=1, device=device)
+    try:
+        f.begin_step(binding.MAKE_LIST_FOR_REUSE)
+        f.set_particles(torch.from_numpy(posm0).to(f.device))
+        f.set_sph(torch.from_numpy(rec0).to(f.device))
+        torch.cuda.synchronize()
+        t = time.perf_counter()
+        f.build_neighbours(n, cfg.n_leaf, cfg.n_grp, cfg.skin)
+        f.sync()
+        t_build = time.perf_counter() - t
+        sizes = f.get_build_sizes()
+        dst = torch.zeros((n, 4), dtype=torch.float32, device=f.device)
+        ms = {"density": [], "hydro": []}
+        inter = 0
+        for it in range(2 + steps):
+            f.begin_step(binding.REUSE_LIST)
+            c0 = f.get_counters()["interactions"]
+            f.dispatch_density(0, 0, sizes["n_group"], cfg.gamma)
+            f.retrieve(0, None)
+            inter = f.get_counters()["interactions"] - c0
+            t_d = f.last_dispatch_ms(0)
+            f.dispatch_hydro(0, 0, sizes["n_group"])
+            f.retrieve(0, dst)
+            if it >= 2:
+                ms["density"].append(t_d); ms["hydro"].append(f.last_dispatch_ms(0))
+    finally:
+        f.close()
+    n_sm = torch.cuda.get_device_properties(device).multi_processor_count
+    peak = n_sm * 256 * (measured_peaks().get("sm_max_mhz") or 1965.0) * 1e6
+    out = {"workload": "short-range: " + cfg.name, "n": n, "n_group": sizes["n_group"], "list_entries": sizes["n_epj"], "interactions_per_pass": int(inter),
+           "device_build_ms": 1e3 * t_build, "what": "mwf_build_neighbours (first call on a fresh ctx), then mwf_dispatch_density / mwf_dispatch_hydro over all groups"}
+    for k, nop in (("density", 25), ("hydro", 45)):
+        m = float(np.median(ms[k]))
+        out[k] = {"kernel_ms": m, "flop_per_interaction": nop, "frac_fp32_peak": nop * inter / (m * 1e-3) / peak}
+    return out
+
+
 # ----------------------------------------------------------------------------- main
 def main():
     ap = argparse.ArgumentParser()
@@ -819,6 +866,14 @@ def main():
     except binding.MwfError as ex:
         order2 = {"error": str(ex)}
 
+    # ---- NEXT-4: the short-range workload, for the record (its own ctx; skipped with --n)
+    sph_step = None
+    if args.n is None and rank == 0:
+        try:
+            sph_step = sph_summary(binding, local)
+        except binding.MwfError as ex:
+            sph_step = {"error": str(ex)}
+
     # ---- NEXT-1: device-resident reuse steps (kick-drift, refresh, force, kick; no host transfer)
     dev_res = None
     if w.vel is not None and cfg.dt > 0:
@@ -952,7 +1007,7 @@ def main():
             "e2e_blocking_call": {"value": e2e_value, "unit": UNIT, "h2d_bytes_per_step": 16 * w.n, "d2h_bytes_per_step": 16 * w.n,
                                   "ms_per_step": ms_e_max / args.steps,
                                   "what": "one blocking mwf_calc_force_all per step, pinned host source and destination (the H2D cannot overlap the kernels)"},
-            "gpu_launches": launches, "clocks": clk, "phases": phases, "device_resident_step": dev_res, "batched_dispatch": batched, "order2_step": order2,
+            "gpu_launches": launches, "clocks": clk, "phases": phases, "device_resident_step": dev_res, "batched_dispatch": batched, "order2_step": order2, "sph_step": sph_step,
             "run_n_reuse_%d" % max(cfg.n_reuse, 0): whole_run,
             "construction_step": {"host_tree_and_lists_s": round(t_build, 3), "upload_tree_and_lists_s": round(t_upload, 3), "on_device": dev_build},
             "context": {"paper_fraction_of_peak": 0.27, "paper_hardware": "TITAN V (P:673), whole step"},
