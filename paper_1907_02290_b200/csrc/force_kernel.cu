@@ -27,7 +27,9 @@
 //     not an fp32 input -- on the fp32 grid it is up to 2^-25 |X| off, which for a cell 1e-3 away at coordinates of
 //     order 1 is the north_star's whole error budget -- so the refresh keeps its rounding remainder (spj_lo) and the
 //     staged position (hi - c) + lo carries 24 bits of the DISTANCE to the item; the i-side switches by adding c to -x_i.
-//     The two runs of a group's list are padded to whole tiles separately.
+//     The two runs of a group's list are padded to whole tiles separately and swept by a tile loop each (run_item).
+//   * order 2 (k_force_quad, reading S22): from a list's first SPJ entry on the tiles also carry the cells' quadrupoles, and the
+//     sweep evaluates the Q terms from the monopole interaction's own distances and rsqrt.
 //   * the self term (an i-particle meets itself in its own EPJ list) contributes exactly 0 to acc and
 //     m_i * rsqrt(eps^2) to the potential sum; the same value is subtracted up front (reading S2).
 #include "mwf_internal.h"

@@ -47,6 +47,8 @@ struct WorkItem {
 #ifndef MWF_COST_STAGE
 #define MWF_COST_STAGE 40
 #endif
+// j-pairs of a tile unrolled in the W = 32 / 16 sweeps of run 1: 16, not all 32 -- the kernel then is 79 KB of SASS; beyond
+// ~95 KB its time falls off a cliff (instruction fetch of 16 warps in differently specialised loops, profiles/r02_kforce_variants.md)
 #ifndef MWF_UNROLL_WIDE
 #define MWF_UNROLL_WIDE 16
 #endif
