@@ -312,9 +312,9 @@ cudaError_t build_tree_device(const BuildBuffers& b, int64_t n, int n_leaf, int 
         BT(scan_exclusive<int32_t>(b.level_cnt, m + 1, b.scan_scratch, s));
         k_level_emit<<<(unsigned)((m + 127) / 128), 128, 0, s>>>(b.cells, b.geom, b.parent, lev_begin, lev_end, b.level_bounds, b.level_cnt, max_cell, b.err);
         BT(cudaGetLastError());
-        int32_t n_new = 0;
-        BT(cudaMemcpyAsync(&n_new, b.level_cnt + m, 4, cudaMemcpyDeviceToHost, s));
+        BT(cudaMemcpyAsync(b.h_i32, b.level_cnt + m, 4, cudaMemcpyDeviceToHost, s));
         BT(cudaStreamSynchronize(s));
+        const int32_t n_new = b.h_i32[0];
         if (n_new == 0) break;
         if (lev_end + n_new > max_cell) { *n_cell_out = lev_end + n_new; *n_group_out = 0; *n_level_out = n_level; return cudaSuccess; }  // err word is set
         lev_begin = lev_end;
@@ -329,9 +329,9 @@ cudaError_t build_tree_device(const BuildBuffers& b, int64_t n, int n_leaf, int 
     k_group_mark<<<(unsigned)((n_cell + 255) / 256), 256, 0, s>>>(b.cells, b.parent, n_cell, n_grp, b.mark);
     BT(cudaGetLastError());
     BT(scan_exclusive<int32_t>(b.mark, n + 1, b.scan_scratch, s));
-    int32_t n_group = 0;
-    BT(cudaMemcpyAsync(&n_group, b.mark + n, 4, cudaMemcpyDeviceToHost, s));
+    BT(cudaMemcpyAsync(b.h_i32 + 1, b.mark + n, 4, cudaMemcpyDeviceToHost, s));
     BT(cudaStreamSynchronize(s));
+    const int32_t n_group = b.h_i32[1];
     *n_group_out = n_group;
     if (n_group > max_group) return cudaSuccess;  // caller reports the capacity error
     k_group_emit<<<(unsigned)((n_cell + 255) / 256), 256, 0, s>>>(b.cells, b.parent, n_cell, n_grp, b.mark, max_group, b.grp_cell, b.grp_first, b.grp_n);

@@ -281,6 +281,7 @@ int mwf_create(mwf_ctx** out, const mwf_params* p, void* arena, int64_t arena_by
     ok = ok && cudaMemset(c->counters, 0, N_COUNTER * 4) == cudaSuccess;
     ok = ok && cudaMemset(c->err, 0, 256) == cudaSuccess;
     ok = ok && cudaHostAlloc(reinterpret_cast<void**>(&c->h_scalars), 16 * sizeof(int64_t), cudaHostAllocDefault) == cudaSuccess;
+    c->bb.h_i32 = ok ? reinterpret_cast<int32_t*>(c->h_scalars + 8) : nullptr;
     ok = ok && cudaHostAlloc(reinterpret_cast<void**>(&c->h_order_cls), (size_t)c->max_items * sizeof(int32_t), cudaHostAllocDefault) == cudaSuccess;
     ok = ok && cudaHostAlloc(reinterpret_cast<void**>(&c->h_groups), (size_t)p->max_group * 5 * sizeof(int32_t), cudaHostAllocDefault) == cudaSuccess;
     ok = ok && cudaEventCreateWithFlags(&c->ev_groups, cudaEventDisableTiming) == cudaSuccess;

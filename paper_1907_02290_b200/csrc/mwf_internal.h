@@ -162,6 +162,7 @@ struct BuildBuffers {
     int32_t* mark; int32_t* grp_cell; int32_t* grp_first; int32_t* grp_n; float* grp_box;
     int32_t* n_epj; int32_t* n_spj; int32_t* n_far; int32_t* run1_len; int64_t* list_off; int64_t* epj_off; int64_t* spj_off; int32_t* list;
     int32_t* walk_stacks; unsigned int* walk_counter; unsigned int* err;
+    int32_t* h_i32;                                     // pinned host memory, 2 ints: the per-level and group counts on their way back
 };
 
 cudaError_t build_tree_device(const BuildBuffers& b, int64_t n, int n_leaf, int n_grp, int64_t max_cell, int64_t max_group, bool with_vel, float4* sph,
