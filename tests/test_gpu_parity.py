@@ -198,6 +198,41 @@ def test_batched_dispatch_over_tags_is_bitwise_identical():
         assert np.array_equal(one, many)
 
 
+@pytest.mark.parametrize("sizes", [[64] * 12, [3] * 40, [64, 1, 200, 7, 64, 33, 2, 129, 16, 64, 5, 255]])
+def test_arbitrary_group_ranges_equal_one_dispatch(sizes):
+    """A dispatch over any group range takes its items widest-first from the class-sorted permutation (five runs per
+    range): ranges of one group, ranges in which some width classes are empty, ranges dispatched out of order -- the
+    results are bitwise those of the whole-workload dispatch, and match direct summation."""
+    n = int(np.sum(sizes))
+    posm, _ = make_particles(CONFIGS[0], n)
+    gf, gn, eo, ei, so, si = synthetic_groups(n, sizes)
+    ng = len(sizes)
+    f = binding.MultiWalkForce(1 / 64, 1.0, max_ptcl=n, max_cell=1, max_group=ng, max_entry=ei.size, n_tag=3)
+    f.begin_step(binding.MAKE_LIST_FOR_REUSE)
+    f.set_particles(posm)
+    f.set_tree(np.array([[0, n, 0, 0]], np.int32))
+    f.set_lists(gf, gn, eo, ei, so, si, binding.MAKE_LIST_FOR_REUSE)
+    f.refresh_monopoles()
+    one = np.full((n, 4), np.nan, np.float32)
+    f.dispatch(0, 0, ng)
+    f.retrieve(0, one)
+    cuts = sorted({0, 1, 2, ng // 3, ng // 2, ng - 1, ng})
+    ranges = list(zip(cuts[:-1], cuts[1:]))[::-1]                  # last range first
+    many = np.full((n, 4), np.nan, np.float32)
+    f.begin_step(binding.REUSE_LIST)
+    for k, (gb, ge) in enumerate(ranges):
+        t = k % 3
+        if k >= 3:
+            f.retrieve(t, many)
+        f.dispatch(t, gb, ge)
+    for t in range(min(3, len(ranges))):
+        f.retrieve(t, many)
+    f.close()
+    assert np.array_equal(one, many)
+    acc, pot = oracle.direct(posm, 1 / 64)
+    check(many, acc, pot, label="arbitrary ranges")
+
+
 def test_calc_force_all_host_and_device_destinations():
     import torch
     cfg = CONFIGS[1]
