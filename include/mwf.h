@@ -306,6 +306,36 @@ int mwf_get_monopoles(mwf_ctx* c, mwf_posm* dst, int dst_on_device);
 /* DEVICE pointers into the arena: store (N particles then n_cell SPJ) and result array. */
 int mwf_device_pointers(mwf_ctx* c, mwf_posm** store, mwf_accp** accp);
 
+/* ---- The monopole pass for callers that must not allocate device memory.
+ * Everything above works through an mwf_ctx, whose arena somebody has to allocate.  Some callers cannot: a plugin inside
+ * an application whose own pool owns the GPU's memory (a guest cudaMalloc may be refused or against the rules), a routine
+ * on a latency-bound path (cudaMalloc and cudaFree synchronise the whole device), code on a nearly full GPU where the
+ * allocation is the one call that may fail.  mwf_monopoles_static() needs no ctx and allocates nothing, on the host side
+ * of CUDA or the device side: its working memory (fp64 moments, parent links, arrival counters; 40 B per cell) is one
+ * fixed array inside the library image, sized for MWF_STATIC_MAX_CELL cells (5 MiB).  Every GPU that loads the library
+ * holds that array until the process exits, which is why the limit is modest; larger trees need an mwf_ctx.
+ *
+ * Computes, for every cell c of the tree, the record (centre of mass x, y, z, total mass) of the particles in its range,
+ * summed in fp64 bottom-up (leaf sums, then children in child order) and rounded once to float -- the
+ * records mwf_refresh_monopoles() + mwf_get_monopoles() give for the same tree and particles, to the last float bit or
+ * one (the ctx path sums by a prefix scan).  A cell of zero mass gets its first particle's position and mass 0.
+ *   cells   DEVICE, n_cell records laid out as mwf_set_tree() wants them (children behind their parent, child ranges
+ *           partitioning the parent's).  NOT validated (that needs a read-back): ranges that leave the arrays are
+ *           clipped or ignored, so a malformed tree gives wrong records, never an out-of-bounds access.
+ *   ptcl    DEVICE, n_ptcl records in tree order.       spj   DEVICE, n_cell records, written.
+ *   All three 16-byte aligned, on the CURRENT device (there is no ctx to name one), owned by the caller and valid until
+ *   the work on `stream` has finished.  Asynchronous on `stream`; the caller synchronises.
+ * Returns MWF_ENOMEM when n_cell > MWF_STATIC_MAX_CELL, MWF_EINVAL for null / misaligned pointers or sizes <= 0,
+ * MWF_ECUDA when a CUDA call fails; mwf_static_last_error() gives this thread's last message in words.
+ * First call on a device: it also looks up the array's device address (once per device).  Make that call before any
+ * stream capture begins.
+ * Sharing: all calls on a GPU use the same array, which keeps the previous call's contents; each call resets, on its
+ * stream, what it needs clean.  Calls that overlap on one GPU (two streams, two threads) race on it -- run them one
+ * after the other. */
+#define MWF_STATIC_MAX_CELL 131072
+int mwf_monopoles_static(const mwf_cell* cells, int64_t n_cell, const mwf_posm* ptcl, int64_t n_ptcl, mwf_posm* spj, void* stream);
+const char* mwf_static_last_error(void);
+
 /* Wait for everything the ctx has enqueued. */
 int mwf_sync(mwf_ctx* c);
 

@@ -28,6 +28,7 @@ SYMBOLS = (
     "mwf_set_sph", "mwf_get_sph", "mwf_dispatch_density", "mwf_dispatch_hydro", "mwf_calc_sph_all",
     "mwf_build", "mwf_build_neighbours", "mwf_get_build_sizes", "mwf_get_permutation", "mwf_get_tree", "mwf_get_groups", "mwf_get_lists", "mwf_get_list_buffer",
     "mwf_set_particles_next", "mwf_swap_store", "mwf_get_tag_split",
+    "mwf_monopoles_static", "mwf_static_last_error",
 )
 
 
@@ -101,6 +102,7 @@ def load_library(path: str | None = None) -> ctypes.CDLL:
         "mwf_get_groups": [vp, vp, vp],
         "mwf_get_lists": [vp, vp, vp, vp, vp],
         "mwf_get_list_buffer": [vp, vp, vp, P(i64), P(i64), ci],
+        "mwf_monopoles_static": [vp, i64, vp, i64, vp, vp],
     }
     for name, args in sig.items():
         fn = getattr(lib, name)
@@ -110,6 +112,8 @@ def load_library(path: str | None = None) -> ctypes.CDLL:
     lib.mwf_strerror.restype = ctypes.c_char_p
     lib.mwf_last_cuda_error.argtypes = [vp]
     lib.mwf_last_cuda_error.restype = ctypes.c_char_p
+    lib.mwf_static_last_error.argtypes = []
+    lib.mwf_static_last_error.restype = ctypes.c_char_p
     _lib = lib
     return lib
 
@@ -137,6 +141,34 @@ def _stream_handle(stream) -> ctypes.c_void_p:
         import torch
         stream = torch.cuda.current_stream()
     return ctypes.c_void_p(int(stream.cuda_stream))
+
+
+STATIC_MAX_CELL = 131072      # MWF_STATIC_MAX_CELL of include/mwf.h
+
+
+def monopoles_static(cells, ptcl, spj, stream=None) -> None:
+    """mwf_monopoles_static: the monopole record of every tree cell, for callers that may not allocate device memory.
+
+    Meant for code that lives inside someone else's memory budget -- a plugin under a host application's pool, a step
+    on a latency-bound path where cudaMalloc would stall the device, a job on a nearly full GPU -- and so cannot create
+    a MultiWalkForce (whose arena has to be allocated by somebody).  Nothing is allocated here either: the three
+    arguments are torch CUDA tensors the caller already owns (cells int32 (n_cell, 4), ptcl float32 (n_ptcl, 4), spj
+    float32 (n_cell, 4), all contiguous, on the current device) and only their pointers are passed on.  The library's
+    working memory is a fixed array in its image, good for at most STATIC_MAX_CELL cells; a larger tree raises MwfError
+    (code ENOMEM) with the limit in its text.  Asynchronous on `stream` (default: torch's current stream).  Calls share
+    that array: do not let two of them run on the same GPU at the same time.  The first call on a device also looks up
+    the array's address; make it before starting a stream capture."""
+    import torch
+    lib = load_library()
+    for t, dt, what in ((cells, torch.int32, "cells"), (ptcl, torch.float32, "ptcl"), (spj, torch.float32, "spj")):
+        if not (isinstance(t, torch.Tensor) and t.is_cuda and t.is_contiguous() and t.dtype == dt and t.dim() == 2 and t.shape[1] == 4):
+            raise TypeError("%s must be a contiguous CUDA tensor of %s with shape (n, 4)" % (what, dt))
+    if spj.shape[0] != cells.shape[0]:
+        raise ValueError("spj needs one record per cell")
+    rc = lib.mwf_monopoles_static(ctypes.c_void_p(cells.data_ptr()), cells.shape[0], ctypes.c_void_p(ptcl.data_ptr()), ptcl.shape[0],
+                                  ctypes.c_void_p(spj.data_ptr()), _stream_handle(stream))
+    if rc != 0:
+        raise MwfError(rc, lib.mwf_static_last_error().decode() or lib.mwf_strerror(rc).decode())
 
 
 class MultiWalkForce:
