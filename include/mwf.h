@@ -116,7 +116,16 @@ int mwf_set_tree(mwf_ctx* c, const mwf_cell* cells, int64_t n_cell, void* stream
  * mode: MWF_MAKE_LIST (lists valid for one evaluation, dropped once every dispatched tag has been
  * retrieved) or MWF_MAKE_LIST_FOR_REUSE (kept until the next mwf_set_lists / mwf_set_tree).
  * Requires mwf_set_tree() first.  Validates on the device, re-encodes into one padded merged list per
- * group and builds the work schedule.  Blocking. */
+ * group and builds the work schedule.  Blocking.
+ * Call order and accuracy (reading S11b of DESIGN.md): every SPJ entry is marked here, once, as FAR (swept from its
+ * fp32 record) or NEAR (swept with the fp64 remainder of its centre of mass, about 3 x the cost), from the particle
+ * positions in the store.  Only positions uploaded for this step are used: all N particles, in the new tree's order,
+ * uploaded since the last dispatch (mwf_set_particles from 0 upwards or mwf_swap_store; mwf_build leaves them so).
+ * If they arrive only after this call, every SPJ entry is treated as NEAR -- always accurate, slower.  The marks are
+ * kept over the reuse steps while the particles drift; FAR allows a margin of 16x over what the error bound needs, so
+ * a group and a cell would have to close a sizeable part of their distance before a mark is wrong -- rebuild the lists
+ * before that, as the opening criterion needs anyway.  The marks hold for ANY list, also one that no opening
+ * criterion produced: the distance used is a lower bound (tight boxes of the group's and of the cell's particles). */
 int mwf_set_lists(mwf_ctx* c, int64_t n_group, const int32_t* grp_first, const int32_t* grp_n,
                   const int64_t* epj_off, const int32_t* epj_id, const int64_t* spj_off, const int32_t* spj_id,
                   int mode, void* stream);
@@ -276,10 +285,14 @@ int mwf_get_groups(mwf_ctx* c, int32_t* grp_first, int32_t* grp_n);
 int mwf_get_lists(mwf_ctx* c, int64_t* epj_off, int32_t* epj_id, int64_t* spj_off, int32_t* spj_id);
 /* The list buffers exactly as the force kernel reads them (pin P9 of SURVEY.md 8(c): "list buffers bit-identical before /
  * after the reuse steps"): list_off[n_group + 1] (offsets in entries, multiples of 64) and the merged,
- * padded index list (per group: EPJ ids, dummy indices up to a whole tile, SPJ ids + N, dummy indices up to a whole tile).  *n_group, *n_entry = groups and
+ * padded index list (per group: run 1 = EPJ ids then FAR SPJ ids + N, dummy indices up to a whole tile; run 2 = NEAR SPJ ids + N, dummy indices up to a whole tile).  *n_group, *n_entry = groups and
  * entries in the merged list (also without destinations: call once to size them).  Destinations HOST or DEVICE, either may be NULL.
  * MWF_ESTATE without lists.  Blocking. */
 int mwf_get_list_buffer(mwf_ctx* c, int64_t* list_off, int32_t* list, int64_t* n_group, int64_t* n_entry, int dst_on_device);
+/* The third array the force kernel reads with them: run1_len[g] = entries of group g's run 1 (its EPJ entries + its FAR SPJ
+ * entries, reading S11b); run 2 (the NEAR SPJ entries) starts at the next multiple of 64 behind it.  n_group values, HOST or
+ * DEVICE.  MWF_ESTATE without lists.  Blocking. */
+int mwf_get_run1_len(mwf_ctx* c, int32_t* run1_len, int dst_on_device);
 
 /* ---- Device-resident reuse step (the paper's own conclusion, P:1171-1185:
  * with the lists resident the per-step host<->device transfers of particles and forces are what is left,

@@ -28,7 +28,7 @@ SYMBOLS = (
     "mwf_set_sph", "mwf_get_sph", "mwf_dispatch_density", "mwf_dispatch_hydro", "mwf_calc_sph_all",
     "mwf_build", "mwf_build_neighbours", "mwf_get_build_sizes", "mwf_get_permutation", "mwf_get_tree", "mwf_get_groups", "mwf_get_lists", "mwf_get_list_buffer",
     "mwf_set_particles_next", "mwf_swap_store", "mwf_get_tag_split",
-    "mwf_monopoles_static", "mwf_static_last_error",
+    "mwf_monopoles_static", "mwf_static_last_error", "mwf_get_run1_len",
 )
 
 
@@ -103,6 +103,7 @@ def load_library(path: str | None = None) -> ctypes.CDLL:
         "mwf_get_lists": [vp, vp, vp, vp, vp],
         "mwf_get_list_buffer": [vp, vp, vp, P(i64), P(i64), ci],
         "mwf_monopoles_static": [vp, i64, vp, i64, vp, vp],
+        "mwf_get_run1_len": [vp, vp, ci],
     }
     for name, args in sig.items():
         fn = getattr(lib, name)
@@ -403,6 +404,14 @@ class MultiWalkForce:
         off, lst = np.empty(g.value + 1, np.int64), np.empty(max(1, n.value), np.int32)
         self._ck(self._lib.mwf_get_list_buffer(self._h, _host_ptr(off, np.int64, "list_off"), _host_ptr(lst, np.int32, "list"), None, None, 0))
         return off, lst[:n.value]
+
+    def get_run1_len(self) -> np.ndarray:
+        """Per group: EPJ + far SPJ entries (run 1 of its merged list); the near SPJ entries are the rest of the list."""
+        g = ctypes.c_int64(0)
+        self._ck(self._lib.mwf_get_list_buffer(self._h, None, None, ctypes.byref(g), None, 0))
+        out = np.empty(g.value, np.int32)
+        self._ck(self._lib.mwf_get_run1_len(self._h, _host_ptr(out, np.int32, "run1_len"), 0))
+        return out
 
     def get_monopoles(self, n_cell: int) -> np.ndarray:
         out = np.empty((n_cell, 4), np.float32)

@@ -12,6 +12,7 @@ using namespace mwf;
 static int build_failed(mwf_ctx* c, cudaStream_t s, int code) {
     after_store_op(c, s);
     c->ptcl_hi = c->vel_hi = c->sph_hi = 0;
+    c->cls_hi = 0;
     c->n_ptcl = 0;
     return code;
 }
@@ -65,6 +66,7 @@ static int build_impl(mwf_ctx* c, int64_t n, int32_t n_leaf, int32_t n_grp, doub
     c->n_ptcl = n;
     c->n_cell = n_cell;
     c->ptcl_hi = n;
+    c->cls_hi = n;  // the store is in the order of the tree just built
     // lists: counting walk, offsets, capacity check, fill walk
     WalkRule rule;
     rule.theta = theta;
@@ -207,6 +209,15 @@ int mwf_get_list_buffer(mwf_ctx* c, int64_t* list_off, int32_t* list, int64_t* n
     const auto kind = dst_on_device ? cudaMemcpyDeviceToDevice : cudaMemcpyDeviceToHost;
     if (list_off) CU(c, cudaMemcpy(list_off, c->list_off, (size_t)(c->n_group + 1) * 8, kind));
     if (list && c->padded_entries > 0) CU(c, cudaMemcpy(list, c->list, (size_t)c->padded_entries * 4, kind));
+    return MWF_OK;
+}
+
+int mwf_get_run1_len(mwf_ctx* c, int32_t* run1_len, int dst_on_device) {
+    MWF_ENTER(c);
+    if (!c || !run1_len) return MWF_EINVAL;
+    if (!c->have_lists) return MWF_ESTATE;
+    CU(c, cudaDeviceSynchronize());
+    CU(c, cudaMemcpy(run1_len, c->grp_run1, (size_t)c->n_group * 4, dst_on_device ? cudaMemcpyDeviceToDevice : cudaMemcpyDeviceToHost));
     return MWF_OK;
 }
 

@@ -202,6 +202,10 @@ int mwf_set_spj_order(mwf_ctx* c, int order) {
     for (int t = 0; t < c->p.n_tag; ++t)
         if (c->tag_inflight[t] || !c->tag_ranges[t].empty()) return MWF_ESTATE;
     if (order == 2 && !c->quad) {
+        // first the shared-memory opt-in of the order-2 kernel on this ctx's device and its occupancy; the arrays only once
+        // that has succeeded, so that a failed call leaves the ctx at order 1 with nothing half set up
+        const int ctas = force_quad_max_ctas_per_sm();
+        if (ctas < 1) return cuda_fail(c, cudaGetLastError(), "order-2 force kernel: shared-memory opt-in / occupancy");
         void *a = nullptr, *b = nullptr;
         if (cudaMalloc(&a, (size_t)c->p.max_cell * 48) != cudaSuccess || cudaMalloc(&b, (size_t)c->p.max_cell * 32) != cudaSuccess) {
             cudaGetLastError();
@@ -210,8 +214,7 @@ int mwf_set_spj_order(mwf_ctx* c, int order) {
         }
         c->quad64 = static_cast<double*>(a);
         c->quad = static_cast<float4*>(b);
-        c->quad_ctas_per_sm = force_quad_max_ctas_per_sm();
-        if (c->quad_ctas_per_sm < 1) return MWF_ECUDA;
+        c->quad_ctas_per_sm = ctas;
     }
     if (order != c->spj_order) {
         c->mono_fresh = false;  // the moments on the device are those of the other order

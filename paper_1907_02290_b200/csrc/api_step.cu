@@ -27,6 +27,7 @@ int pick_order(mwf_ctx* c, int64_t g_begin, int64_t g_end, cudaStream_t s, const
 // Bookkeeping common to every kind of dispatch: the tag is in flight, its particle ranges await a retrieve.
 void book_dispatch(mwf_ctx* c, int32_t tag, int64_t g_begin, int64_t g_end) {
     c->tag_inflight[tag] = true;
+    c->cls_hi = 0;  // the store has been used with the current tree: uploads from here on are the next step's
     ++c->n_launch;
     c->n_inter += c->h_inter[(size_t)g_end] - c->h_inter[(size_t)g_begin];
     // particle range covered (groups are disjoint; contiguous when they come from a tree)
@@ -90,6 +91,7 @@ static int dispatch_launch(mwf_ctx* c, int32_t tag, int64_t g_begin, int64_t g_e
         }
     }
     const int64_t resident = (int64_t)c->n_sm * (a.quad ? c->quad_ctas_per_sm : c->ctas_per_sm);
+    if (resident < 1) return cuda_fail(c, cudaErrorLaunchOutOfResources, "force kernel: no block fits an SM");  // never a silent empty launch
     const int64_t want = (a.n_items + WARPS_PER_CTA - 1) / WARPS_PER_CTA;
     int grid = (int)resident, warps = WARPS_PER_CTA;
     a.counter = nullptr;
@@ -125,6 +127,7 @@ int mwf_set_particles(mwf_ctx* c, const mwf_posm* src, int64_t first, int64_t n,
     CU(c, cudaMemcpyAsync(c->store + first, src, (size_t)n * 16, src_on_device ? cudaMemcpyDeviceToDevice : cudaMemcpyHostToDevice, s));
     c->ptcl_hi = std::max(c->ptcl_hi, first + n);
     if (c->have_tree) c->ptcl_hi = std::min(c->ptcl_hi, c->n_ptcl);
+    if (first <= c->cls_hi) c->cls_hi = std::max(c->cls_hi, first + n);
     c->mono_fresh = false;
     c->acc_full = false;
     return after_store_op(c, s);
@@ -175,6 +178,7 @@ int mwf_swap_store(mwf_ctx* c, void* stream) {
     c->next_ranges.clear();
     c->next_streams.clear();
     c->ptcl_hi = c->n_ptcl;
+    c->cls_hi = c->n_ptcl;
     c->mono_fresh = false;
     c->acc_full = false;
     return after_store_op(c, s);  // every later dispatch / store operation waits for this event, hence for the uploads
@@ -241,6 +245,7 @@ int mwf_set_tree(mwf_ctx* c, const mwf_cell* cells, int64_t n_cell, void* stream
     c->n_ptcl = n;
     c->n_cell = n_cell;
     c->ptcl_hi = std::min(c->ptcl_hi, n);
+    c->cls_hi = std::min(c->cls_hi, n);
     c->have_tree = true;
     return MWF_OK;
 }
@@ -278,9 +283,12 @@ int mwf_set_lists(mwf_ctx* c, int64_t n_group, const int32_t* grp_first, const i
     if (e_epj) CU(c, cudaMemcpyAsync(c->st_ids, epj_id, (size_t)e_epj * 4, H2D, s));
     if (e_spj) CU(c, cudaMemcpyAsync(c->st_ids + e_epj, spj_id, (size_t)e_spj * 4, H2D, s));
     // which SPJ entries are far enough to be swept like particles (run 1); their number per group sizes the two runs
-    CU(c, launch_classify_spj(n_group, c->grp_first, c->grp_n, c->st_spj_off, c->st_ids + e_epj, c->cells, c->store, c->n_ptcl, c->n_cell,
-                              c->ptcl_hi >= c->n_ptcl, c->grp_nfar, s));
-    ++c->n_launch;
+    // (only from positions uploaded for THIS step: what an earlier step left in the store is in the previous tree's order)
+    const bool have_ptcl = c->ptcl_hi >= c->n_ptcl && c->cls_hi >= c->n_ptcl;
+    // (the cells' tight boxes live in mom64 for the moment: 32 B per cell, rewritten from the leaves up by every refresh that reads it)
+    CU(c, launch_classify_spj(n_group, c->grp_first, c->grp_n, c->st_spj_off, c->st_ids + e_epj, c->cells, c->parent, c->arrive,
+                              reinterpret_cast<float4*>(c->mom64), c->store, c->n_ptcl, c->n_cell, have_ptcl, c->grp_nfar, s));
+    c->n_launch += have_ptcl ? 2 : 1;
     std::vector<int32_t> n_far((size_t)n_group);
     CU(c, cudaMemcpyAsync(n_far.data(), c->grp_nfar, (size_t)n_group * 4, cudaMemcpyDeviceToHost, s));
     CU(c, cudaStreamSynchronize(s));

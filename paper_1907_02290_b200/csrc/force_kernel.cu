@@ -581,12 +581,9 @@ cudaError_t launch_force(const ForceArgs& a, int grid, int warps, cudaStream_t s
     if (warps < 1 || warps > WARPS_PER_CTA) return cudaErrorInvalidValue;
     if (a.quad) {
         if (a.jdata) return cudaErrorInvalidValue;
-        static bool optin = false;  // 53 KB of dynamic shared memory per block
-        if (!optin) {
-            const cudaError_t e = cudaFuncSetAttribute(k_force_quad, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)(WARPS_PER_CTA * QUAD_SMEM_PER_WARP));
-            if (e != cudaSuccess) return e;
-            optin = true;
-        }
+        // 8 warps x 544 float4 = 68 KB of dynamic shared memory per block: above the default limit, so the kernel needs the opt-in of
+        // force_quad_max_ctas_per_sm().  Function attributes are per device; mwf_set_spj_order(2) makes that call for every ctx on
+        // the ctx's own device before it hands out a quad pointer, so no process-wide flag is kept here.
         k_force_quad<<<grid, warps * 32, warps * QUAD_SMEM_PER_WARP, s>>>(a);
     } else if (a.jdata)
         k_force_data<<<grid, warps * 32, warps * FORCE_SMEM_PER_WARP, s>>>(a);

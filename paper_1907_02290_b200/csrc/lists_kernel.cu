@@ -18,13 +18,56 @@ namespace {
 
 constexpr unsigned FAR_BIT = 0x40000000u;  // marks a far SPJ entry in the staging ids between the two passes
 
-// Pass 1: classifies every SPJ entry of every group as far or near and counts the far ones.  There are no moments yet
-// at this point of the construction step and an uploaded tree carries no geometry, so the cell is located by its first and
-// last particle (Morton order: the two ends of its range) and the group by the bounding box of its particles; the
-// classification only chooses between two correct ways of sweeping an entry, so a rough distance will do -- entries anywhere
-// near the threshold are accurate either way.  have_ptcl = 0 (the particles are not in the store yet): everything is near.
+// Pass 0: the tight bounding box of every cell's particles, bottom-up over the fixed tree like the climb variant of the
+// monopole refresh: a leaf takes min / max over its particle range, the last child to arrive at a cell (self-resetting
+// arrival counter) combines the children's boxes and carries on.  box[2c] = (lo, -), box[2c + 1] = (hi, -).  An uploaded
+// tree carries no geometry, and min / max of fp32 values are exact, so these boxes are the one bound that holds for any
+// tree and any list: the cell's centre of mass lies inside its box (convex hull of the particles).
+__global__ void __launch_bounds__(128) k_cell_boxes(const mwf_cell* __restrict__ cells, const int32_t* __restrict__ parent, int64_t n_cell,
+                                                    const float4* __restrict__ store, float4* __restrict__ box, int32_t* __restrict__ counter) {
+    const int64_t c0 = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (c0 >= n_cell) return;
+    const mwf_cell leaf = cells[c0];
+    if (leaf.n_child != 0) return;
+    float lo[3] = {INFINITY, INFINITY, INFINITY}, hi[3] = {-INFINITY, -INFINITY, -INFINITY};
+    const float4* __restrict__ p = store + leaf.first_ptcl;
+    for (int k = 0; k < leaf.n_ptcl; ++k) {
+        const float4 q = p[k];
+        lo[0] = fminf(lo[0], q.x); hi[0] = fmaxf(hi[0], q.x);
+        lo[1] = fminf(lo[1], q.y); hi[1] = fmaxf(hi[1], q.y);
+        lo[2] = fminf(lo[2], q.z); hi[2] = fmaxf(hi[2], q.z);
+    }
+    box[2 * c0] = make_float4(lo[0], lo[1], lo[2], 0.f);
+    box[2 * c0 + 1] = make_float4(hi[0], hi[1], hi[2], 0.f);
+    int64_t c = c0;
+    for (;;) {
+        const int32_t par = parent[c];
+        if (par < 0) break;
+        const mwf_cell pc = cells[par];
+        __threadfence();  // publish this cell's box before announcing arrival
+        if (atomicAdd(&counter[par], 1) != pc.n_child - 1) break;
+        counter[par] = 0;
+        __threadfence();
+        for (int a = 0; a < 3; ++a) { lo[a] = INFINITY; hi[a] = -INFINITY; }
+        for (int k = 0; k < pc.n_child; ++k) {
+            const float4 l = __ldcg(&box[2 * (int64_t)(pc.first_child + k)]), h = __ldcg(&box[2 * (int64_t)(pc.first_child + k) + 1]);
+            lo[0] = fminf(lo[0], l.x); hi[0] = fmaxf(hi[0], h.x);
+            lo[1] = fminf(lo[1], l.y); hi[1] = fmaxf(hi[1], h.y);
+            lo[2] = fminf(lo[2], l.z); hi[2] = fmaxf(hi[2], h.z);
+        }
+        box[2 * (int64_t)par] = make_float4(lo[0], lo[1], lo[2], 0.f);
+        box[2 * (int64_t)par + 1] = make_float4(hi[0], hi[1], hi[2], 0.f);
+        c = par;
+    }
+}
+
+// Pass 1: classifies every SPJ entry of every group as far or near and counts the far ones.  There are no moments yet at
+// this point of the construction step, so the cell is located by the tight box of its particles (pass 0) and the group by
+// the tight box of its own: the gap between the two boxes is a lower bound of the distance from any i-particle to the
+// cell's centre of mass, and the largest |coordinate| of the cell's box an upper bound of the centre's -- so "far" is a
+// bound, for any list, not an estimate.  have_ptcl = 0 (the particles of this step are not in the store yet): everything is near.
 __global__ void __launch_bounds__(256) k_classify_spj(int64_t n_group, const int32_t* __restrict__ grp_first, const int32_t* __restrict__ grp_n,
-                                                      const int64_t* __restrict__ spj_off, int32_t* __restrict__ spj_id, const mwf_cell* __restrict__ cells,
+                                                      const int64_t* __restrict__ spj_off, int32_t* __restrict__ spj_id, const float4* __restrict__ box,
                                                       const float4* __restrict__ store, int64_t n_ptcl, int64_t n_cell, int have_ptcl,
                                                       int32_t* __restrict__ n_far) {
     __shared__ float s_box[6][8];
@@ -59,15 +102,16 @@ __global__ void __launch_bounds__(256) k_classify_spj(int64_t n_group, const int
         int far = 0;
         for (int64_t k = threadIdx.x; k < ns; k += blockDim.x) {
             const int32_t id = spj_id[s0 + k];
-            if (!ok || id < 0 || id >= n_cell) continue;  // bad indices are reported by the merge pass
-            const mwf_cell cc = cells[id];
-            if (cc.n_ptcl <= 0 || cc.first_ptcl < 0 || (int64_t)cc.first_ptcl + cc.n_ptcl > n_ptcl) continue;
-            const float4 a = store[cc.first_ptcl], b = store[cc.first_ptcl + cc.n_ptcl - 1];
+            // A bad index is reported by the merge pass.  It is overwritten here, before any far mark is set, so that an uploaded
+            // id that happens to carry FAR_BIT over valid low bits cannot pass for a marked entry (n_cell < 2^30: params_ok).
+            if (id < 0 || id >= n_cell) { spj_id[s0 + k] = -1; continue; }
+            if (!ok) continue;
+            const float4 a = box[2 * (int64_t)id], b = box[2 * (int64_t)id + 1];
             const float pa[3] = {a.x, a.y, a.z}, pb[3] = {b.x, b.y, b.z};
             float d2 = 0.f, amax = 0.f;
 #pragma unroll
             for (int q = 0; q < 3; ++q) {
-                const float clo = fminf(pa[q], pb[q]), chi = fmaxf(pa[q], pb[q]);  // the cell, roughly
+                const float clo = pa[q], chi = pb[q];
                 const float gap = fmaxf(0.f, fmaxf(lo[q] - chi, clo - hi[q]));
                 d2 += gap * gap;
                 amax = fmaxf(amax, fmaxf(fabsf(clo), fabsf(chi)));
@@ -164,12 +208,18 @@ __global__ void __launch_bounds__(256) k_merge_lists(int64_t n_group, const int3
 
 }  // namespace
 
+// box: scratch for 2 float4 per cell; parent / counter: those of the validated tree (counter all zero, left all zero).
 cudaError_t launch_classify_spj(int64_t n_group, const int32_t* grp_first, const int32_t* grp_n, const int64_t* spj_off, int32_t* spj_id,
-                                const mwf_cell* cells, const float4* store, int64_t n_ptcl, int64_t n_cell, bool have_ptcl, int32_t* n_far,
-                                cudaStream_t s) {
+                                const mwf_cell* cells, const int32_t* parent, int32_t* counter, float4* box, const float4* store, int64_t n_ptcl,
+                                int64_t n_cell, bool have_ptcl, int32_t* n_far, cudaStream_t s) {
     if (n_group <= 0) return cudaSuccess;
+    if (have_ptcl) {
+        k_cell_boxes<<<(unsigned)((n_cell + 127) / 128), 128, 0, s>>>(cells, parent, n_cell, store, box, counter);
+        const cudaError_t e = cudaGetLastError();
+        if (e != cudaSuccess) return e;
+    }
     const int64_t grid = n_group < 148 * 16 ? n_group : 148 * 16;
-    k_classify_spj<<<(unsigned)grid, 256, 0, s>>>(n_group, grp_first, grp_n, spj_off, spj_id, cells, store, n_ptcl, n_cell, have_ptcl ? 1 : 0, n_far);
+    k_classify_spj<<<(unsigned)grid, 256, 0, s>>>(n_group, grp_first, grp_n, spj_off, spj_id, box, store, n_ptcl, n_cell, have_ptcl ? 1 : 0, n_far);
     return cudaGetLastError();
 }
 

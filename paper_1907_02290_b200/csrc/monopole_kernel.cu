@@ -18,34 +18,37 @@ namespace mwf {
 __global__ void k_tree_prepare(const mwf_cell* __restrict__ cells, int64_t n_cell, int64_t max_ptcl, int32_t* __restrict__ parent,
                                int32_t* __restrict__ counter, unsigned int* __restrict__ err) {
     const int64_t c = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
-    if (c >= n_cell) return;
-    const mwf_cell cc = cells[c];
-    const int64_t n = cells[0].n_ptcl;
+    const bool live = c < n_cell;  // no early return: every lane of the warp takes part in the reduction at the end
     unsigned int e = 0;
-    if (c == 0) {
-        parent[0] = -1;
-        if (cc.first_ptcl != 0 || cc.n_ptcl <= 0 || cc.n_ptcl > max_ptcl) e |= ERR_CELL_RANGE;
-    }
-    counter[c] = 0;
-    if (cc.n_ptcl <= 0 || cc.first_ptcl < 0 || (int64_t)cc.first_ptcl + cc.n_ptcl > n) e |= ERR_CELL_RANGE;
-    if (cc.n_child < 0 || cc.n_child > 8) e |= ERR_CHILD_RANGE;
-    if (cc.n_child > 0) {
-        if (cc.first_child <= c || (int64_t)cc.first_child + cc.n_child > n_cell) {
-            e |= ERR_CHILD_RANGE;
-        } else {
-            int64_t next = cc.first_ptcl;
-            for (int k = 0; k < cc.n_child; ++k) {
-                const mwf_cell ch = cells[cc.first_child + k];
-                if (ch.first_ptcl != next) e |= ERR_CHILD_PART;
-                next += ch.n_ptcl;
-                parent[cc.first_child + k] = (int32_t)c;
-            }
-            if (next != (int64_t)cc.first_ptcl + cc.n_ptcl) e |= ERR_CHILD_PART;
+    unsigned claims = 0;
+    if (live) {
+        const mwf_cell cc = cells[c];
+        const int64_t n = cells[0].n_ptcl;
+        if (c == 0) {
+            parent[0] = -1;
+            if (cc.first_ptcl != 0 || cc.n_ptcl <= 0 || cc.n_ptcl > max_ptcl) e |= ERR_CELL_RANGE;
         }
+        counter[c] = 0;
+        if (cc.n_ptcl <= 0 || cc.first_ptcl < 0 || (int64_t)cc.first_ptcl + cc.n_ptcl > n) e |= ERR_CELL_RANGE;
+        if (cc.n_child < 0 || cc.n_child > 8) e |= ERR_CHILD_RANGE;
+        if (cc.n_child > 0) {
+            if (cc.first_child <= c || (int64_t)cc.first_child + cc.n_child > n_cell) {
+                e |= ERR_CHILD_RANGE;
+            } else {
+                int64_t next = cc.first_ptcl;
+                for (int k = 0; k < cc.n_child; ++k) {
+                    const mwf_cell ch = cells[cc.first_child + k];
+                    if (ch.first_ptcl != next) e |= ERR_CHILD_PART;
+                    next += ch.n_ptcl;
+                    parent[cc.first_child + k] = (int32_t)c;
+                }
+                if (next != (int64_t)cc.first_ptcl + cc.n_ptcl) e |= ERR_CHILD_PART;
+            }
+        }
+        if (e) atomicOr(err, e);
+        // number of child claims, for k_tree_check (a cell with a bad child range claims nothing)
+        claims = (cc.n_child > 0 && !(e & ERR_CHILD_RANGE)) ? (unsigned)cc.n_child : 0u;
     }
-    if (e) atomicOr(err, e);
-    // number of child claims, for k_tree_check (a cell with a bad child range claims nothing)
-    unsigned claims = (cc.n_child > 0 && !(e & ERR_CHILD_RANGE)) ? (unsigned)cc.n_child : 0u;
 #pragma unroll
     for (int d = 16; d > 0; d >>= 1) claims += __shfl_xor_sync(0xffffffffu, claims, d);
     if ((threadIdx.x & 31) == 0 && claims) atomicAdd(err + 1, claims);

@@ -49,7 +49,7 @@ struct mwf_ctx {
     int64_t* list_off = nullptr;  // [max_group + 1]
     int64_t* st_epj_off = nullptr, *st_spj_off = nullptr;  // [max_group + 1] staging
     int32_t* st_ids = nullptr;    // [max_entry] staging of the uploaded ids
-    int32_t* list = nullptr;      // [max_entry + TILE_J * max_group] merged, padded
+    int32_t* list = nullptr;      // [max_entry + 2 * TILE_J * max_group] merged; each of a group's two runs padded to whole tiles
     mwf::WorkItem* items = nullptr;    // [max_items]
     int32_t* order_full = nullptr, *order_split = nullptr;  // [max_items]
     // items sorted by width class (32, 16, 8, 4, 2), group order inside a class: any contiguous group range then has its
@@ -65,6 +65,10 @@ struct mwf_ctx {
     // state
     int64_t n_ptcl = 0, n_cell = 0, n_group = 0, n_items = 0, ptcl_hi = 0, padded_entries = 0;
     bool have_tree = false, have_lists = false, lists_for_reuse = false, mono_fresh = false;
+    // Particles [0, cls_hi) have been uploaded, contiguously from 0, since the last dispatch: they are the positions of the
+    // step being prepared, so mwf_set_lists may classify SPJ entries as far / near from them (reading S11b).  A dispatch
+    // consumes the store for the tree it ran on and resets this; when mwf_set_lists finds cls_hi < N it calls every entry near.
+    int64_t cls_hi = 0;
     mwf::BuildBuffers bb{};       // device-side construction step (NEXT-2)
     int64_t walk_warps_n = 0;
     bool built_on_device = false;

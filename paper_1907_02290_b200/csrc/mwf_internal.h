@@ -128,8 +128,8 @@ cudaError_t launch_leaf_ranking(const mwf_cell* cells, int64_t n_cell, int64_t n
 cudaError_t launch_monopoles_scan(const mwf_cell* cells, const int2* cell_lr, int64_t n_cell, int64_t n_ptcl, int64_t n_leaf_cells, float4* store,
                                   float4* spj_lo, double4* P, double4* toff, cudaStream_t s);
 cudaError_t launch_classify_spj(int64_t n_group, const int32_t* grp_first, const int32_t* grp_n, const int64_t* spj_off, int32_t* spj_id,
-                                const mwf_cell* cells, const float4* store, int64_t n_ptcl, int64_t n_cell, bool have_ptcl, int32_t* n_far,
-                                cudaStream_t s);
+                                const mwf_cell* cells, const int32_t* parent, int32_t* counter, float4* box, const float4* store, int64_t n_ptcl,
+                                int64_t n_cell, bool have_ptcl, int32_t* n_far, cudaStream_t s);
 cudaError_t launch_merge_lists(int64_t n_group, const int32_t* grp_first, const int32_t* grp_n, const int64_t* epj_off,
                                const int32_t* epj_id, const int64_t* spj_off, const int32_t* spj_id, const int64_t* list_off,
                                const int32_t* n_far, int32_t* run1_len, int64_t n_ptcl, int64_t n_cell, int32_t* list, uint8_t* grp_self,

@@ -577,6 +577,7 @@ def test_state_machine_and_validation():
     assert expect_code(f.dispatch, 0, 0, 1) == binding.ESTATE
     # MAKE_LIST_FOR_REUSE keeps them; evaluation 0 is identical under either mode (pin P9)
     f.begin_step(binding.MAKE_LIST_FOR_REUSE)
+    f.set_particles(w.posm)        # a construction step brings its particles (mwf.h, mwf_set_lists: without them every SPJ entry is near)
     f.set_tree(w.cells)
     f.set_lists(*lists, binding.MAKE_LIST_FOR_REUSE)
     f.refresh_monopoles()
