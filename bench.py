@@ -652,6 +652,102 @@ def sph_summary(binding, device, steps=3):
 
 
 # ----------------------------------------------------------------------------- main
+def pipelined_loop(binding, f, w, src_host, dst_host, steps, device, barrier=None):
+    """Host wall-clock ms of `steps` list-reuse steps through pinned host buffers with the pipelined loop of mwf.h (P:179,
+    P:189): per tag the D2H of its results, then the H2D of its particles of the next step into the shadow store while the
+    other tags' kernels still run; swap, refresh, one dispatch per tag.  The drain (results of the last evaluation) is inside."""
+    import torch
+    split = f.get_tag_split()
+    tags = [t for t in range(f.n_tag) if split[t + 1] > split[t]]
+    pfirst = {t: int(w.grp_first[split[t]]) for t in tags}
+    pend = {t: int(w.grp_first[split[t + 1] - 1] + w.grp_n[split[t + 1] - 1]) for t in tags}
+    up = torch.cuda.Stream(device=device)
+
+    def dispatch_tags():
+        f.refresh_monopoles(f.streams[0])
+        for t in tags:
+            f.dispatch(t, int(split[t]), int(split[t + 1]))
+
+    def step_pipelined():
+        for t in tags:
+            f.retrieve(t, dst_host)
+            f.set_particles_next(src_host[pfirst[t]:pend[t]], pfirst[t], pend[t] - pfirst[t], up)
+        f.swap_store(f.streams[0])
+        dispatch_tags()
+
+    f.begin_step(binding.REUSE_LIST)
+    f.set_particles(src_host, 0, w.n, f.streams[0])
+    dispatch_tags()
+    for _ in range(2):
+        step_pipelined()
+    torch.cuda.synchronize()   # the evaluation in flight is complete: the K evaluations timed below are launched inside
+    if barrier:
+        barrier()
+    t0 = time.perf_counter()
+    for _ in range(steps):
+        step_pipelined()
+    for t in tags:   # drain: the results of the last evaluation (K uploads, K evaluations, K + 1 retrieves in the region)
+        f.retrieve(t, dst_host)
+    torch.cuda.synchronize()
+    return (time.perf_counter() - t0) * 1e3
+
+
+def other_config_leg(binding, cfg, device, n_tag, steps, peak_tflops, label=None, far_from_origin=False):
+    """One more workload beside the headline's, in the same process: its list-reuse step through device buffers (CUDA events:
+    whole step and k_force alone, median of `steps` >= 10), the pipelined loop through pinned host buffers, and the result of
+    the timed step against the fp64 oracle on EVERY particle.  far_from_origin: the particles are moved 40 system diameters
+    away from the origin before the tree is built, so that every SPJ entry is NEAR (reading S11b): the floor of the kernel."""
+    import torch
+    import oracle
+    from paper_1907_02290_b200.workload import build_tree_and_lists, make_particles, make_workload
+    steps = max(10, steps)
+    t = time.perf_counter()
+    if far_from_origin:
+        posm, _ = make_particles(cfg)
+        diam = float(np.linalg.norm(posm[:, :3].max(0) - posm[:, :3].min(0)))
+        posm[:, :3] += np.float32(2.0 ** np.ceil(np.log2(40.0 * diam)))
+        w = build_tree_and_lists(posm, cfg.n_leaf, cfg.n_grp, cfg.theta)
+    else:
+        w = make_workload(cfg)
+    t_host = time.perf_counter() - t
+    f = binding.MultiWalkForce.for_workload(w, eps=cfg.eps, n_tag=n_tag, device=device)
+    f.upload_workload(w, binding.MAKE_LIST_FOR_REUSE)
+    run1 = f.get_run1_len().astype(np.int64)
+    n_far = int((run1 - np.diff(w.epj_off)).sum())
+    src_dev = torch.from_numpy(w.posm).to(f.device)
+    dst_dev = torch.zeros((w.n, 4), dtype=torch.float32, device=f.device)
+    k_ms, step_ms = [], []
+    for it in range(3 + steps):
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        e0.record(f.streams[0])
+        f.begin_step(binding.REUSE_LIST)
+        f.calc_force_all(src_dev, dst_dev)
+        e1.record(f.streams[0])
+        torch.cuda.synchronize()
+        if it >= 3:
+            k_ms.append(f.last_dispatch_ms(0))
+            step_ms.append(e0.elapsed_time(e1))
+    result = dst_dev.cpu().numpy()
+    src_host, dst_host = f.pinned(w.n), f.pinned(w.n)
+    src_host.numpy()[:] = w.posm
+    ms_pipe = pipelined_loop(binding, f, w, src_host, dst_host, steps, device) / steps
+    f.close()
+    del src_dev, dst_dev, src_host, dst_host
+    mom = oracle.monopoles(w.cells, w.posm)
+    t = time.perf_counter()
+    acc, pot = oracle.forces(w.posm, mom, w.grp_first, w.grp_n, w.epj_off, w.epj_id, w.spj_off, w.spj_id, cfg.eps, 1.0)
+    t_oracle = time.perf_counter() - t
+    km, sm = float(np.median(k_ms)), float(np.median(step_ms))
+    return {"workload": label or "config %d: %s" % (cfg_index(cfg) + 1, cfg.name), "n": w.n, "n_group": w.n_group, "interactions_per_step": w.interactions,
+            "spj_entries": int(w.spj_id.size), "near_spj_entries": int(w.spj_id.size) - n_far,
+            "kernel_ms": km, "kernel_ms_min": float(min(k_ms)), "frac": N_OP * w.interactions / (km * 1e-3) / 1e12 / peak_tflops,
+            "ms_per_step": sm, "value": w.interactions / (sm * 1e-3), "unit": UNIT,
+            "e2e_ms_per_step": ms_pipe, "e2e_value": w.interactions / (ms_pipe * 1e-3),
+            "parity": parity_of(w, result, np.arange(w.n_group), acc, pot),
+            "host_tree_and_lists_s": round(t_host, 2), "oracle_s": round(t_oracle, 2),
+            "timing": "CUDA events, median of %d steps after 3 warm-up (device buffers); e2e: pipelined loop through pinned host buffers, host wall clock" % steps}
+
+
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
@@ -662,6 +758,7 @@ def main():
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--cpu-baseline-seconds", type=float, default=15.0)
     ap.add_argument("--n-tag", type=int, default=8)
+    ap.add_argument("--no-other-configs", action="store_true", help="skip the other_configs / all_near_floor legs of the default line")
     ap.add_argument("--leg", default="step", choices=["step", "construction", "sweep", "g1", "quad", "sph"],
                     help="step: the list-reuse step (the contract's JSON line); construction: only the device-side construction step; "
                          "sweep: kernel time per interaction against <n_i> and theta (the paper's Fig. A.1, P:1197-1212); "
@@ -771,38 +868,7 @@ def main():
 
     # ---- end to end, pipelined host loop: per tag the D2H of its results, then the H2D of its particles of
     # the next step into the shadow store while the other tags' kernels still run; swap, refresh, dispatch
-    split = f.get_tag_split()
-    tags = [t for t in range(f.n_tag) if split[t + 1] > split[t]]
-    pfirst = {t: int(w.grp_first[split[t]]) for t in tags}
-    pend = {t: int(w.grp_first[split[t + 1] - 1] + w.grp_n[split[t + 1] - 1]) for t in tags}
-    up = torch.cuda.Stream(device=local)
-
-    def dispatch_tags():
-        f.refresh_monopoles(f.streams[0])
-        for t in tags:
-            f.dispatch(t, int(split[t]), int(split[t + 1]))
-
-    def step_pipelined():
-        for t in tags:
-            f.retrieve(t, dst_host)
-            f.set_particles_next(src_host[pfirst[t]:pend[t]], pfirst[t], pend[t] - pfirst[t], up)
-        f.swap_store(f.streams[0])
-        dispatch_tags()
-
-    f.begin_step(binding.REUSE_LIST)
-    f.set_particles(src_host, 0, w.n, f.streams[0])
-    dispatch_tags()
-    for _ in range(2):
-        step_pipelined()
-    torch.cuda.synchronize()   # the evaluation in flight is complete: the K evaluations timed below are launched inside
-    replicas.barrier(world)
-    t0 = time.perf_counter()
-    for _ in range(args.steps):
-        step_pipelined()
-    for t in tags:   # drain: the results of the last evaluation (K uploads, K evaluations, K + 1 retrieves in the region)
-        f.retrieve(t, dst_host)
-    torch.cuda.synchronize()
-    ms_pipe = (time.perf_counter() - t0) * 1e3
+    ms_pipe = pipelined_loop(binding, f, w, src_host, dst_host, args.steps, local, barrier=lambda: replicas.barrier(world))
     units_p, ms_p_max = replicas.reduce_timing(inter * args.steps, ms_pipe, world)
     e2e_pipe = {"value": units_p / (ms_p_max * 1e-3), "unit": UNIT, "ms_per_step": ms_p_max / args.steps,
                 "h2d_bytes_per_step": 16 * w.n, "d2h_bytes_per_step": 16 * w.n,
@@ -960,6 +1026,30 @@ def main():
         except binding.MwfError as ex:
             whole_run = {"error": str(ex)}
 
+    # ---- the other full-size workloads of BASELINE.json (configs 2-4: Plummer 1M, disk + halo = galaxy-shaped, clumpy box =
+    # cosmology-shaped) and the all-near floor, each on its own ctx after the headline's legs
+    others, near_floor = None, None
+    if args.n is None and rank == 0 and cfg_index(cfg) == 4 and not args.no_other_configs:
+        f.close()
+        del src_dev, dst_dev, src_host, dst_host
+        torch.cuda.empty_cache()
+        pk = torch.cuda.get_device_properties(local).multi_processor_count * 256 * (measured_peaks().get("sm_max_mhz") or 1965.0) * 1e6 / 1e12
+        others = []
+        for ci in (1, 2, 3):
+            try:
+                t = time.perf_counter()
+                others.append(other_config_leg(binding, CONFIGS[ci], local, args.n_tag, args.steps, pk))
+                log("[bench] config %d: k_force %.3f ms, frac %.3f, parity %s (%.0f s)" % (
+                    ci + 1, others[-1]["kernel_ms"], others[-1]["frac"], others[-1]["parity"]["ok"], time.perf_counter() - t))
+            except binding.MwfError as ex:
+                others.append({"workload": "config %d" % (ci + 1), "error": str(ex)})
+        try:
+            near_floor = other_config_leg(binding, cfg, local, args.n_tag, args.steps, pk, far_from_origin=True,
+                                          label="config 5's particles moved 40 diameters from the origin: every SPJ entry near (reading S11b)")
+            log("[bench] all-near floor: k_force %.3f ms, frac %.3f, parity %s" % (near_floor["kernel_ms"], near_floor["frac"], near_floor["parity"]["ok"]))
+        except binding.MwfError as ex:
+            near_floor = {"error": str(ex)}
+
     if rank == 0:
         peaks = measured_peaks()
         clk = clocks.summary()
@@ -1010,6 +1100,7 @@ def main():
             "gpu_launches": launches, "clocks": clk, "phases": phases, "device_resident_step": dev_res, "batched_dispatch": batched, "order2_step": order2, "sph_step": sph_step,
             "run_n_reuse_%d" % max(cfg.n_reuse, 0): whole_run,
             "construction_step": {"host_tree_and_lists_s": round(t_build, 3), "upload_tree_and_lists_s": round(t_upload, 3), "on_device": dev_build},
+            "other_configs": others, "all_near_floor": near_floor,
             "context": {"paper_fraction_of_peak": 0.27, "paper_hardware": "TITAN V (P:673), whole step"},
         }
         print(json.dumps(out), flush=True)
