@@ -143,7 +143,11 @@ int mwf_refresh_monopoles(mwf_ctx* c, void* stream);
 /* (4) Launch the force kernel over groups [g_begin, g_end) on the stream of `tag`; non-blocking.
  * For every particle i of those groups, over the group's list (reading S1-S5 of DESIGN.md):
  *   acc_i =  G sum_k m_k (x_k - x_i) / (|x_k - x_i|^2 + eps^2)^(3/2)
- *   pot_i = -G sum_k m_k / (|x_k - x_i|^2 + eps^2)^(1/2)        (k != i by index) */
+ *   pot_i = -G sum_k m_k / (|x_k - x_i|^2 + eps^2)^(1/2)        (k != i by index)
+ * First-call latency: a dispatch over all groups, or over one of the ranges of mwf_get_tag_split(), uses a schedule made
+ * with the lists.  The FIRST dispatch over any other range after new lists builds, on the host, the permutation that
+ * orders the work items of arbitrary ranges widest first (about 1 ms for 10^5 items, plus one upload); later ones reuse it.
+ * MWF_ECUDA when no block of the kernel fits an SM (never a silent empty launch). */
 int mwf_dispatch(mwf_ctx* c, int32_t tag, int64_t g_begin, int64_t g_end);
 
 /* ---- Method G1 of the paper, for A/B comparison with the index method (paper
