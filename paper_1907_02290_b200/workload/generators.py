@@ -94,6 +94,25 @@ def plummer(n: int, seed: int, a: float = 1.0, mtot: float = 1.0, rcut: float = 
     return pos, vel, mass
 
 
+def planetary_ring(n: int, seed: int, m_ring: float = 1e-6, r_in: float = 0.95, r_out: float = 1.05, h: float = 1e-4):
+    """The paper's third shape ("planetary ring"; list reuse pays most here, the particles barely
+    change neighbours): one central body of mass 1 at the origin (particle 0) and n - 1 equal light particles of total
+    mass m_ring in a thin annulus r_in <= r < r_out (uniform in area), Gaussian thickness h x r, on circular Keplerian
+    orbits (G = 1).  Not one of BASELINE.json's configs: reported beside them.  Returns (pos[n,3], vel[n,3], mass[n]) in fp64."""
+    rng = np.random.default_rng(seed)
+    k = n - 1
+    r = np.sqrt(rng.uniform(r_in * r_in, r_out * r_out, k))
+    phi = rng.uniform(0.0, 2.0 * np.pi, k)
+    pos = np.zeros((n, 3))
+    vel = np.zeros((n, 3))
+    pos[1:, 0], pos[1:, 1], pos[1:, 2] = r * np.cos(phi), r * np.sin(phi), h * r * rng.normal(size=k)
+    v = 1.0 / np.sqrt(r)
+    vel[1:, 0], vel[1:, 1] = -v * np.sin(phi), v * np.cos(phi)
+    mass = np.full(n, m_ring / k)
+    mass[0] = 1.0
+    return pos, vel, mass
+
+
 def disk_halo(n: int, seed: int):
     """90% exponential disk (R_d = 1, sech^2 vertical profile, h = 0.1, total mass 0.1) plus
     10% Hernquist halo (a = 3, total mass 0.9, truncated at r = 100).  Positions only."""
